@@ -1,0 +1,136 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY (see grid.hpp).  C entry points for the ctypes harness (oracle/pyoracle.py).
+// All pointers are host pointers; arrays are contiguous, axis 0 fastest.
+#include <cstring>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#include "solvers.hpp"
+
+using namespace orc;
+
+extern "C" {
+
+void* orc_create(const int* shape, const double* spacing, const double* origin, const double* const* edges,
+                 int coord, int order, const int* bc) {
+    Grid* g = new Grid;
+    for (int a = 0; a < 3; ++a) {
+        g->n[a] = shape[a];
+        g->h[a] = spacing ? spacing[a] : 1.0;
+        g->origin[a] = origin ? origin[a] : 0.0;
+    }
+    g->coord = coord;
+    g->order = order;
+    g->R = (order == 6) ? 3 : 1;
+    for (int f = 0; f < 6; ++f) g->bc[f] = bc[f];
+    for (int f = 0; f < 6; ++f)
+        if (g->bc[f] == BC_DIRICHLET_GHOST) g->ghost[f].assign(g->face_len(f), 0.0);
+    if (coord == SPHERICAL) {
+        for (int a = 0; a < 3; ++a) g->edge[a].assign(edges[a], edges[a] + shape[a] + 1);
+        setup_spherical(*g);
+    }
+    return g;
+}
+
+void orc_destroy(void* h) { delete (Grid*)h; }
+
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+    omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+int orc_get_threads() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_gamma(void* h, double gamma) { ((Grid*)h)->gamma = gamma; }
+
+long orc_face_len(void* h, int f) { return (long)((Grid*)h)->face_len(f); }
+
+void orc_set_ghost_face(void* h, int f, const double* v) {
+    Grid* g = (Grid*)h;
+    g->ghost[f].assign(v, v + g->face_len(f));
+}
+void orc_get_ghost_face(void* h, int f, double* v) {
+    Grid* g = (Grid*)h;
+    if (g->ghost[f].empty()) return;
+    std::memcpy(v, g->ghost[f].data(), g->ghost[f].size() * sizeof(double));
+}
+
+void orc_apply(void* h, const double* phi, double* out, int use_ghost) { apply(*(Grid*)h, phi, out, use_ghost != 0); }
+void orc_apply_f32(void* h, const float* phi, float* out, int use_ghost) { apply(*(Grid*)h, phi, out, use_ghost != 0); }
+void orc_diag(void* h, double* out) {
+    Grid* g = (Grid*)h;
+    for (int k = 0; k < g->n[2]; ++k)
+        for (int j = 0; j < g->n[1]; ++j)
+            for (int i = 0; i < g->n[0]; ++i) out[g->idx(i, j, k)] = diag<double>(*g, i, j, k);
+}
+double orc_residual_norm(void* h, const double* phi, const double* rhs) {
+    return residual_norm(*(Grid*)h, phi, rhs, true);
+}
+
+void orc_rbsor_half(void* h, double* phi, const double* rhs, double omega, int colour) {
+    rbsor_half(*(Grid*)h, phi, rhs, omega, colour, true);
+}
+void orc_rbsor(void* h, double* phi, const double* rhs, double omega, int nsweeps, double* resnorm) {
+    rbsor(*(Grid*)h, phi, rhs, omega, nsweeps, true);
+    if (resnorm) *resnorm = residual_norm(*(Grid*)h, phi, rhs, true);
+}
+void orc_rbsor_f32(void* h, float* phi, const float* rhs, float omega, int nsweeps) {
+    rbsor(*(Grid*)h, phi, rhs, omega, nsweeps, true);
+}
+
+int orc_cg(void* h, double* phi, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
+           double* relres, double* history) {
+    return cg(*(Grid*)h, phi, rhs, rtol, max_iter, fixed_iters, iters, relres, history);
+}
+int orc_bicgstab(void* h, double* phi, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
+                 int* iters, double* relres, double* history) {
+    return bicgstab(*(Grid*)h, phi, rhs, rtol, max_iter, fixed_iters, jacobi, iters, relres, history);
+}
+int orc_vcycle(void* h, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, int coarsest_sweeps,
+               int precision, int restriction, int ncycles, double* resnorms) {
+    return vcycle(*(Grid*)h, phi, rhs, nu1, nu2, coarsest_n, coarsest_sweeps, precision, restriction, ncycles,
+                  resnorms);
+}
+
+// transfer operators between this grid (fine) and its first coarse level, for the pins
+void orc_restrict(void* h, const double* r, double* fc, int restriction) {
+    Grid* g = (Grid*)h;
+    Grid c = coarsen(*g, 1);
+    restrict_fw(*g, c, r, fc, restriction);
+}
+void orc_prolong_add(void* h, const double* ec, double* phi, double coarse_gamma) {
+    Grid* g = (Grid*)h;
+    Grid c = coarsen(*g, 1);
+    c.gamma = coarse_gamma;
+    prolong_add(*g, c, ec, phi);
+}
+
+void orc_multipole_moments(void* h, const double* rho, int lmax, double* q) {
+    multipole_moments(*(Grid*)h, rho, lmax, q);
+}
+double orc_multipole_potential(const double* q, int lmax, double G, double x, double y, double z) {
+    return multipole_potential(q, lmax, G, x, y, z);
+}
+void orc_multipole_bc(void* h, const double* rho, double G, int lmax, double* moments) {
+    multipole_bc(*(Grid*)h, rho, G, lmax, moments);
+}
+
+// spherical helpers for the harness: centres and the outer ghost radius
+void orc_centres(void* h, int axis, double* out) {
+    Grid* g = (Grid*)h;
+    if (g->coord == SPHERICAL)
+        std::memcpy(out, g->ctr[axis].data(), g->ctr[axis].size() * sizeof(double));
+    else
+        for (int i = 0; i < g->n[axis]; ++i) out[i] = g->coordinate(axis, i);
+}
+double orc_r_ghost_out(void* h) { return ((Grid*)h)->r_ghost_out; }
+
+}  // extern "C"

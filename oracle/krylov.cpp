@@ -1,0 +1,162 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY (see grid.hpp).
+// Conjugate gradient and BiCGSTAB, step by step after Saad (2003), which the paper says it follows
+// ("For further details on CG and BICGSTAB we refer the reader to Saad (2003), which our
+// description follows closely").  CG: Alg. 6.18 on the SPD matrix A = -L_h with b = -rhs.
+// BiCGSTAB: Alg. 7.7 on the nonsymmetric spherical operator, with right Jacobi scaling
+// (readings C4/C10).  Inhomogeneous ghost values enter only through r0; search directions see
+// homogeneous ghosts (reading C3).  Dot products: long double, plane partial sums in k order.
+#include <cmath>
+#include <vector>
+
+#include "solvers.hpp"
+
+namespace orc {
+
+static bool all_periodic(const Grid& g) {
+    for (int f = 0; f < 6; ++f)
+        if (g.bc[f] != BC_PERIODIC) return false;
+    return g.coord == CARTESIAN;
+}
+
+static void sub_mean(const Grid& g, double* v) {
+    const double mu = sum(g, v) / (double)g.size();
+    const size_t n = g.size();
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) v[p] -= mu;
+}
+
+int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
+       double* relres, double* history) {
+    const size_t n = g.size();
+    std::vector<double> r(n), p(n), q(n), b(n);
+    const bool project = all_periodic(g);  // A singular, null space = constants (reading C3)
+    // b = -rhs ; projected once onto zero mean for the periodic problem
+    for (size_t m = 0; m < n; ++m) b[m] = -rhs[m];
+    if (project) sub_mean(g, b.data());
+    // r0 = b - A x0 = b + L x0 (ghosts included)
+    apply(g, x, q.data(), true);
+#pragma omp parallel for schedule(static)
+    for (size_t m = 0; m < n; ++m) r[m] = b[m] + q[m];
+    if (project) sub_mean(g, r.data());
+    p = r;
+    double rr = dot(g, r.data(), r.data());
+    const double rr0 = rr;
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    if (history) history[0] = 1.0;
+    int it = 0, status = (fixed_iters > 0) ? ST_OK : ST_NOT_CONVERGED;
+    if (fixed_iters <= 0 && (rr0 == 0.0)) {
+        status = ST_OK;
+    } else {
+        for (it = 0; it < nit;) {
+            // q = A p = -L p (homogeneous ghosts)
+            apply(g, p.data(), q.data(), false);
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) q[m] = -q[m];
+            const double pq = dot(g, p.data(), q.data());
+            const double alpha = rr / pq;
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) {
+                x[m] = std::fma(alpha, p[m], x[m]);
+                r[m] = std::fma(-alpha, q[m], r[m]);
+            }
+            if (project) sub_mean(g, r.data());
+            const double rr_new = dot(g, r.data(), r.data());
+            ++it;
+            if (history) history[it] = std::sqrt(rr_new / rr0);
+            if (fixed_iters <= 0 && std::sqrt(rr_new) <= rtol * std::sqrt(rr0)) {
+                rr = rr_new;
+                status = ST_OK;
+                break;
+            }
+            const double beta = rr_new / rr;
+            rr = rr_new;
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) p[m] = std::fma(beta, p[m], r[m]);
+        }
+    }
+    if (project) sub_mean(g, x);
+    if (iters) *iters = it;
+    if (relres) *relres = (rr0 > 0) ? std::sqrt(rr / rr0) : 0.0;
+    return status;
+}
+
+int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
+             int* iters, double* relres, double* history) {
+    const size_t n = g.size();
+    std::vector<double> r(n), r0(n), p(n), v(n), s(n), t(n), ph(n), sh(n), dg(n);
+    // D = diag(A) for right Jacobi scaling: p^ = D^-1 p, s^ = D^-1 s.  The system solved is L x = rhs as it
+    // stands (A = L, nonsymmetric); its diagonal is -d.
+    for (int k = 0; k < g.n[2]; ++k)
+        for (int j = 0; j < g.n[1]; ++j)
+            for (int i = 0; i < g.n[0]; ++i) dg[g.idx(i, j, k)] = jacobi ? -diag<double>(g, i, j, k) : 1.0;
+    // r0 = b - A x0 (ghosts included)
+    apply(g, x, v.data(), true);
+#pragma omp parallel for schedule(static)
+    for (size_t m = 0; m < n; ++m) r[m] = rhs[m] - v[m];
+    r0 = r;  // shadow residual r^_0 = r_0
+    p = r;
+    double rho = dot(g, r0.data(), r.data());
+    const double rr0 = dot(g, r.data(), r.data());
+    double rr = rr0;
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    if (history) history[0] = 1.0;
+    int it = 0, status = (fixed_iters > 0) ? ST_OK : ST_NOT_CONVERGED;
+    if (fixed_iters <= 0 && rr0 == 0.0) {
+        status = ST_OK;
+    } else {
+        for (it = 0; it < nit;) {
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) ph[m] = p[m] / dg[m];
+            apply(g, ph.data(), v.data(), false);  // v = A p^
+            const double r0v = dot(g, r0.data(), v.data());
+            if (!(std::fabs(r0v) > 0.0) || !std::isfinite(r0v) || !(std::fabs(rho) > 0.0)) {
+                status = ST_BREAKDOWN;
+                break;
+            }
+            const double alpha = rho / r0v;
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) {
+                s[m] = std::fma(-alpha, v[m], r[m]);
+                sh[m] = s[m] / dg[m];
+            }
+            apply(g, sh.data(), t.data(), false);  // t = A s^
+            const double ts = dot(g, t.data(), s.data());
+            const double tt = dot(g, t.data(), t.data());
+            if (!(tt > 0.0) || !std::isfinite(tt)) {
+                status = ST_BREAKDOWN;
+                break;
+            }
+            const double omega = ts / tt;
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) {
+                x[m] = std::fma(omega, sh[m], std::fma(alpha, ph[m], x[m]));
+                r[m] = std::fma(-omega, t[m], s[m]);
+            }
+            rr = dot(g, r.data(), r.data());
+            ++it;
+            if (history) history[it] = std::sqrt(rr / rr0);
+            if (!std::isfinite(rr)) {
+                status = ST_BREAKDOWN;
+                break;
+            }
+            if (fixed_iters <= 0 && std::sqrt(rr) <= rtol * std::sqrt(rr0)) {
+                status = ST_OK;
+                break;
+            }
+            if (!(std::fabs(omega) > 0.0)) {
+                status = ST_BREAKDOWN;
+                break;
+            }
+            const double rho_new = dot(g, r0.data(), r.data());
+            const double beta = (rho_new / rho) * (alpha / omega);
+            rho = rho_new;
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) p[m] = std::fma(beta, std::fma(-omega, v[m], p[m]), r[m]);
+        }
+    }
+    if (iters) *iters = it;
+    if (relres) *relres = (rr0 > 0) ? std::sqrt(rr / rr0) : 0.0;
+    return status;
+}
+
+}  // namespace orc

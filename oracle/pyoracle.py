@@ -1,0 +1,206 @@
+"""ORACLE — TEST INFRASTRUCTURE ONLY.  ctypes wrapper around oracle/liboracle.so (plain C++ CPU oracle).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+It imports nothing from the CUDA package.
+"""
+import ctypes as C
+import importlib.util
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+CARTESIAN, SPHERICAL = 0, 1
+BC_DIRICHLET_GHOST, BC_PERIODIC, BC_NEUMANN0, BC_AXIS = 0, 1, 2, 3
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        spec = importlib.util.spec_from_file_location("_oracle_build", os.path.join(_HERE, "build.py"))
+        mod = importlib.util.module_from_spec(spec)
+        spec.loader.exec_module(mod)
+        _lib = C.CDLL(mod.build())
+        _lib.orc_create.restype = C.c_void_p
+        _lib.orc_residual_norm.restype = C.c_double
+        _lib.orc_multipole_potential.restype = C.c_double
+        _lib.orc_r_ghost_out.restype = C.c_double
+        _lib.orc_face_len.restype = C.c_long
+    return _lib
+
+
+def _p(a, ct=C.c_double):
+    return a.ctypes.data_as(C.POINTER(ct)) if a is not None else None
+
+
+def _f64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+def set_threads(n):
+    lib().orc_set_threads(int(n))
+
+
+def get_threads():
+    return int(lib().orc_get_threads())
+
+
+class Oracle:
+    """One grid + operator.  Arrays are numpy, shape (nz, ny, nx) i.e. axis 0 of the method is the last numpy axis."""
+
+    def __init__(self, shape, spacing=None, origin=None, edges=None, coord=CARTESIAN, order=2, bc=(0,) * 6):
+        L = lib()
+        self.shape = tuple(int(s) for s in shape)  # (n0, n1, n2), n0 fastest
+        self.npshape = self.shape[::-1]
+        self.coord, self.order = coord, order
+        self.bc = tuple(int(b) for b in bc)
+        sh = (C.c_int * 3)(*self.shape)
+        sp = (C.c_double * 3)(*(spacing if spacing is not None else (1.0, 1.0, 1.0)))
+        og = (C.c_double * 3)(*(origin if origin is not None else (0.0, 0.0, 0.0)))
+        self.spacing = tuple(sp)
+        self.origin = tuple(og)
+        bcs = (C.c_int * 6)(*self.bc)
+        if edges is not None:
+            self._edges = [_f64(e) for e in edges]
+            ed = (C.POINTER(C.c_double) * 3)(*[_p(e) for e in self._edges])
+        else:
+            ed = None
+        self.h = C.c_void_p(L.orc_create(sh, sp, og, ed, coord, order, bcs))
+
+    def __del__(self):
+        try:
+            if self.h:
+                lib().orc_destroy(self.h)
+                self.h = None
+        except Exception:
+            pass
+
+    @property
+    def size(self):
+        return self.shape[0] * self.shape[1] * self.shape[2]
+
+    def set_gamma(self, gamma):
+        lib().orc_set_gamma(self.h, C.c_double(gamma))
+
+    def face_len(self, f):
+        return int(lib().orc_face_len(self.h, f))
+
+    def set_ghost_face(self, f, v):
+        v = _f64(v).ravel()
+        assert v.size == self.face_len(f)
+        lib().orc_set_ghost_face(self.h, f, _p(v))
+
+    def get_ghost_face(self, f):
+        v = np.zeros(self.face_len(f))
+        lib().orc_get_ghost_face(self.h, f, _p(v))
+        return v
+
+    def apply(self, phi, use_ghost=True):
+        phi = _f64(phi)
+        out = np.empty_like(phi)
+        lib().orc_apply(self.h, _p(phi), _p(out), int(use_ghost))
+        return out
+
+    def apply_f32(self, phi, use_ghost=True):
+        phi = np.ascontiguousarray(phi, dtype=np.float32)
+        out = np.empty_like(phi)
+        lib().orc_apply_f32(self.h, _p(phi, C.c_float), _p(out, C.c_float), int(use_ghost))
+        return out
+
+    def diag(self):
+        out = np.empty(self.npshape)
+        lib().orc_diag(self.h, _p(out))
+        return out
+
+    def residual_norm(self, phi, rhs):
+        phi, rhs = _f64(phi), _f64(rhs)
+        return float(lib().orc_residual_norm(self.h, _p(phi), _p(rhs)))
+
+    def rbsor_half(self, phi, rhs, omega, colour):
+        """In place on phi (must be a contiguous float64 array)."""
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs = _f64(rhs)
+        lib().orc_rbsor_half(self.h, _p(phi), _p(rhs), C.c_double(omega), int(colour))
+
+    def rbsor(self, phi, rhs, omega, nsweeps, want_resnorm=False):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs = _f64(rhs)
+        rn = C.c_double(0.0)
+        lib().orc_rbsor(self.h, _p(phi), _p(rhs), C.c_double(omega), int(nsweeps),
+                        C.byref(rn) if want_resnorm else None)
+        return rn.value if want_resnorm else None
+
+    def rbsor_f32(self, phi, rhs, omega, nsweeps):
+        assert phi.dtype == np.float32 and phi.flags.c_contiguous
+        rhs = np.ascontiguousarray(rhs, dtype=np.float32)
+        lib().orc_rbsor_f32(self.h, _p(phi, C.c_float), _p(rhs, C.c_float), C.c_float(omega), int(nsweeps))
+
+    def _krylov(self, fn, phi, rhs, rtol, max_iter, fixed_iters, want_history, extra=()):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs = _f64(rhs)
+        iters, relres = C.c_int(0), C.c_double(0.0)
+        nh = (fixed_iters if fixed_iters > 0 else max_iter) + 1
+        hist = np.zeros(nh) if want_history else None
+        st = fn(self.h, _p(phi), _p(rhs), C.c_double(rtol), int(max_iter), int(fixed_iters), *extra,
+                C.byref(iters), C.byref(relres), _p(hist))
+        out = dict(status=int(st), iters=iters.value, relres=relres.value)
+        if want_history:
+            out["history"] = hist[: iters.value + 1]
+        return out
+
+    def cg(self, phi, rhs, rtol=1e-8, max_iter=10000, fixed_iters=0, want_history=False):
+        return self._krylov(lib().orc_cg, phi, rhs, rtol, max_iter, fixed_iters, want_history)
+
+    def bicgstab(self, phi, rhs, rtol=1e-8, max_iter=10000, fixed_iters=0, jacobi=1, want_history=False):
+        return self._krylov(lib().orc_bicgstab, phi, rhs, rtol, max_iter, fixed_iters, want_history,
+                            extra=(int(jacobi),))
+
+    def vcycle(self, phi, rhs, nu1=2, nu2=2, coarsest_n=8, coarsest_sweeps=50, precision=0, restriction=0,
+               ncycles=1):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs = _f64(rhs)
+        rn = np.zeros(ncycles + 1)
+        st = lib().orc_vcycle(self.h, _p(phi), _p(rhs), int(nu1), int(nu2), int(coarsest_n), int(coarsest_sweeps),
+                              int(precision), int(restriction), int(ncycles), _p(rn))
+        return dict(status=int(st), resnorms=rn)
+
+    def restrict(self, r, restriction=0):
+        r = _f64(r)
+        fc = np.zeros(tuple(s // 2 for s in self.npshape))
+        lib().orc_restrict(self.h, _p(r), _p(fc), int(restriction))
+        return fc
+
+    def prolong_add(self, ec, phi, coarse_gamma):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        ec = _f64(ec)
+        lib().orc_prolong_add(self.h, _p(ec), _p(phi), C.c_double(coarse_gamma))
+
+    def multipole_moments(self, rho, lmax):
+        rho = _f64(rho)
+        q = np.zeros((lmax + 1) ** 2)
+        lib().orc_multipole_moments(self.h, _p(rho), int(lmax), _p(q))
+        return q
+
+    def multipole_bc(self, rho, G, lmax):
+        rho = _f64(rho)
+        q = np.zeros((lmax + 1) ** 2)
+        lib().orc_multipole_bc(self.h, _p(rho), C.c_double(G), int(lmax), _p(q))
+        return q
+
+    def centres(self, axis):
+        out = np.zeros(self.shape[axis])
+        lib().orc_centres(self.h, int(axis), _p(out))
+        return out
+
+    def r_ghost_out(self):
+        return float(lib().orc_r_ghost_out(self.h))
+
+
+def multipole_potential(q, lmax, G, x, y, z):
+    q = _f64(q)
+    return float(lib().orc_multipole_potential(_p(q), int(lmax), C.c_double(G), C.c_double(x), C.c_double(y),
+                                               C.c_double(z)))

@@ -1,0 +1,42 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY (see grid.hpp).  Declarations of the solver steps.
+#pragma once
+#include "grid.hpp"
+
+namespace orc {
+
+enum { ST_OK = 0, ST_NOT_CONVERGED = 1, ST_BREAKDOWN = 2 };
+
+// One colour half-sweep of red-black SOR (colour 0 = red = (i+j+k) even, 1 = black).  PAPER.md:59-63.
+template <typename T>
+void rbsor_half(const Grid& g, T* phi, const T* rhs, T omega, int colour, bool use_ghost);
+// nsweeps full sweeps: red then black (PAPER.md:74 footnote: a sweep is one complete round of updates).
+template <typename T>
+void rbsor(const Grid& g, T* phi, const T* rhs, T omega, int nsweeps, bool use_ghost);
+
+// Conjugate gradient, Saad Alg. 6.18 on A = -L_h (SPD), b = -rhs.  PAPER.md:95-105.
+int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
+       double* relres, double* history /* nullable, max_iter+1 relative residuals */);
+
+// BiCGSTAB, Saad Alg. 7.7 with right Jacobi scaling (jacobi != 0).  PAPER.md:105; reading C4/C10.
+int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
+             int* iters, double* relres, double* history);
+
+// Geometric multigrid V-cycles (Eq. 11-13; reading C7).
+//   restriction: 0 = transpose of trilinear (1/8)[1 3 3 1]^3, 1 = mean of the 8 children
+//   precision:   0 = fp64, 1 = mixed (fp64 residual + correction, fp32 error-equation V-cycle)
+int vcycle(const Grid& g, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, int coarsest_sweeps,
+           int precision, int restriction, int ncycles, double* resnorms /* nullable, ncycles+1 */);
+
+// Transfer operators exposed for the pins (R 1 = 1, P 1 = 1, <Pu,v> = 8 <u,Rv>).
+template <typename T>
+void restrict_fw(const Grid& fine, const Grid& coarse, const T* r, T* fc, int restriction);
+template <typename T>
+void prolong_add(const Grid& fine, const Grid& coarse, const T* ec, T* phi);
+Grid coarsen(const Grid& fine, int level_of_coarse);
+
+// Multipole boundary condition, Eq. 19-20.  Fills g.ghost[] on Dirichlet faces.
+void multipole_moments(const Grid& g, const double* rho, int lmax, double* q /* (lmax+1)^2, index l*l+l+m */);
+double multipole_potential(const double* q, int lmax, double G, double x, double y, double z);
+void multipole_bc(Grid& g, const double* rho, double G, int lmax, double* moments /* nullable */);
+
+}  // namespace orc

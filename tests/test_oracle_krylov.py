@@ -1,0 +1,166 @@
+"""Pins for the oracle's CG and BiCGSTAB (oracle/krylov.cpp) — SURVEY.md §8(c) C3, C4, C10; Table 3."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import pyoracle as po
+from helpers import dense_matrix, make_oracle, rel_l2
+from paper_2605_03563_b200 import workloads as wl
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+D6 = (po.BC_DIRICHLET_GHOST,) * 6
+P6 = (po.BC_PERIODIC,) * 6
+COUNTS = {(r[0], int(r[1])): (int(r[2]), int(r[3]))
+          for r in (l.split() for l in open(os.path.join(GOLD, "paper_table3_counts.txt")) if l[0] != "#")}
+
+
+def test_cg_matches_dense_solve_8cubed_with_ghosts():
+    shape, h, org = (8, 8, 8), (0.1, 0.12, 0.09), (0.0, 0.1, 0.2)
+    w = dict(shape=shape, spacing=h, origin=org, bc=D6)
+    o = make_oracle(w)
+    A = dense_matrix(o)
+    g = lambda x, y, z: np.sin(x + 2 * y) * np.exp(z)
+    for k, fa in enumerate(wl.analytic_ghost_faces(w, g)):
+        o.set_ghost_face(k, fa)
+    rhs = wl.random_field(shape, 3)
+    bnd = o.apply(np.zeros(o.npshape))  # L applied to the ghost-only field
+    exact = np.linalg.solve(A, (rhs - bnd).reshape(-1)).reshape(rhs.shape)
+    phi = np.zeros_like(rhs)
+    res = o.cg(phi, rhs, rtol=1e-13, max_iter=500)
+    assert res["status"] == 0
+    assert rel_l2(phi, exact) < 1e-11
+    # warm start: a non-zero initial guess is honoured; the residual is relative to r0 of that guess
+    half = 0.5 * exact
+    res2 = o.cg(half, rhs, rtol=1e-12, max_iter=500)
+    assert res2["status"] == 0 and rel_l2(half, exact) < 1e-10
+
+
+def test_cg_finite_termination_by_distinct_eigenvalues():
+    # CG terminates in at most as many steps as A has distinct eigenvalues: on an isotropic 4^3 Dirichlet grid the
+    # eigenvalues are sums of 3 values out of 4 (20 multisets; 16 distinct because lam1+lam4 = lam2+lam3)
+    shape = (4, 4, 4)
+    o = po.Oracle(shape, (0.2, 0.2, 0.2), bc=D6)
+    ev = np.linalg.eigvalsh(dense_matrix(o))
+    ndist = len(np.unique(np.round(ev / np.abs(ev).max(), 10)))
+    assert ndist == 16
+    rhs = wl.random_field(shape, 5)
+    phi = np.zeros_like(rhs)
+    res = o.cg(phi, rhs, rtol=1e-12, max_iter=64)
+    assert res["status"] == 0 and res["iters"] <= ndist
+
+
+def test_cg_energy_monotone_residual_not():
+    shape = (16, 16, 16)
+    o = po.Oracle(shape, (1 / 16,) * 3, bc=D6)
+    rhs = wl.random_field(shape, 9)
+    energies = []
+    for it in range(1, 25):
+        phi = np.zeros_like(rhs)
+        o.cg(phi, rhs, fixed_iters=it)
+        Ap = -o.apply(phi, use_ghost=False)
+        energies.append(0.5 * np.vdot(phi, Ap) + np.vdot(rhs, phi))
+    assert all(b < a for a, b in zip(energies, energies[1:]))
+
+
+def _two_sphere_counts(order, n):
+    w = wl.two_spheres(n)
+    w["order"] = order
+    o = make_oracle(w)
+    for k, fa in enumerate(wl.analytic_ghost_faces(w, w["potential"], R=3 if order == 6 else 1)):
+        o.set_ghost_face(k, fa)
+    phi = np.zeros_like(w["rhs"])
+    res = o.cg(phi, w["rhs"], rtol=1e-6, max_iter=2000, want_history=True)
+    return int(np.argmax(res["history"] < 1e-4)), res["iters"], phi, w
+
+
+def test_paper_table3_cg2_counts_64():
+    c4, c6, phi, w = _two_sphere_counts(2, 64)
+    assert (c4, c6) == COUNTS[("CG2", 64)]  # 125 / 171
+    # and the solution is the analytic potential up to truncation error (Eq. 24)
+    assert np.abs(phi - w["exact"]).max() / np.abs(w["exact"]).max() < 0.05
+
+
+def test_paper_table3_cg6_counts_64():
+    c4, c6, _, _ = _two_sphere_counts(6, 64)
+    assert (c4, c6) == COUNTS[("CG6", 64)]  # 151 / 207
+
+
+def test_periodic_cg_matches_fft_direct_solve():
+    # exact pin for config 4's operator: x^(k) = b^(k)/lambda(k), x^(0) = 0 with the symbol of the 19-point star
+    w = wl.config4(32)
+    o = make_oracle(w)
+    n, h = 32, w["spacing"][0]
+    t = 2 * math.pi * np.fft.fftfreq(n)
+    s1 = (-49 / 18 + 3 * np.cos(t) - 0.3 * np.cos(2 * t) + np.cos(3 * t) / 45) / h ** 2
+    lam = s1[:, None, None] + s1[None, :, None] + s1[None, None, :]
+    bh = np.fft.fftn(w["rhs"])
+    lam[0, 0, 0] = 1.0
+    xh = bh / lam
+    xh[0, 0, 0] = 0.0
+    exact = np.real(np.fft.ifftn(xh))
+    phi = np.zeros_like(w["rhs"])
+    res = o.cg(phi, w["rhs"], rtol=1e-10, max_iter=1000)
+    assert res["status"] == 0
+    assert res["iters"] == pytest.approx(105, abs=25)  # SURVEY.md C3 probe: 105 at 32^3 (different RNG)
+    assert rel_l2(phi, exact) < 1e-9
+    assert abs(phi.mean()) < 1e-14 * np.abs(phi).max()
+    # the input field itself: zero mean, unit variance, band-limited to |k| <= n/4
+    assert abs(w["rhs"].mean()) < 1e-12 and w["rhs"].std() == pytest.approx(1.0, abs=1e-12)
+    k1 = np.fft.fftfreq(n, 1 / n)
+    kk = np.sqrt(k1[:, None, None] ** 2 + k1[None, :, None] ** 2 + k1[None, None, :] ** 2)
+    assert np.abs(bh[kk > n / 4 + 1e-9]).max() < 1e-9 * np.abs(bh).max()
+
+
+# ---- BiCGSTAB -------------------------------------------------------------------------------------------------------
+def _sph_small():
+    re, te, pe = wl.spherical_edges(8, 4, 8)
+    bc = (po.BC_NEUMANN0, po.BC_DIRICHLET_GHOST, po.BC_AXIS, po.BC_AXIS, po.BC_PERIODIC, po.BC_PERIODIC)
+    return po.Oracle((8, 4, 8), edges=(re, te, pe), coord=po.SPHERICAL, bc=bc)
+
+
+def test_bicgstab_matches_dense_lu_spherical_8x4x8():
+    o = _sph_small()
+    A = dense_matrix(o)
+    ghost = wl.hash_uniform(4, np.arange(o.face_len(1)))
+    o.set_ghost_face(1, ghost)
+    rhs = wl.random_field(o.shape, 6)
+    bnd = o.apply(np.zeros(o.npshape))
+    exact = np.linalg.solve(A, (rhs - bnd).reshape(-1)).reshape(rhs.shape)
+    for jacobi in (1, 0):
+        phi = np.zeros_like(rhs)
+        res = o.bicgstab(phi, rhs, rtol=1e-12, max_iter=2000, jacobi=jacobi)
+        assert res["status"] == 0, res
+        assert rel_l2(phi, exact) < 1e-9
+
+
+def test_bicgstab_agrees_with_cg_on_spd_problem():
+    shape = (12, 12, 12)
+    o = po.Oracle(shape, (0.1,) * 3, bc=D6)
+    rhs = wl.random_field(shape, 8)
+    a, b = np.zeros_like(rhs), np.zeros_like(rhs)
+    o.cg(a, rhs, rtol=1e-12)
+    res = o.bicgstab(b, rhs, rtol=1e-12)
+    assert res["status"] == 0 and rel_l2(b, a) < 1e-10
+
+
+def test_bicgstab_reports_true_residual():
+    o = _sph_small()
+    rhs = wl.random_field(o.shape, 12)
+    phi = np.zeros_like(rhs)
+    res = o.bicgstab(phi, rhs, rtol=1e-9, max_iter=2000)
+    true = o.residual_norm(phi, rhs) / np.linalg.norm(rhs)
+    assert res["status"] == 0 and true < 1e-8 and true == pytest.approx(res["relres"], rel=1e-3, abs=1e-12)
+
+
+def test_config5_reduced_jacobi_scaled_bicgstab_converges():
+    # SURVEY.md C10 probe: with right Jacobi scaling 228 iterations at 32x16x32 (erratic residual)
+    w = wl.config5(32, 16, 32)
+    o = make_oracle(w)
+    o.multipole_bc(w["rho"], w["G"], w["lmax"])
+    phi = np.zeros_like(w["rhs"])
+    res = o.bicgstab(phi, w["rhs"], rtol=1e-8, max_iter=3000, jacobi=1)
+    assert res["status"] == 0
+    assert 100 < res["iters"] < 500
+    assert o.residual_norm(phi, w["rhs"]) <= 1e-7 * o.residual_norm(np.zeros_like(phi), w["rhs"])
