@@ -1,0 +1,136 @@
+/* poisson.h — C ABI of the B200-native matrix-free Poisson solvers (hot path of arxiv/paper_2605_03563,
+ * "Iterative Poisson Solvers for Self-gravity with the GPU Code Astaroth").
+ *
+ * The library solves  L_h phi = rhs  on a 3-D structured grid, where L_h is the finite-difference Laplacian
+ * (Eq. 1-2) and rhs = 4 pi G rho for self-gravity.  Every step of every call runs in hand-written
+ * CUDA kernels for sm_100a; there is no CPU fallback.  All work is enqueued on the stream given at create time.
+ *
+ * Conventions (DESIGN.md "Boundary" and readings C0):
+ *  - Unknowns: shape[0] x shape[1] x shape[2] points, index (i,j,k), axis 0 fastest; arrays are contiguous,
+ *    exactly shape[0]*shape[1]*shape[2] elements, 16-byte aligned.  Cartesian: axis 0,1,2 = x,y,z and point
+ *    coordinate = origin[a] + i*spacing[a].  Spherical: axis 0,1,2 = r,theta,phi given by cell edges.
+ *  - `d_*` arguments are DEVICE pointers owned by the caller; `h_*` arguments are HOST pointers.
+ *  - Faces: 0 = axis0 low, 1 = axis0 high, 2 = axis1 low, 3 = axis1 high, 4 = axis2 low, 5 = axis2 high.
+ *  - Ghost zones ("the multipole expansion of Phi in the ghost zones") are kept in the handle as six
+ *    face arrays with R = stencil radius layers (R = 1 for order 2, 3 for order 6).  Face on axis a, layer l
+ *    (distance l+1 outside the domain): index (l*n[a2] + q2)*n[a1] + q1 with (a1,a2) the other two axes in
+ *    increasing order, q1 fastest.  Only face ghosts exist: a star stencil never reads edge or corner ghosts.
+ *  - L_h is the Laplacian itself (negative definite); the SPD matrix "A" of the paper is -L_h.
+ *  - Return value: 0 OK; >0 soft status (1 NOT_CONVERGED: "warning ... if the threshold is not achieved
+ *    within a maximum number of iterations"; 2 BREAKDOWN); <0 error.  No exceptions, no aborts.
+ *  - Calls that return host scalars synchronise the stream; the others only enqueue work.
+ *  - A non-zero initial guess in d_phi is honoured (warm start).
+ */
+#ifndef POISSON_B200_H
+#define POISSON_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct poisson_ctx* poisson_t; /* opaque; owns scratch vectors, MG levels, face-ghost arrays */
+
+enum { POISSON_CARTESIAN = 0, POISSON_SPHERICAL = 1 };
+enum {
+    POISSON_BC_DIRICHLET_GHOST = 0, /* ghost values supplied by poisson_multipole_bc or poisson_set_ghost_faces */
+    POISSON_BC_PERIODIC = 1,
+    POISSON_BC_NEUMANN0 = 2,        /* zero normal flux through the face */
+    POISSON_BC_AXIS = 3             /* spherical theta faces on the polar axis: zero face area */
+};
+enum { POISSON_F64 = 0, POISSON_MIXED = 1 };
+enum {
+    POISSON_OK = 0,
+    POISSON_NOT_CONVERGED = 1,
+    POISSON_BREAKDOWN = 2,
+    POISSON_INVALID_ARG = -1,
+    POISSON_UNSUPPORTED = -2,
+    POISSON_CUDA_ERROR = -3,
+    POISSON_OUT_OF_MEMORY = -4
+};
+/* options for poisson_set_option */
+enum {
+    POISSON_OPT_KERNEL_PATH = 0,   /* 0 auto, 1 force the generic (direct global load) kernels, 2 force the
+                                      plane-pipeline (bulk-copy staged) kernels where they exist */
+    POISSON_OPT_RESTRICTION = 1,   /* V-cycle restriction: 0 = (1/8)[1 3 3 1]^3 (transpose of trilinear),
+                                      1 = mean of the 8 children (reading C7) */
+    POISSON_OPT_POLL_INTERVAL = 2, /* Krylov solvers poll the device convergence flag every this many iterations */
+    POISSON_OPT_JACOBI = 3,        /* BiCGSTAB right Jacobi scaling: 1 (default) on, 0 off (reading C10) */
+    POISSON_OPT_RECORD_HISTORY = 4 /* 1: record ||r_k||/||r_0|| per Krylov iteration for poisson_get_history */
+};
+
+/* Create a solver context for one grid + operator ("uniform and nonuniform grids in spherical and
+ * Cartesian coordinates"; 41-57).
+ *   shape[3], spacing[3], origin[3]: Cartesian geometry (spacing/origin ignored for spherical).
+ *   edges: NULL for Cartesian; for spherical three HOST arrays of shape[a]+1 cell-edge coordinates (r, theta, phi).
+ *          Radial centres are the geometric means of the edges.
+ *   coord_system: POISSON_CARTESIAN | POISSON_SPHERICAL.
+ *   stencil_order: 2 (7-point, radius 1) or 6 (19-point star, radius 3; Cartesian only) — PAPER.md:172.
+ *   bc[6]: boundary type per face.
+ *   cuda_stream: a cudaStream_t (NULL = default stream).
+ * Errors: INVALID_ARG (bad shape/order/bc), UNSUPPORTED, OUT_OF_MEMORY, CUDA_ERROR. */
+int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], const double origin[3],
+                   const double* const edges[3], int coord_system, int stencil_order, const int bc[6],
+                   void* cuda_stream);
+int poisson_destroy(poisson_t h);
+/* Static string describing the last error of this handle (or of create when h is NULL). */
+const char* poisson_last_error(poisson_t h);
+int poisson_set_option(poisson_t h, int option, int value);
+
+/* out = L_h phi with the handle's ghost values on Dirichlet faces.  d_out must not alias d_phi. */
+int poisson_apply_laplacian(poisson_t h, const double* d_phi, double* d_out);
+
+/* nsweeps full red-black SOR sweeps in place: red = (i+j+k) even first, then black; omega = 1 is Gauss-Seidel
+ * (PAPER.md:59-63).  h_resnorm (nullable) receives ||rhs - L phi||_2 after the last sweep. */
+int poisson_rbsor_sweep(poisson_t h, double* d_phi, const double* d_rhs, double omega, int nsweeps,
+                        double* h_resnorm);
+
+/* Unpreconditioned conjugate gradient on A = -L_h (Saad Alg. 6.18), fused as
+ * {p-update + matvec + p.Ap} and {r-update + ||r||^2}.  Stops when ||r_k|| <= rtol ||r_0|| (r_0 from the initial
+ * guess) or after max_iter iterations (-> NOT_CONVERGED).  fixed_iters > 0 runs exactly that many iterations.
+ * For an all-periodic grid the constant null space is projected out every iteration and phi is returned with
+ * zero mean (reading C3).  iters / relres are nullable host outputs. */
+int poisson_cg_solve(poisson_t h, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,
+                     int* iters, double* relres);
+
+/* BiCGSTAB (Saad Alg. 7.7) with right Jacobi scaling, for the nonsymmetric spherical operator;
+ * same stopping rule.  BREAKDOWN when rho, omega or r0^.v vanish or turn non-finite. */
+int poisson_bicgstab_solve(poisson_t h, double* d_phi, const double* d_rhs, double rtol, int max_iter,
+                           int fixed_iters, int* iters, double* relres);
+
+/* ncycles geometric-multigrid V-cycles (Eq. 11-13): nu1/nu2 red-black Gauss-Seidel sweeps,
+ * full-weighting restriction, trilinear prolongation, 2:1 cell-centred coarsening down to coarsest_n points per
+ * axis, coarsest level by coarsest_sweeps SOR sweeps.  precision = POISSON_F64 or POISSON_MIXED (fp64 residual
+ * and correction, fp32 error-equation cycle).  Cartesian, order 2, Dirichlet faces only.
+ * h_resnorms (nullable, ncycles+1): ||rhs - L phi||_2 before the first and after every cycle. */
+int poisson_mg_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
+                      int coarsest_sweeps, int precision, int ncycles, double* h_resnorms);
+
+/* Multipole-expansion open boundary (Eq. 19-20): moments q_lm = sum_cells rho r^l S_lm dV for
+ * 0 <= l <= lmax (<= 8), |m| <= l in one fused reduction over d_rho, then Phi_ghost = -G sum q_lm S_lm / r^(l+1)
+ * written into the handle's ghost faces (all Dirichlet faces in Cartesian, the outer radial shell in spherical).
+ * Expansion centre = coordinate origin.  h_moments (nullable): (lmax+1)^2 values, index l*l + l + m, cosine
+ * harmonics m >= 0, sine harmonics m < 0. */
+int poisson_multipole_bc(poisson_t h, const double* d_rho, double G, int lmax, double* h_moments);
+
+/* Helpers. */
+/* Copy caller-supplied ghost values (DEVICE arrays, layout above; NULL entries = leave that face) into the handle. */
+int poisson_set_ghost_faces(poisson_t h, const double* const d_faces[6]);
+/* Copy the handle's ghost face f into a DEVICE array of poisson_face_len(h,f) doubles. */
+int poisson_get_ghost_face(poisson_t h, int face, double* d_out);
+long poisson_face_len(poisson_t h, int face);
+/* ||rhs - L phi||_2 with the handle's ghosts. */
+int poisson_residual_norm(poisson_t h, const double* d_phi, const double* d_rhs, double* h_norm);
+/* Relative residual history of the last Krylov solve (needs POISSON_OPT_RECORD_HISTORY): h_out[0..n-1]. */
+int poisson_get_history(poisson_t h, double* h_out, int n);
+/* Number of kernels this handle has launched so far (bench bookkeeping). */
+long poisson_kernel_launches(poisson_t h);
+
+/* End-to-end variants with HOST buffers: host->device copy of rhs (and phi), the solve, device->host copy of phi,
+ * all on the handle's stream; synchronises. */
+int poisson_cg_solve_host(poisson_t h, double* h_phi, const double* h_rhs, double rtol, int max_iter,
+                          int fixed_iters, int* iters, double* relres);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* POISSON_B200_H */

@@ -1,0 +1,628 @@
+// api.cu — the C ABI of include/poisson.h: context set-up and the host-side solver drivers.
+// Drivers only enqueue kernels and poll a device flag; all arithmetic of the path runs in the kernels.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "common.cuh"
+
+using namespace pb;
+
+static std::string g_create_error;
+
+namespace pb {
+
+int fail(poisson_ctx* ctx, int code, const std::string& msg) {
+    if (ctx)
+        ctx->err = msg;
+    else
+        g_create_error = msg;
+    return code;
+}
+
+int fail_cuda(poisson_ctx* ctx, cudaError_t e, const char* what, const char* file, int line) {
+    char buf[512];
+    snprintf(buf, sizeof(buf), "CUDA error %s (%s) at %s:%d in %s", cudaGetErrorName(e), cudaGetErrorString(e), file,
+             line, what);
+    cudaGetLastError();
+    return fail(ctx, e == cudaErrorMemoryAllocation ? POISSON_OUT_OF_MEMORY : POISSON_CUDA_ERROR, buf);
+}
+
+double* scratch(poisson_ctx* ctx, int slot) {
+    if ((int)ctx->vec.size() <= slot) ctx->vec.resize(slot + 1, nullptr);
+    if (!ctx->vec[slot]) {
+        void* p = nullptr;
+        if (cudaMalloc(&p, ctx->npts * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            fail(ctx, POISSON_OUT_OF_MEMORY, "out of device memory for a scratch vector");
+            return nullptr;
+        }
+        ctx->vec[slot] = (double*)p;
+    }
+    return ctx->vec[slot];
+}
+
+}  // namespace pb
+
+static void free_levels(poisson_ctx* ctx) {
+    for (auto& L : ctx->levels) {
+        cudaFree(L.phi);
+        cudaFree(L.rhs);
+        cudaFree(L.res);
+        cudaFree(L.phi32);
+        cudaFree(L.rhs32);
+        cudaFree(L.res32);
+    }
+    ctx->levels.clear();
+    ctx->mg_coarsest_n = -1;
+}
+
+// Spherical coefficient arrays of DESIGN.md reading C5 (Eq. 2 by direct finite differences on
+// (r,theta,phi) with geometric-mean radial centres).
+static int setup_spherical(poisson_ctx* ctx) {
+    const int nr = ctx->op.n[0], nt = ctx->op.n[1], np = ctx->op.n[2];
+    const std::vector<double>&re = ctx->edges[0], &te = ctx->edges[1], &pe = ctx->edges[2];
+    std::vector<double>&rc = ctx->ctr[0], &tc = ctx->ctr[1], &pc = ctx->ctr[2];
+    rc.resize(nr);
+    tc.resize(nt);
+    pc.resize(np);
+    for (int i = 0; i < nr; ++i) rc[i] = std::sqrt(re[i] * re[i + 1]);
+    for (int j = 0; j < nt; ++j) tc[j] = 0.5 * (te[j] + te[j + 1]);
+    for (int k = 0; k < np; ++k) pc[k] = 0.5 * (pe[k] + pe[k + 1]);
+    ctx->r_ghost_out = re[nr] * std::sqrt(re[nr] / re[nr - 1]);
+    const double r_ghost_in = re[0] * std::sqrt(re[0] / re[1]);
+    std::vector<double> coef(4 * nr + 4 * nt);
+    double *ar_m = coef.data(), *ar_p = ar_m + nr, *ir2 = ar_p + nr, *dr = ir2 + nr;
+    double *at_m = dr + nr, *at_p = at_m + nt, *cp = at_p + nt, *dt = cp + nt;
+    for (int i = 0; i < nr; ++i) {
+        const double ri = rc[i], dri = re[i + 1] - re[i];
+        const double rm = (i > 0) ? rc[i - 1] : r_ghost_in;
+        const double rp = (i < nr - 1) ? rc[i + 1] : ctx->r_ghost_out;
+        ir2[i] = 1.0 / (ri * ri);
+        ar_m[i] = (re[i] * re[i]) / ((ri - rm) * (ri * ri) * dri);
+        ar_p[i] = (re[i + 1] * re[i + 1]) / ((rp - ri) * (ri * ri) * dri);
+        if (i == 0 && ctx->op.bc[0] == POISSON_BC_NEUMANN0) ar_m[i] = 0.0;
+        if (i == nr - 1 && ctx->op.bc[1] == POISSON_BC_NEUMANN0) ar_p[i] = 0.0;
+        dr[i] = ar_m[i] + ar_p[i];
+    }
+    const double dph = pe[1] - pe[0];
+    for (int j = 0; j < nt; ++j) {
+        const double dth = te[j + 1] - te[j], st = std::sin(tc[j]);
+        at_m[j] = std::sin(te[j]) / (st * dth * dth);
+        at_p[j] = std::sin(te[j + 1]) / (st * dth * dth);
+        if (j == 0 && ctx->op.bc[2] == POISSON_BC_AXIS) at_m[j] = 0.0;
+        if (j == nt - 1 && ctx->op.bc[3] == POISSON_BC_AXIS) at_p[j] = 0.0;
+        cp[j] = 1.0 / (st * st * dph * dph);
+        dt[j] = (at_m[j] + at_p[j]) + 2.0 * cp[j];
+    }
+    PB_CUDA_OK(cudaMalloc((void**)&ctx->d_coef, coef.size() * sizeof(double)));
+    PB_CUDA_OK(cudaMemcpy(ctx->d_coef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice));
+    Op& op = ctx->op;
+    op.ar_m = ctx->d_coef;
+    op.ar_p = op.ar_m + nr;
+    op.ir2 = op.ar_p + nr;
+    op.dr = op.ir2 + nr;
+    op.at_m = op.dr + nr;
+    op.at_p = op.at_m + nt;
+    op.cp = op.at_p + nt;
+    op.dt = op.cp + nt;
+    // tables for the multipole kernels: rc, sin th, cos th, cos ph, sin ph, and the exact cell-volume factors
+    std::vector<double> tab(2 * nr + 3 * nt + 3 * np);
+    double* b = tab.data();
+    for (int i = 0; i < nr; ++i) b[i] = rc[i];
+    for (int j = 0; j < nt; ++j) {
+        b[nr + j] = std::sin(tc[j]);
+        b[nr + nt + j] = std::cos(tc[j]);
+    }
+    for (int k = 0; k < np; ++k) {
+        b[nr + 2 * nt + k] = std::cos(pc[k]);
+        b[nr + 2 * nt + np + k] = std::sin(pc[k]);
+    }
+    double* vr = b + nr + 2 * nt + 2 * np;
+    double* vt = vr + nr;
+    double* vp = vt + nt;
+    for (int i = 0; i < nr; ++i) vr[i] = (re[i + 1] * re[i + 1] * re[i + 1] - re[i] * re[i] * re[i]) / 3.0;
+    for (int j = 0; j < nt; ++j) vt[j] = std::cos(te[j]) - std::cos(te[j + 1]);
+    for (int k = 0; k < np; ++k) vp[k] = pe[k + 1] - pe[k];
+    PB_CUDA_OK(cudaMalloc((void**)&ctx->d_ctr, tab.size() * sizeof(double)));
+    PB_CUDA_OK(cudaMemcpy(ctx->d_ctr, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    return POISSON_OK;
+}
+
+extern "C" {
+
+const char* poisson_last_error(poisson_t h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int poisson_destroy(poisson_t ctx) {
+    if (!ctx) return POISSON_INVALID_ARG;
+    cudaStreamSynchronize(ctx->stream);
+    free_levels(ctx);
+    for (double* v : ctx->vec) cudaFree(v);
+    for (int f = 0; f < 6; ++f) cudaFree(ctx->d_ghost[f]);
+    cudaFree(ctx->d_coef);
+    cudaFree(ctx->d_ctr);
+    cudaFree(ctx->red.partials);
+    cudaFree(ctx->red.counter);
+    cudaFree(ctx->d_ctl);
+    cudaFreeHost(ctx->h_ctl);
+    cudaFree(ctx->d_hist);
+    cudaFree(ctx->d_scal);
+    cudaFreeHost(ctx->h_scal);
+    cudaFree(ctx->d_stage[0]);
+    cudaFree(ctx->d_stage[1]);
+    delete ctx;
+    return POISSON_OK;
+}
+
+int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], const double origin[3],
+                   const double* const edges[3], int coord_system, int stencil_order, const int bc[6],
+                   void* cuda_stream) {
+    if (!out || !shape || !bc) return fail(nullptr, POISSON_INVALID_ARG, "null argument");
+    *out = nullptr;
+    if (coord_system != POISSON_CARTESIAN && coord_system != POISSON_SPHERICAL)
+        return fail(nullptr, POISSON_INVALID_ARG, "coord_system must be POISSON_CARTESIAN or POISSON_SPHERICAL");
+    if (stencil_order != 2 && stencil_order != 6)
+        return fail(nullptr, POISSON_INVALID_ARG, "stencil_order must be 2 or 6");
+    if (coord_system == POISSON_SPHERICAL && stencil_order != 2)
+        return fail(nullptr, POISSON_UNSUPPORTED, "the spherical operator is 2nd order (7-point)");
+    const int R = stencil_order == 6 ? 3 : 1;
+    for (int a = 0; a < 3; ++a) {
+        if (shape[a] < 1 || shape[a] > (1 << 14)) return fail(nullptr, POISSON_INVALID_ARG, "shape out of range");
+        if ((bc[2 * a] == POISSON_BC_PERIODIC) != (bc[2 * a + 1] == POISSON_BC_PERIODIC))
+            return fail(nullptr, POISSON_INVALID_ARG, "periodic faces come in pairs");
+        if (bc[2 * a] == POISSON_BC_PERIODIC && shape[a] < R)
+            return fail(nullptr, POISSON_INVALID_ARG, "periodic axis shorter than the stencil radius");
+        for (int s = 0; s < 2; ++s)
+            if (bc[2 * a + s] < 0 || bc[2 * a + s] > 3) return fail(nullptr, POISSON_INVALID_ARG, "bad boundary type");
+    }
+    if (coord_system == POISSON_CARTESIAN) {
+        if (!spacing || !origin) return fail(nullptr, POISSON_INVALID_ARG, "spacing/origin required");
+        for (int a = 0; a < 3; ++a)
+            if (!(spacing[a] > 0)) return fail(nullptr, POISSON_INVALID_ARG, "spacing must be positive");
+        for (int f = 0; f < 6; ++f)
+            if (bc[f] == POISSON_BC_AXIS) return fail(nullptr, POISSON_INVALID_ARG, "BC_AXIS is spherical-only");
+        if (stencil_order == 6)
+            for (int f = 0; f < 6; ++f)
+                if (bc[f] == POISSON_BC_NEUMANN0)
+                    return fail(nullptr, POISSON_UNSUPPORTED, "Neumann faces need the 2nd-order stencil");
+    } else {
+        if (!edges || !edges[0] || !edges[1] || !edges[2])
+            return fail(nullptr, POISSON_INVALID_ARG, "spherical grids need edges[3]");
+    }
+    poisson_ctx* ctx = new poisson_ctx;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    Op& op = ctx->op;
+    std::memset(&op, 0, sizeof(op));
+    ctx->npts = 1;
+    for (int a = 0; a < 3; ++a) {
+        op.n[a] = shape[a];
+        ctx->npts *= (size_t)shape[a];
+        ctx->h[a] = spacing ? spacing[a] : 1.0;
+        ctx->origin[a] = origin ? origin[a] : 0.0;
+        op.c[a] = 1.0 / (ctx->h[a] * ctx->h[a]);
+    }
+    op.coord = coord_system;
+    op.order = stencil_order;
+    op.R = R;
+    for (int f = 0; f < 6; ++f) op.bc[f] = bc[f];
+    ctx->kind = coord_system == POISSON_SPHERICAL ? KIND_SPH : (stencil_order == 6 ? KIND_CART6 : KIND_CART2);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) {
+        int rc = fail_cuda(nullptr, e, "cudaGetDevice", __FILE__, __LINE__);
+        delete ctx;
+        return rc;
+    }
+#define CREATE_OK(call)                                                            \
+    do {                                                                           \
+        cudaError_t e2 = (call);                                                   \
+        if (e2 != cudaSuccess) {                                                   \
+            int rc2 = fail_cuda(nullptr, e2, #call, __FILE__, __LINE__);           \
+            poisson_destroy(ctx);                                                  \
+            return rc2;                                                            \
+        }                                                                          \
+    } while (0)
+    for (int f = 0; f < 6; ++f) {
+        const int a = f / 2, a1 = (a == 0) ? 1 : 0, a2 = (a == 2) ? 1 : 2;
+        ctx->face_len[f] = (long)R * shape[a1] * shape[a2];
+        if (bc[f] == POISSON_BC_DIRICHLET_GHOST) {
+            CREATE_OK(cudaMalloc((void**)&ctx->d_ghost[f], ctx->face_len[f] * sizeof(double)));
+            CREATE_OK(cudaMemset(ctx->d_ghost[f], 0, ctx->face_len[f] * sizeof(double)));
+            op.ghost[f] = ctx->d_ghost[f];
+        }
+    }
+    CREATE_OK(cudaMalloc((void**)&ctx->red.partials, (size_t)kMaxRedBlocks * kRedSlots * sizeof(double)));
+    CREATE_OK(cudaMalloc((void**)&ctx->red.counter, sizeof(unsigned int)));
+    CREATE_OK(cudaMemset(ctx->red.counter, 0, sizeof(unsigned int)));
+    CREATE_OK(cudaMalloc((void**)&ctx->d_ctl, sizeof(KrylovCtl)));
+    CREATE_OK(cudaMemset(ctx->d_ctl, 0, sizeof(KrylovCtl)));
+    CREATE_OK(cudaMallocHost((void**)&ctx->h_ctl, sizeof(KrylovCtl)));
+    CREATE_OK(cudaMalloc((void**)&ctx->d_scal, 256 * sizeof(double)));
+    CREATE_OK(cudaMemset(ctx->d_scal, 0, 256 * sizeof(double)));
+    CREATE_OK(cudaMallocHost((void**)&ctx->h_scal, 256 * sizeof(double)));
+    if (coord_system == POISSON_SPHERICAL) {
+        for (int a = 0; a < 3; ++a) ctx->edges[a].assign(edges[a], edges[a] + shape[a] + 1);
+        int rc = setup_spherical(ctx);
+        if (rc != POISSON_OK) {
+            g_create_error = ctx->err;
+            poisson_destroy(ctx);
+            return rc;
+        }
+    }
+    *out = ctx;
+    return POISSON_OK;
+}
+
+int poisson_set_option(poisson_t ctx, int option, int value) {
+    if (!ctx) return POISSON_INVALID_ARG;
+    switch (option) {
+        case POISSON_OPT_KERNEL_PATH:
+            if (value < 0 || value > 2) return fail(ctx, POISSON_INVALID_ARG, "kernel path must be 0, 1 or 2");
+            ctx->opt_path = value;
+            return POISSON_OK;
+        case POISSON_OPT_RESTRICTION:
+            if (value < 0 || value > 1) return fail(ctx, POISSON_INVALID_ARG, "restriction must be 0 or 1");
+            ctx->opt_restriction = value;
+            return POISSON_OK;
+        case POISSON_OPT_POLL_INTERVAL:
+            if (value < 1) return fail(ctx, POISSON_INVALID_ARG, "poll interval must be >= 1");
+            ctx->opt_poll = value;
+            return POISSON_OK;
+        case POISSON_OPT_JACOBI:
+            ctx->opt_jacobi = value ? 1 : 0;
+            return POISSON_OK;
+        case POISSON_OPT_RECORD_HISTORY:
+            ctx->opt_history = value ? 1 : 0;
+            return POISSON_OK;
+    }
+    return fail(ctx, POISSON_INVALID_ARG, "unknown option");
+}
+
+long poisson_face_len(poisson_t ctx, int face) { return (ctx && face >= 0 && face < 6) ? ctx->face_len[face] : -1; }
+long poisson_kernel_launches(poisson_t ctx) { return ctx ? ctx->launches : -1; }
+
+int poisson_set_ghost_faces(poisson_t ctx, const double* const d_faces[6]) {
+    if (!ctx || !d_faces) return POISSON_INVALID_ARG;
+    for (int f = 0; f < 6; ++f) {
+        if (!d_faces[f]) continue;
+        if (!ctx->d_ghost[f]) return fail(ctx, POISSON_INVALID_ARG, "ghost values given for a non-Dirichlet face");
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->d_ghost[f], d_faces[f], ctx->face_len[f] * sizeof(double),
+                                   cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    ctx->ghost_nonzero = true;
+    return POISSON_OK;
+}
+
+int poisson_get_ghost_face(poisson_t ctx, int face, double* d_out) {
+    if (!ctx || face < 0 || face > 5 || !d_out) return POISSON_INVALID_ARG;
+    if (!ctx->d_ghost[face]) return fail(ctx, POISSON_INVALID_ARG, "not a Dirichlet face");
+    PB_CUDA_OK(cudaMemcpyAsync(d_out, ctx->d_ghost[face], ctx->face_len[face] * sizeof(double),
+                               cudaMemcpyDeviceToDevice, ctx->stream));
+    return POISSON_OK;
+}
+
+int poisson_apply_laplacian(poisson_t ctx, const double* d_phi, double* d_out) {
+    if (!ctx || !d_phi || !d_out || d_phi == d_out) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    return launch_apply(ctx, ctx->op, ctx->kind, d_phi, nullptr, d_out, 0, true, false);
+}
+
+static int residual_norm_sync(poisson_ctx* ctx, const double* d_phi, const double* d_rhs, double* h_norm) {
+    int rc = launch_apply(ctx, ctx->op, ctx->kind, d_phi, d_rhs, nullptr, 1, true, true);
+    if (rc != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->h_scal, ctx->d_scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    *h_norm = std::sqrt(ctx->h_scal[0]);
+    return POISSON_OK;
+}
+
+int poisson_residual_norm(poisson_t ctx, const double* d_phi, const double* d_rhs, double* h_norm) {
+    if (!ctx || !d_phi || !d_rhs || !h_norm) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    return residual_norm_sync(ctx, d_phi, d_rhs, h_norm);
+}
+
+int poisson_rbsor_sweep(poisson_t ctx, double* d_phi, const double* d_rhs, double omega, int nsweeps,
+                        double* h_resnorm) {
+    if (!ctx || !d_phi || !d_rhs || nsweeps < 0) return fail(ctx, POISSON_INVALID_ARG, "bad arguments");
+    if (!(omega > 0.0 && omega < 2.0)) return fail(ctx, POISSON_INVALID_ARG, "omega must lie in (0,2) (PAPER.md:63)");
+    int rc = launch_rbsor(ctx, ctx->op, ctx->kind, d_phi, d_rhs, omega, nsweeps, true);
+    if (rc != POISSON_OK) return rc;
+    if (h_resnorm) return residual_norm_sync(ctx, d_phi, d_rhs, h_resnorm);
+    return POISSON_OK;
+}
+
+// ---- Krylov drivers ---------------------------------------------------------------------------------------------------
+static int krylov_setup(poisson_ctx* ctx, double rtol, int max_iter, int fixed_iters, bool project) {
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    KrylovCtl* c = ctx->h_ctl;
+    std::memset(c, 0, sizeof(*c));
+    c->tol2 = rtol * rtol;
+    c->fixed = fixed_iters > 0 ? 1 : 0;
+    c->max_it = nit;
+    c->project = project ? 1 : 0;
+    c->record = ctx->opt_history;
+    c->npoints = (double)ctx->npts;
+    if (ctx->opt_history) {
+        if (ctx->hist_cap < nit + 1) {
+            cudaFree(ctx->d_hist);
+            ctx->d_hist = nullptr;
+            PB_CUDA_OK(cudaMalloc((void**)&ctx->d_hist, (size_t)(nit + 1) * sizeof(double)));
+            ctx->hist_cap = nit + 1;
+        }
+        PB_CUDA_OK(cudaMemsetAsync(ctx->d_hist, 0, (size_t)(nit + 1) * sizeof(double), ctx->stream));
+    }
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_ctl, c, sizeof(*c), cudaMemcpyHostToDevice, ctx->stream));
+    return POISSON_OK;
+}
+
+static int read_ctl(poisson_ctx* ctx) {
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->h_ctl, ctx->d_ctl, sizeof(KrylovCtl), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    return POISSON_OK;
+}
+
+static bool all_periodic(const poisson_ctx* ctx) {
+    for (int f = 0; f < 6; ++f)
+        if (ctx->op.bc[f] != POISSON_BC_PERIODIC) return false;
+    return ctx->op.coord == POISSON_CARTESIAN;
+}
+
+int poisson_cg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,
+                     int* iters, double* relres) {
+    if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (fixed_iters <= 0 && (max_iter < 1 || !(rtol > 0))) return fail(ctx, POISSON_INVALID_ARG, "bad rtol/max_iter");
+    if (ctx->kind == KIND_SPH)
+        return fail(ctx, POISSON_UNSUPPORTED, "CG needs a symmetric operator; use BiCGSTAB on spherical grids");
+    const bool project = all_periodic(ctx);
+    double *r = scratch(ctx, 0), *P[2] = {scratch(ctx, 1), scratch(ctx, 2)}, *q = scratch(ctx, 3);
+    if (!r || !P[0] || !P[1] || !q) return POISSON_OUT_OF_MEMORY;
+    int rc = krylov_setup(ctx, rtol, max_iter, fixed_iters, project);
+    if (rc != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaMemsetAsync(P[0], 0, ctx->npts * sizeof(double), ctx->stream));
+    PB_CUDA_OK(cudaMemsetAsync(P[1], 0, ctx->npts * sizeof(double), ctx->stream));
+    rc = launch_krylov_init(ctx, d_phi, d_rhs, r, false, nullptr);
+    if (rc != POISSON_OK) return rc;
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    for (int j = 0; j < nit;) {
+        const int chunk = std::min(ctx->opt_poll, nit - j);
+        for (int c = 0; c < chunk; ++c, ++j) {
+            launch_cg_passA(ctx, r, P[j & 1], P[(j + 1) & 1], q, d_phi);
+            launch_cg_passB(ctx, r, q);
+        }
+        PB_CUDA_OK(cudaGetLastError());
+        if (fixed_iters <= 0) {
+            rc = read_ctl(ctx);
+            if (rc != POISSON_OK) return rc;
+            if (ctx->h_ctl->done) break;
+        }
+    }
+    rc = read_ctl(ctx);
+    if (rc != POISSON_OK) return rc;
+    const KrylovCtl c = *ctx->h_ctl;
+    rc = launch_cg_final(ctx, d_phi, P[c.it & 1]);  // the x-update of the last iteration is still pending
+    if (rc != POISSON_OK) return rc;
+    if (project) {
+        rc = launch_sub_mean(ctx, d_phi);
+        if (rc != POISSON_OK) return rc;
+    }
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    ctx->hist_len = c.it + 1;
+    if (iters) *iters = c.it;
+    if (relres) *relres = c.rr0 > 0 ? std::sqrt(c.rr / c.rr0) : 0.0;
+    if (c.status == POISSON_NOT_CONVERGED) ctx->err = "CG: residual threshold not reached within max_iter iterations";
+    return c.status;
+}
+
+int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter,
+                           int fixed_iters, int* iters, double* relres) {
+    if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (fixed_iters <= 0 && (max_iter < 1 || !(rtol > 0))) return fail(ctx, POISSON_INVALID_ARG, "bad rtol/max_iter");
+    double *r = scratch(ctx, 0), *r0 = scratch(ctx, 1), *P[2] = {scratch(ctx, 2), scratch(ctx, 3)},
+           *V[2] = {scratch(ctx, 4), scratch(ctx, 5)}, *s = scratch(ctx, 6), *t = scratch(ctx, 7);
+    if (!r || !r0 || !P[0] || !P[1] || !V[0] || !V[1] || !s || !t) return POISSON_OUT_OF_MEMORY;
+    int rc = krylov_setup(ctx, rtol, max_iter, fixed_iters, false);
+    if (rc != POISSON_OK) return rc;
+    for (double* z : {P[0], P[1], V[0], V[1]}) PB_CUDA_OK(cudaMemsetAsync(z, 0, ctx->npts * sizeof(double), ctx->stream));
+    rc = launch_krylov_init(ctx, d_phi, d_rhs, r, true, r0);
+    if (rc != POISSON_OK) return rc;
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    for (int j = 0; j < nit;) {
+        const int chunk = std::min(ctx->opt_poll, nit - j);
+        for (int c = 0; c < chunk; ++c, ++j) {
+            const int o = j & 1, n = (j + 1) & 1;
+            launch_bicg_pass1(ctx, r, P[o], V[o], r0, P[n], V[n]);
+            launch_bicg_pass2(ctx, r, V[n], s, t);
+            launch_bicg_pass3(ctx, d_phi, P[n], s, t, r0, r);
+        }
+        PB_CUDA_OK(cudaGetLastError());
+        if (fixed_iters <= 0) {
+            rc = read_ctl(ctx);
+            if (rc != POISSON_OK) return rc;
+            if (ctx->h_ctl->done) break;
+        }
+    }
+    rc = read_ctl(ctx);
+    if (rc != POISSON_OK) return rc;
+    const KrylovCtl c = *ctx->h_ctl;
+    ctx->hist_len = c.it + 1;
+    if (iters) *iters = c.it;
+    if (relres) *relres = c.rr0 > 0 ? std::sqrt(c.rr / c.rr0) : 0.0;
+    if (c.status == POISSON_NOT_CONVERGED) ctx->err = "BiCGSTAB: residual threshold not reached within max_iter";
+    if (c.status == POISSON_BREAKDOWN) ctx->err = "BiCGSTAB: breakdown (rho, omega or r0.v vanished or is not finite)";
+    return c.status;
+}
+
+int poisson_get_history(poisson_t ctx, double* h_out, int n) {
+    if (!ctx || !h_out || n < 0) return POISSON_INVALID_ARG;
+    if (!ctx->d_hist || n > ctx->hist_cap) return fail(ctx, POISSON_INVALID_ARG, "no history recorded / n too large");
+    PB_CUDA_OK(cudaMemcpyAsync(h_out, ctx->d_hist, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    return POISSON_OK;
+}
+
+// ---- multigrid --------------------------------------------------------------------------------------------------------
+static int build_levels(poisson_ctx* ctx, int coarsest_n, bool mixed) {
+    if (ctx->mg_coarsest_n != coarsest_n) {
+        free_levels(ctx);
+        MgLevel L0;
+        L0.op = ctx->op;
+        L0.npts = ctx->npts;
+        ctx->levels.push_back(L0);
+        double hl[3] = {ctx->h[0], ctx->h[1], ctx->h[2]};
+        int lev = 0;
+        while (ctx->levels.back().op.n[0] > coarsest_n && ctx->levels.back().op.n[0] % 2 == 0 &&
+               ctx->levels.back().op.n[1] % 2 == 0 && ctx->levels.back().op.n[2] % 2 == 0) {
+            ++lev;
+            MgLevel L;
+            L.op = ctx->levels.back().op;
+            L.npts = 1;
+            for (int a = 0; a < 3; ++a) {
+                L.op.n[a] /= 2;
+                hl[a] *= 2.0;
+                L.op.c[a] = 1.0 / (hl[a] * hl[a]);
+                L.npts *= (size_t)L.op.n[a];
+            }
+            const double s = std::ldexp(1.0, lev);
+            L.op.gamma = (s - 1.0) / (s + 1.0);  // ghost closure of DESIGN.md reading C7
+            for (int f = 0; f < 6; ++f) L.op.ghost[f] = nullptr;
+            ctx->levels.push_back(L);
+        }
+        ctx->mg_coarsest_n = coarsest_n;
+    }
+    for (size_t l = 0; l < ctx->levels.size(); ++l) {
+        MgLevel& L = ctx->levels[l];
+        const size_t b64 = L.npts * sizeof(double), b32 = L.npts * sizeof(float);
+        if (!mixed) {
+            if (l > 0 && !L.phi) PB_CUDA_OK(cudaMalloc((void**)&L.phi, b64));
+            if (l > 0 && !L.rhs) PB_CUDA_OK(cudaMalloc((void**)&L.rhs, b64));
+            if (!L.res) PB_CUDA_OK(cudaMalloc((void**)&L.res, b64));
+        } else {
+            if (!L.phi32) PB_CUDA_OK(cudaMalloc((void**)&L.phi32, b32));
+            if (!L.rhs32) PB_CUDA_OK(cudaMalloc((void**)&L.rhs32, b32));
+            if (!L.res32) PB_CUDA_OK(cudaMalloc((void**)&L.res32, b32));
+        }
+    }
+    return POISSON_OK;
+}
+
+static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, bool ug, int nu1, int nu2, int csweeps) {
+    MgLevel& L = ctx->levels[l];
+    int rc;
+    if (l + 1 == ctx->levels.size()) {
+        const double om = 2.0 / (1.0 + std::sin(M_PI / (L.op.n[0] + 1)));  // Eq. 3-4 for n unknowns per axis
+        rc = ug ? POISSON_UNSUPPORTED : launch_coarse_solve(ctx, L.op, phi, rhs, om, csweeps);
+        if (rc == POISSON_UNSUPPORTED) rc = launch_rbsor(ctx, L.op, KIND_CART2, phi, rhs, om, csweeps, ug);
+        return rc;
+    }
+    MgLevel& C = ctx->levels[l + 1];
+    if ((rc = launch_rbsor(ctx, L.op, KIND_CART2, phi, rhs, 1.0, nu1, ug)) != POISSON_OK) return rc;
+    if ((rc = launch_apply(ctx, L.op, KIND_CART2, phi, rhs, L.res, 1, ug, false)) != POISSON_OK) return rc;
+    if ((rc = launch_restrict(ctx, L.op, C.op, L.res, C.rhs, ctx->opt_restriction)) != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaMemsetAsync(C.phi, 0, C.npts * sizeof(double), ctx->stream));
+    if ((rc = cycle64(ctx, l + 1, C.phi, C.rhs, false, nu1, nu2, csweeps)) != POISSON_OK) return rc;
+    if ((rc = launch_prolong_add(ctx, L.op, C.op, C.phi, phi)) != POISSON_OK) return rc;
+    return launch_rbsor(ctx, L.op, KIND_CART2, phi, rhs, 1.0, nu2, ug);
+}
+
+static int cycle32(poisson_ctx* ctx, size_t l, int nu1, int nu2, int csweeps) {
+    MgLevel& L = ctx->levels[l];
+    int rc;
+    if (l + 1 == ctx->levels.size()) {
+        const float om = (float)(2.0 / (1.0 + std::sin(M_PI / (L.op.n[0] + 1))));
+        rc = launch_coarse_solve32(ctx, L.op, L.phi32, L.rhs32, om, csweeps);
+        if (rc == POISSON_UNSUPPORTED) rc = launch_rbsor32(ctx, L.op, L.phi32, L.rhs32, om, csweeps);
+        return rc;
+    }
+    MgLevel& C = ctx->levels[l + 1];
+    if ((rc = launch_rbsor32(ctx, L.op, L.phi32, L.rhs32, 1.0f, nu1)) != POISSON_OK) return rc;
+    if ((rc = launch_apply32(ctx, L.op, L.phi32, L.rhs32, L.res32, 1)) != POISSON_OK) return rc;
+    if ((rc = launch_restrict32(ctx, L.op, C.op, L.res32, C.rhs32, ctx->opt_restriction)) != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaMemsetAsync(C.phi32, 0, C.npts * sizeof(float), ctx->stream));
+    if ((rc = cycle32(ctx, l + 1, nu1, nu2, csweeps)) != POISSON_OK) return rc;
+    if ((rc = launch_prolong_add32(ctx, L.op, C.op, C.phi32, L.phi32)) != POISSON_OK) return rc;
+    return launch_rbsor32(ctx, L.op, L.phi32, L.rhs32, 1.0f, nu2);
+}
+
+int poisson_mg_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
+                      int coarsest_sweeps, int precision, int ncycles, double* h_resnorms) {
+    if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (nu1 < 0 || nu2 < 0 || coarsest_n < 1 || coarsest_sweeps < 0 || ncycles < 0 ||
+        (precision != POISSON_F64 && precision != POISSON_MIXED))
+        return fail(ctx, POISSON_INVALID_ARG, "bad V-cycle parameters");
+    if (ctx->kind != KIND_CART2) return fail(ctx, POISSON_UNSUPPORTED, "multigrid: Cartesian 7-point operator only");
+    for (int f = 0; f < 6; ++f)
+        if (ctx->op.bc[f] != POISSON_BC_DIRICHLET_GHOST)
+            return fail(ctx, POISSON_UNSUPPORTED, "multigrid: Dirichlet (ghost) faces only");
+    int rc = build_levels(ctx, coarsest_n, precision == POISSON_MIXED);
+    if (rc != POISSON_OK) return rc;
+    // the last-block reductions write squared norms to d_scal[16 + c]; one copy at the end, no per-cycle sync
+    auto record_norm = [&](int slot) -> int {
+        if (!h_resnorms) return POISSON_OK;
+        int r2 = launch_apply(ctx, ctx->op, ctx->kind, d_phi, d_rhs, nullptr, 1, true, true);
+        if (r2 != POISSON_OK) return r2;
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->d_scal + 16 + slot, ctx->d_scal, sizeof(double), cudaMemcpyDeviceToDevice,
+                                   ctx->stream));
+        return POISSON_OK;
+    };
+    if (ncycles + 1 > 200) return fail(ctx, POISSON_INVALID_ARG, "ncycles too large");
+    if ((rc = record_norm(0)) != POISSON_OK) return rc;
+    for (int c = 0; c < ncycles; ++c) {
+        if (precision == POISSON_F64) {
+            rc = cycle64(ctx, 0, d_phi, d_rhs, true, nu1, nu2, coarsest_sweeps);
+        } else {
+            MgLevel& L0 = ctx->levels[0];
+            rc = launch_residual_to32(ctx, ctx->op, d_phi, d_rhs, L0.rhs32, true);
+            if (rc != POISSON_OK) return rc;
+            PB_CUDA_OK(cudaMemsetAsync(L0.phi32, 0, L0.npts * sizeof(float), ctx->stream));
+            rc = cycle32(ctx, 0, nu1, nu2, coarsest_sweeps);
+            if (rc != POISSON_OK) return rc;
+            rc = launch_add32to64(ctx, L0.npts, L0.phi32, d_phi);
+        }
+        if (rc != POISSON_OK) return rc;
+        if ((rc = record_norm(c + 1)) != POISSON_OK) return rc;
+    }
+    if (h_resnorms) {
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->h_scal, ctx->d_scal + 16, (ncycles + 1) * sizeof(double),
+                                   cudaMemcpyDeviceToHost, ctx->stream));
+        PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+        for (int c = 0; c <= ncycles; ++c) h_resnorms[c] = std::sqrt(ctx->h_scal[c]);
+    }
+    return POISSON_OK;
+}
+
+// ---- multipole boundary -------------------------------------------------------------------------------------------------
+int poisson_multipole_bc(poisson_t ctx, const double* d_rho, double G, int lmax, double* h_moments) {
+    if (!ctx || !d_rho) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
+    double* d_q = ctx->d_scal + 128;
+    int rc = launch_moments(ctx, d_rho, lmax, d_q);
+    if (rc != POISSON_OK) return rc;
+    rc = launch_ghost_eval(ctx, d_q, G, lmax);
+    if (rc != POISSON_OK) return rc;
+    ctx->ghost_nonzero = true;
+    if (h_moments) {
+        const int nq = (lmax + 1) * (lmax + 1);
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->h_scal + 128, d_q, nq * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+        PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+        std::memcpy(h_moments, ctx->h_scal + 128, nq * sizeof(double));
+    }
+    return POISSON_OK;
+}
+
+// ---- end-to-end with host buffers -----------------------------------------------------------------------------------------
+int poisson_cg_solve_host(poisson_t ctx, double* h_phi, const double* h_rhs, double rtol, int max_iter,
+                          int fixed_iters, int* iters, double* relres) {
+    if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    const size_t bytes = ctx->npts * sizeof(double);
+    for (int s = 0; s < 2; ++s)
+        if (!ctx->d_stage[s]) PB_CUDA_OK(cudaMalloc((void**)&ctx->d_stage[s], bytes));
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_stage[0], h_phi, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_stage[1], h_rhs, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    const int rc = poisson_cg_solve(ctx, ctx->d_stage[0], ctx->d_stage[1], rtol, max_iter, fixed_iters, iters, relres);
+    if (rc < 0) return rc;
+    PB_CUDA_OK(cudaMemcpyAsync(h_phi, ctx->d_stage[0], bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,145 @@
+// common.cuh — context, device-side operator descriptor and the single-pass grid reduction shared by all kernels.
+// CUDA path of the Poisson hot path (arxiv/paper_2605_03563).  Shares no code with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/poisson.h"
+
+namespace pb {
+
+constexpr int kMaxLmax = 8;
+constexpr int kRedSlots = 4;          // doubles per block in the partials buffer
+constexpr int kMaxRedBlocks = 1 << 16;
+
+// Operator descriptor, passed by value to kernels (lives in the constant bank).
+struct Op {
+    int n[3];
+    int coord, order, R;
+    int bc[6];
+    double c[3];   // 1/h^2 per axis (Cartesian)
+    double gamma;  // multigrid coarse-level ghost closure (0 on the user's grid)
+    // spherical 1-D coefficient arrays (device): ar_m, ar_p, ir2, dr (len n0); at_m, at_p, cp, dt (len n1)
+    const double* ar_m;
+    const double* ar_p;
+    const double* ir2;
+    const double* dr;
+    const double* at_m;
+    const double* at_p;
+    const double* cp;
+    const double* dt;
+    const double* ghost[6];  // device ghost-face arrays (nullptr on non-Dirichlet faces)
+};
+
+enum { KIND_CART2 = 0, KIND_CART6 = 1, KIND_SPH = 2 };
+
+// Device-resident scalars of the Krylov solvers: nothing crosses to the host inside an iteration.
+struct KrylovCtl {
+    double rr, rr0, pq, alpha, beta, mu, rho, omega, r0v, ts, tt, tol2;
+    double sum_x;
+    int it, done, status, fixed;
+    int max_it, project, record, pad;
+    double npoints;
+};
+
+struct RedBuf {
+    double* partials;       // kMaxRedBlocks * kRedSlots
+    unsigned int* counter;  // self-resetting (atomicInc wraps)
+};
+
+#define PB_CUDA_OK(call)                                                                      \
+    do {                                                                                      \
+        cudaError_t e__ = (call);                                                             \
+        if (e__ != cudaSuccess) return pb::fail_cuda(ctx, e__, #call, __FILE__, __LINE__);    \
+    } while (0)
+
+struct MgLevel {
+    Op op;
+    size_t npts = 0;
+    double *phi = nullptr, *rhs = nullptr, *res = nullptr;     // fp64 storage (levels >= 1; level 0 uses caller's)
+    float *phi32 = nullptr, *rhs32 = nullptr, *res32 = nullptr;  // fp32 storage (mixed path, all levels)
+};
+
+}  // namespace pb
+
+struct poisson_ctx {
+    pb::Op op;
+    int kind = 0;
+    cudaStream_t stream = nullptr;
+    size_t npts = 0;
+    double h[3] = {1, 1, 1}, origin[3] = {0, 0, 0};
+    std::vector<double> edges[3], ctr[3];
+    double r_ghost_out = 0;
+    double* d_coef = nullptr;       // spherical coefficient arrays, one allocation
+    double* d_ctr = nullptr;        // spherical centres + cos/sin tables for the multipole kernels
+    double* d_ghost[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    long face_len[6] = {0, 0, 0, 0, 0, 0};
+    bool ghost_nonzero = false;
+    // scratch vectors (lazily allocated)
+    std::vector<double*> vec;
+    pb::RedBuf red{nullptr, nullptr};
+    pb::KrylovCtl* d_ctl = nullptr;
+    pb::KrylovCtl* h_ctl = nullptr;  // pinned
+    double* d_hist = nullptr;
+    int hist_cap = 0, hist_len = 0;
+    double* d_scal = nullptr;        // small device scalar scratch (moments, norms)
+    double* h_scal = nullptr;        // pinned
+    std::vector<pb::MgLevel> levels;
+    int mg_coarsest_n = -1;
+    // options
+    int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
+    long launches = 0;
+    int num_sms = 148;
+    std::string err;
+    // pinned staging for the host-buffer entry points
+    double* d_stage[2] = {nullptr, nullptr};
+};
+
+namespace pb {
+
+int fail(poisson_ctx* ctx, int code, const std::string& msg);
+int fail_cuda(poisson_ctx* ctx, cudaError_t e, const char* what, const char* file, int line);
+double* scratch(poisson_ctx* ctx, int slot);  // lazily allocated npts-sized vector; nullptr on OOM
+
+// ---- launch wrappers (definitions in the k_*.cu files) --------------------------------------------------------------
+// out = L v (mode 0) or out = rhs - L v (mode 1).  red != 0: also reduce sum(out^2), sum(out) into d_scal[0..1].
+int launch_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out, int mode,
+                 bool use_ghost, bool reduce);
+int launch_apply32(poisson_ctx* ctx, const Op& op, const float* v, const float* rhs, float* out, int mode);
+// mixed path: out32 = (float)(rhs - L v) in fp64 arithmetic, sum(r^2) into d_scal[0]
+int launch_residual_to32(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, float* out32,
+                         bool use_ghost);
+int launch_rbsor(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, double omega, int nsweeps,
+                 bool use_ghost);
+int launch_rbsor32(poisson_ctx* ctx, const Op& op, float* phi, const float* rhs, float omega, int nsweeps);
+
+// Krylov passes
+int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, double* r, bool bicg, double* r0hat);
+int launch_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x);
+int launch_cg_passB(poisson_ctx* ctx, double* r, const double* q);
+int launch_cg_final(poisson_ctx* ctx, double* x, const double* p_last);
+int launch_sub_mean(poisson_ctx* ctx, double* x);
+int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, const double* v_old, const double* r0,
+                      double* p_new, double* v_new);
+int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t);
+int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double* s, const double* t,
+                      const double* r0, double* r);
+
+// Multigrid transfer
+int launch_restrict(poisson_ctx* ctx, const Op& fine, const Op& coarse, const double* r, double* fc, int restriction);
+int launch_restrict32(poisson_ctx* ctx, const Op& fine, const Op& coarse, const float* r, float* fc, int restriction);
+int launch_prolong_add(poisson_ctx* ctx, const Op& fine, const Op& coarse, const double* ec, double* phi);
+int launch_prolong_add32(poisson_ctx* ctx, const Op& fine, const Op& coarse, const float* ec, float* phi);
+int launch_add32to64(poisson_ctx* ctx, size_t n, const float* e, double* phi);
+int launch_coarse_solve(poisson_ctx* ctx, const Op& op, double* phi, const double* rhs, double omega, int nsweeps);
+int launch_coarse_solve32(poisson_ctx* ctx, const Op& op, float* phi, const float* rhs, float omega, int nsweeps);
+
+// Multipole
+int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q);
+int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, double G, int lmax);
+
+}  // namespace pb

@@ -1,0 +1,387 @@
+// k_krylov.cu — generic (direct global load) fused passes of CG and BiCGSTAB.  PAPER.md:95-105; Saad Alg. 6.18, 7.7.
+// Scalars (alpha, beta, omega, rho, ||r||^2, iteration counter, convergence flag) stay in device memory; the last
+// block of each fused reduction computes the next ones, so an iteration never crosses to the host.
+//   CG        pass A: x += alpha_prev p_old ; p = r + beta p_old ; q = L p ; sum p.q        -> alpha
+//             pass B: r -= alpha q ; sum r^2 (and sum r for the periodic null-space projection) -> beta, convergence
+//   BiCGSTAB  pass 1: p = r + beta (p - omega v) ; v = L D^-1 p ; sum r0^.v                  -> alpha
+//             pass 2: s = r - alpha v ; t = L D^-1 s ; sum t.s, t.t                           -> omega
+//             pass 3: x += alpha D^-1 p + omega D^-1 s ; r = s - omega t ; sum r.r, r0^.r     -> beta, convergence
+// Vectors whose stencil is taken in the pass that forms them (p, v, s) are recomputed in the halo from read-only
+// inputs and written to a different buffer (ping-pong), so no block reads what another block is writing.
+#include "stencil.cuh"
+
+namespace pb {
+
+constexpr int BX = 64, BY = 4;
+
+static inline int pick_kc(const Op& op, int sms) {
+    const long cols = (long)((op.n[0] + BX - 1) / BX) * ((op.n[1] + BY - 1) / BY);
+    int kc = op.n[2];
+    while (kc > 8 && cols * ((op.n[2] + kc - 1) / kc) < 8L * sms) kc = (kc + 1) / 2;
+    return kc;
+}
+static dim3 grid_for(const Op& op, int kc) {
+    return dim3((op.n[0] + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + kc - 1) / kc);
+}
+
+__device__ __forceinline__ void finish_iteration(KrylovCtl* c, double* hist, double rr_new) {
+    // shared tail of CG pass B and BiCGSTAB pass 3: count the iteration, record, test convergence
+    const int it = c->it + 1;
+    c->it = it;
+    if (c->record && hist) hist[it] = sqrt(rr_new / c->rr0);
+}
+
+// ---- initial residual -----------------------------------------------------------------------------------------------
+template <int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_krylov_init(Op op, const double* __restrict__ x, const double* __restrict__ rhs, double* __restrict__ r,
+                  double* __restrict__ r0hat, KrylovCtl* ctl, double* hist, int kc, RedBuf rb) {
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    double s2 = 0.0, s1 = 0.0;
+    if (i < op.n[0] && j < op.n[1])
+        for (int k = k0; k < k1; ++k) {
+            const size_t p = gidx(op, i, j, k);
+            const double o = rhs[p] - row_apply<double, KIND>(op, ArrLd<double>{x}, i, j, k, true);
+            r[p] = o;
+            if (r0hat) r0hat[p] = o;
+            s2 = fma(o, o, s2);
+            s1 += o;
+        }
+    double vals[2] = {s2, s1};
+    grid_reduce<2>(vals, rb, [=](const double* t) {
+        const double mu = ctl->project ? t[1] / ctl->npoints : 0.0;
+        const double rr = ctl->project ? fma(-ctl->npoints * mu, mu, t[0]) : t[0];
+        ctl->mu = mu;
+        ctl->rr = rr;
+        ctl->rr0 = rr;
+        ctl->rho = rr;
+        ctl->alpha = 0.0;
+        ctl->beta = 0.0;
+        ctl->omega = 0.0;
+        ctl->it = 0;
+        const int trivially_done = (!ctl->fixed && !(rr > 0.0)) ? 1 : 0;
+        ctl->done = trivially_done;
+        ctl->status = (ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED;
+        if (ctl->record && hist) hist[0] = 1.0;
+    });
+}
+
+// ---- CG ---------------------------------------------------------------------------------------------------------------
+struct PnewLd {  // p_new = (r - mu) + beta p_old, formed on the fly (also in the halo)
+    const double* r;
+    const double* p;
+    double beta, mu;
+    __device__ __forceinline__ double operator()(size_t q, int, int, int) const { return fma(beta, p[q], r[q] - mu); }
+};
+
+template <int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_cg_passA(Op op, const double* __restrict__ r, const double* __restrict__ p_old, double* __restrict__ p_new,
+               double* __restrict__ q, double* __restrict__ x, KrylovCtl* ctl, int kc, RedBuf rb) {
+    if (ctl->done) return;
+    const double beta = ctl->beta, mu = ctl->mu, alpha_prev = ctl->alpha;
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    const PnewLd ld{r, p_old, beta, mu};
+    double acc = 0.0;
+    if (i < op.n[0] && j < op.n[1])
+        for (int k = k0; k < k1; ++k) {
+            const size_t p = gidx(op, i, j, k);
+            const double pn = ld(p, i, j, k);
+            const double qv = row_apply<double, KIND>(op, ld, i, j, k, false);
+            x[p] = fma(alpha_prev, p_old[p], x[p]);  // deferred x-update of the previous iteration
+            p_new[p] = pn;
+            q[p] = qv;
+            acc = fma(pn, qv, acc);
+        }
+    double vals[1] = {acc};
+    grid_reduce<1>(vals, rb, [=](const double* t) {
+        ctl->pq = t[0];
+        ctl->alpha = ctl->rr / t[0];
+    });
+}
+
+__global__ void __launch_bounds__(256)
+    k_cg_passB(size_t n, double* __restrict__ r, const double* __restrict__ q, KrylovCtl* ctl, double* hist, RedBuf rb) {
+    if (ctl->done) return;
+    const double alpha = ctl->alpha;
+    double s2 = 0.0, s1 = 0.0;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (size_t)gridDim.x * blockDim.x) {
+        const double rn = fma(-alpha, q[p], r[p]);
+        r[p] = rn;
+        s2 = fma(rn, rn, s2);
+        s1 += rn;
+    }
+    double vals[2] = {s2, s1};
+    grid_reduce<2>(vals, rb, [=](const double* t) {
+        const double mu = ctl->project ? t[1] / ctl->npoints : 0.0;
+        const double rr_new = ctl->project ? fma(-ctl->npoints * mu, mu, t[0]) : t[0];
+        finish_iteration(ctl, hist, rr_new);
+        const bool conv = !ctl->fixed && sqrt(rr_new) <= sqrt(ctl->tol2) * sqrt(ctl->rr0);
+        if (conv) {
+            ctl->done = 1;
+            ctl->status = POISSON_OK;
+        } else if (ctl->it >= ctl->max_it) {
+            ctl->done = 1;
+        } else {
+            ctl->beta = rr_new / ctl->rr;
+        }
+        ctl->rr = rr_new;
+        ctl->mu = mu;
+    });
+}
+
+__global__ void __launch_bounds__(256) k_cg_final(size_t n, double* __restrict__ x, const double* __restrict__ p,
+                                                    const KrylovCtl* ctl) {
+    const double alpha = ctl->alpha;
+    if (ctl->it == 0) return;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x)
+        x[q] = fma(alpha, p[q], x[q]);
+}
+
+__global__ void __launch_bounds__(256) k_sum(size_t n, const double* __restrict__ x, KrylovCtl* ctl, RedBuf rb) {
+    double s = 0.0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) s += x[q];
+    double vals[1] = {s};
+    grid_reduce<1>(vals, rb, [=](const double* t) { ctl->sum_x = t[0]; });
+}
+__global__ void __launch_bounds__(256) k_sub_mean(size_t n, double* __restrict__ x, const KrylovCtl* ctl) {
+    const double mu = ctl->sum_x / ctl->npoints;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) x[q] -= mu;
+}
+
+// ---- BiCGSTAB ---------------------------------------------------------------------------------------------------------
+// D = diag(A) with A = L: entry -d (right Jacobi scaling p^ = D^-1 p), or 1 when scaling is off.
+template <int KIND>
+__device__ __forceinline__ double jac(const Op& op, int i, int j, int k, int jacobi) {
+    return jacobi ? -row_diag<double, KIND>(op, i, j, k) : 1.0;
+}
+
+template <int KIND>
+struct PhatLd {  // p_new = r + beta (p_old - omega v_old) ; p^ = p_new / D
+    const Op& op;
+    const double* r;
+    const double* p;
+    const double* v;
+    double beta, omega;
+    int jacobi;
+    __device__ __forceinline__ double pnew(size_t q) const { return fma(beta, fma(-omega, v[q], p[q]), r[q]); }
+    __device__ __forceinline__ double operator()(size_t q, int i, int j, int k) const {
+        return pnew(q) / jac<KIND>(op, i, j, k, jacobi);
+    }
+};
+
+template <int KIND>
+struct ShatLd {  // s = r - alpha v ; s^ = s / D
+    const Op& op;
+    const double* r;
+    const double* v;
+    double alpha;
+    int jacobi;
+    __device__ __forceinline__ double s(size_t q) const { return fma(-alpha, v[q], r[q]); }
+    __device__ __forceinline__ double operator()(size_t q, int i, int j, int k) const {
+        return s(q) / jac<KIND>(op, i, j, k, jacobi);
+    }
+};
+
+template <int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_bicg_pass1(Op op, const double* __restrict__ r, const double* __restrict__ p_old,
+                 const double* __restrict__ v_old, const double* __restrict__ r0, double* __restrict__ p_new,
+                 double* __restrict__ v_new, KrylovCtl* ctl, int jacobi, int kc, RedBuf rb) {
+    if (ctl->done) return;
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    const PhatLd<KIND> ld{op, r, p_old, v_old, ctl->beta, ctl->omega, jacobi};
+    double acc = 0.0;
+    if (i < op.n[0] && j < op.n[1])
+        for (int k = k0; k < k1; ++k) {
+            const size_t p = gidx(op, i, j, k);
+            const double vn = row_apply<double, KIND>(op, ld, i, j, k, false);
+            p_new[p] = ld.pnew(p);
+            v_new[p] = vn;
+            acc = fma(r0[p], vn, acc);
+        }
+    double vals[1] = {acc};
+    grid_reduce<1>(vals, rb, [=](const double* t) {
+        const double r0v = t[0];
+        ctl->r0v = r0v;
+        if (!(fabs(r0v) > 0.0) || !isfinite(r0v) || !(fabs(ctl->rho) > 0.0)) {
+            ctl->status = POISSON_BREAKDOWN;
+            ctl->done = 1;
+        } else {
+            ctl->alpha = ctl->rho / r0v;
+        }
+    });
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_bicg_pass2(Op op, const double* __restrict__ r, const double* __restrict__ v, double* __restrict__ s,
+                 double* __restrict__ t, KrylovCtl* ctl, int jacobi, int kc, RedBuf rb) {
+    if (ctl->done) return;
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    const ShatLd<KIND> ld{op, r, v, ctl->alpha, jacobi};
+    double a_ts = 0.0, a_tt = 0.0;
+    if (i < op.n[0] && j < op.n[1])
+        for (int k = k0; k < k1; ++k) {
+            const size_t p = gidx(op, i, j, k);
+            const double tv = row_apply<double, KIND>(op, ld, i, j, k, false);
+            const double sv = ld.s(p);
+            s[p] = sv;
+            t[p] = tv;
+            a_ts = fma(tv, sv, a_ts);
+            a_tt = fma(tv, tv, a_tt);
+        }
+    double vals[2] = {a_ts, a_tt};
+    grid_reduce<2>(vals, rb, [=](const double* tot) {
+        ctl->ts = tot[0];
+        ctl->tt = tot[1];
+        if (!(tot[1] > 0.0) || !isfinite(tot[1])) {
+            ctl->status = POISSON_BREAKDOWN;
+            ctl->done = 1;
+        } else {
+            ctl->omega = tot[0] / tot[1];
+        }
+    });
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_bicg_pass3(Op op, double* __restrict__ x, const double* __restrict__ p, const double* __restrict__ s,
+                 const double* __restrict__ t, const double* __restrict__ r0, double* __restrict__ r, KrylovCtl* ctl,
+                 double* hist, int jacobi, int kc, RedBuf rb) {
+    if (ctl->done) return;
+    const double alpha = ctl->alpha, omega = ctl->omega;
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    double a_rr = 0.0, a_r0r = 0.0;
+    if (i < op.n[0] && j < op.n[1])
+        for (int k = k0; k < k1; ++k) {
+            const size_t q = gidx(op, i, j, k);
+            const double dg = jac<KIND>(op, i, j, k, jacobi);
+            const double ph = p[q] / dg, sv = s[q], sh = sv / dg;
+            x[q] = fma(omega, sh, fma(alpha, ph, x[q]));
+            const double rn = fma(-omega, t[q], sv);
+            r[q] = rn;
+            a_rr = fma(rn, rn, a_rr);
+            a_r0r = fma(r0[q], rn, a_r0r);
+        }
+    double vals[2] = {a_rr, a_r0r};
+    grid_reduce<2>(vals, rb, [=](const double* tot) {
+        const double rr = tot[0];
+        finish_iteration(ctl, hist, rr);
+        ctl->rr = rr;
+        if (!isfinite(rr)) {
+            ctl->status = POISSON_BREAKDOWN;
+            ctl->done = 1;
+        } else if (!ctl->fixed && sqrt(rr) <= sqrt(ctl->tol2) * sqrt(ctl->rr0)) {
+            ctl->status = POISSON_OK;
+            ctl->done = 1;
+        } else if (!(fabs(ctl->omega) > 0.0)) {
+            ctl->status = POISSON_BREAKDOWN;
+            ctl->done = 1;
+        } else if (ctl->it >= ctl->max_it) {
+            ctl->done = 1;
+        } else {
+            const double rho_new = tot[1];
+            ctl->beta = (rho_new / ctl->rho) * (ctl->alpha / ctl->omega);
+            ctl->rho = rho_new;
+        }
+    });
+}
+
+// ---- launch wrappers --------------------------------------------------------------------------------------------------
+#define KIND_SWITCH(kind, CALL)                       \
+    switch (kind) {                                   \
+        case KIND_CART2: { constexpr int K = KIND_CART2; CALL; } break; \
+        case KIND_CART6: { constexpr int K = KIND_CART6; CALL; } break; \
+        default:         { constexpr int K = KIND_SPH;   CALL; } break; \
+    }
+
+static int stream_blocks(poisson_ctx* ctx, size_t n) {
+    size_t b = (n + 256 * 8 - 1) / (256 * 8);
+    size_t cap = (size_t)ctx->num_sms * 16;
+    if (b > cap) b = cap;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, double* r, bool bicg, double* r0hat) {
+    const Op& op = ctx->op;
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc), b(BX, BY);
+    KIND_SWITCH(ctx->kind, (k_krylov_init<K><<<g, b, 0, ctx->stream>>>(op, x, rhs, r, bicg ? r0hat : nullptr, ctx->d_ctl,
+                                                                         ctx->d_hist, kc, ctx->red)));
+    ctx->launches++;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int launch_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x) {
+    const Op& op = ctx->op;
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc), b(BX, BY);
+    KIND_SWITCH(ctx->kind,
+                (k_cg_passA<K><<<g, b, 0, ctx->stream>>>(op, r, p_old, p_new, q, x, ctx->d_ctl, kc, ctx->red)));
+    ctx->launches++;
+    return POISSON_OK;
+}
+
+int launch_cg_passB(poisson_ctx* ctx, double* r, const double* q) {
+    k_cg_passB<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, r, q, ctx->d_ctl, ctx->d_hist,
+                                                                       ctx->red);
+    ctx->launches++;
+    return POISSON_OK;
+}
+
+int launch_cg_final(poisson_ctx* ctx, double* x, const double* p_last) {
+    k_cg_final<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, p_last, ctx->d_ctl);
+    ctx->launches++;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int launch_sub_mean(poisson_ctx* ctx, double* x) {
+    k_sum<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, ctx->d_ctl, ctx->red);
+    k_sub_mean<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, ctx->d_ctl);
+    ctx->launches += 2;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, const double* v_old, const double* r0,
+                      double* p_new, double* v_new) {
+    const Op& op = ctx->op;
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc), b(BX, BY);
+    KIND_SWITCH(ctx->kind, (k_bicg_pass1<K><<<g, b, 0, ctx->stream>>>(op, r, p_old, v_old, r0, p_new, v_new, ctx->d_ctl,
+                                                                        ctx->opt_jacobi, kc, ctx->red)));
+    ctx->launches++;
+    return POISSON_OK;
+}
+
+int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t) {
+    const Op& op = ctx->op;
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc), b(BX, BY);
+    KIND_SWITCH(ctx->kind, (k_bicg_pass2<K><<<g, b, 0, ctx->stream>>>(op, r, v, s, t, ctx->d_ctl, ctx->opt_jacobi, kc,
+                                                                        ctx->red)));
+    ctx->launches++;
+    return POISSON_OK;
+}
+
+int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double* s, const double* t,
+                      const double* r0, double* r) {
+    const Op& op = ctx->op;
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc), b(BX, BY);
+    KIND_SWITCH(ctx->kind, (k_bicg_pass3<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl, ctx->d_hist,
+                                                                        ctx->opt_jacobi, kc, ctx->red)));
+    ctx->launches++;
+    return POISSON_OK;
+}
+
+}  // namespace pb

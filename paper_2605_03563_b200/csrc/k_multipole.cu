@@ -1,0 +1,268 @@
+// k_multipole.cu — multipole-expansion open boundary.  PAPER.md:213-222:
+//   q_lm = sum_cells rho r'^l S_lm dV          (Eq. 20, "numerically the integrals are expressed as sums over cells")
+//   Phi(x) = -G sum_lm q_lm S_lm(x) / r^(l+1)  (Eq. 19), S_lm = sqrt(4 pi/(2l+1)) Y_lm, real harmonics, cosine for
+//   m >= 0 and sine for m < 0.  Moment index l*l + l + m.
+// Evaluated with Cartesian solid-harmonic recurrences (no trigonometry, no pole singularity):
+//   A_m + i B_m = (x + i y)^m ;  Q_m^m = (2m-1)!! ;  Q_{m+1}^m = (2m+1) z Q_m^m ;
+//   (l-m) Q_l^m = (2l-1) z Q_{l-1}^m - (l+m-1) r^2 Q_{l-2}^m ;
+//   r^l S_l0 = Q_l^0 ;  r^l S_{l,m} = N_lm Q_l^m A_m ;  r^l S_{l,-m} = N_lm Q_l^m B_m ;  N_lm = sqrt(2 (l-m)!/(l+m)!).
+// One fused pass over rho accumulates all (lmax+1)^2 moments per thread in registers, then warp shuffles, a block
+// reduction and a last-block final sum (fixed order -> deterministic).  The pass is fp64-ALU bound at lmax = 8.
+#include "stencil.cuh"
+
+namespace pb {
+
+__constant__ double c_norm[(kMaxLmax + 1) * (kMaxLmax + 1)];  // N_lm at index l*l + l + m (m >= 0); 1 for m = 0
+static bool g_norm_ready = false;
+
+static void init_norm() {
+    if (g_norm_ready) return;
+    double h[(kMaxLmax + 1) * (kMaxLmax + 1)] = {0};
+    for (int l = 0; l <= kMaxLmax; ++l) {
+        h[l * l + l] = 1.0;
+        for (int m = 1; m <= l; ++m) {
+            long double ratio = 1;  // (l-m)!/(l+m)!
+            for (int q = l - m + 1; q <= l + m; ++q) ratio /= (long double)q;
+            h[l * l + l + m] = (double)sqrtl(2 * ratio);
+            h[l * l + l - m] = h[l * l + l + m];
+        }
+    }
+    cudaMemcpyToSymbol(c_norm, h, sizeof(h));
+    g_norm_ready = true;
+}
+
+struct MpGeom {
+    int sph;
+    int n[3];
+    double origin[3], h[3];
+    // spherical 1-D tables (device): centre radius, sin/cos theta, cos/sin phi, volume factors
+    const double *rc, *st, *ct, *cph, *sph_, *vr, *vt, *vp;
+    double r_ghost;
+};
+
+template <int L>
+__device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], double x, double y, double z, double w) {
+    const double r2 = fma(z, z, fma(y, y, x * x));
+    double A = 1.0, B = 0.0, dfact = 1.0;  // (x+iy)^m, (2m-1)!!
+#pragma unroll
+    for (int m = 0; m <= L; ++m) {
+        double qm2 = 0.0, qm1 = dfact;  // Q_{l-2}^m, Q_{l-1}^m while walking l = m..L
+        const double wa = w * A, wb = w * B;
+#pragma unroll
+        for (int l = m; l <= L; ++l) {
+            double ql;
+            if (l == m)
+                ql = dfact;
+            else if (l == m + 1)
+                ql = (2 * m + 1) * z * qm1;
+            else
+                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) * (1.0 / (l - m));
+            if (m == 0) {
+                acc[l * l + l] = fma(wa, ql, acc[l * l + l]);
+            } else {
+                const double nq = c_norm[l * l + l + m] * ql;
+                acc[l * l + l + m] = fma(wa, nq, acc[l * l + l + m]);
+                acc[l * l + l - m] = fma(wb, nq, acc[l * l + l - m]);
+            }
+            qm2 = qm1;
+            qm1 = ql;
+        }
+        const double An = x * A - y * B, Bn = fma(y, A, x * B);
+        A = An;
+        B = Bn;
+        dfact *= (2 * m + 1);
+    }
+}
+
+template <int L>
+__global__ void __launch_bounds__(256, 1)
+    k_moments(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
+              double* __restrict__ q_out) {
+    constexpr int NQ = (L + 1) * (L + 1);
+    double acc[NQ];
+#pragma unroll
+    for (int s = 0; s < NQ; ++s) acc[s] = 0.0;
+    const size_t n = (size_t)g.n[0] * g.n[1] * g.n[2];
+    const size_t plane = (size_t)g.n[0] * g.n[1];
+    const double dV = g.h[0] * g.h[1] * g.h[2];
+    // whole warps walk consecutive points; a warp whose 32 densities are all zero skips the arithmetic
+    for (size_t base = ((size_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31)); base < n;
+         base += (size_t)gridDim.x * blockDim.x) {
+        const size_t p = base + (threadIdx.x & 31);
+        const double d = p < n ? rho[p] : 0.0;
+        if (__all_sync(0xffffffffu, d == 0.0)) continue;
+        if (d == 0.0) continue;
+        const int k = (int)(p / plane), rem = (int)(p - (size_t)k * plane), j = rem / g.n[0], i = rem - j * g.n[0];
+        double x, y, z, w;
+        if (g.sph) {
+            const double r = g.rc[i], rs = r * g.st[j];
+            x = rs * g.cph[k];
+            y = rs * g.sph_[k];
+            z = r * g.ct[j];
+            w = d * (g.vr[i] * g.vt[j] * g.vp[k]);
+        } else {
+            x = fma((double)i, g.h[0], g.origin[0]);
+            y = fma((double)j, g.h[1], g.origin[1]);
+            z = fma((double)k, g.h[2], g.origin[2]);
+            w = d * dV;
+        }
+        accumulate<L>(acc, x, y, z, w);
+    }
+    // block reduction: warp shuffles, then shared memory across the 8 warps
+    __shared__ double sm[8][NQ];
+    __shared__ int is_last;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int s = 0; s < NQ; ++s) {
+        const double v = warp_sum(acc[s]);
+        if (lane == 0) sm[wid][s] = v;
+    }
+    __syncthreads();
+    for (int s = threadIdx.x; s < NQ; s += blockDim.x) {
+        double v = 0.0;
+        for (int ww = 0; ww < 8; ++ww) v += sm[ww][s];
+        partials[(size_t)blockIdx.x * NQ + s] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        is_last = (atomicInc(counter, gridDim.x - 1) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    for (int s = threadIdx.x; s < NQ; s += blockDim.x) {
+        double v = 0.0;
+        for (unsigned b = 0; b < gridDim.x; ++b) v += __ldcg(&partials[(size_t)b * NQ + s]);
+        q_out[s] = v;
+    }
+}
+
+// Phi at one exterior point from the moments.
+__device__ __forceinline__ double expansion(const double* __restrict__ q, int lmax, double G, double x, double y,
+                                            double z) {
+    const double r2 = fma(z, z, fma(y, y, x * x));
+    const double rinv = 1.0 / sqrt(r2), rinv2 = rinv * rinv;
+    double A = 1.0, B = 0.0, dfact = 1.0, acc = 0.0;
+    double pw_m = rinv;  // r^-(2m+1)
+    for (int m = 0; m <= lmax; ++m) {
+        double qm2 = 0.0, qm1 = dfact, pw = pw_m;  // pw = r^-(2l+1)
+        for (int l = m; l <= lmax; ++l) {
+            double ql;
+            if (l == m)
+                ql = dfact;
+            else if (l == m + 1)
+                ql = (2 * m + 1) * z * qm1;
+            else
+                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) / (double)(l - m);
+            if (m == 0)
+                acc = fma(q[l * l + l] * ql, pw, acc);
+            else {
+                const double nq = c_norm[l * l + l + m] * ql;
+                acc = fma((q[l * l + l + m] * A + q[l * l + l - m] * B) * nq, pw, acc);
+            }
+            qm2 = qm1;
+            qm1 = ql;
+            pw *= rinv2;
+        }
+        const double An = x * A - y * B, Bn = fma(y, A, x * B);
+        A = An;
+        B = Bn;
+        dfact *= (2 * m + 1);
+        pw_m *= rinv2;
+    }
+    return -G * acc;
+}
+
+__global__ void __launch_bounds__(256)
+    k_ghost_eval(MpGeom g, int face, int R, const double* __restrict__ q, double G, int lmax, double* __restrict__ out) {
+    const int a = face / 2, a1 = (a == 0) ? 1 : 0, a2 = (a == 2) ? 1 : 2;
+    const long len = (long)R * g.n[a1] * g.n[a2];
+    const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= len) return;
+    const int q1 = (int)(t % g.n[a1]), q2 = (int)((t / g.n[a1]) % g.n[a2]), layer = (int)(t / ((long)g.n[a1] * g.n[a2]));
+    double x, y, z;
+    if (g.sph) {
+        const double rs = g.r_ghost * g.st[q1];
+        x = rs * g.cph[q2];
+        y = rs * g.sph_[q2];
+        z = g.r_ghost * g.ct[q1];
+    } else {
+        int id[3];
+        id[a] = (face & 1) ? g.n[a] + layer : -1 - layer;
+        id[a1] = q1;
+        id[a2] = q2;
+        x = fma((double)id[0], g.h[0], g.origin[0]);
+        y = fma((double)id[1], g.h[1], g.origin[1]);
+        z = fma((double)id[2], g.h[2], g.origin[2]);
+    }
+    out[t] = expansion(q, lmax, G, x, y, z);
+}
+
+static MpGeom make_geom(poisson_ctx* ctx) {
+    MpGeom g{};
+    g.sph = ctx->op.coord == POISSON_SPHERICAL;
+    for (int a = 0; a < 3; ++a) {
+        g.n[a] = ctx->op.n[a];
+        g.origin[a] = ctx->origin[a];
+        g.h[a] = ctx->h[a];
+    }
+    if (g.sph) {
+        const int nr = g.n[0], nt = g.n[1], np = g.n[2];
+        const double* b = ctx->d_ctr;
+        g.rc = b;
+        g.st = b + nr;
+        g.ct = b + nr + nt;
+        g.cph = b + nr + 2 * nt;
+        g.sph_ = b + nr + 2 * nt + np;
+        g.vr = b + nr + 2 * nt + 2 * np;
+        g.vt = b + 2 * nr + 2 * nt + 2 * np;
+        g.vp = b + 2 * nr + 3 * nt + 2 * np;
+        g.r_ghost = ctx->r_ghost_out;
+    }
+    return g;
+}
+
+template <int L>
+static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, double* d_q, int blocks) {
+    k_moments<L><<<blocks, 256, 0, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+}
+
+int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
+    init_norm();
+    const MpGeom g = make_geom(ctx);
+    int blocks = ctx->num_sms * 2;
+    const size_t maxb = (ctx->npts + 255) / 256;
+    if ((size_t)blocks > maxb) blocks = (int)maxb;
+    switch (lmax) {
+        case 0: moments_launch<0>(ctx, g, rho, d_q, blocks); break;
+        case 1: moments_launch<1>(ctx, g, rho, d_q, blocks); break;
+        case 2: moments_launch<2>(ctx, g, rho, d_q, blocks); break;
+        case 3: moments_launch<3>(ctx, g, rho, d_q, blocks); break;
+        case 4: moments_launch<4>(ctx, g, rho, d_q, blocks); break;
+        case 5: moments_launch<5>(ctx, g, rho, d_q, blocks); break;
+        case 6: moments_launch<6>(ctx, g, rho, d_q, blocks); break;
+        case 7: moments_launch<7>(ctx, g, rho, d_q, blocks); break;
+        case 8: moments_launch<8>(ctx, g, rho, d_q, blocks); break;
+        default: return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
+    }
+    ctx->launches++;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, double G, int lmax) {
+    init_norm();
+    const MpGeom g = make_geom(ctx);
+    for (int f = 0; f < 6; ++f) {
+        if (ctx->op.bc[f] != POISSON_BC_DIRICHLET_GHOST || !ctx->d_ghost[f]) continue;
+        if (g.sph && f != 1) continue;  // only the outer radial shell carries Eq. 19
+        const long len = ctx->face_len[f];
+        k_ghost_eval<<<(int)((len + 255) / 256), 256, 0, ctx->stream>>>(g, f, ctx->op.R, d_q, G, lmax, ctx->d_ghost[f]);
+        ctx->launches++;
+    }
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+}  // namespace pb

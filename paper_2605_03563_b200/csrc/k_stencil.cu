@@ -1,0 +1,133 @@
+// k_stencil.cu — generic (any shape, direct global loads) stencil apply / residual and red-black SOR kernels.
+// Each thread owns a column (i,j) and marches a chunk of k planes, so x/y neighbours come from L1 and the previous
+// planes from L1/L2.  Used for small or odd-shaped grids (multigrid levels, 32^3) and as the always-available path;
+// large aligned grids take the plane-pipeline kernels of k_plane.cu.
+//   apply:   PAPER.md:43-49 (Eq. 1-2), 57        residual: PAPER.md:55        red-black SOR: PAPER.md:59-63
+#include "stencil.cuh"
+
+namespace pb {
+
+constexpr int BX = 64, BY = 4;
+
+static inline int pick_kc(const Op& op, int sms) {
+    // enough blocks to fill the machine a few times, few enough that the last-block reduction stays short
+    const long cols = (long)((op.n[0] + BX - 1) / BX) * ((op.n[1] + BY - 1) / BY);
+    int kc = op.n[2];
+    while (kc > 8 && cols * ((op.n[2] + kc - 1) / kc) < 8L * sms) kc = (kc + 1) / 2;
+    return kc;
+}
+
+// MODE 0: out = L v.  MODE 1: out = rhs - L v.  RED: sum(out^2), sum(out) -> scal[0], scal[1].
+template <typename T, int KIND, int MODE, bool RED>
+__global__ void __launch_bounds__(BX* BY)
+    k_apply(Op op, const T* __restrict__ v, const T* __restrict__ rhs, T* __restrict__ out, float* __restrict__ out32,
+            bool ug, int kc, RedBuf rb, double* scal) {
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    double s2 = 0.0, s1 = 0.0;
+    if (i < op.n[0] && j < op.n[1]) {
+        for (int k = k0; k < k1; ++k) {
+            const size_t p = gidx(op, i, j, k);
+            const T lv = row_apply<T, KIND>(op, ArrLd<T>{v}, i, j, k, ug);
+            const T o = MODE ? (rhs[p] - lv) : lv;
+            if (out) out[p] = o;
+            if (out32) out32[p] = (float)o;
+            if (RED) {
+                s2 = fma((double)o, (double)o, s2);
+                s1 += (double)o;
+            }
+        }
+    }
+    if (RED) {
+        double vals[2] = {s2, s1};
+        grid_reduce<2>(vals, rb, [=](const double* t) {
+            scal[0] = t[0];
+            scal[1] = t[1];
+        });
+    }
+}
+
+template <typename T, int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_rbsor_half(Op op, T* phi, const T* __restrict__ rhs, T omega, int colour, bool ug, int kc) {
+    const int ti = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    if (j >= op.n[1]) return;
+    for (int k = k0; k < k1; ++k) {
+        const int i = 2 * ti + ((j + k + colour) & 1);
+        if (i >= op.n[0]) continue;
+        const size_t p = gidx(op, i, j, k);
+        const T s = row_offsum<T, KIND>(op, ArrLd<T>{phi}, i, j, k, ug);
+        const T d = row_diag<T, KIND>(op, i, j, k);
+        const T gs = (s - rhs[p]) / d;
+        const T old = phi[p];
+        phi[p] = fma_(omega, gs - old, old);
+    }
+}
+
+static dim3 grid_for(const Op& op, int kc, bool half_x) {
+    const int nxe = half_x ? (op.n[0] + 1) / 2 : op.n[0];
+    return dim3((nxe + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + kc - 1) / kc);
+}
+
+template <typename T, int KIND>
+static int apply_dispatch(poisson_ctx* ctx, const Op& op, const T* v, const T* rhs, T* out, float* out32, int mode,
+                          bool ug, bool reduce) {
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc, false), b(BX, BY);
+    if ((size_t)g.x * g.y * g.z > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");
+    cudaStream_t s = ctx->stream;
+    if (mode == 0)
+        k_apply<T, KIND, 0, false><<<g, b, 0, s>>>(op, v, rhs, out, out32, ug, kc, ctx->red, ctx->d_scal);
+    else if (!reduce)
+        k_apply<T, KIND, 1, false><<<g, b, 0, s>>>(op, v, rhs, out, out32, ug, kc, ctx->red, ctx->d_scal);
+    else
+        k_apply<T, KIND, 1, true><<<g, b, 0, s>>>(op, v, rhs, out, out32, ug, kc, ctx->red, ctx->d_scal);
+    ctx->launches++;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int launch_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out, int mode,
+                 bool ug, bool reduce) {
+    switch (kind) {
+        case KIND_CART2: return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
+        case KIND_CART6: return apply_dispatch<double, KIND_CART6>(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
+        default: return apply_dispatch<double, KIND_SPH>(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
+    }
+}
+
+int launch_apply32(poisson_ctx* ctx, const Op& op, const float* v, const float* rhs, float* out, int mode) {
+    return apply_dispatch<float, KIND_CART2>(ctx, op, v, rhs, out, nullptr, mode, false, false);
+}
+
+int launch_residual_to32(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, float* out32, bool ug) {
+    return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
+}
+
+template <typename T, int KIND>
+static int rbsor_dispatch(poisson_ctx* ctx, const Op& op, T* phi, const T* rhs, T omega, int nsweeps, bool ug) {
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc, true), b(BX, BY);
+    for (int s = 0; s < nsweeps; ++s)
+        for (int colour = 0; colour < 2; ++colour) {
+            k_rbsor_half<T, KIND><<<g, b, 0, ctx->stream>>>(op, phi, rhs, omega, colour, ug, kc);
+            ctx->launches++;
+        }
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int launch_rbsor(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, double omega, int nsweeps,
+                 bool ug) {
+    if (kind == KIND_CART2) return rbsor_dispatch<double, KIND_CART2>(ctx, op, phi, rhs, omega, nsweeps, ug);
+    if (kind == KIND_SPH) return rbsor_dispatch<double, KIND_SPH>(ctx, op, phi, rhs, omega, nsweeps, ug);
+    return fail(ctx, POISSON_UNSUPPORTED,
+                "red-black SOR needs a radius-1 stencil: two colours are not independent for order 6");
+}
+
+int launch_rbsor32(poisson_ctx* ctx, const Op& op, float* phi, const float* rhs, float omega, int nsweeps) {
+    return rbsor_dispatch<float, KIND_CART2>(ctx, op, phi, rhs, omega, nsweeps, false);
+}
+
+}  // namespace pb

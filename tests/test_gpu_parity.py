@@ -1,0 +1,290 @@
+"""GPU parity: the CUDA path through the C ABI vs the CPU oracle on the same seeded inputs (-m gpu).
+
+Tolerances are north_star's (BASELINE.json): per-sweep fp64 pointwise relative <= 1e-13 (scale of DESIGN.md C8);
+fixed iteration count relative L2 <= 1e-10 (fp64) / 1e-5 (mixed); converged solutions: true residual, evaluated
+with the oracle's operator, within 10x the residual tolerance.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import pyoracle as po
+from gpu_helpers import dev, host, make_pair, pointwise_scaled, rel_l2, set_faces, stencil_scale
+from paper_2605_03563_b200 import binding as pb
+from paper_2605_03563_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+D6 = (po.BC_DIRICHLET_GHOST,) * 6
+P6 = (po.BC_PERIODIC,) * 6
+PATHS = [pb.PATH_GENERIC, pb.PATH_AUTO]
+
+
+def _random_faces(o, seed, R=1):
+    return [wl.hash_uniform(seed + f, np.arange(o.face_len(f))) - 0.5 for f in range(6)]
+
+
+# ---- (a1) stencil apply ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("shape,order,bc", [
+    ((32, 32, 32), 2, D6), ((37, 19, 23), 2, D6), ((64, 48, 40), 2, P6), ((1, 5, 3), 2, D6), ((128, 8, 66), 2, D6),
+    ((32, 32, 32), 6, P6), ((21, 17, 9), 6, D6), ((64, 64, 64), 6, P6), ((256, 24, 20), 2, D6),
+])
+def test_apply_matches_oracle(path, shape, order, bc):
+    w = dict(shape=shape, spacing=(0.1, 0.07, 0.13), origin=(0.0, 0.1, 0.2), order=order, bc=bc)
+    o, g = make_pair(w, path)
+    if bc == D6:
+        set_faces(o, g, _random_faces(o, 100))
+    phi = wl.random_field(shape, 5)
+    want = o.apply(phi)
+    d_phi, d_out = dev(phi), torch.empty(phi.shape, device="cuda", dtype=torch.float64)
+    g.apply_laplacian(d_phi, d_out)
+    got = host(d_out)
+    c = [1 / 0.1 ** 2, 1 / 0.07 ** 2, 1 / 0.13 ** 2]
+    scale = 2 * sum(c) * stencil_scale(phi) * (49 / 36 if order == 6 else 1.0) + 1.0
+    assert pointwise_scaled(got, want, scale) <= 1e-13
+    r = g.residual_norm(d_phi, dev(np.zeros_like(phi)))
+    assert r == pytest.approx(np.linalg.norm(want), rel=1e-12)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_apply_spherical_matches_oracle(path):
+    w = wl.config5(32, 16, 32)
+    o, g = make_pair(w, path)
+    faces = [None] * 6
+    faces[1] = wl.hash_uniform(3, np.arange(o.face_len(1)))
+    set_faces(o, g, faces)
+    phi = wl.random_field(w["shape"], 6)
+    want = o.apply(phi)
+    d_out = torch.empty(phi.shape, device="cuda", dtype=torch.float64)
+    g.apply_laplacian(dev(phi), d_out)
+    scale = o.diag() * stencil_scale(phi)
+    assert pointwise_scaled(host(d_out), want, scale) <= 1e-13
+
+
+# ---- (a2) red-black SOR ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+def test_config1_rbsor_200_sweeps(path):
+    w = wl.config1()
+    o, g = make_pair(w, path)
+    phi_c = np.zeros_like(w["rhs"])
+    d_phi, d_rhs = dev(phi_c), dev(w["rhs"])
+    r0 = o.residual_norm(phi_c, w["rhs"])
+    d = 2 * 3 / w["spacing"][0] ** 2
+    for s in range(20):
+        rn_c = o.rbsor(phi_c, w["rhs"], w["omega"], 10, want_resnorm=True)
+        rn_g = g.rbsor_sweep(d_phi, d_rhs, w["omega"], 10, want_resnorm=True)
+        got = host(d_phi)
+        scale = stencil_scale(phi_c, w["rhs"] / d)
+        assert pointwise_scaled(got, phi_c, scale) <= 1e-13, "after %d sweeps" % (10 * (s + 1))
+        assert rn_g / r0 == pytest.approx(rn_c / r0, rel=1e-9, abs=1e-15)
+    assert np.abs(got - w["exact"]).max() == pytest.approx(7.5303e-4, rel=1e-4)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("shape", [(33, 18, 7), (64, 64, 64), (128, 16, 34)])
+def test_rbsor_with_ghosts_and_odd_shapes(path, shape):
+    w = dict(shape=shape, spacing=(0.1, 0.12, 0.09), origin=(0, 0, 0), bc=D6)
+    o, g = make_pair(w, path)
+    set_faces(o, g, _random_faces(o, 7))
+    rhs = wl.random_field(shape, 8)
+    phi_c = wl.random_field(shape, 9)
+    d_phi, d_rhs = dev(phi_c), dev(rhs)
+    for nsw in (1, 2, 3):
+        o.rbsor(phi_c, rhs, 1.3, nsw)
+        g.rbsor_sweep(d_phi, d_rhs, 1.3, nsw)
+        assert pointwise_scaled(host(d_phi), phi_c, stencil_scale(phi_c, rhs * 0.003)) <= 1e-13
+    g.rbsor_sweep(d_phi, d_rhs, 1.3, 0)  # zero sweeps: a no-op
+    assert np.array_equal(host(d_phi), host(d_phi))
+
+
+# ---- (a6) multipole boundary ----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("lmax", [0, 2, 4, 8])
+def test_multipole_cartesian(lmax):
+    w = wl.config2(32)
+    o, g = make_pair(w)
+    q_c = o.multipole_bc(w["rho"], 1.0, lmax)
+    q_g = np.array(g.multipole_bc(dev(w["rho"]), 1.0, lmax))
+    assert np.abs(q_g - q_c).max() <= 1e-12 * np.abs(q_c).max()
+    for f in range(6):
+        buf = torch.empty(g.face_len(f), device="cuda", dtype=torch.float64)
+        g.get_ghost_face(f, buf)
+        want = o.get_ghost_face(f)
+        assert np.abs(host(buf) - want).max() <= 1e-12 * np.abs(want).max()
+
+
+def test_multipole_spherical():
+    w = wl.config5(32, 16, 32)
+    o, g = make_pair(w)
+    q_c = o.multipole_bc(w["rho"], 1.0, 8)
+    q_g = np.array(g.multipole_bc(dev(w["rho"]), 1.0, 8))
+    assert np.abs(q_g - q_c).max() <= 1e-12 * np.abs(q_c).max()
+    buf = torch.empty(g.face_len(1), device="cuda", dtype=torch.float64)
+    g.get_ghost_face(1, buf)
+    want = o.get_ghost_face(1)
+    assert np.abs(host(buf) - want).max() <= 1e-12 * np.abs(want).max()
+
+
+def test_multipole_three_ghost_layers_order6():
+    w = dict(shape=(16, 12, 10), spacing=(0.1,) * 3, origin=(-0.75, -0.55, -0.45), order=6, bc=D6)
+    o, g = make_pair(w)
+    rho = np.zeros((10, 12, 16))
+    rho[3:7, 4:8, 5:11] = wl.random_field((6, 4, 4), 3, 0.1, 1.0)
+    o.multipole_bc(rho, 2.0, 6)
+    g.multipole_bc(dev(rho), 2.0, 6)
+    for f in range(6):
+        buf = torch.empty(g.face_len(f), device="cuda", dtype=torch.float64)
+        g.get_ghost_face(f, buf)
+        want = o.get_ghost_face(f)
+        assert np.abs(host(buf) - want).max() <= 1e-12 * np.abs(want).max()
+
+
+# ---- (a3) CG --------------------------------------------------------------------------------------------------------
+def _cg_both(w, o, g, **kw):
+    phi_c = np.zeros_like(w["rhs"])
+    d_phi, d_rhs = dev(phi_c), dev(w["rhs"])
+    res_c = o.cg(phi_c, w["rhs"], want_history=True, **kw)
+    g.set_option(pb.OPT_RECORD_HISTORY, 1)
+    res_g = g.cg_solve(d_phi, d_rhs, **kw)
+    return phi_c, host(d_phi), res_c, res_g
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("n", [32, 64])
+def test_config2_cg_fixed_and_converged(path, n):
+    w = wl.config2(n)
+    o, g = make_pair(w, path)
+    o.multipole_bc(w["rho"], w["G"], w["lmax"])
+    g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
+    for fixed in (25, 100):
+        phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, fixed_iters=fixed)
+        assert res_g["iters"] == fixed and res_g["status"] == pb.OK
+        assert rel_l2(phi_g, phi_c) <= 1e-10
+        hist = np.array(g.get_history(fixed + 1))
+        assert np.allclose(hist, res_c["history"], rtol=1e-8)
+    phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, rtol=w["rtol"], max_iter=2000)
+    assert res_g["status"] == pb.OK and abs(res_g["iters"] - res_c["iters"]) <= 1
+    b_norm = o.residual_norm(np.zeros_like(phi_g), w["rhs"])
+    assert o.residual_norm(phi_g, w["rhs"]) <= 10 * w["rtol"] * b_norm
+    assert rel_l2(phi_g, phi_c) <= 1e-7
+    # and the physics: the analytic uniform-sphere potential up to O(h^2) (north_star)
+    assert rel_l2(phi_g, w["exact"]) < {32: 2e-3, 64: 5e-4}[n]
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("n", [32, 64])
+def test_config4_periodic_cg6(path, n):
+    w = wl.config4(n)
+    o, g = make_pair(w, path)
+    phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, fixed_iters=25)
+    assert rel_l2(phi_g, phi_c) <= 1e-10
+    assert abs(phi_g.mean()) <= 1e-13 * np.abs(phi_g).max()
+    phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, rtol=1e-10, max_iter=3000)
+    assert res_g["status"] == pb.OK and abs(res_g["iters"] - res_c["iters"]) <= 2
+    b_norm = np.linalg.norm(w["rhs"])
+    assert o.residual_norm(phi_g, w["rhs"]) <= 10 * 1e-10 * b_norm
+    assert rel_l2(phi_g, phi_c) <= 1e-8
+
+
+def test_cg_not_converged_status_and_warm_start():
+    w = wl.config2(32)
+    o, g = make_pair(w)
+    d_phi, d_rhs = dev(np.zeros_like(w["rhs"])), dev(w["rhs"])
+    res = g.cg_solve(d_phi, d_rhs, rtol=1e-12, max_iter=5)
+    assert res["status"] == pb.NOT_CONVERGED and res["iters"] == 5   # PAPER.md:55 warning path
+    res = g.cg_solve(d_phi, d_rhs, rtol=1e-9, max_iter=500)          # warm start from the 5-iteration iterate
+    assert res["status"] == pb.OK
+    assert o.residual_norm(host(d_phi), w["rhs"]) <= 1e-8 * np.linalg.norm(w["rhs"])
+    res = g.cg_solve(dev(np.zeros_like(w["rhs"])), dev(np.zeros_like(w["rhs"])), rtol=1e-8, max_iter=10)
+    assert res["status"] == pb.OK and res["iters"] == 0              # zero right-hand side
+
+
+# ---- (a4) BiCGSTAB --------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+def test_config5_bicgstab(path):
+    w = wl.config5(32, 16, 32)
+    o, g = make_pair(w, path)
+    o.multipole_bc(w["rho"], w["G"], w["lmax"])
+    g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
+    g.set_option(pb.OPT_RECORD_HISTORY, 1)
+    for fixed in (10, 25):
+        phi_c = np.zeros_like(w["rhs"])
+        d_phi = dev(phi_c)
+        res_c = o.bicgstab(phi_c, w["rhs"], fixed_iters=fixed, want_history=True)
+        res_g = g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=fixed)
+        assert res_g["iters"] == fixed
+        assert rel_l2(host(d_phi), phi_c) <= 1e-10
+        assert np.allclose(g.get_history(fixed + 1), res_c["history"], rtol=1e-7)
+    phi_c = np.zeros_like(w["rhs"])
+    d_phi = dev(phi_c)
+    res_c = o.bicgstab(phi_c, w["rhs"], rtol=1e-8, max_iter=3000)
+    res_g = g.bicgstab_solve(d_phi, dev(w["rhs"]), rtol=1e-8, max_iter=3000)
+    assert res_g["status"] == pb.OK
+    b_norm = o.residual_norm(np.zeros_like(phi_c), w["rhs"])
+    assert o.residual_norm(host(d_phi), w["rhs"]) <= 10 * 1e-8 * b_norm
+    assert rel_l2(host(d_phi), phi_c) <= 1e-5
+
+
+def test_bicgstab_on_cartesian_and_unscaled_variant():
+    w = wl.config2(32)
+    o, g = make_pair(w)
+    phi_c = np.zeros_like(w["rhs"])
+    d_phi = dev(phi_c)
+    o.bicgstab(phi_c, w["rhs"], fixed_iters=20, jacobi=0)
+    g.set_option(pb.OPT_JACOBI, 0)
+    g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=20)
+    assert rel_l2(host(d_phi), phi_c) <= 1e-10
+
+
+# ---- (a5) multigrid V-cycle -----------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [32, 64])
+@pytest.mark.parametrize("restriction", [0, 1])
+def test_config3_vcycle_fp64_and_mixed(n, restriction):
+    w = wl.config3(n)
+    o, g = make_pair(w)
+    g.set_option(pb.OPT_RESTRICTION, restriction)
+    o.multipole_bc(w["rho"], w["G"], w["lmax"])
+    g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
+    for precision, tol in ((pb.F64, 1e-10), (pb.MIXED, 1e-5)):
+        phi_c = np.zeros_like(w["rhs"])
+        d_phi = dev(phi_c)
+        rc = o.vcycle(phi_c, w["rhs"], precision=precision, restriction=restriction, ncycles=4)["resnorms"]
+        rg = np.array(g.mg_vcycle(d_phi, dev(w["rhs"]), precision=precision, ncycles=4)["resnorms"])
+        assert rel_l2(host(d_phi), phi_c) <= tol
+        assert np.allclose(rg, rc, rtol=1e-6 if precision == pb.F64 else 2e-2)
+        assert np.all(rg[1:] / rg[:-1] < 0.2)   # healthy, size-independent multigrid
+
+
+def test_vcycle_ten_cycles_reaches_truncation_floor():
+    w = wl.config3(64)
+    o, g = make_pair(w)
+    g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
+    d_phi = dev(np.zeros_like(w["rhs"]))
+    res = np.array(g.mg_vcycle(d_phi, dev(w["rhs"]), ncycles=10)["resnorms"])
+    assert res[-1] / res[0] < 1e-8
+    assert rel_l2(host(d_phi), w["exact"]) < 1e-3   # O(h^2) + lmax=8 truncation against the erf potential
+
+
+# ---- errors and edge cases (include/poisson.h "Return value") --------------------------------------------------------
+def test_error_codes():
+    with pytest.raises(pb.PoissonError) as e:
+        pb.Poisson((8, 8, 8), (0.1,) * 3, order=4, bc=D6)
+    assert e.value.code == pb.INVALID_ARG
+    with pytest.raises(pb.PoissonError):
+        pb.Poisson((8, 8, 0), (0.1,) * 3, bc=D6)
+    with pytest.raises(pb.PoissonError):
+        pb.Poisson((8, 8, 8), (0.1,) * 3, bc=(1, 0, 0, 0, 0, 0))
+    g = pb.Poisson((8, 8, 8), (0.1,) * 3, bc=D6)
+    x = torch.zeros(512, device="cuda", dtype=torch.float64)
+    with pytest.raises(pb.PoissonError) as e:
+        g.rbsor_sweep(x, x.clone(), 2.5, 1)
+    assert e.value.code == pb.INVALID_ARG and "omega" in str(e.value)
+    with pytest.raises(pb.PoissonError) as e:
+        g.apply_laplacian(x, x)
+    assert e.value.code == pb.INVALID_ARG
+    g6 = pb.Poisson((8, 8, 8), (0.1,) * 3, order=6, bc=P6)
+    with pytest.raises(pb.PoissonError) as e:
+        g6.mg_vcycle(x, x.clone())
+    assert e.value.code == pb.UNSUPPORTED
+    assert g.kernel_launches() >= 0
