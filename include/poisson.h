@@ -55,7 +55,9 @@ enum {
                                       1 = mean of the 8 children (reading C7) */
     POISSON_OPT_POLL_INTERVAL = 2, /* Krylov solvers poll the device convergence flag every this many iterations */
     POISSON_OPT_JACOBI = 3,        /* BiCGSTAB right Jacobi scaling: 1 (default) on, 0 off (reading C10) */
-    POISSON_OPT_RECORD_HISTORY = 4 /* 1: record ||r_k||/||r_0|| per Krylov iteration for poisson_get_history */
+    POISSON_OPT_RECORD_HISTORY = 4,/* 1: record ||r_k||/||r_0|| per Krylov iteration for poisson_get_history */
+    POISSON_OPT_TIME_KERNELS = 5   /* bracket every launch of one kernel class (0..poisson_kernel_classes()-1) with
+                                      CUDA events on the handle's stream; -2 = every class, -1 = off (default) */
 };
 
 /* Create a solver context for one grid + operator ("uniform and nonuniform grids in spherical and
@@ -125,10 +127,28 @@ int poisson_get_history(poisson_t h, double* h_out, int n);
 /* Number of kernels this handle has launched so far (bench bookkeeping). */
 long poisson_kernel_launches(poisson_t h);
 
-/* End-to-end variants with HOST buffers: host->device copy of rhs (and phi), the solve, device->host copy of phi,
- * all on the handle's stream; synchronises. */
+/* Kernel-class bookkeeping for the bench: the classes are the rows of the hot path
+ * (apply, rbsor, cg_pass_a, ...).  poisson_kernel_time synchronises the stream and returns the summed CUDA-event
+ * duration (ms) and the number of timed launches of one class since the last reset. */
+int poisson_kernel_classes(void);
+const char* poisson_kernel_name(int kernel_class);
+long poisson_kernel_class_launches(poisson_t h, int kernel_class);
+int poisson_kernel_time(poisson_t h, int kernel_class, double* h_ms_total, long* h_count);
+int poisson_reset_kernel_times(poisson_t h);
+
+/* End-to-end variants with HOST buffers (all h_* below, including the fields): host->device copy of the inputs on
+ * the handle's stream, the device entry point of the same name, device->host copy of the result, synchronise.
+ * Same arguments, statuses and errors as the device versions.  Pinned host memory gives full PCIe speed. */
+int poisson_apply_laplacian_host(poisson_t h, const double* h_phi, double* h_out);
+int poisson_rbsor_sweep_host(poisson_t h, double* h_phi, const double* h_rhs, double omega, int nsweeps,
+                             double* h_resnorm);
 int poisson_cg_solve_host(poisson_t h, double* h_phi, const double* h_rhs, double rtol, int max_iter,
                           int fixed_iters, int* iters, double* relres);
+int poisson_bicgstab_solve_host(poisson_t h, double* h_phi, const double* h_rhs, double rtol, int max_iter,
+                                int fixed_iters, int* iters, double* relres);
+int poisson_mg_vcycle_host(poisson_t h, double* h_phi, const double* h_rhs, int nu1, int nu2, int coarsest_n,
+                           int coarsest_sweeps, int precision, int ncycles, double* h_resnorms);
+int poisson_multipole_bc_host(poisson_t h, const double* h_rho, double G, int lmax, double* h_moments);
 
 #ifdef __cplusplus
 }

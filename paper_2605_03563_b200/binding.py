@@ -15,14 +15,17 @@ BC_DIRICHLET_GHOST, BC_PERIODIC, BC_NEUMANN0, BC_AXIS = 0, 1, 2, 3
 F64, MIXED = 0, 1
 OK, NOT_CONVERGED, BREAKDOWN = 0, 1, 2
 INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY = -1, -2, -3, -4
-OPT_KERNEL_PATH, OPT_RESTRICTION, OPT_POLL_INTERVAL, OPT_JACOBI, OPT_RECORD_HISTORY = 0, 1, 2, 3, 4
+OPT_KERNEL_PATH, OPT_RESTRICTION, OPT_POLL_INTERVAL, OPT_JACOBI, OPT_RECORD_HISTORY, OPT_TIME_KERNELS = 0, 1, 2, 3, 4, 5
 PATH_AUTO, PATH_GENERIC, PATH_PLANE = 0, 1, 2
 
 SYMBOLS = [
     "poisson_create", "poisson_destroy", "poisson_last_error", "poisson_set_option", "poisson_apply_laplacian",
     "poisson_rbsor_sweep", "poisson_cg_solve", "poisson_bicgstab_solve", "poisson_mg_vcycle", "poisson_multipole_bc",
     "poisson_set_ghost_faces", "poisson_get_ghost_face", "poisson_face_len", "poisson_residual_norm",
-    "poisson_get_history", "poisson_kernel_launches", "poisson_cg_solve_host",
+    "poisson_get_history", "poisson_kernel_launches", "poisson_kernel_classes", "poisson_kernel_name",
+    "poisson_kernel_class_launches", "poisson_kernel_time", "poisson_reset_kernel_times",
+    "poisson_apply_laplacian_host", "poisson_rbsor_sweep_host", "poisson_cg_solve_host",
+    "poisson_bicgstab_solve_host", "poisson_mg_vcycle_host", "poisson_multipole_bc_host",
 ]
 
 _lib = None
@@ -48,16 +51,29 @@ def lib():
         L.poisson_face_len.argtypes = [C.c_void_p, C.c_int]
         L.poisson_kernel_launches.restype = C.c_long
         L.poisson_kernel_launches.argtypes = [C.c_void_p]
+        L.poisson_kernel_name.restype = C.c_char_p
+        L.poisson_kernel_name.argtypes = [C.c_int]
+        L.poisson_kernel_class_launches.restype = C.c_long
+        L.poisson_kernel_class_launches.argtypes = [C.c_void_p, C.c_int]
         _lib = L
     return _lib
 
 
+def kernel_classes():
+    """Names of the kernel classes (rows of the hot path), indexed by class id."""
+    L = lib()
+    return [L.poisson_kernel_name(i).decode() for i in range(L.poisson_kernel_classes())]
+
+
 def _ptr(t):
-    """Device (or pinned host) pointer of a torch tensor / raw integer address."""
+    """Device (or pinned host) pointer of a torch tensor / numpy array / raw integer address."""
     if t is None:
         return C.c_void_p(0)
     if isinstance(t, int):
         return C.c_void_p(t)
+    if hasattr(t, "ctypes"):  # numpy array (host entry points only)
+        assert t.flags.c_contiguous, "arrays must be contiguous"
+        return C.c_void_p(t.ctypes.data)
     assert t.is_contiguous(), "arrays must be contiguous"
     return C.c_void_p(t.data_ptr())
 
@@ -113,11 +129,27 @@ class Poisson:
     def kernel_launches(self):
         return int(lib().poisson_kernel_launches(self.h))
 
+    def kernel_class_launches(self):
+        L = lib()
+        return {n: int(L.poisson_kernel_class_launches(self.h, i)) for i, n in enumerate(kernel_classes())}
+
+    def kernel_time(self, kernel_class):
+        """(total ms, launches) of the event-timed launches of one class (set OPT_TIME_KERNELS first)."""
+        ms, cnt = C.c_double(0.0), C.c_long(0)
+        self._check(lib().poisson_kernel_time(self.h, int(kernel_class), C.byref(ms), C.byref(cnt)))
+        return ms.value, cnt.value
+
+    def reset_kernel_times(self):
+        self._check(lib().poisson_reset_kernel_times(self.h))
+
     def face_len(self, f):
         return int(lib().poisson_face_len(self.h, int(f)))
 
     def apply_laplacian(self, d_phi, d_out):
         self._check(lib().poisson_apply_laplacian(self.h, _ptr(d_phi), _ptr(d_out)))
+
+    def apply_laplacian_host(self, h_phi, h_out):
+        self._check(lib().poisson_apply_laplacian_host(self.h, _ptr(h_phi), _ptr(h_out)))
 
     def residual_norm(self, d_phi, d_rhs):
         out = C.c_double(0.0)
@@ -128,6 +160,12 @@ class Poisson:
         out = C.c_double(0.0)
         self._check(lib().poisson_rbsor_sweep(self.h, _ptr(d_phi), _ptr(d_rhs), C.c_double(omega), int(nsweeps),
                                               C.byref(out) if want_resnorm else None))
+        return out.value if want_resnorm else None
+
+    def rbsor_sweep_host(self, h_phi, h_rhs, omega, nsweeps, want_resnorm=False):
+        out = C.c_double(0.0)
+        self._check(lib().poisson_rbsor_sweep_host(self.h, _ptr(h_phi), _ptr(h_rhs), C.c_double(omega), int(nsweeps),
+                                                   C.byref(out) if want_resnorm else None))
         return out.value if want_resnorm else None
 
     def _krylov(self, fn, d_phi, d_rhs, rtol, max_iter, fixed_iters):
@@ -145,6 +183,9 @@ class Poisson:
     def bicgstab_solve(self, d_phi, d_rhs, rtol=1e-8, max_iter=10000, fixed_iters=0):
         return self._krylov(lib().poisson_bicgstab_solve, d_phi, d_rhs, rtol, max_iter, fixed_iters)
 
+    def bicgstab_solve_host(self, h_phi, h_rhs, rtol=1e-8, max_iter=10000, fixed_iters=0):
+        return self._krylov(lib().poisson_bicgstab_solve_host, h_phi, h_rhs, rtol, max_iter, fixed_iters)
+
     def get_history(self, n):
         buf = (C.c_double * n)()
         self._check(lib().poisson_get_history(self.h, buf, int(n)))
@@ -158,12 +199,23 @@ class Poisson:
                                                  buf if want_resnorms else None))
         return dict(status=rc, resnorms=list(buf) if want_resnorms else None)
 
-    def multipole_bc(self, d_rho, G, lmax, want_moments=True):
+    def mg_vcycle_host(self, h_phi, h_rhs, nu1=2, nu2=2, coarsest_n=8, coarsest_sweeps=50, precision=F64, ncycles=1,
+                       want_resnorms=True):
+        buf = (C.c_double * (ncycles + 1))()
+        rc = self._check(lib().poisson_mg_vcycle_host(self.h, _ptr(h_phi), _ptr(h_rhs), int(nu1), int(nu2),
+                                                      int(coarsest_n), int(coarsest_sweeps), int(precision),
+                                                      int(ncycles), buf if want_resnorms else None))
+        return dict(status=rc, resnorms=list(buf) if want_resnorms else None)
+
+    def multipole_bc(self, d_rho, G, lmax, want_moments=True, _fn=None):
         nq = (lmax + 1) ** 2
         buf = (C.c_double * nq)()
-        self._check(lib().poisson_multipole_bc(self.h, _ptr(d_rho), C.c_double(G), int(lmax),
-                                               buf if want_moments else None))
+        fn = _fn or lib().poisson_multipole_bc
+        self._check(fn(self.h, _ptr(d_rho), C.c_double(G), int(lmax), buf if want_moments else None))
         return list(buf) if want_moments else None
+
+    def multipole_bc_host(self, h_rho, G, lmax, want_moments=True):
+        return self.multipole_bc(h_rho, G, lmax, want_moments, _fn=lib().poisson_multipole_bc_host)
 
     def set_ghost_faces(self, d_faces):
         arr = (C.c_void_p * 6)(*[_ptr(f) for f in d_faces])

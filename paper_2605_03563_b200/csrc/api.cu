@@ -42,7 +42,37 @@ double* scratch(poisson_ctx* ctx, int slot) {
     return ctx->vec[slot];
 }
 
+void pre_launch(poisson_ctx* ctx, int kid) {
+    if (ctx->time_kid != kid && ctx->time_kid != -2) return;
+    if (ctx->ev_used + 2 > ctx->ev_pool.size()) {
+        cudaEvent_t a = nullptr, b = nullptr;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
+            cudaGetLastError();
+            return;
+        }
+        ctx->ev_pool.push_back(a);
+        ctx->ev_pool.push_back(b);
+        ctx->ev_kid.push_back(kid);
+    } else {
+        ctx->ev_kid[ctx->ev_used / 2] = kid;
+    }
+    cudaEventRecord(ctx->ev_pool[ctx->ev_used], ctx->stream);
+}
+
+void post_launch(poisson_ctx* ctx, int kid) {
+    ctx->launches++;
+    ctx->launches_by_kid[kid]++;
+    if (ctx->time_kid != kid && ctx->time_kid != -2) return;
+    if (ctx->ev_used + 2 > ctx->ev_pool.size()) return;
+    cudaEventRecord(ctx->ev_pool[ctx->ev_used + 1], ctx->stream);
+    ctx->ev_used += 2;
+}
+
 }  // namespace pb
+
+static const char* const kKernelNames[pb::KID_COUNT] = {
+    "apply", "rbsor", "krylov_init", "cg_pass_a", "cg_pass_b", "cg_final", "bicg_pass1", "bicg_pass2", "bicg_pass3",
+    "mg_restrict", "mg_prolong", "mg_coarse", "mg_axpy", "mp_moments", "mp_ghosts"};
 
 static void free_levels(poisson_ctx* ctx) {
     for (auto& L : ctx->levels) {
@@ -148,8 +178,8 @@ int poisson_destroy(poisson_t ctx) {
     cudaFree(ctx->d_hist);
     cudaFree(ctx->d_scal);
     cudaFreeHost(ctx->h_scal);
-    cudaFree(ctx->d_stage[0]);
-    cudaFree(ctx->d_stage[1]);
+    for (double* s : ctx->d_stage) cudaFree(s);
+    for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
     return POISSON_OK;
 }
@@ -275,12 +305,46 @@ int poisson_set_option(poisson_t ctx, int option, int value) {
         case POISSON_OPT_RECORD_HISTORY:
             ctx->opt_history = value ? 1 : 0;
             return POISSON_OK;
+        case POISSON_OPT_TIME_KERNELS:
+            if (value < -2 || value >= KID_COUNT) return fail(ctx, POISSON_INVALID_ARG, "bad kernel class");
+            ctx->time_kid = value;
+            return POISSON_OK;
     }
     return fail(ctx, POISSON_INVALID_ARG, "unknown option");
 }
 
 long poisson_face_len(poisson_t ctx, int face) { return (ctx && face >= 0 && face < 6) ? ctx->face_len[face] : -1; }
 long poisson_kernel_launches(poisson_t ctx) { return ctx ? ctx->launches : -1; }
+
+int poisson_kernel_classes(void) { return KID_COUNT; }
+const char* poisson_kernel_name(int kernel_class) {
+    return (kernel_class >= 0 && kernel_class < KID_COUNT) ? kKernelNames[kernel_class] : "";
+}
+long poisson_kernel_class_launches(poisson_t ctx, int kernel_class) {
+    return (ctx && kernel_class >= 0 && kernel_class < KID_COUNT) ? ctx->launches_by_kid[kernel_class] : -1;
+}
+int poisson_kernel_time(poisson_t ctx, int kernel_class, double* h_ms_total, long* h_count) {
+    if (!ctx || kernel_class < 0 || kernel_class >= KID_COUNT) return POISSON_INVALID_ARG;
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    double tot = 0;
+    long cnt = 0;
+    for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+        if (ctx->ev_kid[i / 2] != kernel_class) continue;
+        float ms = 0;
+        PB_CUDA_OK(cudaEventElapsedTime(&ms, ctx->ev_pool[i], ctx->ev_pool[i + 1]));
+        tot += ms;
+        ++cnt;
+    }
+    if (h_ms_total) *h_ms_total = tot;
+    if (h_count) *h_count = cnt;
+    return POISSON_OK;
+}
+int poisson_reset_kernel_times(poisson_t ctx) {
+    if (!ctx) return POISSON_INVALID_ARG;
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    ctx->ev_used = 0;
+    return POISSON_OK;
+}
 
 int poisson_set_ghost_faces(poisson_t ctx, const double* const d_faces[6]) {
     if (!ctx || !d_faces) return POISSON_INVALID_ARG;
@@ -610,17 +674,84 @@ int poisson_multipole_bc(poisson_t ctx, const double* d_rho, double G, int lmax,
 }
 
 // ---- end-to-end with host buffers -----------------------------------------------------------------------------------------
+// Each call copies its inputs host->device on the handle's stream, runs the device entry point above, copies the
+// result back and synchronises.  Host buffers should be pinned for full PCIe speed; pageable memory also works.
+static int stage(poisson_ctx* ctx, int slot, const double* h_src) {
+    const size_t bytes = ctx->npts * sizeof(double);
+    if (!ctx->d_stage[slot]) PB_CUDA_OK(cudaMalloc((void**)&ctx->d_stage[slot], bytes));
+    if (h_src) PB_CUDA_OK(cudaMemcpyAsync(ctx->d_stage[slot], h_src, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    return POISSON_OK;
+}
+static int unstage(poisson_ctx* ctx, int slot, double* h_dst) {
+    PB_CUDA_OK(cudaMemcpyAsync(h_dst, ctx->d_stage[slot], ctx->npts * sizeof(double), cudaMemcpyDeviceToHost,
+                               ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    return POISSON_OK;
+}
+#define STAGE_OK(call)                  \
+    do {                                \
+        int rc__ = (call);              \
+        if (rc__ != POISSON_OK) return rc__; \
+    } while (0)
+
+int poisson_apply_laplacian_host(poisson_t ctx, const double* h_phi, double* h_out) {
+    if (!ctx || !h_phi || !h_out) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    STAGE_OK(stage(ctx, 0, h_phi));
+    STAGE_OK(stage(ctx, 1, nullptr));
+    const int rc = poisson_apply_laplacian(ctx, ctx->d_stage[0], ctx->d_stage[1]);
+    if (rc < 0) return rc;
+    return unstage(ctx, 1, h_out);
+}
+
+int poisson_rbsor_sweep_host(poisson_t ctx, double* h_phi, const double* h_rhs, double omega, int nsweeps,
+                             double* h_resnorm) {
+    if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    STAGE_OK(stage(ctx, 0, h_phi));
+    STAGE_OK(stage(ctx, 1, h_rhs));
+    const int rc = poisson_rbsor_sweep(ctx, ctx->d_stage[0], ctx->d_stage[1], omega, nsweeps, h_resnorm);
+    if (rc < 0) return rc;
+    return unstage(ctx, 0, h_phi);
+}
+
 int poisson_cg_solve_host(poisson_t ctx, double* h_phi, const double* h_rhs, double rtol, int max_iter,
                           int fixed_iters, int* iters, double* relres) {
     if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
-    const size_t bytes = ctx->npts * sizeof(double);
-    for (int s = 0; s < 2; ++s)
-        if (!ctx->d_stage[s]) PB_CUDA_OK(cudaMalloc((void**)&ctx->d_stage[s], bytes));
-    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_stage[0], h_phi, bytes, cudaMemcpyHostToDevice, ctx->stream));
-    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_stage[1], h_rhs, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    STAGE_OK(stage(ctx, 0, h_phi));
+    STAGE_OK(stage(ctx, 1, h_rhs));
     const int rc = poisson_cg_solve(ctx, ctx->d_stage[0], ctx->d_stage[1], rtol, max_iter, fixed_iters, iters, relres);
     if (rc < 0) return rc;
-    PB_CUDA_OK(cudaMemcpyAsync(h_phi, ctx->d_stage[0], bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    const int rc2 = unstage(ctx, 0, h_phi);
+    return rc2 != POISSON_OK ? rc2 : rc;
+}
+
+int poisson_bicgstab_solve_host(poisson_t ctx, double* h_phi, const double* h_rhs, double rtol, int max_iter,
+                                int fixed_iters, int* iters, double* relres) {
+    if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    STAGE_OK(stage(ctx, 0, h_phi));
+    STAGE_OK(stage(ctx, 1, h_rhs));
+    const int rc =
+        poisson_bicgstab_solve(ctx, ctx->d_stage[0], ctx->d_stage[1], rtol, max_iter, fixed_iters, iters, relres);
+    if (rc < 0) return rc;
+    const int rc2 = unstage(ctx, 0, h_phi);
+    return rc2 != POISSON_OK ? rc2 : rc;
+}
+
+int poisson_mg_vcycle_host(poisson_t ctx, double* h_phi, const double* h_rhs, int nu1, int nu2, int coarsest_n,
+                           int coarsest_sweeps, int precision, int ncycles, double* h_resnorms) {
+    if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    STAGE_OK(stage(ctx, 0, h_phi));
+    STAGE_OK(stage(ctx, 1, h_rhs));
+    const int rc = poisson_mg_vcycle(ctx, ctx->d_stage[0], ctx->d_stage[1], nu1, nu2, coarsest_n, coarsest_sweeps,
+                                     precision, ncycles, h_resnorms);
+    if (rc < 0) return rc;
+    return unstage(ctx, 0, h_phi);
+}
+
+int poisson_multipole_bc_host(poisson_t ctx, const double* h_rho, double G, int lmax, double* h_moments) {
+    if (!ctx || !h_rho) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    STAGE_OK(stage(ctx, 1, h_rho));
+    const int rc = poisson_multipole_bc(ctx, ctx->d_stage[1], G, lmax, h_moments);
+    if (rc < 0) return rc;
     PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
     return rc;
 }

@@ -37,6 +37,26 @@ struct Op {
 
 enum { KIND_CART2 = 0, KIND_CART6 = 1, KIND_SPH = 2 };
 
+// Kernel classes, for launch counting and the optional per-class CUDA-event timing (POISSON_OPT_TIME_KERNELS).
+enum KernelId {
+    KID_APPLY = 0,      // stencil apply / residual (a1, a7)
+    KID_RBSOR,          // red-black SOR sweeps (a2)
+    KID_KRYLOV_INIT,    // initial residual of CG / BiCGSTAB
+    KID_CG_PASS_A,      // p-update + matvec + p.Ap (+ deferred x-update) (a3)
+    KID_CG_PASS_B,      // r-update + ||r||^2 (a3)
+    KID_CG_FINAL,       // pending x-update / mean removal
+    KID_BICG_PASS1,     // (a4)
+    KID_BICG_PASS2,
+    KID_BICG_PASS3,
+    KID_MG_RESTRICT,    // residual + restriction (a5)
+    KID_MG_PROLONG,     // prolongation + correction (+ smoothing) (a5)
+    KID_MG_COARSE,      // coarsest-level solver (a5)
+    KID_MG_AXPY,        // mixed path: phi += (double) e32
+    KID_MP_MOMENTS,     // multipole moments (a6)
+    KID_MP_GHOSTS,      // ghost-zone evaluation (a6)
+    KID_COUNT
+};
+
 // Device-resident scalars of the Krylov solvers: nothing crosses to the host inside an iteration.
 struct KrylovCtl {
     double rr, rr0, pq, alpha, beta, mu, rho, omega, r0v, ts, tt, tol2;
@@ -93,6 +113,12 @@ struct poisson_ctx {
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
     long launches = 0;
+    long launches_by_kid[pb::KID_COUNT] = {0};
+    // optional event timing of one kernel class (or all with -2): pairs of events around every such launch
+    int time_kid = -1;
+    std::vector<cudaEvent_t> ev_pool;           // start/stop pairs, reused after poisson_reset_kernel_times
+    std::vector<int> ev_kid;                    // kernel class of pair i
+    size_t ev_used = 0;
     int num_sms = 148;
     std::string err;
     // pinned staging for the host-buffer entry points
@@ -104,6 +130,16 @@ namespace pb {
 int fail(poisson_ctx* ctx, int code, const std::string& msg);
 int fail_cuda(poisson_ctx* ctx, cudaError_t e, const char* what, const char* file, int line);
 double* scratch(poisson_ctx* ctx, int slot);  // lazily allocated npts-sized vector; nullptr on OOM
+void pre_launch(poisson_ctx* ctx, int kid);
+void post_launch(poisson_ctx* ctx, int kid);
+
+// Every kernel launch of the library goes through this: counts it and, when asked, brackets it with CUDA events.
+#define PB_LAUNCH(ctx, kid, ...)       \
+    do {                               \
+        pb::pre_launch((ctx), (kid));  \
+        __VA_ARGS__;                   \
+        pb::post_launch((ctx), (kid)); \
+    } while (0)
 
 // ---- launch wrappers (definitions in the k_*.cu files) --------------------------------------------------------------
 // out = L v (mode 0) or out = rhs - L v (mode 1).  red != 0: also reduce sum(out^2), sum(out) into d_scal[0..1].

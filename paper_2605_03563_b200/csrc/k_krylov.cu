@@ -313,9 +313,10 @@ int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, dou
     const Op& op = ctx->op;
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
+    pre_launch(ctx, KID_KRYLOV_INIT);
     KIND_SWITCH(ctx->kind, (k_krylov_init<K><<<g, b, 0, ctx->stream>>>(op, x, rhs, r, bicg ? r0hat : nullptr, ctx->d_ctl,
                                                                          ctx->d_hist, kc, ctx->red)));
-    ctx->launches++;
+    post_launch(ctx, KID_KRYLOV_INIT);
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -324,30 +325,31 @@ int launch_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, doub
     const Op& op = ctx->op;
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
+    pre_launch(ctx, KID_CG_PASS_A);
     KIND_SWITCH(ctx->kind,
                 (k_cg_passA<K><<<g, b, 0, ctx->stream>>>(op, r, p_old, p_new, q, x, ctx->d_ctl, kc, ctx->red)));
-    ctx->launches++;
+    post_launch(ctx, KID_CG_PASS_A);
     return POISSON_OK;
 }
 
 int launch_cg_passB(poisson_ctx* ctx, double* r, const double* q) {
-    k_cg_passB<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, r, q, ctx->d_ctl, ctx->d_hist,
-                                                                       ctx->red);
-    ctx->launches++;
+    PB_LAUNCH(ctx, KID_CG_PASS_B, (k_cg_passB<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(
+                                      ctx->npts, r, q, ctx->d_ctl, ctx->d_hist, ctx->red)));
     return POISSON_OK;
 }
 
 int launch_cg_final(poisson_ctx* ctx, double* x, const double* p_last) {
-    k_cg_final<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, p_last, ctx->d_ctl);
-    ctx->launches++;
+    PB_LAUNCH(ctx, KID_CG_FINAL,
+              (k_cg_final<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, p_last, ctx->d_ctl)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
 
 int launch_sub_mean(poisson_ctx* ctx, double* x) {
-    k_sum<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, ctx->d_ctl, ctx->red);
-    k_sub_mean<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, ctx->d_ctl);
-    ctx->launches += 2;
+    PB_LAUNCH(ctx, KID_CG_FINAL,
+              (k_sum<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, ctx->d_ctl, ctx->red)));
+    PB_LAUNCH(ctx, KID_CG_FINAL,
+              (k_sub_mean<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, x, ctx->d_ctl)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -357,9 +359,10 @@ int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, co
     const Op& op = ctx->op;
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
+    pre_launch(ctx, KID_BICG_PASS1);
     KIND_SWITCH(ctx->kind, (k_bicg_pass1<K><<<g, b, 0, ctx->stream>>>(op, r, p_old, v_old, r0, p_new, v_new, ctx->d_ctl,
                                                                         ctx->opt_jacobi, kc, ctx->red)));
-    ctx->launches++;
+    post_launch(ctx, KID_BICG_PASS1);
     return POISSON_OK;
 }
 
@@ -367,9 +370,10 @@ int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double
     const Op& op = ctx->op;
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
+    pre_launch(ctx, KID_BICG_PASS2);
     KIND_SWITCH(ctx->kind, (k_bicg_pass2<K><<<g, b, 0, ctx->stream>>>(op, r, v, s, t, ctx->d_ctl, ctx->opt_jacobi, kc,
                                                                         ctx->red)));
-    ctx->launches++;
+    post_launch(ctx, KID_BICG_PASS2);
     return POISSON_OK;
 }
 
@@ -378,9 +382,10 @@ int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double
     const Op& op = ctx->op;
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
+    pre_launch(ctx, KID_BICG_PASS3);
     KIND_SWITCH(ctx->kind, (k_bicg_pass3<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl, ctx->d_hist,
                                                                         ctx->opt_jacobi, kc, ctx->red)));
-    ctx->launches++;
+    post_launch(ctx, KID_BICG_PASS3);
     return POISSON_OK;
 }
 

@@ -103,8 +103,7 @@ __global__ void __launch_bounds__(512)
 template <typename T>
 static int restrict_t(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T* r, T* fc, int restriction) {
     dim3 b(32, 8), g((coarse.n[0] + 31) / 32, (coarse.n[1] + 7) / 8, coarse.n[2]);
-    k_restrict<T><<<g, b, 0, ctx->stream>>>(fine, coarse, r, fc, restriction);
-    ctx->launches++;
+    PB_LAUNCH(ctx, KID_MG_RESTRICT, (k_restrict<T><<<g, b, 0, ctx->stream>>>(fine, coarse, r, fc, restriction)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -118,8 +117,7 @@ int launch_restrict32(poisson_ctx* ctx, const Op& f, const Op& c, const float* r
 template <typename T>
 static int prolong_t(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T* ec, T* phi) {
     dim3 b(64, 4), g((fine.n[0] + 63) / 64, (fine.n[1] + 3) / 4, fine.n[2]);
-    k_prolong_add<T><<<g, b, 0, ctx->stream>>>(fine, coarse, ec, phi);
-    ctx->launches++;
+    PB_LAUNCH(ctx, KID_MG_PROLONG, (k_prolong_add<T><<<g, b, 0, ctx->stream>>>(fine, coarse, ec, phi)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -133,8 +131,7 @@ int launch_prolong_add32(poisson_ctx* ctx, const Op& f, const Op& c, const float
 int launch_add32to64(poisson_ctx* ctx, size_t n, const float* e, double* phi) {
     size_t blocks = (n + 2047) / 2048;
     if (blocks > (size_t)ctx->num_sms * 16) blocks = (size_t)ctx->num_sms * 16;
-    k_add32to64<<<(int)blocks, 256, 0, ctx->stream>>>(n, e, phi);
-    ctx->launches++;
+    PB_LAUNCH(ctx, KID_MG_AXPY, (k_add32to64<<<(int)blocks, 256, 0, ctx->stream>>>(n, e, phi)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -146,8 +143,7 @@ static int coarse_t(poisson_ctx* ctx, const Op& op, T* phi, const T* rhs, T omeg
     if (bytes > 200 * 1024) return POISSON_UNSUPPORTED;  // caller falls back to per-colour launches
     if (bytes > 48 * 1024)
         PB_CUDA_OK(cudaFuncSetAttribute(k_coarse_solve<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    k_coarse_solve<T><<<1, 512, bytes, ctx->stream>>>(op, phi, rhs, omega, nsweeps);
-    ctx->launches++;
+    PB_LAUNCH(ctx, KID_MG_COARSE, (k_coarse_solve<T><<<1, 512, bytes, ctx->stream>>>(op, phi, rhs, omega, nsweeps)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }

@@ -229,11 +229,13 @@ static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho,
 }
 
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
+    if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     init_norm();
     const MpGeom g = make_geom(ctx);
     int blocks = ctx->num_sms * 2;
     const size_t maxb = (ctx->npts + 255) / 256;
     if ((size_t)blocks > maxb) blocks = (int)maxb;
+    pre_launch(ctx, KID_MP_MOMENTS);
     switch (lmax) {
         case 0: moments_launch<0>(ctx, g, rho, d_q, blocks); break;
         case 1: moments_launch<1>(ctx, g, rho, d_q, blocks); break;
@@ -244,9 +246,9 @@ int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
         case 6: moments_launch<6>(ctx, g, rho, d_q, blocks); break;
         case 7: moments_launch<7>(ctx, g, rho, d_q, blocks); break;
         case 8: moments_launch<8>(ctx, g, rho, d_q, blocks); break;
-        default: return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
+        default: break;  // range checked by the caller
     }
-    ctx->launches++;
+    post_launch(ctx, KID_MP_MOMENTS);
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -258,8 +260,8 @@ int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, double G, int lmax) {
         if (ctx->op.bc[f] != POISSON_BC_DIRICHLET_GHOST || !ctx->d_ghost[f]) continue;
         if (g.sph && f != 1) continue;  // only the outer radial shell carries Eq. 19
         const long len = ctx->face_len[f];
-        k_ghost_eval<<<(int)((len + 255) / 256), 256, 0, ctx->stream>>>(g, f, ctx->op.R, d_q, G, lmax, ctx->d_ghost[f]);
-        ctx->launches++;
+        PB_LAUNCH(ctx, KID_MP_GHOSTS, (k_ghost_eval<<<(int)((len + 255) / 256), 256, 0, ctx->stream>>>(
+                                          g, f, ctx->op.R, d_q, G, lmax, ctx->d_ghost[f])));
     }
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;

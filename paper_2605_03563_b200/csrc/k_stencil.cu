@@ -77,13 +77,14 @@ static int apply_dispatch(poisson_ctx* ctx, const Op& op, const T* v, const T* r
     const dim3 g = grid_for(op, kc, false), b(BX, BY);
     if ((size_t)g.x * g.y * g.z > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");
     cudaStream_t s = ctx->stream;
+    pre_launch(ctx, KID_APPLY);
     if (mode == 0)
         k_apply<T, KIND, 0, false><<<g, b, 0, s>>>(op, v, rhs, out, out32, ug, kc, ctx->red, ctx->d_scal);
     else if (!reduce)
         k_apply<T, KIND, 1, false><<<g, b, 0, s>>>(op, v, rhs, out, out32, ug, kc, ctx->red, ctx->d_scal);
     else
         k_apply<T, KIND, 1, true><<<g, b, 0, s>>>(op, v, rhs, out, out32, ug, kc, ctx->red, ctx->d_scal);
-    ctx->launches++;
+    post_launch(ctx, KID_APPLY);
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -111,8 +112,7 @@ static int rbsor_dispatch(poisson_ctx* ctx, const Op& op, T* phi, const T* rhs, 
     const dim3 g = grid_for(op, kc, true), b(BX, BY);
     for (int s = 0; s < nsweeps; ++s)
         for (int colour = 0; colour < 2; ++colour) {
-            k_rbsor_half<T, KIND><<<g, b, 0, ctx->stream>>>(op, phi, rhs, omega, colour, ug, kc);
-            ctx->launches++;
+            PB_LAUNCH(ctx, KID_RBSOR, (k_rbsor_half<T, KIND><<<g, b, 0, ctx->stream>>>(op, phi, rhs, omega, colour, ug, kc)));
         }
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
