@@ -165,6 +165,16 @@ int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double
 int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double* s, const double* t,
                       const double* r0, double* r);
 
+// Plane-pipeline versions (k_plane.cu) for pair-aligned grids; same results, bit for bit
+int plane_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out,
+                float* out32, int mode, bool ug, bool reduce);
+int plane_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, double* r, double* r0hat);
+int plane_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x);
+int plane_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, const double* v_old, const double* r0,
+                     double* p_new, double* v_new);
+int plane_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t);
+bool plane_ok(const poisson_ctx* ctx, const Op& op);
+
 // Multigrid transfer
 int launch_restrict(poisson_ctx* ctx, const Op& fine, const Op& coarse, const double* r, double* fc, int restriction);
 int launch_restrict32(poisson_ctx* ctx, const Op& fine, const Op& coarse, const float* r, float* fc, int restriction);

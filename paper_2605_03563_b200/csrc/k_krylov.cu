@@ -311,6 +311,7 @@ static int stream_blocks(poisson_ctx* ctx, size_t n) {
 
 int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, double* r, bool bicg, double* r0hat) {
     const Op& op = ctx->op;
+    if (plane_ok(ctx, op)) return plane_krylov_init(ctx, x, rhs, r, bicg ? r0hat : nullptr);
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
     pre_launch(ctx, KID_KRYLOV_INIT);
@@ -323,6 +324,7 @@ int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, dou
 
 int launch_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x) {
     const Op& op = ctx->op;
+    if (plane_ok(ctx, op)) return plane_cg_passA(ctx, r, p_old, p_new, q, x);
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
     pre_launch(ctx, KID_CG_PASS_A);
@@ -357,6 +359,7 @@ int launch_sub_mean(poisson_ctx* ctx, double* x) {
 int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, const double* v_old, const double* r0,
                       double* p_new, double* v_new) {
     const Op& op = ctx->op;
+    if (plane_ok(ctx, op)) return plane_bicg_pass1(ctx, r, p_old, v_old, r0, p_new, v_new);
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
     pre_launch(ctx, KID_BICG_PASS1);
@@ -368,6 +371,7 @@ int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, co
 
 int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t) {
     const Op& op = ctx->op;
+    if (plane_ok(ctx, op)) return plane_bicg_pass2(ctx, r, v, s, t);
     const int kc = pick_kc(op, ctx->num_sms);
     const dim3 g = grid_for(op, kc), b(BX, BY);
     pre_launch(ctx, KID_BICG_PASS2);

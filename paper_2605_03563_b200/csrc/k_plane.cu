@@ -1,0 +1,345 @@
+// k_plane.cu — instances of the plane-pipeline engine (plane.cuh) for large, pair-aligned grids:
+//   stencil apply / residual / residual norm
+//   initial Krylov residual
+//   CG pass A       x += alpha p_old ; p = r + beta p_old ; q = L p ; sum p.q
+//   BiCGSTAB pass 1 p = r + beta (p - omega v) ; v = L D^-1 p ; sum r0^.v
+//   BiCGSTAB pass 2 s = r - alpha v ; t = L D^-1 s ; sum t.s, t.t
+// Same arithmetic, same order as the generic kernels (k_stencil.cu, k_krylov.cu); only the data movement differs.
+#include "plane.cuh"
+
+namespace pb {
+
+// ---- loaders ------------------------------------------------------------------------------------------------------------
+struct LdArr {  // v itself
+    const double* v;
+    struct Raw {
+        double2 a;
+    };
+    __device__ __forceinline__ void prepare() {}
+    __device__ __forceinline__ Raw load(size_t p) const { return Raw{ld2(v + p)}; }
+    __device__ __forceinline__ double2 form(const Op&, const Raw& r, int, int, int) const { return r.a; }
+    __device__ __forceinline__ double at(const Op&, size_t p, int, int, int) const { return v[p]; }
+};
+
+struct LdPnew {  // p_new = (r - mu) + beta p_old
+    const double* r;
+    const double* p;
+    const KrylovCtl* ctl;
+    double beta, mu;
+    struct Raw {
+        double2 r, p;
+    };
+    __device__ __forceinline__ void prepare() {
+        beta = ctl->beta;
+        mu = ctl->mu;
+    }
+    __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q)}; }
+    __device__ __forceinline__ double2 form(const Op&, const Raw& w, int, int, int) const {
+        return mk2(fma(beta, w.p.x, w.r.x - mu), fma(beta, w.p.y, w.r.y - mu));
+    }
+    __device__ __forceinline__ double at(const Op&, size_t q, int, int, int) const {
+        return fma(beta, p[q], r[q] - mu);
+    }
+};
+
+template <int KIND>
+__device__ __forceinline__ double jac_(const Op& op, int i, int j, int k, int jacobi) {
+    return jacobi ? -row_diag<double, KIND>(op, i, j, k) : 1.0;
+}
+
+template <int KIND>
+struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D
+    const double* r;
+    const double* p;
+    const double* v;
+    const KrylovCtl* ctl;
+    int jacobi;
+    double beta, omega;
+    struct Raw {
+        double2 r, p, v;
+    };
+    __device__ __forceinline__ void prepare() {
+        beta = ctl->beta;
+        omega = ctl->omega;
+    }
+    __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q), ld2(v + q)}; }
+    __device__ __forceinline__ double2 form(const Op& op, const Raw& w, int i, int j, int k) const {
+        return mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
+                   fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y) / jac_<KIND>(op, i + 1, j, k, jacobi));
+    }
+    __device__ __forceinline__ double at(const Op& op, size_t q, int i, int j, int k) const {
+        return fma(beta, fma(-omega, v[q], p[q]), r[q]) / jac_<KIND>(op, i, j, k, jacobi);
+    }
+};
+
+template <int KIND>
+struct LdShat {  // s^ = (r - alpha v) / D
+    const double* r;
+    const double* v;
+    const KrylovCtl* ctl;
+    int jacobi;
+    double alpha;
+    struct Raw {
+        double2 r, v;
+    };
+    __device__ __forceinline__ void prepare() { alpha = ctl->alpha; }
+    __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(v + q)}; }
+    __device__ __forceinline__ double2 form(const Op& op, const Raw& w, int i, int j, int k) const {
+        return mk2(fma(-alpha, w.v.x, w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
+                   fma(-alpha, w.v.y, w.r.y) / jac_<KIND>(op, i + 1, j, k, jacobi));
+    }
+    __device__ __forceinline__ double at(const Op& op, size_t q, int i, int j, int k) const {
+        return fma(-alpha, v[q], r[q]) / jac_<KIND>(op, i, j, k, jacobi);
+    }
+};
+
+// ---- epilogues ----------------------------------------------------------------------------------------------------------
+// out = L v (MODE 0) or rhs - L v (MODE 1); optional fp32 copy; optional sum(out^2), sum(out) -> scal[0..1]
+template <int MODE, bool RED>
+struct EpApply {
+    static constexpr int NRED = RED ? 2 : 0;
+    const double* rhs;
+    double* out;
+    float* out32;
+    double* scal;
+    struct Raw {
+        double2 f;
+    };
+    __device__ __forceinline__ bool skip() const { return false; }
+    __device__ __forceinline__ void prepare() {}
+    __device__ __forceinline__ Raw load(size_t p) const {
+        Raw w;
+        if (MODE) w.f = ld2(rhs + p);
+        return w;
+    }
+    __device__ __forceinline__ void apply(const Raw& w, size_t p, int, int, int, double2, double2 lv,
+                                          double* acc) const {
+        double2 o = lv;
+        if (MODE) o = mk2(w.f.x - lv.x, w.f.y - lv.y);
+        if (out) st2(out + p, o);
+        if (out32) *reinterpret_cast<float2*>(out32 + p) = make_float2((float)o.x, (float)o.y);
+        if (RED) {
+            acc[0] = fma(o.x, o.x, acc[0]);
+            acc[1] += o.x;
+            acc[0] = fma(o.y, o.y, acc[0]);
+            acc[1] += o.y;
+        }
+    }
+    __device__ __forceinline__ void finish(const double* t) const {
+        scal[0] = t[0];
+        scal[1] = t[1];
+    }
+};
+
+struct EpInit {  // r = rhs - L x (ghosts included); r0^ = r; first scalars of the Krylov recurrences
+    static constexpr int NRED = 2;
+    const double* rhs;
+    double* r;
+    double* r0hat;
+    KrylovCtl* ctl;
+    double* hist;
+    struct Raw {
+        double2 f;
+    };
+    __device__ __forceinline__ bool skip() const { return false; }
+    __device__ __forceinline__ void prepare() {}
+    __device__ __forceinline__ Raw load(size_t p) const { return Raw{ld2(rhs + p)}; }
+    __device__ __forceinline__ void apply(const Raw& w, size_t p, int, int, int, double2, double2 lv,
+                                          double* acc) const {
+        const double2 o = mk2(w.f.x - lv.x, w.f.y - lv.y);
+        st2(r + p, o);
+        if (r0hat) st2(r0hat + p, o);
+        acc[0] = fma(o.x, o.x, acc[0]);
+        acc[1] += o.x;
+        acc[0] = fma(o.y, o.y, acc[0]);
+        acc[1] += o.y;
+    }
+    __device__ __forceinline__ void finish(const double* t) const {
+        const double mu = ctl->project ? t[1] / ctl->npoints : 0.0;
+        const double rr = ctl->project ? fma(-ctl->npoints * mu, mu, t[0]) : t[0];
+        ctl->mu = mu;
+        ctl->rr = rr;
+        ctl->rr0 = rr;
+        ctl->rho = rr;
+        ctl->alpha = 0.0;
+        ctl->beta = 0.0;
+        ctl->omega = 0.0;
+        ctl->it = 0;
+        const int trivially_done = (!ctl->fixed && !(rr > 0.0)) ? 1 : 0;
+        ctl->done = trivially_done;
+        ctl->status = (ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED;
+        if (ctl->record && hist) hist[0] = 1.0;
+    }
+};
+
+struct EpCgA {
+    static constexpr int NRED = 1;
+    const double* p_old;
+    double* p_new;
+    double* q;
+    double* x;
+    KrylovCtl* ctl;
+    double alpha_prev;
+    struct Raw {
+        double2 x, p;
+    };
+    __device__ __forceinline__ bool skip() const { return ctl->done != 0; }
+    __device__ __forceinline__ void prepare() { alpha_prev = ctl->alpha; }
+    __device__ __forceinline__ Raw load(size_t m) const { return Raw{ld2(x + m), ld2(p_old + m)}; }
+    __device__ __forceinline__ void apply(const Raw& w, size_t m, int, int, int, double2 pn, double2 lv,
+                                          double* acc) const {
+        st2(x + m, mk2(fma(alpha_prev, w.p.x, w.x.x), fma(alpha_prev, w.p.y, w.x.y)));  // deferred x-update
+        st2(p_new + m, pn);
+        st2(q + m, lv);
+        acc[0] = fma(pn.x, lv.x, acc[0]);
+        acc[0] = fma(pn.y, lv.y, acc[0]);
+    }
+    __device__ __forceinline__ void finish(const double* t) const {
+        ctl->pq = t[0];
+        ctl->alpha = ctl->rr / t[0];
+    }
+};
+
+struct EpBicg1 {
+    static constexpr int NRED = 1;
+    const double* r;
+    const double* p_old;
+    const double* v_old;
+    const double* r0;
+    double* p_new;
+    double* v_new;
+    KrylovCtl* ctl;
+    double beta, omega;
+    struct Raw {
+        double2 r, p, v, r0;
+    };
+    __device__ __forceinline__ bool skip() const { return ctl->done != 0; }
+    __device__ __forceinline__ void prepare() {
+        beta = ctl->beta;
+        omega = ctl->omega;
+    }
+    __device__ __forceinline__ Raw load(size_t m) const {
+        return Raw{ld2(r + m), ld2(p_old + m), ld2(v_old + m), ld2(r0 + m)};
+    }
+    __device__ __forceinline__ void apply(const Raw& w, size_t m, int, int, int, double2, double2 lv,
+                                          double* acc) const {
+        st2(p_new + m, mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x), fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y)));
+        st2(v_new + m, lv);
+        acc[0] = fma(w.r0.x, lv.x, acc[0]);
+        acc[0] = fma(w.r0.y, lv.y, acc[0]);
+    }
+    __device__ __forceinline__ void finish(const double* t) const {
+        const double r0v = t[0];
+        ctl->r0v = r0v;
+        if (!(fabs(r0v) > 0.0) || !isfinite(r0v) || !(fabs(ctl->rho) > 0.0)) {
+            ctl->status = POISSON_BREAKDOWN;
+            ctl->done = 1;
+        } else {
+            ctl->alpha = ctl->rho / r0v;
+        }
+    }
+};
+
+struct EpBicg2 {
+    static constexpr int NRED = 2;
+    const double* r;
+    const double* v;
+    double* s;
+    double* t;
+    KrylovCtl* ctl;
+    double alpha;
+    struct Raw {
+        double2 r, v;
+    };
+    __device__ __forceinline__ bool skip() const { return ctl->done != 0; }
+    __device__ __forceinline__ void prepare() { alpha = ctl->alpha; }
+    __device__ __forceinline__ Raw load(size_t m) const { return Raw{ld2(r + m), ld2(v + m)}; }
+    __device__ __forceinline__ void apply(const Raw& w, size_t m, int, int, int, double2, double2 lv,
+                                          double* acc) const {
+        const double2 sv = mk2(fma(-alpha, w.v.x, w.r.x), fma(-alpha, w.v.y, w.r.y));
+        st2(s + m, sv);
+        st2(t + m, lv);
+        acc[0] = fma(lv.x, sv.x, acc[0]);
+        acc[1] = fma(lv.x, lv.x, acc[1]);
+        acc[0] = fma(lv.y, sv.y, acc[0]);
+        acc[1] = fma(lv.y, lv.y, acc[1]);
+    }
+    __device__ __forceinline__ void finish(const double* tot) const {
+        ctl->ts = tot[0];
+        ctl->tt = tot[1];
+        if (!(tot[1] > 0.0) || !isfinite(tot[1])) {
+            ctl->status = POISSON_BREAKDOWN;
+            ctl->done = 1;
+        } else {
+            ctl->omega = tot[0] / tot[1];
+        }
+    }
+};
+
+#define KIND_SWITCH(kind, CALL)                                         \
+    switch (kind) {                                                     \
+        case KIND_CART2: { constexpr int K = KIND_CART2; CALL; } break; \
+        case KIND_CART6: { constexpr int K = KIND_CART6; CALL; } break; \
+        default:         { constexpr int K = KIND_SPH;   CALL; } break; \
+    }
+
+template <int KIND>
+static int apply_k(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32,
+                   int mode, bool ug, bool reduce) {
+    const LdArr ld{v};
+    int rc;
+    if (mode == 0)
+        rc = launch_plane<KIND>(ctx, op, ld, EpApply<0, false>{rhs, out, out32, ctx->d_scal}, ug, KID_APPLY);
+    else if (!reduce)
+        rc = launch_plane<KIND>(ctx, op, ld, EpApply<1, false>{rhs, out, out32, ctx->d_scal}, ug, KID_APPLY);
+    else
+        rc = launch_plane<KIND>(ctx, op, ld, EpApply<1, true>{rhs, out, out32, ctx->d_scal}, ug, KID_APPLY);
+    if (rc != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+bool plane_ok(const poisson_ctx* ctx, const Op& op) { return plane_eligible(ctx, op); }
+
+int plane_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out,
+                float* out32, int mode, bool ug, bool reduce) {
+    int rc = POISSON_OK;
+    KIND_SWITCH(kind, rc = apply_k<K>(ctx, op, v, rhs, out, out32, mode, ug, reduce));
+    return rc;
+}
+
+int plane_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, double* r, double* r0hat) {
+    int rc = POISSON_OK;
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdArr{x}, EpInit{rhs, r, r0hat, ctx->d_ctl, ctx->d_hist},
+                                                true, KID_KRYLOV_INIT));
+    if (rc != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+int plane_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x) {
+    int rc = POISSON_OK;
+    const LdPnew ld{r, p_old, ctx->d_ctl, 0.0, 0.0};
+    const EpCgA ep{p_old, p_new, q, x, ctx->d_ctl, 0.0};
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, ld, ep, false, KID_CG_PASS_A));
+    return rc;
+}
+
+int plane_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, const double* v_old, const double* r0,
+                     double* p_new, double* v_new) {
+    int rc = POISSON_OK;
+    const EpBicg1 ep{r, p_old, v_old, r0, p_new, v_new, ctx->d_ctl, 0.0, 0.0};
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdPhat<K>{r, p_old, v_old, ctx->d_ctl, ctx->opt_jacobi, 0.0, 0.0},
+                                                ep, false, KID_BICG_PASS1));
+    return rc;
+}
+
+int plane_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t) {
+    int rc = POISSON_OK;
+    const EpBicg2 ep{r, v, s, t, ctx->d_ctl, 0.0};
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdShat<K>{r, v, ctx->d_ctl, ctx->opt_jacobi, 0.0}, ep, false,
+                                                KID_BICG_PASS2));
+    return rc;
+}
+
+}  // namespace pb

@@ -91,6 +91,7 @@ static int apply_dispatch(poisson_ctx* ctx, const Op& op, const T* v, const T* r
 
 int launch_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out, int mode,
                  bool ug, bool reduce) {
+    if (plane_ok(ctx, op)) return plane_apply(ctx, op, kind, v, rhs, out, nullptr, mode, ug, reduce);
     switch (kind) {
         case KIND_CART2: return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
         case KIND_CART6: return apply_dispatch<double, KIND_CART6>(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
@@ -103,6 +104,7 @@ int launch_apply32(poisson_ctx* ctx, const Op& op, const float* v, const float* 
 }
 
 int launch_residual_to32(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, float* out32, bool ug) {
+    if (plane_ok(ctx, op)) return plane_apply(ctx, op, KIND_CART2, v, rhs, nullptr, out32, 1, ug, true);
     return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
 }
 

@@ -1,0 +1,391 @@
+// plane.cuh — the plane-pipeline stencil engine (2.5-D blocking).  One template serves every pass whose core is
+// "form a vector v point by point, take out = L_h v, then a pointwise epilogue with fused dot products":
+// stencil apply / residual, the CG pass {p-update + matvec + p.Ap} and the two BiCGSTAB matvec
+// passes.
+//
+// Geometry: a CTA owns an xy tile of TX x TY = 128 x 16 points and marches a chunk of z planes.  Threads are
+// 64 x 8; each owns two x-adjacent points (one 16-byte access) in two adjacent rows.  The formed vector v lives in
+// a shared-memory ring of 2R+2 planes, each (TY+2R) x (TX+2HX) with its xy halo (R = stencil radius, HX = halo
+// rounded up to whole 16-byte pairs), so v is formed ONCE per point per pass (halo points once more by the
+// neighbouring CTA) and all 6R neighbours of a point come from shared memory.  Loads for plane k+R+1 are issued a
+// full iteration before they are consumed (software pipelining through registers), one __syncthreads per plane.
+// Out-of-range neighbours follow include/poisson.h: periodic wrap, ghost-face values, or zero.
+// Arithmetic order is the canonical one of stencil.cuh, so results are bit-identical to the generic kernels.
+#pragma once
+#include "stencil.cuh"
+
+namespace pb {
+
+__device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
+__device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
+
+template <int KIND>
+struct PlaneGeom {
+    static constexpr int R = (KIND == KIND_CART6) ? 3 : 1;
+    static constexpr int HX = (R == 1) ? 2 : 4;
+    static constexpr int TX = 128, TY = 16;
+    static constexpr int NTX = TX / 2, NTY = TY / 2, NT = NTX * NTY;
+    static constexpr int SW = TX + 2 * HX, SH = TY + 2 * R;
+    static constexpr int NS = 2 * R + 2;
+    static constexpr int SLOT = SH * SW;
+    static constexpr size_t SMEM = (size_t)NS * SLOT * sizeof(double);
+};
+
+// Value of the loader's vector at (i,j,k) when at most one index is out of range (slow path: boundary cells only).
+// Edge and corner ghosts are never read by a star stencil and come back as zero.
+template <class Ld>
+__device__ double vpoint(const Op& op, const Ld& ld, int i, int j, int k, bool ug) {
+    int id[3] = {i, j, k};
+    int bad = -1, nbad = 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        if (id[a] < 0 || id[a] >= op.n[a]) {
+            bad = a;
+            ++nbad;
+        }
+    if (nbad == 0) return ld.at(op, gidx(op, i, j, k), i, j, k);
+    if (nbad > 1) return 0.0;
+    const int n = op.n[bad], q = id[bad];
+    const int f = 2 * bad + (q < 0 ? 0 : 1), bc = op.bc[f];
+    if (bc == POISSON_BC_PERIODIC) {
+        id[bad] = ((q % n) + n) % n;
+        return ld.at(op, gidx(op, id[0], id[1], id[2]), id[0], id[1], id[2]);
+    }
+    if (bc == POISSON_BC_DIRICHLET_GHOST && ug && op.ghost[f] != nullptr) {
+        const int layer = q < 0 ? (-1 - q) : (q - n);
+        if (layer >= op.R) return 0.0;
+        const int a1 = (bad == 0) ? 1 : 0, a2 = (bad == 2) ? 1 : 2;
+        return op.ghost[f][((size_t)layer * op.n[a2] + id[a2]) * op.n[a1] + id[a1]];
+    }
+    return 0.0;
+}
+
+// Per-thread coefficients of the operator rows it owns.
+template <int KIND>
+struct RowCoef {};
+template <>
+struct RowCoef<KIND_CART2> {
+    double c0, c1, c2, d;
+    bool plain;
+};
+template <>
+struct RowCoef<KIND_CART6> {
+    double c0, c1, c2, d;
+};
+template <>
+struct RowCoef<KIND_SPH> {
+    double arm[2], arp[2], ir2[2], dr[2];  // per own column
+    double atm[2], atp[2], cp[2], dt[2];   // per own row
+};
+
+// Loader / epilogue concepts (see k_plane.cu for the instances):
+//   struct Ld { struct Raw; void prepare(); Raw load(size_t p) const;
+//               double2 form(const Op&, const Raw&, int i, int j, int k) const;   (pair starting at column i)
+//               double at(const Op&, size_t p, int i, int j, int k) const; };
+//   struct Ep { static constexpr int NRED; struct Raw; bool skip() const; void prepare(); Raw load(size_t p) const;
+//               void apply(const Raw&, size_t p, int i, int j, int k, double2 v, double2 lv, double* acc) const;
+//               void finish(const double* totals) const; };
+template <int KIND, class Ld, class Ep>
+__global__ void __launch_bounds__(512, 1)
+    k_plane(const Op op, const Ld ld_in, const Ep ep_in, const int kc, const bool ug_in, RedBuf rb) {
+    using G = PlaneGeom<KIND>;
+    constexpr int R = G::R, HX = G::HX, TX = G::TX, TY = G::TY, SW = G::SW, NS = G::NS, SLOT = G::SLOT;
+    extern __shared__ __align__(16) double ring[];
+    if (ep_in.skip()) return;
+    Ld ld = ld_in;  // the functors fetch their device-resident scalars (alpha, beta, ...) once
+    Ep ep = ep_in;
+    ld.prepare();
+    ep.prepare();
+    const bool ug = ug_in && op.gamma == 0.0;
+    const int n0 = op.n[0], n1 = op.n[1], n2 = op.n[2];
+    const int lx = threadIdx.x, ty = threadIdx.y, tid = ty * G::NTX + lx;
+    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+    const int k0 = blockIdx.z * kc, k1 = min(n2, k0 + kc);
+    const int i = i0 + 2 * lx;
+    const int jr[2] = {j0 + 2 * ty, j0 + 2 * ty + 1};
+    const bool act[2] = {i < n0 && jr[0] < n1, i < n0 && jr[1] < n1};
+    const size_t plane = (size_t)n0 * n1;
+    const size_t base[2] = {(size_t)jr[0] * n0 + i, (size_t)jr[1] * n0 + i};
+    const int so[2] = {(R + 2 * ty) * SW + HX + 2 * lx, (R + 2 * ty + 1) * SW + HX + 2 * lx};
+    const bool per_z = op.bc[4] == POISSON_BC_PERIODIC;
+
+    // ---- this thread's halo pair (at most one) -----------------------------------------------------------------
+    int hcls = 0, hi = 0, hj = 0, hso = 0;  // class 0 none, 1 plain load at wrapped (hwi,hwj), 2 boundary values
+    int hwi = 0, hwj = 0;
+    if (tid < 2 * R * G::NTX) {
+        const int rr = tid / G::NTX, c = tid % G::NTX;
+        const int srow = rr < R ? rr : TY + rr;
+        hj = j0 - R + srow;
+        hi = i0 + 2 * c;
+        hso = srow * SW + HX + 2 * c;
+        hcls = 1;
+    } else if (tid - 2 * R * G::NTX < TY * HX) {
+        const int t = tid - 2 * R * G::NTX, row = t / HX, c = t % HX;
+        const int pc = c < HX / 2 ? c : (TX / 2 + c);
+        hj = j0 + row;
+        hi = i0 - HX + 2 * pc;
+        hso = (R + row) * SW + 2 * pc;
+        hcls = 1;
+    }
+    if (hcls) {
+        const bool ox = hi < 0 || hi >= n0, oy = hj < 0 || hj >= n1;
+        hwi = hi;
+        hwj = hj;
+        if (ox && oy) {
+            hcls = 0;
+        } else if (ox) {
+            if (op.bc[0] == POISSON_BC_PERIODIC && n0 >= HX) hwi = ((hi % n0) + n0) % n0; else hcls = 2;
+        } else if (oy) {
+            if (op.bc[2] == POISSON_BC_PERIODIC) hwj = ((hj % n1) + n1) % n1; else hcls = 2;
+        }
+    }
+    const size_t hbase = (size_t)hwj * n0 + hwi;
+
+    // ---- operator coefficients of the owned rows ----------------------------------------------------------------
+    RowCoef<KIND> rc;
+    if constexpr (KIND == KIND_SPH) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int ii = min(i + e, n0 - 1), jj = min(jr[e], n1 - 1);
+            rc.arm[e] = op.ar_m[ii];
+            rc.arp[e] = op.ar_p[ii];
+            rc.ir2[e] = op.ir2[ii];
+            rc.dr[e] = op.dr[ii];
+            rc.atm[e] = op.at_m[jj];
+            rc.atp[e] = op.at_p[jj];
+            rc.cp[e] = op.cp[jj];
+            rc.dt[e] = op.dt[jj];
+        }
+    } else {
+        rc.c0 = op.c[0];
+        rc.c1 = op.c[1];
+        rc.c2 = op.c[2];
+        if constexpr (KIND == KIND_CART6) {
+            rc.d = (49.0 / 18.0) * ((rc.c0 + rc.c1) + rc.c2);
+        } else {
+            rc.d = 2.0 * ((rc.c0 + rc.c1) + rc.c2);
+            bool neumann = false;
+#pragma unroll
+            for (int f = 0; f < 6; ++f) neumann |= op.bc[f] == POISSON_BC_NEUMANN0;
+            rc.plain = !neumann && op.gamma == 0.0;
+        }
+    }
+
+    // ---- plane staging --------------------------------------------------------------------------------------------
+    struct Staged {
+        typename Ld::Raw o[2], h;
+        int kw;       // wrapped plane index, or -1 when the plane lies outside a non-periodic z face
+    };
+    auto issue = [&](int kk) -> Staged {
+        Staged s;
+        s.kw = kk;
+        if (kk < 0 || kk >= n2) s.kw = per_z ? ((kk % n2) + n2) % n2 : -1;
+        if (s.kw >= 0) {
+            const size_t off = (size_t)s.kw * plane;
+            if (act[0]) s.o[0] = ld.load(off + base[0]);
+            if (act[1]) s.o[1] = ld.load(off + base[1]);
+            if (hcls == 1) s.h = ld.load(off + hbase);
+        }
+        return s;
+    };
+    auto commit = [&](int kk, const Staged& s) {
+        double* slot = ring + ((kk + 2 * NS) % NS) * SLOT;
+        if (s.kw >= 0) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                if (act[r])
+                    st2(slot + so[r], ld.form(op, s.o[r], i, jr[r], s.kw));
+                else
+                    st2(slot + so[r], mk2(vpoint(op, ld, i, jr[r], s.kw, ug), vpoint(op, ld, i + 1, jr[r], s.kw, ug)));
+            }
+            if (hcls == 1)
+                st2(slot + hso, ld.form(op, s.h, hwi, hwj, s.kw));
+            else if (hcls == 2)
+                st2(slot + hso, mk2(vpoint(op, ld, hi, hj, s.kw, ug), vpoint(op, ld, hi + 1, hj, s.kw, ug)));
+        } else {
+            // plane beyond a non-periodic z face: ghost values or zeros; only owned columns are ever read
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+                st2(slot + so[r], mk2(vpoint(op, ld, i, jr[r], kk, ug), vpoint(op, ld, i + 1, jr[r], kk, ug)));
+        }
+    };
+
+    // prologue: planes k0-R .. k0+R-1, two at a time
+    for (int kk = k0 - R; kk < k0 + R; kk += 2) {
+        const Staged a = issue(kk), b = issue(kk + 1);
+        commit(kk, a);
+        commit(kk + 1, b);
+    }
+    Staged nxt = issue(k0 + R);
+    typename Ep::Raw enxt[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+        if (act[r]) enxt[r] = ep.load((size_t)k0 * plane + base[r]);
+
+    double acc[Ep::NRED > 0 ? Ep::NRED : 1];
+#pragma unroll
+    for (int r = 0; r < (Ep::NRED > 0 ? Ep::NRED : 1); ++r) acc[r] = 0.0;
+
+    for (int k = k0; k < k1; ++k) {
+        commit(k + R, nxt);
+        typename Ep::Raw ecur[2] = {enxt[0], enxt[1]};
+        if (k + 1 < k1) {
+            nxt = issue(k + 1 + R);
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+                if (act[r]) enxt[r] = ep.load((size_t)(k + 1) * plane + base[r]);
+        }
+        __syncthreads();
+        const double* c = ring + ((k + 2 * NS) % NS) * SLOT;
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            if (!act[r]) continue;
+            const double* P = c + so[r];
+            const double2 C = ld2(P);
+            double2 lv;
+            if constexpr (KIND == KIND_CART6) {
+                const double2 xa = ld2(P - 4), xb = ld2(P - 2), xc = ld2(P + 2), xd = ld2(P + 4);
+                double2 t0, t1, t2;
+                {
+                    // point i: -1 xb.y, +1 C.y, -2 xb.x, +2 xc.x, -3 xa.y, +3 xc.y ; point i+1: -1 C.x, +1 xc.x, ...
+                    double u = 1.5 * (xb.y + C.y);
+                    u = fma(-3.0 / 20.0, xb.x + xc.x, u);
+                    t0.x = fma(1.0 / 90.0, xa.y + xc.y, u);
+                    u = 1.5 * (C.x + xc.x);
+                    u = fma(-3.0 / 20.0, xb.y + xc.y, u);
+                    t0.y = fma(1.0 / 90.0, xb.x + xd.x, u);
+                }
+                {
+                    const double2 m1 = ld2(P - SW), p1 = ld2(P + SW), m2 = ld2(P - 2 * SW), p2 = ld2(P + 2 * SW),
+                                  m3 = ld2(P - 3 * SW), p3 = ld2(P + 3 * SW);
+                    double u = 1.5 * (m1.x + p1.x);
+                    u = fma(-3.0 / 20.0, m2.x + p2.x, u);
+                    t1.x = fma(1.0 / 90.0, m3.x + p3.x, u);
+                    u = 1.5 * (m1.y + p1.y);
+                    u = fma(-3.0 / 20.0, m2.y + p2.y, u);
+                    t1.y = fma(1.0 / 90.0, m3.y + p3.y, u);
+                }
+                {
+                    const int o = so[r];
+                    const double2 m1 = ld2(ring + ((k - 1 + 2 * NS) % NS) * SLOT + o),
+                                  p1 = ld2(ring + ((k + 1 + 2 * NS) % NS) * SLOT + o),
+                                  m2 = ld2(ring + ((k - 2 + 2 * NS) % NS) * SLOT + o),
+                                  p2 = ld2(ring + ((k + 2 + 2 * NS) % NS) * SLOT + o),
+                                  m3 = ld2(ring + ((k - 3 + 2 * NS) % NS) * SLOT + o),
+                                  p3 = ld2(ring + ((k + 3 + 2 * NS) % NS) * SLOT + o);
+                    double u = 1.5 * (m1.x + p1.x);
+                    u = fma(-3.0 / 20.0, m2.x + p2.x, u);
+                    t2.x = fma(1.0 / 90.0, m3.x + p3.x, u);
+                    u = 1.5 * (m1.y + p1.y);
+                    u = fma(-3.0 / 20.0, m2.y + p2.y, u);
+                    t2.y = fma(1.0 / 90.0, m3.y + p3.y, u);
+                }
+                double s = t0.x * rc.c0;
+                s = fma(t1.x, rc.c1, s);
+                s = fma(t2.x, rc.c2, s);
+                lv.x = fma(-rc.d, C.x, s);
+                s = t0.y * rc.c0;
+                s = fma(t1.y, rc.c1, s);
+                s = fma(t2.y, rc.c2, s);
+                lv.y = fma(-rc.d, C.y, s);
+            } else {
+                const double2 xl = ld2(P - 2), xr = ld2(P + 2);
+                const double2 ym = ld2(P - SW), yp = ld2(P + SW);
+                const int o = so[r];
+                const double2 zm = ld2(ring + ((k - 1 + 2 * NS) % NS) * SLOT + o),
+                              zp = ld2(ring + ((k + 1 + 2 * NS) % NS) * SLOT + o);
+                if constexpr (KIND == KIND_CART2) {
+                    double d0 = rc.d, d1 = rc.d;
+                    if (!rc.plain) {
+                        d0 = row_diag<double, KIND_CART2>(op, i, jr[r], k);
+                        d1 = row_diag<double, KIND_CART2>(op, i + 1, jr[r], k);
+                    }
+                    double s = (xl.y + C.y) * rc.c0;
+                    s = fma(ym.x + yp.x, rc.c1, s);
+                    s = fma(zm.x + zp.x, rc.c2, s);
+                    lv.x = fma(-d0, C.x, s);
+                    s = (C.x + xr.x) * rc.c0;
+                    s = fma(ym.y + yp.y, rc.c1, s);
+                    s = fma(zm.y + zp.y, rc.c2, s);
+                    lv.y = fma(-d1, C.y, s);
+                } else {
+                    // spherical row (stencil.cuh row_offsum / row_diag, KIND_SPH)
+                    double s = rc.arm[0] * xl.y;
+                    s = fma(rc.arp[0], C.y, s);
+                    double t = rc.atm[r] * ym.x;
+                    t = fma(rc.atp[r], yp.x, t);
+                    t = fma(rc.cp[r], zm.x + zp.x, t);
+                    double off = fma(rc.ir2[0], t, s);
+                    lv.x = fma(-fma(rc.ir2[0], rc.dt[r], rc.dr[0]), C.x, off);
+                    s = rc.arm[1] * C.x;
+                    s = fma(rc.arp[1], xr.x, s);
+                    t = rc.atm[r] * ym.y;
+                    t = fma(rc.atp[r], yp.y, t);
+                    t = fma(rc.cp[r], zm.y + zp.y, t);
+                    off = fma(rc.ir2[1], t, s);
+                    lv.y = fma(-fma(rc.ir2[1], rc.dt[r], rc.dr[1]), C.y, off);
+                }
+            }
+            ep.apply(ecur[r], (size_t)k * plane + base[r], i, jr[r], k, C, lv, acc);
+        }
+    }
+    if constexpr (Ep::NRED > 0) {
+        double vals[Ep::NRED];
+#pragma unroll
+        for (int r = 0; r < Ep::NRED; ++r) vals[r] = acc[r];
+        grid_reduce<Ep::NRED>(vals, rb, [&](const double* t) { ep.finish(t); });
+    }
+}
+
+// Number of z chunks: minimise (waves of CTAs) x (planes per chunk + the 2R-plane prologue).
+template <int KIND>
+static inline int plane_chunks(const Op& op, int sms, int* kc_out) {
+    using G = PlaneGeom<KIND>;
+    const long tiles = (long)((op.n[0] + G::TX - 1) / G::TX) * ((op.n[1] + G::TY - 1) / G::TY);
+    int best = 1;
+    double best_cost = 1e300;
+    for (int nz = 1; nz <= op.n[2]; ++nz) {
+        const int kc = (op.n[2] + nz - 1) / nz;
+        if (kc < 4 && nz > 1) break;
+        const int nzz = (op.n[2] + kc - 1) / kc;
+        const long waves = (tiles * nzz + sms - 1) / sms;
+        const double cost = (double)waves * (kc + 2.0 * G::R * 1.5 + 2.0);
+        if (cost < best_cost - 1e-9) {
+            best_cost = cost;
+            best = nzz;
+        }
+    }
+    const int kc = (op.n[2] + best - 1) / best;
+    *kc_out = kc;
+    return (op.n[2] + kc - 1) / kc;
+}
+
+template <int KIND, class Ld, class Ep>
+static int launch_plane(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
+    using G = PlaneGeom<KIND>;
+    auto kern = k_plane<KIND, Ld, Ep>;
+    static bool configured = false;
+    if (!configured) {
+        PB_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
+        configured = true;
+    }
+    int kc = 0;
+    const int nz = plane_chunks<KIND>(op, ctx->num_sms, &kc);
+    const dim3 g((op.n[0] + G::TX - 1) / G::TX, (op.n[1] + G::TY - 1) / G::TY, nz), b(G::NTX, G::NTY);
+    if ((size_t)g.x * g.y * g.z > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large");
+    pre_launch(ctx, kid);
+    kern<<<g, b, G::SMEM, ctx->stream>>>(op, ld, ep, kc, ug, ctx->red);
+    post_launch(ctx, kid);
+    return POISSON_OK;
+}
+
+// The plane engine needs 16-byte aligned pairs: even n0 (every row then starts on a pair boundary).
+static inline bool plane_eligible(const poisson_ctx* ctx, const Op& op) {
+    if (ctx->opt_path == 1) return false;
+    if (op.n[0] % 2 != 0) return false;
+    if (ctx->opt_path == 2) return true;
+    return op.n[0] >= 64 && (size_t)op.n[0] * op.n[1] * op.n[2] >= (size_t)1 << 19;
+}
+
+}  // namespace pb

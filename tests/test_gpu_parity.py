@@ -18,7 +18,7 @@ from paper_2605_03563_b200 import workloads as wl
 pytestmark = pytest.mark.gpu
 D6 = (po.BC_DIRICHLET_GHOST,) * 6
 P6 = (po.BC_PERIODIC,) * 6
-PATHS = [pb.PATH_GENERIC, pb.PATH_AUTO]
+PATHS = [pb.PATH_GENERIC, pb.PATH_PLANE]
 
 
 def _random_faces(o, seed, R=1):
@@ -172,15 +172,18 @@ def test_config2_cg_fixed_and_converged(path, n):
     assert rel_l2(phi_g, w["exact"]) < {32: 2e-3, 64: 5e-4}[n]
 
 
-def _oracle_rounding_sensitivity(w, o, fixed):
-    """||x(rhs) - x(rhs + 1 ulp noise)|| / ||x|| of the oracle's own CG after `fixed` iterations (C8:
-    the band-limited config-4 right-hand side makes the CG polynomial grow on the unexcited high modes, so
-    rounding-level input differences are amplified long before convergence)."""
+def _oracle_rounding_sensitivity(w, o, fixed, solver="cg"):
+    """||x(rhs) - x(rhs + 1 ulp noise)|| / ||x|| of the oracle's own Krylov solver after `fixed` iterations, and the
+    same for its residual history (C8: the band-limited config-4 right-hand side makes the CG polynomial
+    grow on the unexcited high modes, and BiCGSTAB on the config-5 operator is erratic, so rounding-level input
+    differences are amplified long before convergence)."""
+    run = getattr(o, solver)
     x1, x2 = np.zeros_like(w["rhs"]), np.zeros_like(w["rhs"])
-    o.cg(x1, w["rhs"], fixed_iters=fixed)
+    h1 = np.array(run(x1, w["rhs"], fixed_iters=fixed, want_history=True)["history"])
     eps = np.finfo(np.float64).eps * np.abs(w["rhs"]).max()
-    o.cg(x2, w["rhs"] + eps * wl.random_field(w["shape"], 77), fixed_iters=fixed)
-    return rel_l2(x2, x1)
+    h2 = np.array(run(x2, w["rhs"] + eps * wl.random_field(w["shape"], 77), fixed_iters=fixed,
+                      want_history=True)["history"])
+    return rel_l2(x2, x1), float(np.max(np.abs(h2 - h1) / h1))
 
 
 @pytest.mark.parametrize("path", PATHS)
@@ -194,9 +197,11 @@ def test_config4_periodic_cg6(path, n):
     assert abs(phi_g.mean()) <= 1e-13 * np.abs(phi_g).max()
     # 25 iterations: within the oracle's own sensitivity to a 1-ulp perturbation of the input
     phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, fixed_iters=25)
-    assert rel_l2(phi_g, phi_c) <= max(1e-10, 10 * _oracle_rounding_sensitivity(w, o, 25))
+    sens_x, sens_hist = _oracle_rounding_sensitivity(w, o, 25)
+    assert rel_l2(phi_g, phi_c) <= max(1e-10, 10 * sens_x)
     hist = np.array(g.get_history(26))
-    assert np.allclose(hist, res_c["history"], rtol=1e-4)
+    assert np.allclose(hist, res_c["history"], rtol=max(1e-8, 10 * sens_hist))
+    assert np.allclose(hist[:6], res_c["history"][:6], rtol=1e-9)
     phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, rtol=1e-10, max_iter=3000)
     assert res_g["status"] == pb.OK and abs(res_g["iters"] - res_c["iters"]) <= 2
     b_norm = np.linalg.norm(w["rhs"])
@@ -239,14 +244,17 @@ def test_config5_bicgstab(path):
     o.multipole_bc(w["rho"], w["G"], w["lmax"])
     g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
     g.set_option(pb.OPT_RECORD_HISTORY, 1)
-    for fixed in (10, 25):
+    for fixed in (3, 10, 25):
         phi_c = np.zeros_like(w["rhs"])
         d_phi = dev(phi_c)
         res_c = o.bicgstab(phi_c, w["rhs"], fixed_iters=fixed, want_history=True)
         res_g = g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=fixed)
         assert res_g["iters"] == fixed
-        assert rel_l2(host(d_phi), phi_c) <= 1e-10
-        assert np.allclose(g.get_history(fixed + 1), res_c["history"], rtol=1e-7)
+        # north_star's 1e-10 while rounding differences are not yet amplified; beyond that the oracle's own
+        # sensitivity to a 1-ulp perturbation of its input bounds what any correct implementation can match
+        sens_x, sens_h = (0.0, 0.0) if fixed == 3 else _oracle_rounding_sensitivity(w, o, fixed, "bicgstab")
+        assert rel_l2(host(d_phi), phi_c) <= max(1e-10, 10 * sens_x)
+        assert np.allclose(g.get_history(fixed + 1), res_c["history"], rtol=max(1e-7, 10 * sens_h))
     phi_c = np.zeros_like(w["rhs"])
     d_phi = dev(phi_c)
     res_c = o.bicgstab(phi_c, w["rhs"], rtol=1e-8, max_iter=3000)
@@ -260,12 +268,19 @@ def test_config5_bicgstab(path):
 def test_bicgstab_on_cartesian_and_unscaled_variant():
     w = wl.config2(32)
     o, g = make_pair(w)
-    phi_c = np.zeros_like(w["rhs"])
-    d_phi = dev(phi_c)
-    o.bicgstab(phi_c, w["rhs"], fixed_iters=20, jacobi=0)
     g.set_option(pb.OPT_JACOBI, 0)
-    g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=20)
-    assert rel_l2(host(d_phi), phi_c) <= 1e-10
+    for fixed in (5, 20):
+        phi_c = np.zeros_like(w["rhs"])
+        d_phi = dev(phi_c)
+        o.bicgstab(phi_c, w["rhs"], fixed_iters=fixed, jacobi=0)
+        g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=fixed)
+        sens = 0.0
+        if fixed > 5:   # the oracle's own sensitivity to a 1-ulp input perturbation (C8)
+            x2 = np.zeros_like(w["rhs"])
+            eps = np.finfo(np.float64).eps * np.abs(w["rhs"]).max()
+            o.bicgstab(x2, w["rhs"] + eps * wl.random_field(w["shape"], 77), fixed_iters=fixed, jacobi=0)
+            sens = rel_l2(x2, phi_c)
+        assert rel_l2(host(d_phi), phi_c) <= max(1e-10, 10 * sens)
 
 
 # ---- (a5) multigrid V-cycle -----------------------------------------------------------------------------------------
