@@ -167,8 +167,21 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     pb.lib()
     p = plan(args.small)
+    if args.divide > 1:
+        for key in ("apply", "sor", "vc64", "vcmx", "cg", "bicg"):
+            p[key] = max(1, p[key] // args.divide)
+    if args.rows:   # profiling aid: a subset of the rows (the reported value then covers only those)
+        keep = set(args.rows.split(","))
+        if "cg_iteration_19pt" not in keep:
+            p["n4"] = 32          # grids of unselected rows are shrunk so that set-up stays short
+        if not keep & {"multipole_bc_spherical", "bicgstab_iteration"}:
+            p["n5"] = (32, 16, 32)
+        if keep <= {"cg_iteration_19pt", "multipole_bc_spherical", "bicgstab_iteration"}:
+            p["n3"] = 32
     w3, w4, w5 = build_inputs(p)
     units = row_units(p)
+    if args.rows:
+        units = [u for u in units if u[0] in keep]
     kids = pb.kernel_classes()
     stream = torch.cuda.current_stream()
     mk = lambda w: pb.Poisson(w["shape"], w.get("spacing"), w.get("origin"), edges=w.get("edges"),
@@ -190,47 +203,64 @@ def run_ours(args):
     omega3 = 2.0 / (1.0 + math.sin(math.pi / (p["n3"] + 1)))
     row_names = [u[0] for u in units]
 
+    def _apply():
+        for _ in range(p["apply"]):
+            g3.apply_laplacian(d["phi3"], d["out3"])
+
+    def _resn():
+        for _ in range(p["resn"]):
+            g3.residual_norm(d["phi3"], d["rhs3"])
+
+    row_fn = {
+        "multipole_bc": lambda: g3.multipole_bc(d["rho3"], 1.0, 8, want_moments=False),
+        "apply_laplacian": _apply,
+        "rbsor_sweep": lambda: g3.rbsor_sweep(d["sor3"], d["rhs3"], omega3, p["sor"]),
+        "mg_vcycle_f64": lambda: g3.mg_vcycle(d["phi3"], d["rhs3"], ncycles=p["vc64"], precision=pb.F64,
+                                              want_resnorms=False),
+        "mg_vcycle_mixed": lambda: g3.mg_vcycle(d["mx3"], d["rhs3"], ncycles=p["vcmx"], precision=pb.MIXED,
+                                                want_resnorms=False),
+        "residual_norm": _resn,
+        "cg_iteration_19pt": lambda: g4.cg_solve(d["phi4"], d["rhs4"], fixed_iters=p["cg"]),
+        "multipole_bc_spherical": lambda: g5.multipole_bc(d["rho5"], 1.0, 8, want_moments=False),
+        "bicgstab_iteration": lambda: g5.bicgstab_solve(d["phi5"], d["rhs5"], fixed_iters=p["bicg"]),
+    }
+
     def step_device(ev=None):
         mark = (lambda: (ev.append(torch.cuda.Event(enable_timing=True)), ev[-1].record())) if ev is not None \
             else (lambda: None)
         mark()
-        g3.multipole_bc(d["rho3"], 1.0, 8, want_moments=False)
-        mark()
-        for _ in range(p["apply"]):
-            g3.apply_laplacian(d["phi3"], d["out3"])
-        mark()
-        g3.rbsor_sweep(d["sor3"], d["rhs3"], omega3, p["sor"])
-        mark()
-        g3.mg_vcycle(d["phi3"], d["rhs3"], ncycles=p["vc64"], precision=pb.F64, want_resnorms=False)
-        mark()
-        g3.mg_vcycle(d["mx3"], d["rhs3"], ncycles=p["vcmx"], precision=pb.MIXED, want_resnorms=False)
-        mark()
-        for _ in range(p["resn"]):
-            g3.residual_norm(d["phi3"], d["rhs3"])
-        mark()
-        g4.cg_solve(d["phi4"], d["rhs4"], fixed_iters=p["cg"])
-        mark()
-        g5.multipole_bc(d["rho5"], 1.0, 8, want_moments=False)
-        mark()
-        g5.bicgstab_solve(d["phi5"], d["rhs5"], fixed_iters=p["bicg"])
-        mark()
+        for name in row_names:
+            row_fn[name]()
+            mark()
 
-    def step_host():
-        # the same rows through the host-buffer entry points: every input crosses PCIe, every result comes back
-        g3.multipole_bc_host(h["rho3"], 1.0, 8, want_moments=False)
+    def _apply_host():
         for _ in range(p["apply"]):
             g3.apply_laplacian_host(h["phi3"], h["out3"])
-        g3.rbsor_sweep_host(h["phi3"], h["rhs3"], omega3, p["sor"])
-        g3.mg_vcycle_host(h["phi3"], h["rhs3"], ncycles=p["vc64"], precision=pb.F64, want_resnorms=False)
-        g3.mg_vcycle_host(h["phi3"], h["rhs3"], ncycles=p["vcmx"], precision=pb.MIXED, want_resnorms=False)
-        g3.rbsor_sweep_host(h["phi3"], h["rhs3"], 1.0, 0, want_resnorm=True)  # residual norm of host data
-        g4.cg_solve_host(h["phi4"], h["rhs4"], fixed_iters=p["cg"])
-        g5.multipole_bc_host(h["rho5"], 1.0, 8, want_moments=False)
-        g5.bicgstab_solve_host(h["phi5"], h["rhs5"], fixed_iters=p["bicg"])
 
     n3b, n4b, n5b = d["rhs3"].numel() * 8, d["rhs4"].numel() * 8, d["rhs5"].numel() * 8
-    h2d = n3b * (1 + p["apply"] + 2 + 2 + 2 + 2) + 2 * n4b + 3 * n5b
-    d2h = n3b * (p["apply"] + 1 + 1 + 1 + 1) + n4b + n5b
+    # the same rows through the host-buffer entry points: every input crosses PCIe, every result comes back
+    host_fn = {  # name -> (call, h2d bytes, d2h bytes)
+        "multipole_bc": (lambda: g3.multipole_bc_host(h["rho3"], 1.0, 8, want_moments=False), n3b, 0),
+        "apply_laplacian": (_apply_host, n3b * p["apply"], n3b * p["apply"]),
+        "rbsor_sweep": (lambda: g3.rbsor_sweep_host(h["phi3"], h["rhs3"], omega3, p["sor"]), 2 * n3b, n3b),
+        "mg_vcycle_f64": (lambda: g3.mg_vcycle_host(h["phi3"], h["rhs3"], ncycles=p["vc64"], precision=pb.F64,
+                                                    want_resnorms=False), 2 * n3b, n3b),
+        "mg_vcycle_mixed": (lambda: g3.mg_vcycle_host(h["phi3"], h["rhs3"], ncycles=p["vcmx"], precision=pb.MIXED,
+                                                      want_resnorms=False), 2 * n3b, n3b),
+        # residual norm of host data: zero sweeps + the norm
+        "residual_norm": (lambda: g3.rbsor_sweep_host(h["phi3"], h["rhs3"], 1.0, 0, want_resnorm=True), 2 * n3b, n3b),
+        "cg_iteration_19pt": (lambda: g4.cg_solve_host(h["phi4"], h["rhs4"], fixed_iters=p["cg"]), 2 * n4b, n4b),
+        "multipole_bc_spherical": (lambda: g5.multipole_bc_host(h["rho5"], 1.0, 8, want_moments=False), n5b, 0),
+        "bicgstab_iteration": (lambda: g5.bicgstab_solve_host(h["phi5"], h["rhs5"], fixed_iters=p["bicg"]),
+                               2 * n5b, n5b),
+    }
+
+    def step_host():
+        for name in row_names:
+            host_fn[name][0]()
+
+    h2d = sum(host_fn[nm][1] for nm in row_names)
+    d2h = sum(host_fn[nm][2] for nm in row_names)
 
     def barrier():
         if world > 1:
@@ -477,6 +507,8 @@ def main():
     ap.add_argument("--small", action="store_true", help="tiny grids: a functional check, not a measurement")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--path", type=int, default=None, help="force POISSON_OPT_KERNEL_PATH (1 generic, 2 plane)")
+    ap.add_argument("--rows", default=None, help="comma list of row names: time only these (profiling aid)")
+    ap.add_argument("--divide", type=int, default=1, help="divide the per-row unit counts (profiling aid)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

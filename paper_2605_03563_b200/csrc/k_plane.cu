@@ -5,12 +5,24 @@
 //   BiCGSTAB pass 1 p = r + beta (p - omega v) ; v = L D^-1 p ; sum r0^.v
 //   BiCGSTAB pass 2 s = r - alpha v ; t = L D^-1 s ; sum t.s, t.t
 // Same arithmetic, same order as the generic kernels (k_stencil.cu, k_krylov.cu); only the data movement differs.
+#include <cstdlib>
+
 #include "plane.cuh"
 
 namespace pb {
 
+int plane_cfg_override() {
+    static int v = -1;
+    if (v < 0) {
+        const char* e = getenv("POISSON_PLANE_CFG");
+        v = e ? atoi(e) : 0;
+    }
+    return v;
+}
+
 // ---- loaders ------------------------------------------------------------------------------------------------------------
 struct LdArr {  // v itself
+    static constexpr bool PLAIN = true;
     const double* v;
     struct Raw {
         double2 a;
@@ -22,6 +34,7 @@ struct LdArr {  // v itself
 };
 
 struct LdPnew {  // p_new = (r - mu) + beta p_old
+    static constexpr bool PLAIN = false;
     const double* r;
     const double* p;
     const KrylovCtl* ctl;
@@ -49,6 +62,7 @@ __device__ __forceinline__ double jac_(const Op& op, int i, int j, int k, int ja
 
 template <int KIND>
 struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D
+    static constexpr bool PLAIN = false;
     const double* r;
     const double* p;
     const double* v;
@@ -74,6 +88,7 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D
 
 template <int KIND>
 struct LdShat {  // s^ = (r - alpha v) / D
+    static constexpr bool PLAIN = false;
     const double* r;
     const double* v;
     const KrylovCtl* ctl;

@@ -20,16 +20,25 @@ __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_ca
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
 __device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
 
-template <int KIND>
+// Tile configuration: TX x TY points per CTA, RPT rows per thread (threads = TX/2 x TY/RPT), MINB resident CTAs per
+// SM asked of the compiler, PF = how many planes ahead the global loads run.
+template <int TX_, int TY_, int RPT_, int MINB_, int PF_>
+struct TileCfg {
+    static constexpr int TX = TX_, TY = TY_, RPT = RPT_, MINB = MINB_, PF = PF_;
+};
+
+template <int KIND, class Cfg>
 struct PlaneGeom {
     static constexpr int R = (KIND == KIND_CART6) ? 3 : 1;
     static constexpr int HX = (R == 1) ? 2 : 4;
-    static constexpr int TX = 128, TY = 16;
-    static constexpr int NTX = TX / 2, NTY = TY / 2, NT = NTX * NTY;
+    static constexpr int TX = Cfg::TX, TY = Cfg::TY, RPT = Cfg::RPT, PF = Cfg::PF;
+    static constexpr int NTX = TX / 2, NTY = TY / RPT, NT = NTX * NTY;
     static constexpr int SW = TX + 2 * HX, SH = TY + 2 * R;
-    static constexpr int NS = 2 * R + 2;
+    static constexpr int NS = 2 * R + 2;  // power of two (4 or 8)
     static constexpr int SLOT = SH * SW;
     static constexpr size_t SMEM = (size_t)NS * SLOT * sizeof(double);
+    static constexpr int NHALO = R * TX + TY * HX;        // halo pairs per plane: 2R rows x TX/2 + TY rows x HX
+    static constexpr int NH = (NHALO + NT - 1) / NT;      // halo pairs per thread
 };
 
 // Value of the loader's vector at (i,j,k) when at most one index is out of range (slow path: boundary cells only).
@@ -62,21 +71,21 @@ __device__ double vpoint(const Op& op, const Ld& ld, int i, int j, int k, bool u
 }
 
 // Per-thread coefficients of the operator rows it owns.
-template <int KIND>
+template <int KIND, int RPT>
 struct RowCoef {};
-template <>
-struct RowCoef<KIND_CART2> {
+template <int RPT>
+struct RowCoef<KIND_CART2, RPT> {
     double c0, c1, c2, d;
     bool plain;
 };
-template <>
-struct RowCoef<KIND_CART6> {
+template <int RPT>
+struct RowCoef<KIND_CART6, RPT> {
     double c0, c1, c2, d;
 };
-template <>
-struct RowCoef<KIND_SPH> {
-    double arm[2], arp[2], ir2[2], dr[2];  // per own column
-    double atm[2], atp[2], cp[2], dt[2];   // per own row
+template <int RPT>
+struct RowCoef<KIND_SPH, RPT> {
+    double arm[2], arp[2], ir2[2], dr[2];          // per own column
+    double atm[RPT], atp[RPT], cp[RPT], dt[RPT];   // per own row
 };
 
 // Loader / epilogue concepts (see k_plane.cu for the instances):
@@ -86,11 +95,12 @@ struct RowCoef<KIND_SPH> {
 //   struct Ep { static constexpr int NRED; struct Raw; bool skip() const; void prepare(); Raw load(size_t p) const;
 //               void apply(const Raw&, size_t p, int i, int j, int k, double2 v, double2 lv, double* acc) const;
 //               void finish(const double* totals) const; };
-template <int KIND, class Ld, class Ep>
-__global__ void __launch_bounds__(512, 1)
+template <int KIND, class Cfg, class Ld, class Ep>
+__global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
     k_plane(const Op op, const Ld ld_in, const Ep ep_in, const int kc, const bool ug_in, RedBuf rb) {
-    using G = PlaneGeom<KIND>;
+    using G = PlaneGeom<KIND, Cfg>;
     constexpr int R = G::R, HX = G::HX, TX = G::TX, TY = G::TY, SW = G::SW, NS = G::NS, SLOT = G::SLOT;
+    constexpr int RPT = G::RPT, NH = G::NH, PF = G::PF;
     extern __shared__ __align__(16) double ring[];
     if (ep_in.skip()) return;
     Ld ld = ld_in;  // the functors fetch their device-resident scalars (alpha, beta, ...) once
@@ -103,59 +113,70 @@ __global__ void __launch_bounds__(512, 1)
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
     const int k0 = blockIdx.z * kc, k1 = min(n2, k0 + kc);
     const int i = i0 + 2 * lx;
-    const int jr[2] = {j0 + 2 * ty, j0 + 2 * ty + 1};
-    const bool act[2] = {i < n0 && jr[0] < n1, i < n0 && jr[1] < n1};
+    const int jrow = j0 + RPT * ty;  // first owned row
+    bool act[RPT];
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) act[r] = i < n0 && jrow + r < n1;
     const size_t plane = (size_t)n0 * n1;
-    const size_t base[2] = {(size_t)jr[0] * n0 + i, (size_t)jr[1] * n0 + i};
-    const int so[2] = {(R + 2 * ty) * SW + HX + 2 * lx, (R + 2 * ty + 1) * SW + HX + 2 * lx};
+    const size_t base0 = (size_t)jrow * n0 + i;               // row r: base0 + r*n0
+    const int so0 = (R + RPT * ty) * SW + HX + 2 * lx;        // row r: so0 + r*SW
     const bool per_z = op.bc[4] == POISSON_BC_PERIODIC;
 
-    // ---- this thread's halo pair (at most one) -----------------------------------------------------------------
-    int hcls = 0, hi = 0, hj = 0, hso = 0;  // class 0 none, 1 plain load at wrapped (hwi,hwj), 2 boundary values
-    int hwi = 0, hwj = 0;
-    if (tid < 2 * R * G::NTX) {
-        const int rr = tid / G::NTX, c = tid % G::NTX;
-        const int srow = rr < R ? rr : TY + rr;
-        hj = j0 - R + srow;
-        hi = i0 + 2 * c;
-        hso = srow * SW + HX + 2 * c;
-        hcls = 1;
-    } else if (tid - 2 * R * G::NTX < TY * HX) {
-        const int t = tid - 2 * R * G::NTX, row = t / HX, c = t % HX;
-        const int pc = c < HX / 2 ? c : (TX / 2 + c);
-        hj = j0 + row;
-        hi = i0 - HX + 2 * pc;
-        hso = (R + row) * SW + 2 * pc;
-        hcls = 1;
-    }
-    if (hcls) {
-        const bool ox = hi < 0 || hi >= n0, oy = hj < 0 || hj >= n1;
-        hwi = hi;
-        hwj = hj;
-        if (ox && oy) {
-            hcls = 0;
-        } else if (ox) {
-            if (op.bc[0] == POISSON_BC_PERIODIC && n0 >= HX) hwi = ((hi % n0) + n0) % n0; else hcls = 2;
-        } else if (oy) {
-            if (op.bc[2] == POISSON_BC_PERIODIC) hwj = ((hj % n1) + n1) % n1; else hcls = 2;
+    // ---- this thread's halo pairs ----------------------------------------------------------------------------------
+    // class 0 none, 1 plain load at the wrapped (hwi,hwj), 2 boundary values through vpoint()
+    int hcls[NH], hi[NH], hj[NH], hso[NH], hwi[NH], hwj[NH];
+#pragma unroll
+    for (int m = 0; m < NH; ++m) {
+        const int h = tid + m * G::NT;
+        hcls[m] = 0;
+        hi[m] = hj[m] = hso[m] = hwi[m] = hwj[m] = 0;
+        if (h < R * TX) {  // rows above and below the tile
+            const int rr = h / G::NTX, c = h % G::NTX;
+            const int srow = rr < R ? rr : TY + rr;
+            hj[m] = j0 - R + srow;
+            hi[m] = i0 + 2 * c;
+            hso[m] = srow * SW + HX + 2 * c;
+            hcls[m] = 1;
+        } else if (h < G::NHALO) {  // columns left and right of the tile
+            const int t = h - R * TX, row = t / HX, c = t % HX;
+            const int pc = c < HX / 2 ? c : (TX / 2 + c);
+            hj[m] = j0 + row;
+            hi[m] = i0 - HX + 2 * pc;
+            hso[m] = (R + row) * SW + 2 * pc;
+            hcls[m] = 1;
+        }
+        if (hcls[m]) {
+            const bool ox = hi[m] < 0 || hi[m] >= n0, oy = hj[m] < 0 || hj[m] >= n1;
+            hwi[m] = hi[m];
+            hwj[m] = hj[m];
+            if (ox && oy) {
+                hcls[m] = 0;
+            } else if (ox) {
+                if (op.bc[0] == POISSON_BC_PERIODIC && n0 >= HX) hwi[m] = ((hi[m] % n0) + n0) % n0; else hcls[m] = 2;
+            } else if (oy) {
+                if (op.bc[2] == POISSON_BC_PERIODIC) hwj[m] = ((hj[m] % n1) + n1) % n1; else hcls[m] = 2;
+            }
         }
     }
-    const size_t hbase = (size_t)hwj * n0 + hwi;
 
     // ---- operator coefficients of the owned rows ----------------------------------------------------------------
-    RowCoef<KIND> rc;
+    RowCoef<KIND, RPT> rc;
     if constexpr (KIND == KIND_SPH) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const int ii = min(i + e, n0 - 1), jj = min(jr[e], n1 - 1);
+            const int ii = min(i + e, n0 - 1);
             rc.arm[e] = op.ar_m[ii];
             rc.arp[e] = op.ar_p[ii];
             rc.ir2[e] = op.ir2[ii];
             rc.dr[e] = op.dr[ii];
-            rc.atm[e] = op.at_m[jj];
-            rc.atp[e] = op.at_p[jj];
-            rc.cp[e] = op.cp[jj];
-            rc.dt[e] = op.dt[jj];
+        }
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            const int jj = min(jrow + r, n1 - 1);
+            rc.atm[r] = op.at_m[jj];
+            rc.atp[r] = op.at_p[jj];
+            rc.cp[r] = op.cp[jj];
+            rc.dt[r] = op.dt[jj];
         }
     } else {
         rc.c0 = op.c[0];
@@ -174,160 +195,196 @@ __global__ void __launch_bounds__(512, 1)
 
     // ---- plane staging --------------------------------------------------------------------------------------------
     struct Staged {
-        typename Ld::Raw o[2], h;
+        typename Ld::Raw o[RPT], h[NH];
         int kw;       // wrapped plane index, or -1 when the plane lies outside a non-periodic z face
     };
-    auto issue = [&](int kk) -> Staged {
-        Staged s;
+    // Boundary values (ghost faces, zeros, wrapped tiny grids) come through vpoint().  For a PLAIN loader (the vector is
+    // an array: Raw is the pair itself) they are fetched here, with the plane's other loads, so that their latency is
+    // hidden like any other; the Krylov loaders never see ghost values and resolve them at commit time.
+    auto bpair = [&](int ii, int jj, int kk) { return mk2(vpoint(op, ld, ii, jj, kk, ug), vpoint(op, ld, ii + 1, jj, kk, ug)); };
+    auto issue = [&](int kk, Staged& s) {
         s.kw = kk;
         if (kk < 0 || kk >= n2) s.kw = per_z ? ((kk % n2) + n2) % n2 : -1;
         if (s.kw >= 0) {
             const size_t off = (size_t)s.kw * plane;
-            if (act[0]) s.o[0] = ld.load(off + base[0]);
-            if (act[1]) s.o[1] = ld.load(off + base[1]);
-            if (hcls == 1) s.h = ld.load(off + hbase);
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                if (act[r]) s.o[r] = ld.load(off + base0 + (size_t)r * n0);
+                else if constexpr (Ld::PLAIN) s.o[r].a = bpair(i, jrow + r, s.kw);
+            }
+#pragma unroll
+            for (int m = 0; m < NH; ++m) {
+                if (hcls[m] == 1) s.h[m] = ld.load(off + (size_t)hwj[m] * n0 + hwi[m]);
+                else if constexpr (Ld::PLAIN) { if (hcls[m] == 2) s.h[m].a = bpair(hi[m], hj[m], s.kw); }
+            }
+        } else if constexpr (Ld::PLAIN) {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) s.o[r].a = bpair(i, jrow + r, kk);
         }
-        return s;
     };
     auto commit = [&](int kk, const Staged& s) {
-        double* slot = ring + ((kk + 2 * NS) % NS) * SLOT;
-        if (s.kw >= 0) {
+        double* slot = ring + ((kk + 2 * NS) & (NS - 1)) * SLOT;
+        if constexpr (Ld::PLAIN) {
 #pragma unroll
-            for (int r = 0; r < 2; ++r) {
-                if (act[r])
-                    st2(slot + so[r], ld.form(op, s.o[r], i, jr[r], s.kw));
-                else
-                    st2(slot + so[r], mk2(vpoint(op, ld, i, jr[r], s.kw, ug), vpoint(op, ld, i + 1, jr[r], s.kw, ug)));
+            for (int r = 0; r < RPT; ++r) st2(slot + so0 + r * SW, s.o[r].a);
+            if (s.kw >= 0) {
+#pragma unroll
+                for (int m = 0; m < NH; ++m)
+                    if (hcls[m] != 0) st2(slot + hso[m], s.h[m].a);
             }
-            if (hcls == 1)
-                st2(slot + hso, ld.form(op, s.h, hwi, hwj, s.kw));
-            else if (hcls == 2)
-                st2(slot + hso, mk2(vpoint(op, ld, hi, hj, s.kw, ug), vpoint(op, ld, hi + 1, hj, s.kw, ug)));
-        } else {
-            // plane beyond a non-periodic z face: ghost values or zeros; only owned columns are ever read
+        } else if (s.kw >= 0) {
 #pragma unroll
-            for (int r = 0; r < 2; ++r)
-                st2(slot + so[r], mk2(vpoint(op, ld, i, jr[r], kk, ug), vpoint(op, ld, i + 1, jr[r], kk, ug)));
+            for (int r = 0; r < RPT; ++r) {
+                if (act[r])
+                    st2(slot + so0 + r * SW, ld.form(op, s.o[r], i, jrow + r, s.kw));
+                else
+                    st2(slot + so0 + r * SW, bpair(i, jrow + r, s.kw));
+            }
+#pragma unroll
+            for (int m = 0; m < NH; ++m) {
+                if (hcls[m] == 1)
+                    st2(slot + hso[m], ld.form(op, s.h[m], hwi[m], hwj[m], s.kw));
+                else if (hcls[m] == 2)
+                    st2(slot + hso[m], bpair(hi[m], hj[m], s.kw));
+            }
+        } else {
+            // plane beyond a non-periodic z face: zeros (or a wrapped tiny grid); only owned columns are ever read
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) st2(slot + so0 + r * SW, bpair(i, jrow + r, kk));
         }
     };
 
     // prologue: planes k0-R .. k0+R-1, two at a time
     for (int kk = k0 - R; kk < k0 + R; kk += 2) {
-        const Staged a = issue(kk), b = issue(kk + 1);
+        Staged a, b;
+        issue(kk, a);
+        issue(kk + 1, b);
         commit(kk, a);
         commit(kk + 1, b);
     }
-    Staged nxt = issue(k0 + R);
-    typename Ep::Raw enxt[2];
+    Staged st[PF];
+    typename Ep::Raw est[PF][RPT];
 #pragma unroll
-    for (int r = 0; r < 2; ++r)
-        if (act[r]) enxt[r] = ep.load((size_t)k0 * plane + base[r]);
+    for (int u = 0; u < PF; ++u) {
+        issue(k0 + R + u, st[u]);
+        if (k0 + u < k1) {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r)
+                if (act[r]) est[u][r] = ep.load((size_t)(k0 + u) * plane + base0 + (size_t)r * n0);
+        }
+    }
 
     double acc[Ep::NRED > 0 ? Ep::NRED : 1];
 #pragma unroll
     for (int r = 0; r < (Ep::NRED > 0 ? Ep::NRED : 1); ++r) acc[r] = 0.0;
 
-    for (int k = k0; k < k1; ++k) {
-        commit(k + R, nxt);
-        typename Ep::Raw ecur[2] = {enxt[0], enxt[1]};
-        if (k + 1 < k1) {
-            nxt = issue(k + 1 + R);
+    for (int kb = k0; kb < k1; kb += PF) {
 #pragma unroll
-            for (int r = 0; r < 2; ++r)
-                if (act[r]) enxt[r] = ep.load((size_t)(k + 1) * plane + base[r]);
-        }
-        __syncthreads();
-        const double* c = ring + ((k + 2 * NS) % NS) * SLOT;
+        for (int u = 0; u < PF; ++u) {
+            const int k = kb + u;
+            if (k >= k1) break;  // uniform over the CTA
+            commit(k + R, st[u]);
+            typename Ep::Raw ecur[RPT];
 #pragma unroll
-        for (int r = 0; r < 2; ++r) {
-            if (!act[r]) continue;
-            const double* P = c + so[r];
-            const double2 C = ld2(P);
-            double2 lv;
-            if constexpr (KIND == KIND_CART6) {
-                const double2 xa = ld2(P - 4), xb = ld2(P - 2), xc = ld2(P + 2), xd = ld2(P + 4);
-                double2 t0, t1, t2;
-                {
-                    // point i: -1 xb.y, +1 C.y, -2 xb.x, +2 xc.x, -3 xa.y, +3 xc.y ; point i+1: -1 C.x, +1 xc.x, ...
-                    double u = 1.5 * (xb.y + C.y);
-                    u = fma(-3.0 / 20.0, xb.x + xc.x, u);
-                    t0.x = fma(1.0 / 90.0, xa.y + xc.y, u);
-                    u = 1.5 * (C.x + xc.x);
-                    u = fma(-3.0 / 20.0, xb.y + xc.y, u);
-                    t0.y = fma(1.0 / 90.0, xb.x + xd.x, u);
-                }
-                {
-                    const double2 m1 = ld2(P - SW), p1 = ld2(P + SW), m2 = ld2(P - 2 * SW), p2 = ld2(P + 2 * SW),
-                                  m3 = ld2(P - 3 * SW), p3 = ld2(P + 3 * SW);
-                    double u = 1.5 * (m1.x + p1.x);
-                    u = fma(-3.0 / 20.0, m2.x + p2.x, u);
-                    t1.x = fma(1.0 / 90.0, m3.x + p3.x, u);
-                    u = 1.5 * (m1.y + p1.y);
-                    u = fma(-3.0 / 20.0, m2.y + p2.y, u);
-                    t1.y = fma(1.0 / 90.0, m3.y + p3.y, u);
-                }
-                {
-                    const int o = so[r];
-                    const double2 m1 = ld2(ring + ((k - 1 + 2 * NS) % NS) * SLOT + o),
-                                  p1 = ld2(ring + ((k + 1 + 2 * NS) % NS) * SLOT + o),
-                                  m2 = ld2(ring + ((k - 2 + 2 * NS) % NS) * SLOT + o),
-                                  p2 = ld2(ring + ((k + 2 + 2 * NS) % NS) * SLOT + o),
-                                  m3 = ld2(ring + ((k - 3 + 2 * NS) % NS) * SLOT + o),
-                                  p3 = ld2(ring + ((k + 3 + 2 * NS) % NS) * SLOT + o);
-                    double u = 1.5 * (m1.x + p1.x);
-                    u = fma(-3.0 / 20.0, m2.x + p2.x, u);
-                    t2.x = fma(1.0 / 90.0, m3.x + p3.x, u);
-                    u = 1.5 * (m1.y + p1.y);
-                    u = fma(-3.0 / 20.0, m2.y + p2.y, u);
-                    t2.y = fma(1.0 / 90.0, m3.y + p3.y, u);
-                }
-                double s = t0.x * rc.c0;
-                s = fma(t1.x, rc.c1, s);
-                s = fma(t2.x, rc.c2, s);
-                lv.x = fma(-rc.d, C.x, s);
-                s = t0.y * rc.c0;
-                s = fma(t1.y, rc.c1, s);
-                s = fma(t2.y, rc.c2, s);
-                lv.y = fma(-rc.d, C.y, s);
-            } else {
-                const double2 xl = ld2(P - 2), xr = ld2(P + 2);
-                const double2 ym = ld2(P - SW), yp = ld2(P + SW);
-                const int o = so[r];
-                const double2 zm = ld2(ring + ((k - 1 + 2 * NS) % NS) * SLOT + o),
-                              zp = ld2(ring + ((k + 1 + 2 * NS) % NS) * SLOT + o);
-                if constexpr (KIND == KIND_CART2) {
-                    double d0 = rc.d, d1 = rc.d;
-                    if (!rc.plain) {
-                        d0 = row_diag<double, KIND_CART2>(op, i, jr[r], k);
-                        d1 = row_diag<double, KIND_CART2>(op, i + 1, jr[r], k);
-                    }
-                    double s = (xl.y + C.y) * rc.c0;
-                    s = fma(ym.x + yp.x, rc.c1, s);
-                    s = fma(zm.x + zp.x, rc.c2, s);
-                    lv.x = fma(-d0, C.x, s);
-                    s = (C.x + xr.x) * rc.c0;
-                    s = fma(ym.y + yp.y, rc.c1, s);
-                    s = fma(zm.y + zp.y, rc.c2, s);
-                    lv.y = fma(-d1, C.y, s);
-                } else {
-                    // spherical row (stencil.cuh row_offsum / row_diag, KIND_SPH)
-                    double s = rc.arm[0] * xl.y;
-                    s = fma(rc.arp[0], C.y, s);
-                    double t = rc.atm[r] * ym.x;
-                    t = fma(rc.atp[r], yp.x, t);
-                    t = fma(rc.cp[r], zm.x + zp.x, t);
-                    double off = fma(rc.ir2[0], t, s);
-                    lv.x = fma(-fma(rc.ir2[0], rc.dt[r], rc.dr[0]), C.x, off);
-                    s = rc.arm[1] * C.x;
-                    s = fma(rc.arp[1], xr.x, s);
-                    t = rc.atm[r] * ym.y;
-                    t = fma(rc.atp[r], yp.y, t);
-                    t = fma(rc.cp[r], zm.y + zp.y, t);
-                    off = fma(rc.ir2[1], t, s);
-                    lv.y = fma(-fma(rc.ir2[1], rc.dt[r], rc.dr[1]), C.y, off);
-                }
+            for (int r = 0; r < RPT; ++r) ecur[r] = est[u][r];
+            if (k + PF < k1) {
+                issue(k + PF + R, st[u]);
+#pragma unroll
+                for (int r = 0; r < RPT; ++r)
+                    if (act[r]) est[u][r] = ep.load((size_t)(k + PF) * plane + base0 + (size_t)r * n0);
             }
-            ep.apply(ecur[r], (size_t)k * plane + base[r], i, jr[r], k, C, lv, acc);
+            __syncthreads();
+            const double* c0p = ring + ((k + 2 * NS) & (NS - 1)) * SLOT + so0;
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                if (!act[r]) continue;
+                const double* P = c0p + r * SW;
+                const int o = so0 + r * SW;
+                const double2 C = ld2(P);
+                double2 lv;
+                if constexpr (KIND == KIND_CART6) {
+                    const double2 xa = ld2(P - 4), xb = ld2(P - 2), xc = ld2(P + 2), xd = ld2(P + 4);
+                    double2 t0, t1, t2;
+                    {
+                        // point i: -1 xb.y, +1 C.y, -2 xb.x, +2 xc.x, -3 xa.y, +3 xc.y ; point i+1 shifted by one
+                        double w = 1.5 * (xb.y + C.y);
+                        w = fma(-3.0 / 20.0, xb.x + xc.x, w);
+                        t0.x = fma(1.0 / 90.0, xa.y + xc.y, w);
+                        w = 1.5 * (C.x + xc.x);
+                        w = fma(-3.0 / 20.0, xb.y + xc.y, w);
+                        t0.y = fma(1.0 / 90.0, xb.x + xd.x, w);
+                    }
+                    {
+                        const double2 m1 = ld2(P - SW), p1 = ld2(P + SW), m2 = ld2(P - 2 * SW), p2 = ld2(P + 2 * SW),
+                                      m3 = ld2(P - 3 * SW), p3 = ld2(P + 3 * SW);
+                        double w = 1.5 * (m1.x + p1.x);
+                        w = fma(-3.0 / 20.0, m2.x + p2.x, w);
+                        t1.x = fma(1.0 / 90.0, m3.x + p3.x, w);
+                        w = 1.5 * (m1.y + p1.y);
+                        w = fma(-3.0 / 20.0, m2.y + p2.y, w);
+                        t1.y = fma(1.0 / 90.0, m3.y + p3.y, w);
+                    }
+                    {
+                        const double2 m1 = ld2(ring + ((k - 1 + 2 * NS) & (NS - 1)) * SLOT + o),
+                                      p1 = ld2(ring + ((k + 1 + 2 * NS) & (NS - 1)) * SLOT + o),
+                                      m2 = ld2(ring + ((k - 2 + 2 * NS) & (NS - 1)) * SLOT + o),
+                                      p2 = ld2(ring + ((k + 2 + 2 * NS) & (NS - 1)) * SLOT + o),
+                                      m3 = ld2(ring + ((k - 3 + 2 * NS) & (NS - 1)) * SLOT + o),
+                                      p3 = ld2(ring + ((k + 3 + 2 * NS) & (NS - 1)) * SLOT + o);
+                        double w = 1.5 * (m1.x + p1.x);
+                        w = fma(-3.0 / 20.0, m2.x + p2.x, w);
+                        t2.x = fma(1.0 / 90.0, m3.x + p3.x, w);
+                        w = 1.5 * (m1.y + p1.y);
+                        w = fma(-3.0 / 20.0, m2.y + p2.y, w);
+                        t2.y = fma(1.0 / 90.0, m3.y + p3.y, w);
+                    }
+                    double s = t0.x * rc.c0;
+                    s = fma(t1.x, rc.c1, s);
+                    s = fma(t2.x, rc.c2, s);
+                    lv.x = fma(-rc.d, C.x, s);
+                    s = t0.y * rc.c0;
+                    s = fma(t1.y, rc.c1, s);
+                    s = fma(t2.y, rc.c2, s);
+                    lv.y = fma(-rc.d, C.y, s);
+                } else {
+                    const double2 xl = ld2(P - 2), xr = ld2(P + 2);
+                    const double2 ym = ld2(P - SW), yp = ld2(P + SW);
+                    const double2 zm = ld2(ring + ((k - 1 + 2 * NS) & (NS - 1)) * SLOT + o),
+                                  zp = ld2(ring + ((k + 1 + 2 * NS) & (NS - 1)) * SLOT + o);
+                    if constexpr (KIND == KIND_CART2) {
+                        double d0 = rc.d, d1 = rc.d;
+                        if (!rc.plain) {
+                            d0 = row_diag<double, KIND_CART2>(op, i, jrow + r, k);
+                            d1 = row_diag<double, KIND_CART2>(op, i + 1, jrow + r, k);
+                        }
+                        double s = (xl.y + C.y) * rc.c0;
+                        s = fma(ym.x + yp.x, rc.c1, s);
+                        s = fma(zm.x + zp.x, rc.c2, s);
+                        lv.x = fma(-d0, C.x, s);
+                        s = (C.x + xr.x) * rc.c0;
+                        s = fma(ym.y + yp.y, rc.c1, s);
+                        s = fma(zm.y + zp.y, rc.c2, s);
+                        lv.y = fma(-d1, C.y, s);
+                    } else {
+                        // spherical row (stencil.cuh row_offsum / row_diag, KIND_SPH)
+                        double s = rc.arm[0] * xl.y;
+                        s = fma(rc.arp[0], C.y, s);
+                        double t = rc.atm[r] * ym.x;
+                        t = fma(rc.atp[r], yp.x, t);
+                        t = fma(rc.cp[r], zm.x + zp.x, t);
+                        double off = fma(rc.ir2[0], t, s);
+                        lv.x = fma(-fma(rc.ir2[0], rc.dt[r], rc.dr[0]), C.x, off);
+                        s = rc.arm[1] * C.x;
+                        s = fma(rc.arp[1], xr.x, s);
+                        t = rc.atm[r] * ym.y;
+                        t = fma(rc.atp[r], yp.y, t);
+                        t = fma(rc.cp[r], zm.y + zp.y, t);
+                        off = fma(rc.ir2[1], t, s);
+                        lv.y = fma(-fma(rc.ir2[1], rc.dt[r], rc.dr[1]), C.y, off);
+                    }
+                }
+                ep.apply(ecur[r], (size_t)k * plane + base0 + (size_t)r * n0, i, jrow + r, k, C, lv, acc);
+            }
         }
     }
     if constexpr (Ep::NRED > 0) {
@@ -338,10 +395,9 @@ __global__ void __launch_bounds__(512, 1)
     }
 }
 
-// Number of z chunks: minimise (waves of CTAs) x (planes per chunk + the 2R-plane prologue).
-template <int KIND>
-static inline int plane_chunks(const Op& op, int sms, int* kc_out) {
-    using G = PlaneGeom<KIND>;
+// Number of z chunks: minimise (waves of CTAs) x (planes per chunk + the prologue of 2R planes).
+template <class G>
+static inline int plane_chunks(const Op& op, int slots, int* kc_out) {
     const long tiles = (long)((op.n[0] + G::TX - 1) / G::TX) * ((op.n[1] + G::TY - 1) / G::TY);
     int best = 1;
     double best_cost = 1e300;
@@ -349,8 +405,8 @@ static inline int plane_chunks(const Op& op, int sms, int* kc_out) {
         const int kc = (op.n[2] + nz - 1) / nz;
         if (kc < 4 && nz > 1) break;
         const int nzz = (op.n[2] + kc - 1) / kc;
-        const long waves = (tiles * nzz + sms - 1) / sms;
-        const double cost = (double)waves * (kc + 2.0 * G::R * 1.5 + 2.0);
+        const long waves = (tiles * nzz + slots - 1) / slots;
+        const double cost = (double)waves * (kc + G::R + 1.0);
         if (cost < best_cost - 1e-9) {
             best_cost = cost;
             best = nzz;
@@ -361,23 +417,46 @@ static inline int plane_chunks(const Op& op, int sms, int* kc_out) {
     return (op.n[2] + kc - 1) / kc;
 }
 
-template <int KIND, class Ld, class Ep>
-static int launch_plane(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
-    using G = PlaneGeom<KIND>;
-    auto kern = k_plane<KIND, Ld, Ep>;
-    static bool configured = false;
-    if (!configured) {
+template <int KIND, class Cfg, class Ld, class Ep>
+static int launch_plane_cfg(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
+    using G = PlaneGeom<KIND, Cfg>;
+    auto kern = k_plane<KIND, Cfg, Ld, Ep>;
+    static int resident = 0;
+    if (!resident) {
         PB_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-        configured = true;
+        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, G::NT, G::SMEM));
+        if (resident < 1) return fail(ctx, POISSON_CUDA_ERROR, "plane kernel does not fit on an SM");
     }
     int kc = 0;
-    const int nz = plane_chunks<KIND>(op, ctx->num_sms, &kc);
+    const int nz = plane_chunks<G>(op, ctx->num_sms * resident, &kc);
     const dim3 g((op.n[0] + G::TX - 1) / G::TX, (op.n[1] + G::TY - 1) / G::TY, nz), b(G::NTX, G::NTY);
     if ((size_t)g.x * g.y * g.z > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large");
     pre_launch(ctx, kid);
     kern<<<g, b, G::SMEM, ctx->stream>>>(op, ld, ep, kc, ug, ctx->red);
     post_launch(ctx, kid);
     return POISSON_OK;
+}
+
+// Tile choice per kernel class (measured on B200); POISSON_PLANE_CFG=<n> overrides for tuning.
+using CfgA = TileCfg<128, 16, 2, 1, 1>;
+using CfgB = TileCfg<128, 16, 1, 1, 1>;
+using CfgC = TileCfg<64, 16, 2, 2, 1>;
+using CfgD = TileCfg<64, 16, 1, 2, 1>;
+using CfgE = TileCfg<128, 16, 2, 1, 2>;
+using CfgF = TileCfg<64, 16, 2, 2, 2>;
+
+int plane_cfg_override();
+
+template <int KIND, class Ld, class Ep>
+static int launch_plane(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
+    switch (plane_cfg_override()) {
+        case 1: return launch_plane_cfg<KIND, CfgB>(ctx, op, ld, ep, ug, kid);
+        case 2: return launch_plane_cfg<KIND, CfgC>(ctx, op, ld, ep, ug, kid);
+        case 3: return launch_plane_cfg<KIND, CfgD>(ctx, op, ld, ep, ug, kid);
+        case 4: return launch_plane_cfg<KIND, CfgE>(ctx, op, ld, ep, ug, kid);
+        case 5: return launch_plane_cfg<KIND, CfgF>(ctx, op, ld, ep, ug, kid);
+        default: return launch_plane_cfg<KIND, CfgA>(ctx, op, ld, ep, ug, kid);
+    }
 }
 
 // The plane engine needs 16-byte aligned pairs: even n0 (every row then starts on a pair boundary).
