@@ -36,8 +36,15 @@ def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
 
+    hdr_mtime = max(os.path.getmtime(os.path.join(CSRC, f)) for f in os.listdir(CSRC) if not f.endswith(".cu"))
+    hdr_mtime = max(hdr_mtime, os.path.getmtime(os.path.join(HERE, "..", "include", "poisson.h")),
+                    os.path.getmtime(os.path.abspath(__file__)))
+
     def compile_one(src):
         obj = os.path.join(OBJ, src[:-3] + ".o")
+        if not force and not verbose and os.path.exists(obj) and \
+                os.path.getmtime(obj) > max(hdr_mtime, os.path.getmtime(os.path.join(CSRC, src))):
+            return obj  # up to date
         cmd = [NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:

@@ -2,6 +2,7 @@
 // Drivers only enqueue kernels and poll a device flag; all arithmetic of the path runs in the kernels.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "common.cuh"
@@ -40,6 +41,21 @@ double* scratch(poisson_ctx* ctx, int slot) {
         ctx->vec[slot] = (double*)p;
     }
     return ctx->vec[slot];
+}
+
+void* sor_scratch(poisson_ctx* ctx, size_t bytes) {
+    if (ctx->sor_tmp_bytes < bytes) {
+        cudaFree(ctx->sor_tmp);
+        ctx->sor_tmp = nullptr;
+        ctx->sor_tmp_bytes = 0;
+        if (cudaMalloc(&ctx->sor_tmp, bytes) != cudaSuccess) {
+            cudaGetLastError();
+            fail(ctx, POISSON_OUT_OF_MEMORY, "out of device memory for the red-black ping-pong buffer");
+            return nullptr;
+        }
+        ctx->sor_tmp_bytes = bytes;
+    }
+    return ctx->sor_tmp;
 }
 
 void pre_launch(poisson_ctx* ctx, int kid) {
@@ -169,6 +185,7 @@ int poisson_destroy(poisson_t ctx) {
     free_levels(ctx);
     for (double* v : ctx->vec) cudaFree(v);
     for (int f = 0; f < 6; ++f) cudaFree(ctx->d_ghost[f]);
+    cudaFree(ctx->sor_tmp);
     cudaFree(ctx->d_coef);
     cudaFree(ctx->d_ctr);
     cudaFree(ctx->red.partials);
@@ -221,6 +238,7 @@ int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], 
     }
     poisson_ctx* ctx = new poisson_ctx;
     ctx->stream = (cudaStream_t)cuda_stream;
+    if (const char* e = getenv("POISSON_SOR_HALFSTEPS")) ctx->opt_sor_nhs = atoi(e) == 4 ? 4 : 2;  // tuning aid
     Op& op = ctx->op;
     std::memset(&op, 0, sizeof(op));
     ctx->npts = 1;
@@ -304,6 +322,10 @@ int poisson_set_option(poisson_t ctx, int option, int value) {
             return POISSON_OK;
         case POISSON_OPT_RECORD_HISTORY:
             ctx->opt_history = value ? 1 : 0;
+            return POISSON_OK;
+        case POISSON_OPT_SOR_HALFSTEPS:
+            if (value != 2 && value != 4) return fail(ctx, POISSON_INVALID_ARG, "half-steps per pass must be 2 or 4");
+            ctx->opt_sor_nhs = value;
             return POISSON_OK;
         case POISSON_OPT_TIME_KERNELS:
             if (value < -2 || value >= KID_COUNT) return fail(ctx, POISSON_INVALID_ARG, "bad kernel class");

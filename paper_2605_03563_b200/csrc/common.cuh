@@ -112,6 +112,9 @@ struct poisson_ctx {
     int mg_coarsest_n = -1;
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
+    int opt_sor_nhs = 2;             // colour half-steps fused per HBM pass of the red-black kernel (2 or 4)
+    void* sor_tmp = nullptr;         // ping-pong buffer of the fused red-black kernel
+    size_t sor_tmp_bytes = 0;
     long launches = 0;
     long launches_by_kid[pb::KID_COUNT] = {0};
     // optional event timing of one kernel class (or all with -2): pairs of events around every such launch
@@ -164,6 +167,13 @@ int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, co
 int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t);
 int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double* s, const double* t,
                       const double* r0, double* r);
+
+// Fused red-black sweeps (k_sor_fused.cu): both colours (or two sweeps) per HBM pass, ping-pong through tmp
+bool sor_fused_ok(const poisson_ctx* ctx, const Op& op);
+int sor_fused(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, double omega, int nsweeps,
+              bool ug);
+int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps);
+void* sor_scratch(poisson_ctx* ctx, size_t bytes);  // nullptr on OOM
 
 // Plane-pipeline versions (k_plane.cu) for pair-aligned grids; same results, bit for bit
 int plane_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out,

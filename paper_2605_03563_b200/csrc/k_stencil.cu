@@ -122,6 +122,11 @@ static int rbsor_dispatch(poisson_ctx* ctx, const Op& op, T* phi, const T* rhs, 
 
 int launch_rbsor(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, double omega, int nsweeps,
                  bool ug) {
+    if (kind == KIND_CART2 && nsweeps > 0 && sor_fused_ok(ctx, op)) {
+        double* tmp = (double*)sor_scratch(ctx, (size_t)op.n[0] * op.n[1] * op.n[2] * sizeof(double));
+        if (!tmp) return POISSON_OUT_OF_MEMORY;
+        return sor_fused(ctx, op, phi, tmp, rhs, omega, nsweeps, ug);
+    }
     if (kind == KIND_CART2) return rbsor_dispatch<double, KIND_CART2>(ctx, op, phi, rhs, omega, nsweeps, ug);
     if (kind == KIND_SPH) return rbsor_dispatch<double, KIND_SPH>(ctx, op, phi, rhs, omega, nsweeps, ug);
     return fail(ctx, POISSON_UNSUPPORTED,
@@ -129,6 +134,11 @@ int launch_rbsor(poisson_ctx* ctx, const Op& op, int kind, double* phi, const do
 }
 
 int launch_rbsor32(poisson_ctx* ctx, const Op& op, float* phi, const float* rhs, float omega, int nsweeps) {
+    if (nsweeps > 0 && sor_fused_ok(ctx, op)) {
+        float* tmp = (float*)sor_scratch(ctx, (size_t)op.n[0] * op.n[1] * op.n[2] * sizeof(float));
+        if (!tmp) return POISSON_OUT_OF_MEMORY;
+        return sor_fused32(ctx, op, phi, tmp, rhs, omega, nsweeps);
+    }
     return rbsor_dispatch<float, KIND_CART2>(ctx, op, phi, rhs, omega, nsweeps, false);
 }
 
