@@ -125,9 +125,9 @@ __device__ __forceinline__ typename PairT<T>::type sor_bpair(const Op& op, int i
 }
 
 // Tile configuration: extended tile of PXN pairs x EY rows (threads in use = PXN * EY), NHS colour half-steps per pass.
-template <int NHS_, int PXN_, int EY_>
+template <int NHS_, int PXN_, int EY_, int PF_ = 1>
 struct SorTile {
-    static constexpr int NHS = NHS_, PXN = PXN_, EY = EY_;
+    static constexpr int NHS = NHS_, PXN = PXN_, EY = EY_, PF = PF_;  // PF = planes of load prefetch (1 or 2)
     static constexpr int D = NHS + 2;                       // queue depth = ring slots
     static constexpr int NT = ((PXN * EY + 31) / 32) * 32;  // threads per CTA
     static constexpr int SW = 2 * PXN, SLOT = SW * EY;
@@ -174,6 +174,8 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
         const int xoB = cA ? (lx > 0 ? -1 : 0) : (lx < PXN - 1 ? 2 : 1);
         const int ymA = cA + (ly > 0 ? -SW : 0), ypA = cA + (ly < EY - 1 ? SW : 0);
         const int ymB = (1 - cA) + (ly > 0 ? -SW : 0), ypB = (1 - cA) + (ly < EY - 1 ? SW : 0);
+        T* const mineA = mine + cA;
+        T* const mineB = mine + 1 - cA;
         T dA = dplain, dB = dplain, rdA = rdplain, rdB = rdplain;
         if (!PLAIN && col_in) {
             dA = sor_diag_xy<T>(op, i + cA, j);
@@ -212,7 +214,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
             if (op.bc[4] == POISSON_BC_DIRICHLET_GHOST && op.ghost[4]) zlo = reinterpret_cast<const T*>(op.ghost[4]) + (size_t)j * n0 + i;
             if (op.bc[5] == POISSON_BC_DIRICHLET_GHOST && op.ghost[5]) zhi = reinterpret_cast<const T*>(op.ghost[5]) + (size_t)j * n0 + i;
         }
-        vp += (ptrdiff_t)kstart * vs;
+        vp += (ptrdiff_t)kstart * vs;  // vp / prh always point at the next plane to load
         const T* prh = rhs + (col_in ? (size_t)j * n0 + i : 0) + (ptrdiff_t)kstart * (ptrdiff_t)plane;
         T* pout = out + (col_in ? (size_t)j * n0 + i : 0) + ((ptrdiff_t)kstart - NHS - 1) * (ptrdiff_t)plane;
         // vp / prh point at plane kk (the next plane to load); they are only dereferenced when that plane exists
@@ -237,7 +239,16 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
         T qA[D], qB[D], fA[D], fB[D];
 #pragma unroll
         for (int m = 0; m < D; ++m) qA[m] = qB[m] = fA[m] = fB[m] = (T)0;
-        P2 nv = loadv(kstart), nr = loadr(kstart);
+        // loads run PF planes ahead of their use: nvq[m] / nrq[m] hold plane (next plane to consume) + m
+        constexpr int PF = Cfg::PF;
+        P2 nvq[PF], nrq[PF];
+#pragma unroll
+        for (int m = 0; m < PF; ++m) {
+            nvq[m] = loadv(kstart + m);
+            nrq[m] = loadr(kstart + m);
+            vp += vs;
+            prh += plane;
+        }
         __syncthreads();  // the previous segment's readers are done with the ring
         for (int kin0 = kstart; kin0 <= kend; kin0 += D) {
 #pragma unroll
@@ -245,45 +256,53 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                 const int kin = kin0 + u;
                 if (kin > kend) break;
                 const int p0 = (D - u) % D;  // index of plane kin (m = 0)
+                const P2 nv = nvq[u % PF], nr = nrq[u % PF];
                 qA[p0] = cA ? nv.y : nv.x;
                 qB[p0] = cA ? nv.x : nv.y;
                 fA[p0] = cA ? nr.y : nr.x;
                 fB[p0] = cA ? nr.x : nr.y;
                 if (live) *reinterpret_cast<P2*>(mine + u * SLOT) = nv;  // slot of plane kin is u
+                pout += plane;
+                if (kin + PF <= kend) {
+                    nvq[u % PF] = loadv(kin + PF);
+                    nrq[u % PF] = loadr(kin + PF);
+                }
                 vp += vs;
                 prh += plane;
-                pout += plane;
-                if (kin < kend) {
-                    nv = loadv(kin + 1);
-                    nr = loadr(kin + 1);
-                }
                 __syncthreads();
+                // (1) everything that does not depend on this iteration's updates: the shared-memory neighbours belong
+                // to columns that are not updated now, so the x/y part of every half-step can be formed up front
+                const bool actA = (u % 2) == 0;
+                T sxy[NHS];
+#pragma unroll
+                for (int h = 1; h <= NHS; ++h) {
+                    const T* const sp = mine + ((u - h + D) % D) * SLOT;
+                    const int ph = (h - u + 2 * D) % D;
+                    const T partner = actA ? qB[ph] : qA[ph];
+                    const T outer = sp[actA ? xoA : xoB];
+                    const T ym = sp[actA ? ymA : ymB], yp = sp[actA ? ypA : ypB];
+                    sxy[h - 1] = fma_(ym + yp, c1, (outer + partner) * c0);
+                }
+                // (2) the dependent chain plane kin-1 -> kin-2 -> ... through the z neighbours, in registers
 #pragma unroll
                 for (int h = 1; h <= NHS; ++h) {
                     const int kz = kin - h;
                     const bool upd = col_in && kz >= 0 && kz < n2;
-                    T* const sp = mine + ((u - h + D) % D) * SLOT;
                     const int ph = (h - u + 2 * D) % D, pm = (h + 1 - u + 2 * D) % D, pp = (h - 1 - u + 2 * D) % D;
-                    const bool actA = (u % 2) == 0;
-                    const T partner = actA ? qB[ph] : qA[ph];
-                    const T outer = sp[actA ? xoA : xoB];
-                    const T ym = sp[actA ? ymA : ymB], yp = sp[actA ? ypA : ypB];
                     const T zp = actA ? qA[pp] : qB[pp], zm = actA ? qA[pm] : qB[pm];
                     const T old = actA ? qA[ph] : qB[ph];
                     const T f = actA ? fA[ph] : fB[ph];
-                    T d = actA ? dA : dB, rd = actA ? rdA : rdB;
+                    T d = PLAIN ? dplain : (actA ? dA : dB), rd = PLAIN ? rdplain : (actA ? rdA : rdB);
                     if (!PLAIN && (kz == 0 || kz == n2 - 1)) {
                         d = sor_diag_z<T>(op, d, kz);
                         rd = (T)1 / d;
                     }
-                    T s = (outer + partner) * c0;
-                    s = fma_(ym + yp, c1, s);
-                    s = fma_(zm + zp, c2, s);
+                    const T s = fma_(zm + zp, c2, sxy[h - 1]);
                     const T gs = div_by<T>(s - f, d, rd);
                     const T nw = fma_(omega, gs - old, old);
                     if (upd) {
                         if (actA) qA[ph] = nw; else qB[ph] = nw;
-                        sp[actA ? cA : 1 - cA] = nw;
+                        (actA ? mineA : mineB)[((u - h + D) % D) * SLOT] = nw;
                     }
                 }
                 const int ko = kin - NHS;
@@ -351,10 +370,10 @@ static int sor_cfg_override() {
 // Tile choice: the compiled configuration with the smallest estimated pass time (POISSON_SOR_CFG=<n> overrides).
 template <typename T, int NHS>
 static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, T omega, bool ug) {
-    using C0 = SorTile<NHS, 32 + NHS, 14 + 2 * NHS>;   // 64 x 14 valid, 612 threads at NHS = 2
+    using C0 = SorTile<NHS, 32 + NHS, 14 + 2 * NHS>;   // 64 x 14 valid, 612 threads at NHS = 2 (best at 256^3 on B200)
     using C1 = SorTile<NHS, 16 + NHS, 28 + 2 * NHS>;   // 32 x 28 valid, 576 threads
     using C2 = SorTile<NHS, 16 + NHS, 10 + 2 * NHS>;   // 32 x 10 valid, 252 threads, two CTAs per SM
-    using C3 = SorTile<NHS, 32 + NHS, 10 + 2 * NHS>;   // 64 x 10 valid, 476 threads
+    using C3 = SorTile<NHS, 32 + NHS, 8 + 2 * NHS>;    // 64 x 8 valid, 408 threads
     SorGeom g[4];
     int grid[4];
     double cost[4] = {sor_cfg_cost<C0>(ctx, op, sizeof(T), &g[0], &grid[0]), sor_cfg_cost<C1>(ctx, op, sizeof(T), &g[1], &grid[1]),
