@@ -22,31 +22,39 @@ int plane_cfg_override() {
 
 // ---- loaders ------------------------------------------------------------------------------------------------------------
 struct LdArr {  // v itself
-    static constexpr bool PLAIN = true;
+    static constexpr bool PLAIN = true, SIDE = false;
     const double* v;
     struct Raw {
         double2 a;
     };
     __device__ __forceinline__ void prepare() {}
     __device__ __forceinline__ Raw load(size_t p) const { return Raw{ld2(v + p)}; }
+    __device__ __forceinline__ Raw load_own(size_t p) const { return load(p); }
+    __device__ __forceinline__ void side(const Raw&, size_t) const {}
     __device__ __forceinline__ double2 form(const Op&, const Raw& r, int, int, int) const { return r.a; }
     __device__ __forceinline__ double at(const Op&, size_t p, int, int, int) const { return v[p]; }
 };
 
-struct LdPnew {  // p_new = (r - mu) + beta p_old
-    static constexpr bool PLAIN = false;
+struct LdPnew {  // p_new = (r - mu) + beta p_old; side effect on owned points: x += alpha_prev p_old (deferred x-update)
+    static constexpr bool PLAIN = false, SIDE = true;
     const double* r;
     const double* p;
+    double* x;
     const KrylovCtl* ctl;
-    double beta, mu;
+    double beta, mu, alpha_prev;
     struct Raw {
-        double2 r, p;
+        double2 r, p, x;
     };
     __device__ __forceinline__ void prepare() {
         beta = ctl->beta;
         mu = ctl->mu;
+        alpha_prev = ctl->alpha;
     }
-    __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q)}; }
+    __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q), mk2(0.0, 0.0)}; }
+    __device__ __forceinline__ Raw load_own(size_t q) const { return Raw{ld2(r + q), ld2(p + q), ld2(x + q)}; }
+    __device__ __forceinline__ void side(const Raw& w, size_t q) const {
+        st2(x + q, mk2(fma(alpha_prev, w.p.x, w.x.x), fma(alpha_prev, w.p.y, w.x.y)));
+    }
     __device__ __forceinline__ double2 form(const Op&, const Raw& w, int, int, int) const {
         return mk2(fma(beta, w.p.x, w.r.x - mu), fma(beta, w.p.y, w.r.y - mu));
     }
@@ -61,11 +69,12 @@ __device__ __forceinline__ double jac_(const Op& op, int i, int j, int k, int ja
 }
 
 template <int KIND>
-struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D
-    static constexpr bool PLAIN = false;
+struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D; side effect on owned points: store p_new
+    static constexpr bool PLAIN = false, SIDE = true;
     const double* r;
     const double* p;
     const double* v;
+    double* p_new;
     const KrylovCtl* ctl;
     int jacobi;
     double beta, omega;
@@ -77,6 +86,10 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D
         omega = ctl->omega;
     }
     __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q), ld2(v + q)}; }
+    __device__ __forceinline__ Raw load_own(size_t q) const { return load(q); }
+    __device__ __forceinline__ void side(const Raw& w, size_t q) const {
+        st2(p_new + q, mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x), fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y)));
+    }
     __device__ __forceinline__ double2 form(const Op& op, const Raw& w, int i, int j, int k) const {
         return mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
                    fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y) / jac_<KIND>(op, i + 1, j, k, jacobi));
@@ -87,10 +100,11 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D
 };
 
 template <int KIND>
-struct LdShat {  // s^ = (r - alpha v) / D
-    static constexpr bool PLAIN = false;
+struct LdShat {  // s^ = (r - alpha v) / D; side effect on owned points: store s
+    static constexpr bool PLAIN = false, SIDE = true;
     const double* r;
     const double* v;
+    double* s;
     const KrylovCtl* ctl;
     int jacobi;
     double alpha;
@@ -99,6 +113,10 @@ struct LdShat {  // s^ = (r - alpha v) / D
     };
     __device__ __forceinline__ void prepare() { alpha = ctl->alpha; }
     __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(v + q)}; }
+    __device__ __forceinline__ Raw load_own(size_t q) const { return load(q); }
+    __device__ __forceinline__ void side(const Raw& w, size_t q) const {
+        st2(s + q, mk2(fma(-alpha, w.v.x, w.r.x), fma(-alpha, w.v.y, w.r.y)));
+    }
     __device__ __forceinline__ double2 form(const Op& op, const Raw& w, int i, int j, int k) const {
         return mk2(fma(-alpha, w.v.x, w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
                    fma(-alpha, w.v.y, w.r.y) / jac_<KIND>(op, i + 1, j, k, jacobi));
@@ -187,23 +205,16 @@ struct EpInit {  // r = rhs - L x (ghosts included); r0^ = r; first scalars of t
     }
 };
 
-struct EpCgA {
+struct EpCgA {  // stores p_new and q = L p_new, sum p.q -> alpha (the x-update rides on the loader, LdPnew::side)
     static constexpr int NRED = 1;
-    const double* p_old;
     double* p_new;
     double* q;
-    double* x;
     KrylovCtl* ctl;
-    double alpha_prev;
-    struct Raw {
-        double2 x, p;
-    };
+    struct Raw {};
     __device__ __forceinline__ bool skip() const { return ctl->done != 0; }
-    __device__ __forceinline__ void prepare() { alpha_prev = ctl->alpha; }
-    __device__ __forceinline__ Raw load(size_t m) const { return Raw{ld2(x + m), ld2(p_old + m)}; }
-    __device__ __forceinline__ void apply(const Raw& w, size_t m, int, int, int, double2 pn, double2 lv,
-                                          double* acc) const {
-        st2(x + m, mk2(fma(alpha_prev, w.p.x, w.x.x), fma(alpha_prev, w.p.y, w.x.y)));  // deferred x-update
+    __device__ __forceinline__ void prepare() {}
+    __device__ __forceinline__ Raw load(size_t) const { return Raw{}; }
+    __device__ __forceinline__ void apply(const Raw&, size_t m, int, int, int, double2 pn, double2 lv, double* acc) const {
         st2(p_new + m, pn);
         st2(q + m, lv);
         acc[0] = fma(pn.x, lv.x, acc[0]);
@@ -215,30 +226,19 @@ struct EpCgA {
     }
 };
 
-struct EpBicg1 {
+struct EpBicg1 {  // v_new = L p^, sum r0^.v -> alpha (p_new is stored by the loader, LdPhat::side)
     static constexpr int NRED = 1;
-    const double* r;
-    const double* p_old;
-    const double* v_old;
     const double* r0;
-    double* p_new;
     double* v_new;
     KrylovCtl* ctl;
-    double beta, omega;
     struct Raw {
-        double2 r, p, v, r0;
+        double2 r0;
     };
     __device__ __forceinline__ bool skip() const { return ctl->done != 0; }
-    __device__ __forceinline__ void prepare() {
-        beta = ctl->beta;
-        omega = ctl->omega;
-    }
-    __device__ __forceinline__ Raw load(size_t m) const {
-        return Raw{ld2(r + m), ld2(p_old + m), ld2(v_old + m), ld2(r0 + m)};
-    }
+    __device__ __forceinline__ void prepare() {}
+    __device__ __forceinline__ Raw load(size_t m) const { return Raw{ld2(r0 + m)}; }
     __device__ __forceinline__ void apply(const Raw& w, size_t m, int, int, int, double2, double2 lv,
                                           double* acc) const {
-        st2(p_new + m, mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x), fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y)));
         st2(v_new + m, lv);
         acc[0] = fma(w.r0.x, lv.x, acc[0]);
         acc[0] = fma(w.r0.y, lv.y, acc[0]);
@@ -255,28 +255,23 @@ struct EpBicg1 {
     }
 };
 
-struct EpBicg2 {
+struct EpBicg2 {  // t = L s^, sum t.s, t.t -> omega (s was stored by the loader of this same thread, LdShat::side)
     static constexpr int NRED = 2;
-    const double* r;
-    const double* v;
-    double* s;
+    const double* s;
     double* t;
     KrylovCtl* ctl;
-    double alpha;
     struct Raw {
-        double2 r, v;
+        double2 s;
     };
     __device__ __forceinline__ bool skip() const { return ctl->done != 0; }
-    __device__ __forceinline__ void prepare() { alpha = ctl->alpha; }
-    __device__ __forceinline__ Raw load(size_t m) const { return Raw{ld2(r + m), ld2(v + m)}; }
+    __device__ __forceinline__ void prepare() {}
+    __device__ __forceinline__ Raw load(size_t m) const { return Raw{ld2(s + m)}; }
     __device__ __forceinline__ void apply(const Raw& w, size_t m, int, int, int, double2, double2 lv,
                                           double* acc) const {
-        const double2 sv = mk2(fma(-alpha, w.v.x, w.r.x), fma(-alpha, w.v.y, w.r.y));
-        st2(s + m, sv);
         st2(t + m, lv);
-        acc[0] = fma(lv.x, sv.x, acc[0]);
+        acc[0] = fma(lv.x, w.s.x, acc[0]);
         acc[1] = fma(lv.x, lv.x, acc[1]);
-        acc[0] = fma(lv.y, sv.y, acc[0]);
+        acc[0] = fma(lv.y, w.s.y, acc[0]);
         acc[1] = fma(lv.y, lv.y, acc[1]);
     }
     __device__ __forceinline__ void finish(const double* tot) const {
@@ -334,8 +329,8 @@ int plane_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, doub
 
 int plane_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x) {
     int rc = POISSON_OK;
-    const LdPnew ld{r, p_old, ctx->d_ctl, 0.0, 0.0};
-    const EpCgA ep{p_old, p_new, q, x, ctx->d_ctl, 0.0};
+    const LdPnew ld{r, p_old, x, ctx->d_ctl, 0.0, 0.0, 0.0};
+    const EpCgA ep{p_new, q, ctx->d_ctl};
     KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, ld, ep, false, KID_CG_PASS_A));
     return rc;
 }
@@ -343,16 +338,16 @@ int plane_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, doubl
 int plane_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, const double* v_old, const double* r0,
                      double* p_new, double* v_new) {
     int rc = POISSON_OK;
-    const EpBicg1 ep{r, p_old, v_old, r0, p_new, v_new, ctx->d_ctl, 0.0, 0.0};
-    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdPhat<K>{r, p_old, v_old, ctx->d_ctl, ctx->opt_jacobi, 0.0, 0.0},
+    const EpBicg1 ep{r0, v_new, ctx->d_ctl};
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdPhat<K>{r, p_old, v_old, p_new, ctx->d_ctl, ctx->opt_jacobi, 0.0, 0.0},
                                                 ep, false, KID_BICG_PASS1));
     return rc;
 }
 
 int plane_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t) {
     int rc = POISSON_OK;
-    const EpBicg2 ep{r, v, s, t, ctx->d_ctl, 0.0};
-    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdShat<K>{r, v, ctx->d_ctl, ctx->opt_jacobi, 0.0}, ep, false,
+    const EpBicg2 ep{s, t, ctx->d_ctl};
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdShat<K>{r, v, s, ctx->d_ctl, ctx->opt_jacobi, 0.0}, ep, false,
                                                 KID_BICG_PASS2));
     return rc;
 }

@@ -89,7 +89,8 @@ struct RowCoef<KIND_SPH, RPT> {
 };
 
 // Loader / epilogue concepts (see k_plane.cu for the instances):
-//   struct Ld { struct Raw; void prepare(); Raw load(size_t p) const;
+//   struct Ld { struct Raw; static bool PLAIN, SIDE; void prepare(); Raw load(size_t p) const; Raw load_own(size_t p) const;
+//               void side(const Raw&, size_t p) const;   (pointwise side effect on owned points, e.g. the CG x-update)
 //               double2 form(const Op&, const Raw&, int i, int j, int k) const;   (pair starting at column i)
 //               double at(const Op&, size_t p, int i, int j, int k) const; };
 //   struct Ep { static constexpr int NRED; struct Raw; bool skip() const; void prepare(); Raw load(size_t p) const;
@@ -97,7 +98,8 @@ struct RowCoef<KIND_SPH, RPT> {
 //               void finish(const double* totals) const; };
 template <int KIND, class Cfg, class Ld, class Ep>
 __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
-    k_plane(const Op op, const Ld ld_in, const Ep ep_in, const int kc, const bool ug_in, RedBuf rb) {
+    k_plane(const Op op, const Ld ld_in, const Ep ep_in, const long items, const int per_tile, const int ntx, const bool ug_in,
+            RedBuf rb) {
     using G = PlaneGeom<KIND, Cfg>;
     constexpr int R = G::R, HX = G::HX, TX = G::TX, TY = G::TY, SW = G::SW, NS = G::NS, SLOT = G::SLOT;
     constexpr int RPT = G::RPT, NH = G::NH, PF = G::PF;
@@ -110,8 +112,25 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
     const bool ug = ug_in && op.gamma == 0.0;
     const int n0 = op.n[0], n1 = op.n[1], n2 = op.n[2];
     const int lx = threadIdx.x, ty = threadIdx.y, tid = ty * G::NTX + lx;
-    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
-    const int k0 = blockIdx.z * kc, k1 = min(n2, k0 + kc);
+    double acc[Ep::NRED > 0 ? Ep::NRED : 1];
+#pragma unroll
+    for (int r = 0; r < (Ep::NRED > 0 ? Ep::NRED : 1); ++r) acc[r] = 0.0;
+    // Work = (tile, plane) items; every CTA takes one contiguous run of them, cut into (tile, k0..k1) segments.
+    const long total = (long)ntx * ((n1 + TY - 1) / TY) * n2;
+    // per_tile > 0: whole z chunks, per_tile runs per tile (a run never straddles two tiles); else one linear split
+    long pos = (long)blockIdx.x * items;
+    long pend = min(total, pos + items);
+    if (per_tile > 0) {
+        const long t0 = (long)(blockIdx.x / per_tile) * n2;
+        pos = t0 + (long)(blockIdx.x % per_tile) * items;
+        pend = min(t0 + n2, pos + items);
+    }
+    while (pos < pend) {
+    const int tile = (int)(pos / n2), k0 = (int)(pos % n2);
+    const int k1 = (int)min((long)n2, (long)k0 + (pend - pos));
+    pos += k1 - k0;
+    const int i0 = (tile % ntx) * TX, j0 = (tile / ntx) * TY;
+    __syncthreads();  // the previous segment's readers are done with the ring
     const int i = i0 + 2 * lx;
     const int jrow = j0 + RPT * ty;  // first owned row
     bool act[RPT];
@@ -209,7 +228,7 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
             const size_t off = (size_t)s.kw * plane;
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                if (act[r]) s.o[r] = ld.load(off + base0 + (size_t)r * n0);
+                if (act[r]) s.o[r] = ld.load_own(off + base0 + (size_t)r * n0);
                 else if constexpr (Ld::PLAIN) s.o[r].a = bpair(i, jrow + r, s.kw);
             }
 #pragma unroll
@@ -235,9 +254,12 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
         } else if (s.kw >= 0) {
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                if (act[r])
+                if (act[r]) {
                     st2(slot + so0 + r * SW, ld.form(op, s.o[r], i, jrow + r, s.kw));
-                else
+                    if constexpr (Ld::SIDE) {
+                        if (kk >= k0 && kk < k1) ld.side(s.o[r], (size_t)s.kw * plane + base0 + (size_t)r * n0);
+                    }
+                } else
                     st2(slot + so0 + r * SW, bpair(i, jrow + r, s.kw));
             }
 #pragma unroll
@@ -273,10 +295,6 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                 if (act[r]) est[u][r] = ep.load((size_t)(k0 + u) * plane + base0 + (size_t)r * n0);
         }
     }
-
-    double acc[Ep::NRED > 0 ? Ep::NRED : 1];
-#pragma unroll
-    for (int r = 0; r < (Ep::NRED > 0 ? Ep::NRED : 1); ++r) acc[r] = 0.0;
 
     for (int kb = k0; kb < k1; kb += PF) {
 #pragma unroll
@@ -387,34 +405,13 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
             }
         }
     }
+    }  // segments
     if constexpr (Ep::NRED > 0) {
         double vals[Ep::NRED];
 #pragma unroll
         for (int r = 0; r < Ep::NRED; ++r) vals[r] = acc[r];
         grid_reduce<Ep::NRED>(vals, rb, [&](const double* t) { ep.finish(t); });
     }
-}
-
-// Number of z chunks: minimise (waves of CTAs) x (planes per chunk + the prologue of 2R planes).
-template <class G>
-static inline int plane_chunks(const Op& op, int slots, int* kc_out) {
-    const long tiles = (long)((op.n[0] + G::TX - 1) / G::TX) * ((op.n[1] + G::TY - 1) / G::TY);
-    int best = 1;
-    double best_cost = 1e300;
-    for (int nz = 1; nz <= op.n[2]; ++nz) {
-        const int kc = (op.n[2] + nz - 1) / nz;
-        if (kc < 4 && nz > 1) break;
-        const int nzz = (op.n[2] + kc - 1) / kc;
-        const long waves = (tiles * nzz + slots - 1) / slots;
-        const double cost = (double)waves * (kc + G::R + 1.0);
-        if (cost < best_cost - 1e-9) {
-            best_cost = cost;
-            best = nzz;
-        }
-    }
-    const int kc = (op.n[2] + best - 1) / best;
-    *kc_out = kc;
-    return (op.n[2] + kc - 1) / kc;
 }
 
 template <int KIND, class Cfg, class Ld, class Ep>
@@ -427,36 +424,52 @@ static int launch_plane_cfg(poisson_ctx* ctx, const Op& op, const Ld& ld, const 
         PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, G::NT, G::SMEM));
         if (resident < 1) return fail(ctx, POISSON_CUDA_ERROR, "plane kernel does not fit on an SM");
     }
-    int kc = 0;
-    const int nz = plane_chunks<G>(op, ctx->num_sms * resident, &kc);
-    const dim3 g((op.n[0] + G::TX - 1) / G::TX, (op.n[1] + G::TY - 1) / G::TY, nz), b(G::NTX, G::NTY);
-    if ((size_t)g.x * g.y * g.z > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large");
+    // equal runs of (tile, plane) items for all resident CTAs; a run shorter than ~4 planes is not worth a prologue
+    const int ntx = (op.n[0] + G::TX - 1) / G::TX, nty = (op.n[1] + G::TY - 1) / G::TY;
+    const long total = (long)ntx * nty * op.n[2];
+    const long slots = (long)ctx->num_sms * resident;
+    long items = (total + slots - 1) / slots;
+    if (items < 4) items = 4;
+    int per_tile = 0;
+    long nctas = (total + items - 1) / items;
+    {
+        // Alternative: whole z chunks (every CTA exactly one run inside one tile).  Estimated time = waves x (planes +
+        // prologue); the linear split pays about one more prologue and set-up per CTA.  Take the cheaper one.
+        const double cost_split = (double)items + 2.0 * (G::R + 1) + 4.0;
+        double best_cost = cost_split;
+        for (int nz = 1; nz <= op.n[2]; ++nz) {
+            const int kc = (op.n[2] + nz - 1) / nz;
+            if (kc < 4 && nz > 1) break;
+            const int nzz = (op.n[2] + kc - 1) / kc;
+            const long ctas = (long)ntx * nty * nzz;
+            const double cost = (double)((ctas + slots - 1) / slots) * (kc + G::R + 1.0);
+            if (cost < best_cost - 1e-9) {
+                best_cost = cost;
+                items = kc;
+                per_tile = nzz;
+                nctas = ctas;
+            }
+        }
+    }
+    const dim3 g((unsigned)nctas), b(G::NTX, G::NTY);
+    if ((size_t)g.x > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large");
     pre_launch(ctx, kid);
-    kern<<<g, b, G::SMEM, ctx->stream>>>(op, ld, ep, kc, ug, ctx->red);
+    kern<<<g, b, G::SMEM, ctx->stream>>>(op, ld, ep, items, per_tile, ntx, ug, ctx->red);
     post_launch(ctx, kid);
     return POISSON_OK;
 }
 
-// Tile choice per kernel class (measured on B200); POISSON_PLANE_CFG=<n> overrides for tuning.
+// Tile choice (measured on B200): 128 x 16 points, two rows per thread, one CTA per SM.
+// POISSON_PLANE_CFG=1 selects the 64 x 16 / two-CTAs-per-SM variant for tuning runs.
 using CfgA = TileCfg<128, 16, 2, 1, 1>;
-using CfgB = TileCfg<128, 16, 1, 1, 1>;
 using CfgC = TileCfg<64, 16, 2, 2, 1>;
-using CfgD = TileCfg<64, 16, 1, 2, 1>;
-using CfgE = TileCfg<128, 16, 2, 1, 2>;
-using CfgF = TileCfg<64, 16, 2, 2, 2>;
 
 int plane_cfg_override();
 
 template <int KIND, class Ld, class Ep>
 static int launch_plane(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
-    switch (plane_cfg_override()) {
-        case 1: return launch_plane_cfg<KIND, CfgB>(ctx, op, ld, ep, ug, kid);
-        case 2: return launch_plane_cfg<KIND, CfgC>(ctx, op, ld, ep, ug, kid);
-        case 3: return launch_plane_cfg<KIND, CfgD>(ctx, op, ld, ep, ug, kid);
-        case 4: return launch_plane_cfg<KIND, CfgE>(ctx, op, ld, ep, ug, kid);
-        case 5: return launch_plane_cfg<KIND, CfgF>(ctx, op, ld, ep, ug, kid);
-        default: return launch_plane_cfg<KIND, CfgA>(ctx, op, ld, ep, ug, kid);
-    }
+    if (plane_cfg_override() == 1) return launch_plane_cfg<KIND, CfgC>(ctx, op, ld, ep, ug, kid);
+    return launch_plane_cfg<KIND, CfgA>(ctx, op, ld, ep, ug, kid);
 }
 
 // The plane engine needs 16-byte aligned pairs: even n0 (every row then starts on a pair boundary).
