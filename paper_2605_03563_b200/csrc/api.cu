@@ -594,6 +594,16 @@ static int build_levels(poisson_ctx* ctx, int coarsest_n, bool mixed) {
 static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, bool ug, int nu1, int nu2, int csweeps) {
     MgLevel& L = ctx->levels[l];
     int rc;
+    if (!ug && L.npts <= 4096 && ctx->opt_path != 1) {  // the rest of the cycle fits one CTA's shared memory
+        Op ops[8];
+        const size_t nl = ctx->levels.size() - l;
+        if (nl <= 4) {
+            for (size_t m = 0; m < nl; ++m) ops[m] = ctx->levels[l + m].op;
+            const double omc = 2.0 / (1.0 + std::sin(M_PI / (ops[nl - 1].n[0] + 1)));
+            rc = launch_mg_bottom(ctx, ops, (int)nl, phi, rhs, nu1, nu2, csweeps, omc);
+            if (rc != POISSON_UNSUPPORTED) return rc;
+        }
+    }
     if (l + 1 == ctx->levels.size()) {
         const double om = 2.0 / (1.0 + std::sin(M_PI / (L.op.n[0] + 1)));  // Eq. 3-4 for n unknowns per axis
         rc = ug ? POISSON_UNSUPPORTED : launch_coarse_solve(ctx, L.op, phi, rhs, om, csweeps);
@@ -613,6 +623,16 @@ static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, b
 static int cycle32(poisson_ctx* ctx, size_t l, int nu1, int nu2, int csweeps) {
     MgLevel& L = ctx->levels[l];
     int rc;
+    if (L.npts <= 4096 && ctx->opt_path != 1) {
+        Op ops[8];
+        const size_t nl = ctx->levels.size() - l;
+        if (nl <= 4) {
+            for (size_t m = 0; m < nl; ++m) ops[m] = ctx->levels[l + m].op;
+            const double omc = 2.0 / (1.0 + std::sin(M_PI / (ops[nl - 1].n[0] + 1)));
+            rc = launch_mg_bottom32(ctx, ops, (int)nl, L.phi32, L.rhs32, nu1, nu2, csweeps, omc);
+            if (rc != POISSON_UNSUPPORTED) return rc;
+        }
+    }
     if (l + 1 == ctx->levels.size()) {
         const float om = (float)(2.0 / (1.0 + std::sin(M_PI / (L.op.n[0] + 1))));
         rc = launch_coarse_solve32(ctx, L.op, L.phi32, L.rhs32, om, csweeps);

@@ -175,6 +175,12 @@ int sor_fused(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const do
 int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps);
 void* sor_scratch(poisson_ctx* ctx, size_t bytes);  // nullptr on OOM
 
+// Lean 7-point apply / residual for non-periodic Cartesian grids (k_apply7.cu), fp64 and fp32
+bool apply7_ok(const poisson_ctx* ctx, const Op& op);
+int apply7(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32, int mode,
+           bool ug, bool reduce);
+int apply7_32(poisson_ctx* ctx, const Op& op, const float* v, const float* rhs, float* out, int mode);
+
 // Plane-pipeline versions (k_plane.cu) for pair-aligned grids; same results, bit for bit
 int plane_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out,
                 float* out32, int mode, bool ug, bool reduce);
@@ -193,6 +199,11 @@ int launch_prolong_add32(poisson_ctx* ctx, const Op& fine, const Op& coarse, con
 int launch_add32to64(poisson_ctx* ctx, size_t n, const float* e, double* phi);
 int launch_coarse_solve(poisson_ctx* ctx, const Op& op, double* phi, const double* rhs, double omega, int nsweeps);
 int launch_coarse_solve32(poisson_ctx* ctx, const Op& op, float* phi, const float* rhs, float omega, int nsweeps);
+// levels first..last (nlev operators) of the V-cycle in one CTA's shared memory; UNSUPPORTED when they do not fit
+int launch_mg_bottom(poisson_ctx* ctx, const Op* ops, int nlev, double* phi, const double* rhs, int nu1, int nu2,
+                     int csweeps, double omega_c);
+int launch_mg_bottom32(poisson_ctx* ctx, const Op* ops, int nlev, float* phi, const float* rhs, int nu1, int nu2,
+                       int csweeps, double omega_c);
 
 // Multipole
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q);

@@ -45,27 +45,56 @@ __device__ __forceinline__ T coarse_val(const Op& c, const T* __restrict__ e, in
 }
 
 template <typename T>
+struct Vec2 {};
+template <>
+struct Vec2<double> {
+    using type = double2;
+};
+template <>
+struct Vec2<float> {
+    using type = float2;
+};
+
+// phi += P e_c (trilinear, "P = c R^T").  One thread per COARSE cell: it reads the 3 x 3 x 3 coarse
+// neighbourhood once (ghost closure applied by coarse_val) and updates its 8 fine children, two x-adjacent ones per
+// 16-byte (fp64) access.  Per fine point the arithmetic is exactly
+//   ex = fma(3/4, e[I], 1/4 e[I +- 1]) ; ey = fma(3/4, ex[J], 1/4 ex[J +- 1]) ; v = fma(3/4, ey[K], 1/4 ey[K +- 1]).
+template <typename T>
 __global__ void __launch_bounds__(256)
     k_prolong_add(Op fine, Op coarse, const T* __restrict__ ec, T* __restrict__ phi) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
-    if (i >= fine.n[0] || j >= fine.n[1]) return;
-    const int I = i >> 1, J = j >> 1, K = k >> 1;
-    const int In = I + ((i & 1) ? 1 : -1), Jn = J + ((j & 1) ? 1 : -1), Kn = K + ((k & 1) ? 1 : -1);
-    T ey[2];
+    using V2 = typename Vec2<T>::type;
+    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    if (I >= coarse.n[0] || J >= coarse.n[1]) return;
+    T ex[2][3][3];  // [x parity][dJ][dK]
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
-        const int KK = c ? Kn : K;
-        T ex[2];
+    for (int dk = 0; dk < 3; ++dk)
 #pragma unroll
-        for (int b = 0; b < 2; ++b) {
-            const int JJ = b ? Jn : J;
-            const T nearv = coarse_val(coarse, ec, I, JJ, KK), farv = coarse_val(coarse, ec, In, JJ, KK);
-            ex[b] = fma_((T)0.75, nearv, (T)0.25 * farv);
+        for (int dj = 0; dj < 3; ++dj) {
+            const T em = coarse_val(coarse, ec, I - 1, J + dj - 1, K + dk - 1);
+            const T e0 = coarse_val(coarse, ec, I, J + dj - 1, K + dk - 1);
+            const T ep = coarse_val(coarse, ec, I + 1, J + dj - 1, K + dk - 1);
+            ex[0][dj][dk] = fma_((T)0.75, e0, (T)0.25 * em);
+            ex[1][dj][dk] = fma_((T)0.75, e0, (T)0.25 * ep);
         }
-        ey[c] = fma_((T)0.75, ex[0], (T)0.25 * ex[1]);
-    }
-    const T v = fma_((T)0.75, ey[0], (T)0.25 * ey[1]);
-    phi[gidx(fine, i, j, k)] += v;
+#pragma unroll
+    for (int pk = 0; pk < 2; ++pk)
+#pragma unroll
+        for (int pj = 0; pj < 2; ++pj) {
+            T v[2];
+#pragma unroll
+            for (int pi = 0; pi < 2; ++pi) {
+                // y: near row J (dj = 1), far row J - 1 (even fine j) or J + 1 (odd); same in z
+                const int fj = pj ? 2 : 0, fk = pk ? 2 : 0;
+                const T ey_near = fma_((T)0.75, ex[pi][1][1], (T)0.25 * ex[pi][fj][1]);
+                const T ey_far = fma_((T)0.75, ex[pi][1][fk], (T)0.25 * ex[pi][fj][fk]);
+                v[pi] = fma_((T)0.75, ey_near, (T)0.25 * ey_far);
+            }
+            V2* q = reinterpret_cast<V2*>(phi + gidx(fine, 2 * I, 2 * J + pj, 2 * K + pk));
+            V2 w = *q;
+            w.x += v[0];
+            w.y += v[1];
+            *q = w;
+        }
 }
 
 __global__ void __launch_bounds__(256) k_add32to64(size_t n, const float* __restrict__ e, double* __restrict__ phi) {
@@ -100,6 +129,185 @@ __global__ void __launch_bounds__(512)
     for (int q = threadIdx.x; q < n; q += blockDim.x) phi[q] = s[q];
 }
 
+// ---- the bottom of the V-cycle in one CTA ---------------------------------------------------------------------------------
+// Levels of at most 16^3 points are launch-latency bound (a dozen kernels of ~10 us each, plus 2 x 50 colour
+// half-sweeps on the coarsest grid).  This kernel runs the whole sub-cycle below such a level — pre-smoothing,
+// residual, restriction, recursion, coarsest-level SOR, prolongation + correction, post-smoothing — in the shared memory
+// of a single CTA, with the same arithmetic (row_offsum / row_diag, restriction and interpolation weights, order of
+// operations) as the per-level kernels above, so the results are bit-identical to the multi-launch path.
+constexpr int kBottomMaxLevels = 4;
+struct BottomArgs {
+    Op op[kBottomMaxLevels];
+    int nlev;
+    int nu1, nu2, csweeps, restriction;
+    double omega_c;
+};
+
+// nsweeps red-black sweeps on a grid of at most 4 x 1024 points held in shared memory.  Every thread first works out,
+// once, what its (up to four) points need — which neighbours exist, the diagonal and its reciprocal, the right-hand side
+// — so that a colour half-sweep is a handful of shared-memory reads and one exact division (div_by).
+template <typename T>
+__device__ void bottom_smooth(const Op& op, T* phi, const T* rhs, T omega, int nsweeps) {
+    constexpr int MP = 4;
+    const int n0 = op.n[0], n1 = op.n[1], n2 = op.n[2], n01 = n0 * n1, n = n01 * n2;
+    const T c0 = (T)op.c[0], c1 = (T)op.c[1], c2 = (T)op.c[2];
+    int msk[MP];
+    T dd[MP], rd[MP], f[MP];
+#pragma unroll
+    for (int m = 0; m < MP; ++m) {
+        const int q = threadIdx.x + m * 1024;
+        msk[m] = 0;
+        dd[m] = rd[m] = f[m] = (T)1;
+        if (q < n) {
+            const int i = q % n0, j = (q / n0) % n1, k = q / n01;
+            msk[m] = (i > 0 ? 1 : 0) | (i < n0 - 1 ? 2 : 0) | (j > 0 ? 4 : 0) | (j < n1 - 1 ? 8 : 0) | (k > 0 ? 16 : 0) |
+                     (k < n2 - 1 ? 32 : 0) | (((i + j + k) & 1) << 6) | 128;
+            dd[m] = row_diag<T, KIND_CART2>(op, i, j, k);
+            rd[m] = (T)1 / dd[m];
+            f[m] = rhs[q];
+        }
+    }
+    for (int sw = 0; sw < nsweeps; ++sw)
+        for (int colour = 0; colour < 2; ++colour) {
+#pragma unroll
+            for (int m = 0; m < MP; ++m) {
+                const int q = threadIdx.x + m * 1024, k = msk[m];
+                if (!(k & 128) || ((k >> 6) & 1) != colour) continue;
+                const T xm = (k & 1) ? phi[q - 1] : (T)0, xp = (k & 2) ? phi[q + 1] : (T)0;
+                const T ym = (k & 4) ? phi[q - n0] : (T)0, yp = (k & 8) ? phi[q + n0] : (T)0;
+                const T zm = (k & 16) ? phi[q - n01] : (T)0, zp = (k & 32) ? phi[q + n01] : (T)0;
+                T s = (xm + xp) * c0;
+                s = fma_(ym + yp, c1, s);
+                s = fma_(zm + zp, c2, s);
+                const T gs = div_by<T>(s - f[m], dd[m], rd[m]);
+                const T old = phi[q];
+                phi[q] = fma_(omega, gs - old, old);
+            }
+            __syncthreads();
+        }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(1024) k_mg_bottom(const BottomArgs a, T* __restrict__ g_phi, const T* __restrict__ g_rhs) {
+    extern __shared__ __align__(16) unsigned char smraw[];
+    T* base = reinterpret_cast<T*>(smraw);
+    T *phi[kBottomMaxLevels], *rhs[kBottomMaxLevels], *res[kBottomMaxLevels];
+    int npt[kBottomMaxLevels];
+    for (int l = 0; l < a.nlev; ++l) {
+        npt[l] = a.op[l].n[0] * a.op[l].n[1] * a.op[l].n[2];
+        phi[l] = base;
+        rhs[l] = base + npt[l];
+        res[l] = base + 2 * npt[l];
+        base += 3 * npt[l];
+    }
+    for (int q = threadIdx.x; q < npt[0]; q += blockDim.x) {
+        phi[0][q] = g_phi[q];
+        rhs[0][q] = g_rhs[q];
+    }
+    __syncthreads();
+    // downward leg
+    for (int l = 0; l + 1 < a.nlev; ++l) {
+        const Op& f = a.op[l];
+        const Op& c = a.op[l + 1];
+        bottom_smooth<T>(f, phi[l], rhs[l], (T)1, a.nu1);
+        const ArrLd<T> ld{phi[l]};
+        for (int q = threadIdx.x; q < npt[l]; q += blockDim.x) {
+            const int i = q % f.n[0], j = (q / f.n[0]) % f.n[1], k = q / (f.n[0] * f.n[1]);
+            res[l][q] = rhs[l][q] - row_apply<T, KIND_CART2>(f, ld, i, j, k, false);
+        }
+        __syncthreads();
+        const double W[4] = {0.125, 0.375, 0.375, 0.125};
+        for (int q = threadIdx.x; q < npt[l + 1]; q += blockDim.x) {
+            const int I = q % c.n[0], J = (q / c.n[0]) % c.n[1], K = q / (c.n[0] * c.n[1]);
+            T acc = 0;
+            if (a.restriction == 1) {
+                for (int cc = 0; cc < 2; ++cc)
+                    for (int b = 0; b < 2; ++b)
+                        for (int aa = 0; aa < 2; ++aa) acc += res[l][gidx(f, 2 * I + aa, 2 * J + b, 2 * K + cc)];
+                acc *= (T)0.125;
+            } else {
+                for (int cc = 0; cc < 4; ++cc)
+                    for (int b = 0; b < 4; ++b)
+                        for (int aa = 0; aa < 4; ++aa) {
+                            const int i = 2 * I - 1 + aa, j = 2 * J - 1 + b, k = 2 * K - 1 + cc;
+                            if (i < 0 || i >= f.n[0] || j < 0 || j >= f.n[1] || k < 0 || k >= f.n[2]) continue;
+                            acc += (T)(W[aa] * W[b] * W[cc]) * res[l][gidx(f, i, j, k)];
+                        }
+            }
+            rhs[l + 1][q] = acc;
+            phi[l + 1][q] = (T)0;
+        }
+        __syncthreads();
+    }
+    // coarsest level
+    {
+        const int l = a.nlev - 1;
+        bottom_smooth<T>(a.op[l], phi[l], rhs[l], (T)a.omega_c, a.csweeps);
+    }
+    // upward leg
+    for (int l = a.nlev - 2; l >= 0; --l) {
+        const Op& f = a.op[l];
+        const Op& c = a.op[l + 1];
+        for (int q = threadIdx.x; q < npt[l]; q += blockDim.x) {
+            const int i = q % f.n[0], j = (q / f.n[0]) % f.n[1], k = q / (f.n[0] * f.n[1]);
+            const int I = i >> 1, J = j >> 1, K = k >> 1;
+            const int In = I + ((i & 1) ? 1 : -1), Jn = J + ((j & 1) ? 1 : -1), Kn = K + ((k & 1) ? 1 : -1);
+            T ey[2];
+            for (int cc = 0; cc < 2; ++cc) {
+                const int KK = cc ? Kn : K;
+                T ex[2];
+                for (int b = 0; b < 2; ++b) {
+                    const int JJ = b ? Jn : J;
+                    const T nearv = coarse_val(c, phi[l + 1], I, JJ, KK), farv = coarse_val(c, phi[l + 1], In, JJ, KK);
+                    ex[b] = fma_((T)0.75, nearv, (T)0.25 * farv);
+                }
+                ey[cc] = fma_((T)0.75, ex[0], (T)0.25 * ex[1]);
+            }
+            phi[l][q] += fma_((T)0.75, ey[0], (T)0.25 * ey[1]);
+        }
+        __syncthreads();
+        bottom_smooth<T>(f, phi[l], rhs[l], (T)1, a.nu2);
+    }
+    for (int q = threadIdx.x; q < npt[0]; q += blockDim.x) g_phi[q] = phi[0][q];
+}
+
+// Runs levels first..last of the hierarchy (ops[] = their operators) in one CTA; UNSUPPORTED if they do not fit.
+template <typename T>
+static int bottom_t(poisson_ctx* ctx, const Op* ops, int nlev, T* phi, const T* rhs, int nu1, int nu2, int csweeps,
+                    double omega_c) {
+    if (nlev < 1 || nlev > kBottomMaxLevels) return POISSON_UNSUPPORTED;
+    BottomArgs a;
+    size_t elems = 0;
+    for (int l = 0; l < nlev; ++l) {
+        a.op[l] = ops[l];
+        elems += 3 * (size_t)ops[l].n[0] * ops[l].n[1] * ops[l].n[2];
+    }
+    const size_t bytes = elems * sizeof(T);
+    if (bytes > 200 * 1024) return POISSON_UNSUPPORTED;
+    a.nlev = nlev;
+    a.nu1 = nu1;
+    a.nu2 = nu2;
+    a.csweeps = csweeps;
+    a.restriction = ctx->opt_restriction;
+    a.omega_c = omega_c;
+    static bool attr_set = false;
+    if (!attr_set) {
+        PB_CUDA_OK(cudaFuncSetAttribute(k_mg_bottom<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_set = true;
+    }
+    PB_LAUNCH(ctx, KID_MG_COARSE, (k_mg_bottom<T><<<1, 1024, bytes, ctx->stream>>>(a, phi, rhs)));
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+int launch_mg_bottom(poisson_ctx* ctx, const Op* ops, int nlev, double* phi, const double* rhs, int nu1, int nu2,
+                     int csweeps, double omega_c) {
+    return bottom_t<double>(ctx, ops, nlev, phi, rhs, nu1, nu2, csweeps, omega_c);
+}
+int launch_mg_bottom32(poisson_ctx* ctx, const Op* ops, int nlev, float* phi, const float* rhs, int nu1, int nu2,
+                       int csweeps, double omega_c) {
+    return bottom_t<float>(ctx, ops, nlev, phi, rhs, nu1, nu2, csweeps, omega_c);
+}
+
 template <typename T>
 static int restrict_t(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T* r, T* fc, int restriction) {
     dim3 b(32, 8), g((coarse.n[0] + 31) / 32, (coarse.n[1] + 7) / 8, coarse.n[2]);
@@ -116,7 +324,7 @@ int launch_restrict32(poisson_ctx* ctx, const Op& f, const Op& c, const float* r
 
 template <typename T>
 static int prolong_t(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T* ec, T* phi) {
-    dim3 b(64, 4), g((fine.n[0] + 63) / 64, (fine.n[1] + 3) / 4, fine.n[2]);
+    dim3 b(32, 8), g((coarse.n[0] + 31) / 32, (coarse.n[1] + 7) / 8, coarse.n[2]);
     PB_LAUNCH(ctx, KID_MG_PROLONG, (k_prolong_add<T><<<g, b, 0, ctx->stream>>>(fine, coarse, ec, phi)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;

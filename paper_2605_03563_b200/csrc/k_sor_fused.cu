@@ -108,17 +108,6 @@ __device__ __forceinline__ T sor_diag_z(const Op& op, T d, int k) {
     return d;
 }
 
-// Correctly rounded a / d from the correctly rounded reciprocal rd = 1/d: two Markstein corrections (exact residuals
-// by fma).  Same result as IEEE division (no overflow / underflow on this path) without its slow-path branches.
-template <typename T>
-__device__ __forceinline__ T div_by(T a, T d, T rd) {
-    T q = a * rd;
-    T r = fma_(-d, q, a);
-    q = fma_(r, rd, q);
-    r = fma_(-d, q, a);
-    return fma_(r, rd, q);
-}
-
 template <typename T>
 __device__ __forceinline__ typename PairT<T>::type sor_bpair(const Op& op, int i, int j, int k, bool ug) {
     return PairT<T>::make(sor_bval<T>(op, i, j, k, ug), sor_bval<T>(op, i + 1, j, k, ug));

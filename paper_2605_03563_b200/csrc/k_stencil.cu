@@ -91,6 +91,7 @@ static int apply_dispatch(poisson_ctx* ctx, const Op& op, const T* v, const T* r
 
 int launch_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out, int mode,
                  bool ug, bool reduce) {
+    if (kind == KIND_CART2 && apply7_ok(ctx, op)) return apply7(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
     if (plane_ok(ctx, op)) return plane_apply(ctx, op, kind, v, rhs, out, nullptr, mode, ug, reduce);
     switch (kind) {
         case KIND_CART2: return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
@@ -100,10 +101,12 @@ int launch_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, cons
 }
 
 int launch_apply32(poisson_ctx* ctx, const Op& op, const float* v, const float* rhs, float* out, int mode) {
+    if (apply7_ok(ctx, op)) return apply7_32(ctx, op, v, rhs, out, mode);
     return apply_dispatch<float, KIND_CART2>(ctx, op, v, rhs, out, nullptr, mode, false, false);
 }
 
 int launch_residual_to32(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, float* out32, bool ug) {
+    if (apply7_ok(ctx, op)) return apply7(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
     if (plane_ok(ctx, op)) return plane_apply(ctx, op, KIND_CART2, v, rhs, nullptr, out32, 1, ug, true);
     return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
 }

@@ -131,6 +131,18 @@ __device__ __forceinline__ T row_apply(const Op& op, const Ld& v, int i, int j, 
                 row_offsum<T, KIND>(op, v, i, j, k, use_ghost));
 }
 
+// ---- division by a repeated divisor --------------------------------------------------------------------------------
+// Correctly rounded a / d from the correctly rounded reciprocal rd = 1/d: two Markstein corrections (exact residuals
+// by fma).  Same result as IEEE division (no overflow / underflow on this path) without its slow-path branches.
+template <typename T>
+__device__ __forceinline__ T div_by(T a, T d, T rd) {
+    T q = a * rd;
+    T r = fma_(-d, q, a);
+    q = fma_(r, rd, q);
+    r = fma_(-d, q, a);
+    return fma_(r, rd, q);
+}
+
 // ---- single-pass grid reduction -------------------------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double x) {
 #pragma unroll
