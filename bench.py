@@ -84,14 +84,35 @@ def measured_peak():
 
 
 def stored_traffic():
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture, or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(path):
-        try:
-            return json.load(open(path))
-        except Exception:
-            return None
-    return None
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.csv:
+    lines `kernel,dram_bytes_per_launch`), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    out = {}
+    try:
+        for line in open(path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 2 and f[0] and not f[0].startswith("#") and f[0] != "kernel":
+                out[f[0]] = float(f[1])
+    except Exception:
+        return None
+    return out or None
+
+
+def max_over_ranks(values, world, device="cpu"):
+    """Replicas only: the only cross-rank traffic of the bench is this MAX over the ranks' device
+    times (nccl on GPUs; gloo in the CPU test).  Returns the list of per-entry maxima."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_value(units_per_rank, world, ms_max, steps):
+    """Whole-job throughput in Gpoint-updates/s: every rank did `units_per_rank` point-updates per step."""
+    return world * units_per_rank * steps / (ms_max * 1e-3) / 1e9
 
 
 class ClockSampler:
@@ -323,10 +344,7 @@ def run_ours(args):
                 ktab["%s:%s" % (gname, kname)] = {"launches": cnt, "avg_ms": ms / cnt, "total_ms": ms}
         g.set_option(pb.OPT_TIME_KERNELS, -1)
 
-    tt = torch.tensor([ms_total, ms_e2e], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(tt[0]), float(tt[1])
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, "cuda")
     total_updates = sum(pts * u for _, pts, u in units)
     peak, peak_src = measured_peak()
     rows = []
@@ -340,7 +358,7 @@ def run_ours(args):
     achieved = 48.0 * n4 / (dom_ms / max(dom_cnt, 1) * 1e-3) / 1e9 if dom_cnt else None
     tr = stored_traffic()
     out = {
-        "metric": METRIC, "value": round(world * total_updates * args.steps / (ms_total * 1e-3) / 1e9, 3),
+        "metric": METRIC, "value": round(aggregate_value(total_updates, world, ms_total, args.steps), 3),
         "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": round(ms_total / args.steps, 3), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -354,13 +372,13 @@ def run_ours(args):
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "gpu_launches": launches,
         "clocks": clocks,
-        "e2e": {"value": round(world * total_updates * e2e_steps / (ms_e2e * 1e-3) / 1e9, 3), "unit": UNIT,
+        "e2e": {"value": round(aggregate_value(total_updates, world, ms_e2e, e2e_steps), 3), "unit": UNIT,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
                 "ms_per_step": round(ms_e2e / e2e_steps, 3)},
         "roofline": {"kernel": "cg_pass_a (19-point, 512^3): x += a p_old; p = r + b p_old; q = L p; sum p.q",
                      "bound": "hbm", "achieved": round(achieved, 1) if achieved else None, "peak": peak,
                      "unit": "GB/s", "frac": round(achieved / peak, 4) if achieved else None,
-                     "traffic": (tr or {}).get("cg_pass_a_dram_bytes_per_launch"),
+                     "traffic": (tr or {}).get("cg_pass_a"),
                      "algorithmic_bytes_per_launch": 48 * n4, "avg_launch_ms": round(dom_ms / max(dom_cnt, 1), 4),
                      "launches_timed": dom_cnt, "peak_source": peak_src},
         "rows": rows,

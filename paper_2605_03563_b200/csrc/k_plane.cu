@@ -11,15 +11,6 @@
 
 namespace pb {
 
-int plane_cfg_override() {
-    static int v = -1;
-    if (v < 0) {
-        const char* e = getenv("POISSON_PLANE_CFG");
-        v = e ? atoi(e) : 0;
-    }
-    return v;
-}
-
 // ---- loaders ------------------------------------------------------------------------------------------------------------
 struct LdArr {  // v itself
     static constexpr bool PLAIN = true, SIDE = false;

@@ -12,6 +12,9 @@
 // Out-of-range neighbours follow include/poisson.h: periodic wrap, ghost-face values, or zero.
 // Arithmetic order is the canonical one of stencil.cuh, so results are bit-identical to the generic kernels.
 #pragma once
+#include <algorithm>
+#include <cstdlib>
+
 #include "stencil.cuh"
 
 namespace pb {
@@ -414,8 +417,48 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
     }
 }
 
+// How one launch is cut into runs of (tile, plane) items, and what it is expected to cost (arbitrary time unit:
+// planes x rows of the tile, per wave).
+struct PlanePlan {
+    long items = 0, nctas = 0;
+    int per_tile = 0, ntx = 0;
+    double cost = 1e300;
+};
+
+// Two ways to schedule: whole z chunks (per_tile runs per tile, all tiles march z together, so the xy halo of a tile is
+// still in L2 when its neighbour asks for it) or one linear split into equal runs (all SMs busy for any grid, but
+// neighbouring tiles drift apart in z and their halos come from HBM again: measured +22 % DRAM traffic on the 512^3
+// 19-point CG pass).  The linear split therefore carries a penalty and wins only when chunks leave SMs idle.
+template <class G>
+static PlanePlan plane_plan(const Op& op, long slots) {
+    PlanePlan pl;
+    pl.ntx = (op.n[0] + G::TX - 1) / G::TX;
+    const int nty = (op.n[1] + G::TY - 1) / G::TY;
+    const long total = (long)pl.ntx * nty * op.n[2];
+    static const char* force_split = getenv("POISSON_PLANE_SPLIT");  // tuning aid: 1 = always split, 0 = never
+    const double halo_pen = force_split ? (atoi(force_split) ? 1e-3 : 1e3) : 1.0 + 0.15 * G::R;
+    pl.items = std::max(4L, (total + slots - 1) / slots);
+    pl.nctas = (total + pl.items - 1) / pl.items;
+    pl.per_tile = 0;
+    pl.cost = ((double)pl.items + 2.0 * (G::R + 1) + 4.0) * G::TY * halo_pen;
+    for (int nz = 1; nz <= op.n[2]; ++nz) {
+        const int kc = (op.n[2] + nz - 1) / nz;
+        if (kc < 4 && nz > 1) break;
+        const int nzz = (op.n[2] + kc - 1) / kc;
+        const long ctas = (long)pl.ntx * nty * nzz;
+        const double cost = (double)((ctas + slots - 1) / slots) * (kc + G::R + 1.0) * G::TY;
+        if (cost < pl.cost - 1e-9) {
+            pl.cost = cost;
+            pl.items = kc;
+            pl.per_tile = nzz;
+            pl.nctas = ctas;
+        }
+    }
+    return pl;
+}
+
 template <int KIND, class Cfg, class Ld, class Ep>
-static int launch_plane_cfg(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
+static int plane_resident(poisson_ctx* ctx, int* out) {
     using G = PlaneGeom<KIND, Cfg>;
     auto kern = k_plane<KIND, Cfg, Ld, Ep>;
     static int resident = 0;
@@ -424,52 +467,31 @@ static int launch_plane_cfg(poisson_ctx* ctx, const Op& op, const Ld& ld, const 
         PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, G::NT, G::SMEM));
         if (resident < 1) return fail(ctx, POISSON_CUDA_ERROR, "plane kernel does not fit on an SM");
     }
-    // equal runs of (tile, plane) items for all resident CTAs; a run shorter than ~4 planes is not worth a prologue
-    const int ntx = (op.n[0] + G::TX - 1) / G::TX, nty = (op.n[1] + G::TY - 1) / G::TY;
-    const long total = (long)ntx * nty * op.n[2];
-    const long slots = (long)ctx->num_sms * resident;
-    long items = (total + slots - 1) / slots;
-    if (items < 4) items = 4;
-    int per_tile = 0;
-    long nctas = (total + items - 1) / items;
-    {
-        // Alternative: whole z chunks (every CTA exactly one run inside one tile).  Estimated time = waves x (planes +
-        // prologue); the linear split pays about one more prologue and set-up per CTA.  Take the cheaper one.
-        const double cost_split = (double)items + 2.0 * (G::R + 1) + 4.0;
-        double best_cost = cost_split;
-        for (int nz = 1; nz <= op.n[2]; ++nz) {
-            const int kc = (op.n[2] + nz - 1) / nz;
-            if (kc < 4 && nz > 1) break;
-            const int nzz = (op.n[2] + kc - 1) / kc;
-            const long ctas = (long)ntx * nty * nzz;
-            const double cost = (double)((ctas + slots - 1) / slots) * (kc + G::R + 1.0);
-            if (cost < best_cost - 1e-9) {
-                best_cost = cost;
-                items = kc;
-                per_tile = nzz;
-                nctas = ctas;
-            }
-        }
-    }
-    const dim3 g((unsigned)nctas), b(G::NTX, G::NTY);
+    *out = resident;
+    return POISSON_OK;
+}
+
+template <int KIND, class Cfg, class Ld, class Ep>
+static int plane_run(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid, const PlanePlan& pl) {
+    using G = PlaneGeom<KIND, Cfg>;
+    const dim3 g((unsigned)pl.nctas), b(G::NTX, G::NTY);
     if ((size_t)g.x > (size_t)kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large");
     pre_launch(ctx, kid);
-    kern<<<g, b, G::SMEM, ctx->stream>>>(op, ld, ep, items, per_tile, ntx, ug, ctx->red);
+    k_plane<KIND, Cfg, Ld, Ep><<<g, b, G::SMEM, ctx->stream>>>(op, ld, ep, pl.items, pl.per_tile, pl.ntx, ug, ctx->red);
     post_launch(ctx, kid);
     return POISSON_OK;
 }
 
-// Tile choice (measured on B200): 128 x 16 points, two rows per thread, one CTA per SM.
-// POISSON_PLANE_CFG=1 selects the 64 x 16 / two-CTAs-per-SM variant for tuning runs.
+// Tile: 128 x 16 points, two rows per thread, one CTA per SM (measured on B200: 64 x 16 with two CTAs per SM, one row
+// per thread, 128 x 14 — which would give exactly 148 tiles on a 512^2 plane — and two-plane prefetch were all slower).
 using CfgA = TileCfg<128, 16, 2, 1, 1>;
-using CfgC = TileCfg<64, 16, 2, 2, 1>;
-
-int plane_cfg_override();
 
 template <int KIND, class Ld, class Ep>
 static int launch_plane(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
-    if (plane_cfg_override() == 1) return launch_plane_cfg<KIND, CfgC>(ctx, op, ld, ep, ug, kid);
-    return launch_plane_cfg<KIND, CfgA>(ctx, op, ld, ep, ug, kid);
+    int ra = 0, rc;
+    if ((rc = plane_resident<KIND, CfgA, Ld, Ep>(ctx, &ra)) != POISSON_OK) return rc;
+    const PlanePlan pa = plane_plan<PlaneGeom<KIND, CfgA>>(op, (long)ctx->num_sms * ra);
+    return plane_run<KIND, CfgA, Ld, Ep>(ctx, op, ld, ep, ug, kid, pa);
 }
 
 // The plane engine needs 16-byte aligned pairs: even n0 (every row then starts on a pair boundary).
