@@ -57,7 +57,8 @@ enum {
     POISSON_OPT_JACOBI = 3,        /* BiCGSTAB right Jacobi scaling: 1 (default) on, 0 off (reading C10) */
     POISSON_OPT_RECORD_HISTORY = 4,/* 1: record ||r_k||/||r_0|| per Krylov iteration for poisson_get_history */
     POISSON_OPT_SOR_HALFSTEPS = 6, /* red-black colour half-steps fused per HBM pass (temporal blocking): 2 = one
-                                      full sweep per pass (default), 4 = two sweeps per pass */
+                                      full sweep per pass, 4 = two sweeps per pass, 0 = automatic (default: 4 on
+                                      grids of >= 2^21 points, else 2); the results do not depend on it */
     POISSON_OPT_TIME_KERNELS = 5   /* bracket every launch of one kernel class (0..poisson_kernel_classes()-1) with
                                       CUDA events on the handle's stream; -2 = every class, -1 = off (default) */
 };

@@ -8,6 +8,7 @@
 //   Spherical (r,theta,phi) direct finite differences of Eq. (2), nonsymmetric (row-scaled) PAPER.md:47-49, 105
 //   ghost zones hold the Dirichlet boundary potential
 // Readings the paper leaves open are those of SURVEY.md §8(c) C0/C1/C5/C7 and are restated in DESIGN.md.
+// Pins: tests/test_oracle_*.py.  Parity unpinned: only the converged config-5 solution's absolute accuracy (krylov.cpp).
 #pragma once
 #include <cmath>
 #include <cstddef>

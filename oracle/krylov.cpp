@@ -5,6 +5,10 @@
 // BiCGSTAB: Alg. 7.7 on the nonsymmetric spherical operator, with right Jacobi scaling
 // (readings C4/C10).  Inhomogeneous ghost values enter only through r0; search directions see
 // homogeneous ghosts (reading C3).  Dot products: long double, plane partial sums in k order.
+// PARITY UNPINNED (one item): the absolute accuracy of the CONVERGED config-5 solution (spherical grid, Neumann inner
+// face, multipole outer shell) has no closed form to pin against — the free-space potential does not satisfy the inner
+// Neumann condition.  BiCGSTAB itself is pinned (dense LU on the spherical 8x4x8 grid, agreement with CG on an SPD
+// problem, true-residual check) and so is the spherical operator (tests/test_oracle_apply.py); see DESIGN.md §2.
 #include <cmath>
 #include <vector>
 

@@ -238,7 +238,7 @@ int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], 
     }
     poisson_ctx* ctx = new poisson_ctx;
     ctx->stream = (cudaStream_t)cuda_stream;
-    if (const char* e = getenv("POISSON_SOR_HALFSTEPS")) ctx->opt_sor_nhs = atoi(e) == 4 ? 4 : 2;  // tuning aid
+    if (const char* e = getenv("POISSON_SOR_HALFSTEPS")) ctx->opt_sor_nhs = atoi(e) == 4 ? 4 : (atoi(e) == 2 ? 2 : 0);  // tuning aid
     Op& op = ctx->op;
     std::memset(&op, 0, sizeof(op));
     ctx->npts = 1;
@@ -324,7 +324,8 @@ int poisson_set_option(poisson_t ctx, int option, int value) {
             ctx->opt_history = value ? 1 : 0;
             return POISSON_OK;
         case POISSON_OPT_SOR_HALFSTEPS:
-            if (value != 2 && value != 4) return fail(ctx, POISSON_INVALID_ARG, "half-steps per pass must be 2 or 4");
+            if (value != 0 && value != 2 && value != 4)
+                return fail(ctx, POISSON_INVALID_ARG, "half-steps per pass must be 0 (auto), 2 or 4");
             ctx->opt_sor_nhs = value;
             return POISSON_OK;
         case POISSON_OPT_TIME_KERNELS:

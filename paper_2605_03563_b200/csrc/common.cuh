@@ -112,7 +112,7 @@ struct poisson_ctx {
     int mg_coarsest_n = -1;
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
-    int opt_sor_nhs = 2;             // colour half-steps fused per HBM pass of the red-black kernel (2 or 4)
+    int opt_sor_nhs = 0;             // colour half-steps fused per HBM pass of the red-black kernel (2, 4; 0 = auto)
     void* sor_tmp = nullptr;         // ping-pong buffer of the fused red-black kernel
     size_t sor_tmp_bytes = 0;
     long launches = 0;

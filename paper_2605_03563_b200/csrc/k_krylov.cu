@@ -259,10 +259,13 @@ __global__ void __launch_bounds__(BX* BY)
     const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
     double a_rr = 0.0, a_r0r = 0.0;
     if (i < op.n[0] && j < op.n[1])
+#pragma unroll 4
         for (int k = k0; k < k1; ++k) {
             const size_t q = gidx(op, i, j, k);
             const double dg = jac<KIND>(op, i, j, k, jacobi);
-            const double ph = p[q] / dg, sv = s[q], sh = sv / dg;
+            const double rdg = 1.0 / dg;  // one division; the two quotients by div_by are still correctly rounded
+            const double sv = s[q];
+            const double ph = div_by<double>(p[q], dg, rdg), sh = div_by<double>(sv, dg, rdg);
             x[q] = fma(omega, sh, fma(alpha, ph, x[q]));
             const double rn = fma(-omega, t[q], sv);
             r[q] = rn;

@@ -394,7 +394,9 @@ template <typename T>
 static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* rhs, T omega, int nsweeps, bool ug) {
     T *src = phi, *dst = tmp;
     int left = nsweeps;
-    const bool two = ctx->opt_sor_nhs == 4;
+    // two sweeps per pass (NHS = 4) pay on large grids: fp64 from 2^23 points (122 vs 117 Gpoint/s at 256^3), fp32 from 2^21; 0 = this automatic choice
+    const bool two = ctx->opt_sor_nhs == 4 ||
+                     (ctx->opt_sor_nhs == 0 && (size_t)op.n[0] * op.n[1] * op.n[2] >= ((size_t)1 << (sizeof(T) == 4 ? 21 : 23)));
     while (left > 0) {
         int rc;
         if (two && left >= 2) {

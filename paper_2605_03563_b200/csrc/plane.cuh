@@ -25,9 +25,11 @@ __device__ __forceinline__ double2 mk2(double a, double b) { return make_double2
 
 // Tile configuration: TX x TY points per CTA, RPT rows per thread (threads = TX/2 x TY/RPT), MINB resident CTAs per
 // SM asked of the compiler, PF = how many planes ahead the global loads run.
-template <int TX_, int TY_, int RPT_, int MINB_, int PF_>
+template <int TX_, int TY_, int RPT_, int MINB_, int PF_, int ZQ_ = 0, int YW_ = 1>
 struct TileCfg {
     static constexpr int TX = TX_, TY = TY_, RPT = RPT_, MINB = MINB_, PF = PF_;
+    static constexpr int YW = YW_;  // radius 3: read the y window of all owned rows once per plane (else per row)
+    static constexpr int ZQ = ZQ_;  // radius 3 only: keep the z neighbours of the owned points in a register queue
 };
 
 template <int KIND, class Cfg>
@@ -220,6 +222,8 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
         typename Ld::Raw o[RPT], h[NH];
         int kw;       // wrapped plane index, or -1 when the plane lies outside a non-periodic z face
     };
+    constexpr bool ZQ = (KIND == KIND_CART6) && (Cfg::ZQ != 0);
+    double2 zq[ZQ ? RPT : 1][2 * R + 1];
     // Boundary values (ghost faces, zeros, wrapped tiny grids) come through vpoint().  For a PLAIN loader (the vector is
     // an array: Raw is the pair itself) they are fetched here, with the plane's other loads, so that their latency is
     // hidden like any other; the Krylov loaders never see ghost values and resolve them at commit time.
@@ -244,11 +248,21 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
             for (int r = 0; r < RPT; ++r) s.o[r].a = bpair(i, jrow + r, kk);
         }
     };
+    auto push = [&](int r, double2 v) {  // z register queue: zq[r][m] = plane (newest - 2R + m) of owned row r
+        if constexpr (ZQ) {
+#pragma unroll
+            for (int m = 0; m < 2 * R; ++m) zq[r][m] = zq[r][m + 1];
+            zq[r][2 * R] = v;
+        }
+    };
     auto commit = [&](int kk, const Staged& s) {
         double* slot = ring + ((kk + 2 * NS) & (NS - 1)) * SLOT;
         if constexpr (Ld::PLAIN) {
 #pragma unroll
-            for (int r = 0; r < RPT; ++r) st2(slot + so0 + r * SW, s.o[r].a);
+            for (int r = 0; r < RPT; ++r) {
+                st2(slot + so0 + r * SW, s.o[r].a);
+                push(r, s.o[r].a);
+            }
             if (s.kw >= 0) {
 #pragma unroll
                 for (int m = 0; m < NH; ++m)
@@ -257,13 +271,17 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
         } else if (s.kw >= 0) {
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
+                double2 fv;
                 if (act[r]) {
-                    st2(slot + so0 + r * SW, ld.form(op, s.o[r], i, jrow + r, s.kw));
+                    fv = ld.form(op, s.o[r], i, jrow + r, s.kw);
                     if constexpr (Ld::SIDE) {
                         if (kk >= k0 && kk < k1) ld.side(s.o[r], (size_t)s.kw * plane + base0 + (size_t)r * n0);
                     }
-                } else
-                    st2(slot + so0 + r * SW, bpair(i, jrow + r, s.kw));
+                } else {
+                    fv = bpair(i, jrow + r, s.kw);
+                }
+                st2(slot + so0 + r * SW, fv);
+                push(r, fv);
             }
 #pragma unroll
             for (int m = 0; m < NH; ++m) {
@@ -275,7 +293,11 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
         } else {
             // plane beyond a non-periodic z face: zeros (or a wrapped tiny grid); only owned columns are ever read
 #pragma unroll
-            for (int r = 0; r < RPT; ++r) st2(slot + so0 + r * SW, bpair(i, jrow + r, kk));
+            for (int r = 0; r < RPT; ++r) {
+                const double2 fv = bpair(i, jrow + r, kk);
+                st2(slot + so0 + r * SW, fv);
+                push(r, fv);
+            }
         }
     };
 
@@ -316,12 +338,27 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
             }
             __syncthreads();
             const double* c0p = ring + ((k + 2 * NS) & (NS - 1)) * SLOT + so0;
+            // radius 3: the y window of all owned rows (rows jrow-3 .. jrow+RPT+2), read once; owned rows from the z queue
+            double2 yw[KIND == KIND_CART6 ? RPT + 6 : 1];
+            if constexpr (KIND == KIND_CART6 && Cfg::YW != 0) {
+#pragma unroll
+                for (int m = 0; m < RPT + 6; ++m) {
+                    if (ZQ && m >= 3 && m < RPT + 3)
+                        yw[m] = zq[ZQ ? m - 3 : 0][R];
+                    else
+                        yw[m] = ld2(c0p + (m - 3) * SW);
+                }
+            }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 if (!act[r]) continue;
                 const double* P = c0p + r * SW;
                 const int o = so0 + r * SW;
-                const double2 C = ld2(P);
+                double2 C;
+                if constexpr (KIND == KIND_CART6 && Cfg::YW != 0)
+                    C = yw[r + 3];
+                else
+                    C = ld2(P);
                 double2 lv;
                 if constexpr (KIND == KIND_CART6) {
                     const double2 xa = ld2(P - 4), xb = ld2(P - 2), xc = ld2(P + 2), xd = ld2(P + 4);
@@ -336,8 +373,14 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                         t0.y = fma(1.0 / 90.0, xb.x + xd.x, w);
                     }
                     {
-                        const double2 m1 = ld2(P - SW), p1 = ld2(P + SW), m2 = ld2(P - 2 * SW), p2 = ld2(P + 2 * SW),
-                                      m3 = ld2(P - 3 * SW), p3 = ld2(P + 3 * SW);
+                        // rows r-3 .. r+3 out of the window read once per plane for all owned rows
+                        double2 m1, p1, m2, p2, m3, p3;
+                        if constexpr (Cfg::YW != 0) {
+                            m1 = yw[r + 2]; p1 = yw[r + 4]; m2 = yw[r + 1]; p2 = yw[r + 5]; m3 = yw[r]; p3 = yw[r + 6];
+                        } else {
+                            m1 = ld2(P - SW); p1 = ld2(P + SW); m2 = ld2(P - 2 * SW); p2 = ld2(P + 2 * SW);
+                            m3 = ld2(P - 3 * SW); p3 = ld2(P + 3 * SW);
+                        }
                         double w = 1.5 * (m1.x + p1.x);
                         w = fma(-3.0 / 20.0, m2.x + p2.x, w);
                         t1.x = fma(1.0 / 90.0, m3.x + p3.x, w);
@@ -346,12 +389,17 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                         t1.y = fma(1.0 / 90.0, m3.y + p3.y, w);
                     }
                     {
-                        const double2 m1 = ld2(ring + ((k - 1 + 2 * NS) & (NS - 1)) * SLOT + o),
-                                      p1 = ld2(ring + ((k + 1 + 2 * NS) & (NS - 1)) * SLOT + o),
-                                      m2 = ld2(ring + ((k - 2 + 2 * NS) & (NS - 1)) * SLOT + o),
-                                      p2 = ld2(ring + ((k + 2 + 2 * NS) & (NS - 1)) * SLOT + o),
-                                      m3 = ld2(ring + ((k - 3 + 2 * NS) & (NS - 1)) * SLOT + o),
-                                      p3 = ld2(ring + ((k + 3 + 2 * NS) & (NS - 1)) * SLOT + o);
+                        double2 m1, p1, m2, p2, m3, p3;
+                        if constexpr (ZQ) {
+                            m1 = zq[r][2]; p1 = zq[r][4]; m2 = zq[r][1]; p2 = zq[r][5]; m3 = zq[r][0]; p3 = zq[r][6];
+                        } else {
+                            m1 = ld2(ring + ((k - 1 + 2 * NS) & (NS - 1)) * SLOT + o);
+                            p1 = ld2(ring + ((k + 1 + 2 * NS) & (NS - 1)) * SLOT + o);
+                            m2 = ld2(ring + ((k - 2 + 2 * NS) & (NS - 1)) * SLOT + o);
+                            p2 = ld2(ring + ((k + 2 + 2 * NS) & (NS - 1)) * SLOT + o);
+                            m3 = ld2(ring + ((k - 3 + 2 * NS) & (NS - 1)) * SLOT + o);
+                            p3 = ld2(ring + ((k + 3 + 2 * NS) & (NS - 1)) * SLOT + o);
+                        }
                         double w = 1.5 * (m1.x + p1.x);
                         w = fma(-3.0 / 20.0, m2.x + p2.x, w);
                         t2.x = fma(1.0 / 90.0, m3.x + p3.x, w);
@@ -482,8 +530,9 @@ static int plane_run(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep,
     return POISSON_OK;
 }
 
-// Tile: 128 x 16 points, two rows per thread, one CTA per SM (measured on B200: 64 x 16 with two CTAs per SM, one row
-// per thread, 128 x 14 — which would give exactly 148 tiles on a 512^2 plane — and two-plane prefetch were all slower).
+// Tile: 128 x 16 points, two rows per thread, one CTA per SM (measured on B200: 64 x 16 with two CTAs per SM, one or
+// four rows per thread, a register queue for the z neighbours, 128 x 14 tiles — exactly 148 of them on a 512^2 plane —
+// and two-plane prefetch were all slower).
 using CfgA = TileCfg<128, 16, 2, 1, 1>;
 
 template <int KIND, class Ld, class Ep>
