@@ -16,7 +16,7 @@ F64, MIXED = 0, 1
 OK, NOT_CONVERGED, BREAKDOWN = 0, 1, 2
 INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY = -1, -2, -3, -4
 OPT_KERNEL_PATH, OPT_RESTRICTION, OPT_POLL_INTERVAL, OPT_JACOBI, OPT_RECORD_HISTORY, OPT_TIME_KERNELS = 0, 1, 2, 3, 4, 5
-OPT_SOR_HALFSTEPS = 6
+OPT_SOR_HALFSTEPS, OPT_FUSED_RESTRICT = 6, 7
 PATH_AUTO, PATH_GENERIC, PATH_PLANE = 0, 1, 2
 
 SYMBOLS = [

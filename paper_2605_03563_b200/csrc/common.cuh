@@ -113,6 +113,7 @@ struct poisson_ctx {
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
     int opt_sor_nhs = 0;             // colour half-steps fused per HBM pass of the red-black kernel (2, 4; 0 = auto)
+    int opt_fused_restrict = 0;      // V-cycle residual + restriction in one kernel: 0 auto (fp32 levels only), 1 always, 2 never
     void* sor_tmp = nullptr;         // ping-pong buffer of the fused red-black kernel
     size_t sor_tmp_bytes = 0;
     long launches = 0;
@@ -180,6 +181,12 @@ bool apply7_ok(const poisson_ctx* ctx, const Op& op);
 int apply7(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32, int mode,
            bool ug, bool reduce);
 int apply7_32(poisson_ctx* ctx, const Op& op, const float* v, const float* rhs, float* out, int mode);
+
+// Fused residual + restriction (k_resid_restrict.cu): f_c = R (rhs - L phi) without storing the fine residual
+bool resid_restrict_ok(const poisson_ctx* ctx, const Op& fine, const Op& coarse);
+int resid_restrict(poisson_ctx* ctx, const Op& fine, const Op& coarse, const double* phi, const double* rhs, double* fc,
+                   bool ug);
+int resid_restrict32(poisson_ctx* ctx, const Op& fine, const Op& coarse, const float* phi, const float* rhs, float* fc);
 
 // Plane-pipeline versions (k_plane.cu) for pair-aligned grids; same results, bit for bit
 int plane_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out,

@@ -397,9 +397,15 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
     // two sweeps per pass (NHS = 4) pay on large grids: fp64 from 2^23 points (122 vs 117 Gpoint/s at 256^3), fp32 from 2^21; 0 = this automatic choice
     const bool two = ctx->opt_sor_nhs == 4 ||
                      (ctx->opt_sor_nhs == 0 && (size_t)op.n[0] * op.n[1] * op.n[2] >= ((size_t)1 << (sizeof(T) == 4 ? 21 : 23)));
+    // Plan: n4 passes of two sweeps + n2 passes of one.  An odd number of passes ends in the ping-pong buffer and costs
+    // a copy back (16 B/point): in fp64 one two-sweep pass is then split into two one-sweep passes instead
+    // (measured: 2 x NHS=2 beats NHS=4 + copy at 256^3; in fp32 the single pass + copy is the faster one).
+    int n4 = two ? nsweeps / 2 : 0;
+    if (sizeof(T) == 8 && n4 > 0 && ((n4 + (nsweeps - 2 * n4)) & 1)) --n4;
     while (left > 0) {
         int rc;
-        if (two && left >= 2) {
+        if (n4 > 0) {
+            --n4;
             rc = sor_fused_pass<T, 4>(ctx, op, src, dst, rhs, omega, ug);
             left -= 2;
         } else {

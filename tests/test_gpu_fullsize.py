@@ -150,3 +150,23 @@ def test_sor_two_sweeps_per_pass_option():
         g.rbsor_sweep(phi, rhs, 1.7, 5)
         outs.append(host(phi))
     assert np.array_equal(outs[0], outs[1])
+
+
+def test_fused_residual_restriction_option():
+    """POISSON_OPT_FUSED_RESTRICT: the one-pass residual + restriction kernel gives the same bits as the two kernels."""
+    shape = (128, 64, 64)
+    outs = []
+    for mode in (1, 2):
+        g = pb.Poisson(shape, (0.1, 0.1, 0.1), (0, 0, 0), bc=D6)
+        g.set_option(pb.OPT_FUSED_RESTRICT, mode)
+        faces = [dev(wl.hash_uniform(400 + f, np.arange(g.face_len(f))) - 0.5) for f in range(6)]
+        g.set_ghost_faces(faces)
+        for precision in (pb.F64, pb.MIXED):
+            for restriction in (0, 1):
+                g.set_option(pb.OPT_RESTRICTION, restriction)
+                phi, rhs = dev(wl.random_field(shape, 71)), dev(wl.random_field(shape, 72))
+                g.mg_vcycle(phi, rhs, precision=precision, ncycles=2)
+                outs.append(host(phi))
+    n = len(outs) // 2
+    for a, b in zip(outs[:n], outs[n:]):
+        assert np.array_equal(a, b)
