@@ -98,6 +98,8 @@ static void free_levels(poisson_ctx* ctx) {
         cudaFree(L.phi32);
         cudaFree(L.rhs32);
         cudaFree(L.res32);
+        cudaFree(L.alt);
+        cudaFree(L.alt32);
     }
     ctx->levels.clear();
     ctx->mg_coarsest_n = -1;
@@ -587,18 +589,24 @@ static int build_levels(poisson_ctx* ctx, int coarsest_n, bool mixed) {
             if (l > 0 && !L.phi) PB_CUDA_OK(cudaMalloc((void**)&L.phi, b64));
             if (l > 0 && !L.rhs) PB_CUDA_OK(cudaMalloc((void**)&L.rhs, b64));
             if (!L.res) PB_CUDA_OK(cudaMalloc((void**)&L.res, b64));
+            if (!L.alt) PB_CUDA_OK(cudaMalloc((void**)&L.alt, b64));
         } else {
             if (!L.phi32) PB_CUDA_OK(cudaMalloc((void**)&L.phi32, b32));
             if (!L.rhs32) PB_CUDA_OK(cudaMalloc((void**)&L.rhs32, b32));
             if (!L.res32) PB_CUDA_OK(cudaMalloc((void**)&L.res32, b32));
+            if (!L.alt32) PB_CUDA_OK(cudaMalloc((void**)&L.alt32, b32));
         }
     }
     return POISSON_OK;
 }
 
-static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, bool ug, int nu1, int nu2, int csweeps) {
+// One V-cycle on level l and below.  The field of the level starts in `phi`; the red-black passes ping-pong between it
+// and the level's second buffer, and *result tells the caller which of the two holds the outcome (no copies).
+static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, bool ug, int nu1, int nu2, int csweeps,
+                   double** result) {
     MgLevel& L = ctx->levels[l];
     int rc;
+    *result = phi;
     if (!ug && L.npts <= 4096 && ctx->opt_path != 1) {  // the rest of the cycle fits one CTA's shared memory
         Op ops[8];
         const size_t nl = ctx->levels.size() - l;
@@ -616,24 +624,29 @@ static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, b
         return rc;
     }
     MgLevel& C = ctx->levels[l + 1];
-    if ((rc = launch_rbsor(ctx, L.op, KIND_CART2, phi, rhs, 1.0, nu1, ug)) != POISSON_OK) return rc;
+    double* cur = phi;
+    if ((rc = launch_rbsor_pp(ctx, L.op, &cur, phi, L.alt, rhs, 1.0, nu1, ug)) != POISSON_OK) return rc;
     // residual and restriction in one pass (no fine residual in memory): in fp64 the two separate kernels are still
     // ~10 % faster at 256^3 (the 64-term ordered sum stalls the CTA), so the fused kernel is opt-in there
     if (ctx->opt_fused_restrict == 1 && resid_restrict_ok(ctx, L.op, C.op)) {
-        if ((rc = resid_restrict(ctx, L.op, C.op, phi, rhs, C.rhs, ug)) != POISSON_OK) return rc;
+        if ((rc = resid_restrict(ctx, L.op, C.op, cur, rhs, C.rhs, ug)) != POISSON_OK) return rc;
     } else {
-        if ((rc = launch_apply(ctx, L.op, KIND_CART2, phi, rhs, L.res, 1, ug, false)) != POISSON_OK) return rc;
+        if ((rc = launch_apply(ctx, L.op, KIND_CART2, cur, rhs, L.res, 1, ug, false)) != POISSON_OK) return rc;
         if ((rc = launch_restrict(ctx, L.op, C.op, L.res, C.rhs, ctx->opt_restriction)) != POISSON_OK) return rc;
     }
     PB_CUDA_OK(cudaMemsetAsync(C.phi, 0, C.npts * sizeof(double), ctx->stream));
-    if ((rc = cycle64(ctx, l + 1, C.phi, C.rhs, false, nu1, nu2, csweeps)) != POISSON_OK) return rc;
-    if ((rc = launch_prolong_add(ctx, L.op, C.op, C.phi, phi)) != POISSON_OK) return rc;
-    return launch_rbsor(ctx, L.op, KIND_CART2, phi, rhs, 1.0, nu2, ug);
+    double* ec = C.phi;
+    if ((rc = cycle64(ctx, l + 1, C.phi, C.rhs, false, nu1, nu2, csweeps, &ec)) != POISSON_OK) return rc;
+    if ((rc = launch_prolong_add(ctx, L.op, C.op, ec, cur)) != POISSON_OK) return rc;
+    if ((rc = launch_rbsor_pp(ctx, L.op, &cur, phi, L.alt, rhs, 1.0, nu2, ug)) != POISSON_OK) return rc;
+    *result = cur;
+    return POISSON_OK;
 }
 
-static int cycle32(poisson_ctx* ctx, size_t l, int nu1, int nu2, int csweeps) {
+static int cycle32(poisson_ctx* ctx, size_t l, int nu1, int nu2, int csweeps, float** result) {
     MgLevel& L = ctx->levels[l];
     int rc;
+    *result = L.phi32;
     if (L.npts <= 4096 && ctx->opt_path != 1) {
         Op ops[8];
         const size_t nl = ctx->levels.size() - l;
@@ -651,17 +664,21 @@ static int cycle32(poisson_ctx* ctx, size_t l, int nu1, int nu2, int csweeps) {
         return rc;
     }
     MgLevel& C = ctx->levels[l + 1];
-    if ((rc = launch_rbsor32(ctx, L.op, L.phi32, L.rhs32, 1.0f, nu1)) != POISSON_OK) return rc;
+    float* cur = L.phi32;
+    if ((rc = launch_rbsor_pp32(ctx, L.op, &cur, L.phi32, L.alt32, L.rhs32, 1.0f, nu1)) != POISSON_OK) return rc;
     if (ctx->opt_fused_restrict != 2 && resid_restrict_ok(ctx, L.op, C.op)) {
-        if ((rc = resid_restrict32(ctx, L.op, C.op, L.phi32, L.rhs32, C.rhs32)) != POISSON_OK) return rc;
+        if ((rc = resid_restrict32(ctx, L.op, C.op, cur, L.rhs32, C.rhs32)) != POISSON_OK) return rc;
     } else {
-        if ((rc = launch_apply32(ctx, L.op, L.phi32, L.rhs32, L.res32, 1)) != POISSON_OK) return rc;
+        if ((rc = launch_apply32(ctx, L.op, cur, L.rhs32, L.res32, 1)) != POISSON_OK) return rc;
         if ((rc = launch_restrict32(ctx, L.op, C.op, L.res32, C.rhs32, ctx->opt_restriction)) != POISSON_OK) return rc;
     }
     PB_CUDA_OK(cudaMemsetAsync(C.phi32, 0, C.npts * sizeof(float), ctx->stream));
-    if ((rc = cycle32(ctx, l + 1, nu1, nu2, csweeps)) != POISSON_OK) return rc;
-    if ((rc = launch_prolong_add32(ctx, L.op, C.op, C.phi32, L.phi32)) != POISSON_OK) return rc;
-    return launch_rbsor32(ctx, L.op, L.phi32, L.rhs32, 1.0f, nu2);
+    float* ec = C.phi32;
+    if ((rc = cycle32(ctx, l + 1, nu1, nu2, csweeps, &ec)) != POISSON_OK) return rc;
+    if ((rc = launch_prolong_add32(ctx, L.op, C.op, ec, cur)) != POISSON_OK) return rc;
+    if ((rc = launch_rbsor_pp32(ctx, L.op, &cur, L.phi32, L.alt32, L.rhs32, 1.0f, nu2)) != POISSON_OK) return rc;
+    *result = cur;
+    return POISSON_OK;
 }
 
 int poisson_mg_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
@@ -689,15 +706,19 @@ int poisson_mg_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1
     if ((rc = record_norm(0)) != POISSON_OK) return rc;
     for (int c = 0; c < ncycles; ++c) {
         if (precision == POISSON_F64) {
-            rc = cycle64(ctx, 0, d_phi, d_rhs, true, nu1, nu2, coarsest_sweeps);
+            double* res = d_phi;
+            rc = cycle64(ctx, 0, d_phi, d_rhs, true, nu1, nu2, coarsest_sweeps, &res);
+            if (rc == POISSON_OK && res != d_phi)  // an odd number of ping-pong passes on level 0
+                PB_CUDA_OK(cudaMemcpyAsync(d_phi, res, ctx->npts * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
         } else {
             MgLevel& L0 = ctx->levels[0];
             rc = launch_residual_to32(ctx, ctx->op, d_phi, d_rhs, L0.rhs32, true);
             if (rc != POISSON_OK) return rc;
             PB_CUDA_OK(cudaMemsetAsync(L0.phi32, 0, L0.npts * sizeof(float), ctx->stream));
-            rc = cycle32(ctx, 0, nu1, nu2, coarsest_sweeps);
+            float* e32 = L0.phi32;
+            rc = cycle32(ctx, 0, nu1, nu2, coarsest_sweeps, &e32);
             if (rc != POISSON_OK) return rc;
-            rc = launch_add32to64(ctx, L0.npts, L0.phi32, d_phi);
+            rc = launch_add32to64(ctx, L0.npts, e32, d_phi);
         }
         if (rc != POISSON_OK) return rc;
         if ((rc = record_norm(c + 1)) != POISSON_OK) return rc;

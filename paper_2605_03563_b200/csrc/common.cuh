@@ -82,6 +82,8 @@ struct MgLevel {
     size_t npts = 0;
     double *phi = nullptr, *rhs = nullptr, *res = nullptr;     // fp64 storage (levels >= 1; level 0 uses caller's)
     float *phi32 = nullptr, *rhs32 = nullptr, *res32 = nullptr;  // fp32 storage (mixed path, all levels)
+    double* alt = nullptr;   // second buffer of the level's field for the ping-pong red-black sweeps
+    float* alt32 = nullptr;
 };
 
 }  // namespace pb
@@ -171,9 +173,17 @@ int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double
 
 // Fused red-black sweeps (k_sor_fused.cu): both colours (or two sweeps) per HBM pass, ping-pong through tmp
 bool sor_fused_ok(const poisson_ctx* ctx, const Op& op);
+// result == nullptr: the sweeps end in phi (copy back if needed); else *result = the buffer (phi or tmp) that holds them
 int sor_fused(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, double omega, int nsweeps,
-              bool ug);
-int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps);
+              bool ug, double** result = nullptr);
+int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps,
+                float** result = nullptr);
+// V-cycle smoothing: nsweeps sweeps of the field in *cur (one of the level's two buffers a, b); *cur then points at the
+// buffer that holds the result — never a copy back
+int launch_rbsor_pp(poisson_ctx* ctx, const Op& op, double** cur, double* a, double* b, const double* rhs, double omega,
+                    int nsweeps, bool ug);
+int launch_rbsor_pp32(poisson_ctx* ctx, const Op& op, float** cur, float* a, float* b, const float* rhs, float omega,
+                      int nsweeps);
 void* sor_scratch(poisson_ctx* ctx, size_t bytes);  // nullptr on OOM
 
 // Lean 7-point apply / residual for non-periodic Cartesian grids (k_apply7.cu), fp64 and fp32

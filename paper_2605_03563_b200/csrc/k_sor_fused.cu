@@ -141,7 +141,9 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
     const T dplain = (T)2 * ((c0 + c1) + c2);
     const T rdplain = (T)1 / dplain;
     const size_t plane = (size_t)n0 * n1;
-    T* const mine = ring + ly * SW + 2 * lx;  // this thread's pair in slot 0
+    // Shared-memory planes are stored de-interleaved: row = [even columns | odd columns], so that the 8-byte reads of
+    // one column parity by consecutive lanes are consecutive words (no bank conflicts; the interleaved layout had 2-way)
+    T* const mine = ring + ly * SW + lx;  // column 0 of this thread's pair in slot 0; column 1 is PXN words further
 
     const long total = (long)g.ntx * g.nty * n2;
     long pos = (long)blockIdx.x * g.items;
@@ -159,12 +161,14 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
         // (i + c + j + kin) odd with i even  ->  cA = 1 - (j & 1).
         const int cA = 1 - (j & 1);
         // shared-memory offsets (relative to `mine`) of each column's own cell and of its three outside neighbours
-        const int xoA = cA ? (lx < PXN - 1 ? 2 : 1) : (lx > 0 ? -1 : 0);
-        const int xoB = cA ? (lx > 0 ? -1 : 0) : (lx < PXN - 1 ? 2 : 1);
-        const int ymA = cA + (ly > 0 ? -SW : 0), ypA = cA + (ly < EY - 1 ? SW : 0);
-        const int ymB = (1 - cA) + (ly > 0 ? -SW : 0), ypB = (1 - cA) + (ly < EY - 1 ? SW : 0);
-        T* const mineA = mine + cA;
-        T* const mineB = mine + 1 - cA;
+        const int selfA = cA * PXN, selfB = (1 - cA) * PXN;
+        // outer x neighbour: left of column 0 = column 1 of the pair to the left; right of column 1 = column 0 of the next
+        const int xo0 = lx > 0 ? PXN - 1 : 0, xo1 = lx < PXN - 1 ? 1 : PXN;
+        const int xoA = cA ? xo1 : xo0, xoB = cA ? xo0 : xo1;
+        const int ymA = selfA + (ly > 0 ? -SW : 0), ypA = selfA + (ly < EY - 1 ? SW : 0);
+        const int ymB = selfB + (ly > 0 ? -SW : 0), ypB = selfB + (ly < EY - 1 ? SW : 0);
+        T* const mineA = mine + selfA;
+        T* const mineB = mine + selfB;
         T dA = dplain, dB = dplain, rdA = rdplain, rdB = rdplain;
         if (!PLAIN && col_in) {
             dA = sor_diag_xy<T>(op, i + cA, j);
@@ -250,7 +254,10 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                 qB[p0] = cA ? nv.x : nv.y;
                 fA[p0] = cA ? nr.y : nr.x;
                 fB[p0] = cA ? nr.x : nr.y;
-                if (live) *reinterpret_cast<P2*>(mine + u * SLOT) = nv;  // slot of plane kin is u
+                if (live) {  // slot of plane kin is u
+                    mine[u * SLOT] = nv.x;
+                    mine[u * SLOT + PXN] = nv.y;
+                }
                 pout += plane;
                 if (kin + PF <= kend) {
                     nvq[u % PF] = loadv(kin + PF);
@@ -391,7 +398,8 @@ bool sor_fused_ok(const poisson_ctx* ctx, const Op& op) {
 
 // nsweeps full sweeps phi -> phi through the ping-pong buffer tmp (same size as phi).
 template <typename T>
-static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* rhs, T omega, int nsweeps, bool ug) {
+static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* rhs, T omega, int nsweeps, bool ug,
+                       T** result) {
     T *src = phi, *dst = tmp;
     int left = nsweeps;
     // two sweeps per pass (NHS = 4) pay on large grids: fp64 from 2^23 points (122 vs 117 Gpoint/s at 256^3), fp32 from 2^21; 0 = this automatic choice
@@ -401,7 +409,7 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
     // a copy back (16 B/point): in fp64 one two-sweep pass is then split into two one-sweep passes instead
     // (measured: 2 x NHS=2 beats NHS=4 + copy at 256^3; in fp32 the single pass + copy is the faster one).
     int n4 = two ? nsweeps / 2 : 0;
-    if (sizeof(T) == 8 && n4 > 0 && ((n4 + (nsweeps - 2 * n4)) & 1)) --n4;
+    if (!result && sizeof(T) == 8 && n4 > 0 && ((n4 + (nsweeps - 2 * n4)) & 1)) --n4;
     while (left > 0) {
         int rc;
         if (n4 > 0) {
@@ -416,7 +424,9 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
         std::swap(src, dst);
     }
     PB_CUDA_OK(cudaGetLastError());
-    if (src != phi) {
+    if (result) {
+        *result = src;  // the caller carries on with whichever buffer holds the result (V-cycle: no copy back)
+    } else if (src != phi) {
         const size_t bytes = (size_t)op.n[0] * op.n[1] * op.n[2] * sizeof(T);
         PB_CUDA_OK(cudaMemcpyAsync(phi, src, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
     }
@@ -424,11 +434,12 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
 }
 
 int sor_fused(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, double omega, int nsweeps,
-              bool ug) {
-    return sor_fused_t<double>(ctx, op, phi, tmp, rhs, omega, nsweeps, ug);
+              bool ug, double** result) {
+    return sor_fused_t<double>(ctx, op, phi, tmp, rhs, omega, nsweeps, ug, result);
 }
-int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps) {
-    return sor_fused_t<float>(ctx, op, phi, tmp, rhs, omega, nsweeps, false);
+int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps,
+                float** result) {
+    return sor_fused_t<float>(ctx, op, phi, tmp, rhs, omega, nsweeps, false, result);
 }
 
 }  // namespace pb

@@ -145,4 +145,18 @@ int launch_rbsor32(poisson_ctx* ctx, const Op& op, float* phi, const float* rhs,
     return rbsor_dispatch<float, KIND_CART2>(ctx, op, phi, rhs, omega, nsweeps, false);
 }
 
+int launch_rbsor_pp(poisson_ctx* ctx, const Op& op, double** cur, double* a, double* b, const double* rhs, double omega,
+                    int nsweeps, bool ug) {
+    if (nsweeps > 0 && a && b && sor_fused_ok(ctx, op))
+        return sor_fused(ctx, op, *cur, *cur == a ? b : a, rhs, omega, nsweeps, ug, cur);
+    return launch_rbsor(ctx, op, KIND_CART2, *cur, rhs, omega, nsweeps, ug);
+}
+
+int launch_rbsor_pp32(poisson_ctx* ctx, const Op& op, float** cur, float* a, float* b, const float* rhs, float omega,
+                      int nsweeps) {
+    if (nsweeps > 0 && a && b && sor_fused_ok(ctx, op))
+        return sor_fused32(ctx, op, *cur, *cur == a ? b : a, rhs, omega, nsweeps, cur);
+    return launch_rbsor32(ctx, op, *cur, rhs, omega, nsweeps);
+}
+
 }  // namespace pb
