@@ -228,19 +228,16 @@ static int a7_cfg_override() {
 
 template <typename T, int MODE, bool RED>
 static int apply7_cfg(poisson_ctx* ctx, const Op& op, const T* v, const T* rhs, T* out, float* out32, bool ug) {
-    using CA = A7Tile<34, 18, 1, 3>;  // 64 x 16 valid, 612 threads
-    using CB = A7Tile<34, 14, 2>;  // 64 x 12 valid, 476 threads
-    using CC = A7Tile<18, 14, 4>;  // 32 x 12 valid, 252 threads (small grids)
-    using CD = A7Tile<34, 14, 1, 3>;  // 64 x 12 valid, loads 3 planes ahead
-    using CE = A7Tile<34, 18, 1, 1>;
+    // measured at 256^3 fp64 on B200 (us per apply): CE 82.7, CA 85.1, CB 87.4, whole-row tiles 107
+    using CE = A7Tile<34, 10, 2, 3>;  // 64 x 8 valid, 340 threads, two CTAs per SM, loads 3 planes ahead
+    using CA = A7Tile<34, 18, 1, 3>;  // 64 x 16 valid, 612 threads, one CTA per SM
+    using CC = A7Tile<18, 14, 4>;     // 32 x 12 valid, 252 threads (small grids)
     int c = (size_t)op.n[0] * op.n[1] * op.n[2] >= ((size_t)1 << 21) ? 0 : 2;
     const int ov = a7_cfg_override();
-    if (ov >= 0 && ov < 5) c = ov;
+    if (ov >= 0 && ov < 3) c = ov;
     switch (c) {
-        case 0: return apply7_launch<T, CA, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 1);
-        case 1: return apply7_launch<T, CB, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 2);
-        case 3: return apply7_launch<T, CD, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 1);
-        case 4: return apply7_launch<T, CE, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 1);
+        case 0: return apply7_launch<T, CE, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 2);
+        case 1: return apply7_launch<T, CA, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 1);
         default: return apply7_launch<T, CC, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 4);
     }
 }
