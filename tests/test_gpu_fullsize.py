@@ -170,3 +170,48 @@ def test_fused_residual_restriction_option():
     n = len(outs) // 2
     for a, b in zip(outs[:n], outs[n:]):
         assert np.array_equal(a, b)
+
+
+# ---- edge cases of the fused / staged kernels ---------------------------------------------------------------------------
+N6 = (po.BC_NEUMANN0, po.BC_DIRICHLET_GHOST, po.BC_DIRICHLET_GHOST, po.BC_NEUMANN0, po.BC_NEUMANN0, po.BC_DIRICHLET_GHOST)
+
+
+@pytest.mark.parametrize("shape", [(2, 2, 2), (4, 6, 2), (2, 40, 3), (66, 14, 5), (130, 30, 9), (64, 2, 70)])
+@pytest.mark.parametrize("bc", [D6, N6])
+def test_small_and_ragged_grids_through_the_fused_kernels(shape, bc):
+    """Tiny, thin and ragged grids (tiles mostly outside the domain, runs shorter than the wavefront, one plane) with
+    Dirichlet ghosts and with Neumann faces, forced through k_apply7 / k_sor_fused (kernel path 2)."""
+    w = dict(shape=shape, spacing=(0.1, 0.07, 0.13), origin=(0.0, 0.1, 0.2), bc=bc)
+    o, g = make_pair(w, pb.PATH_PLANE)
+    faces = [wl.hash_uniform(500 + f, np.arange(o.face_len(f))) - 0.5 if bc[f] == po.BC_DIRICHLET_GHOST else None
+             for f in range(6)]
+    from gpu_helpers import set_faces
+    set_faces(o, g, faces)
+    phi_c, rhs = wl.random_field(shape, 81), wl.random_field(shape, 82)
+    d_phi, d_rhs = dev(phi_c), dev(rhs)
+    d_out = torch.empty_like(d_phi)
+    g.apply_laplacian(d_phi, d_out)
+    c = [1 / 0.1 ** 2, 1 / 0.07 ** 2, 1 / 0.13 ** 2]
+    assert pointwise_scaled(host(d_out), o.apply(phi_c), 2 * sum(c) * stencil_scale(phi_c) + 1.0) <= 1e-13
+    assert g.residual_norm(d_phi, d_rhs) == pytest.approx(o.residual_norm(phi_c, rhs), rel=1e-12)
+    for nhs in (2, 4):
+        g.set_option(pb.OPT_SOR_HALFSTEPS, nhs)
+        for nsw in (1, 2, 5):
+            o.rbsor(phi_c, rhs, 1.2, nsw)
+            g.rbsor_sweep(d_phi, d_rhs, 1.2, nsw)
+            assert pointwise_scaled(host(d_phi), phi_c, stencil_scale(phi_c, rhs * 0.002)) <= 1e-13
+
+
+def test_vcycle_anisotropic_spacing_and_non_cubic_grid():
+    """V-cycles on a 128 x 64 x 32 grid with three different spacings (every level has its own tile geometry)."""
+    w = dict(shape=(128, 64, 32), spacing=(0.01, 0.013, 0.017), origin=(0.0, 0.0, 0.0), bc=D6)
+    o, g = make_pair(w)
+    from gpu_helpers import set_faces
+    set_faces(o, g, [wl.hash_uniform(600 + f, np.arange(o.face_len(f))) - 0.5 for f in range(6)])
+    rhs = wl.random_field(w["shape"], 91)
+    for precision, tol in ((pb.F64, 1e-10), (pb.MIXED, 1e-5)):
+        phi_c = np.zeros_like(rhs)
+        d_phi = dev(phi_c)
+        o.vcycle(phi_c, rhs, precision=precision, ncycles=3)
+        g.mg_vcycle(d_phi, dev(rhs), precision=precision, ncycles=3)
+        assert rel_l2(host(d_phi), phi_c) <= tol
