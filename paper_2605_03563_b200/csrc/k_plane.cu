@@ -13,7 +13,7 @@ namespace pb {
 
 // ---- loaders ------------------------------------------------------------------------------------------------------------
 struct LdArr {  // v itself
-    static constexpr bool PLAIN = true, SIDE = false;
+    static constexpr bool PLAIN = true, SIDE = false, USES_DIAG = false;
     const double* v;
     struct Raw {
         double2 a;
@@ -27,7 +27,7 @@ struct LdArr {  // v itself
 };
 
 struct LdPnew {  // p_new = (r - mu) + beta p_old; side effect on owned points: x += alpha_prev p_old (deferred x-update)
-    static constexpr bool PLAIN = false, SIDE = true;
+    static constexpr bool PLAIN = false, SIDE = true, USES_DIAG = false;
     const double* r;
     const double* p;
     double* x;
@@ -61,7 +61,7 @@ __device__ __forceinline__ double jac_(const Op& op, int i, int j, int k, int ja
 
 template <int KIND>
 struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D; side effect on owned points: store p_new
-    static constexpr bool PLAIN = false, SIDE = true;
+    static constexpr bool PLAIN = false, SIDE = true, USES_DIAG = true;
     const double* r;
     const double* p;
     const double* v;
@@ -85,6 +85,10 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D; side effect on ow
         return mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
                    fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y) / jac_<KIND>(op, i + 1, j, k, jacobi));
     }
+    __device__ __forceinline__ double2 form_own(const Raw& w, double d0, double d1) const {  // d = row diagonal
+        return mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x) / (jacobi ? -d0 : 1.0),
+                   fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y) / (jacobi ? -d1 : 1.0));
+    }
     __device__ __forceinline__ double at(const Op& op, size_t q, int i, int j, int k) const {
         return fma(beta, fma(-omega, v[q], p[q]), r[q]) / jac_<KIND>(op, i, j, k, jacobi);
     }
@@ -92,7 +96,7 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D; side effect on ow
 
 template <int KIND>
 struct LdShat {  // s^ = (r - alpha v) / D; side effect on owned points: store s
-    static constexpr bool PLAIN = false, SIDE = true;
+    static constexpr bool PLAIN = false, SIDE = true, USES_DIAG = true;
     const double* r;
     const double* v;
     double* s;
@@ -111,6 +115,9 @@ struct LdShat {  // s^ = (r - alpha v) / D; side effect on owned points: store s
     __device__ __forceinline__ double2 form(const Op& op, const Raw& w, int i, int j, int k) const {
         return mk2(fma(-alpha, w.v.x, w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
                    fma(-alpha, w.v.y, w.r.y) / jac_<KIND>(op, i + 1, j, k, jacobi));
+    }
+    __device__ __forceinline__ double2 form_own(const Raw& w, double d0, double d1) const {
+        return mk2(fma(-alpha, w.v.x, w.r.x) / (jacobi ? -d0 : 1.0), fma(-alpha, w.v.y, w.r.y) / (jacobi ? -d1 : 1.0));
     }
     __device__ __forceinline__ double at(const Op& op, size_t q, int i, int j, int k) const {
         return fma(-alpha, v[q], r[q]) / jac_<KIND>(op, i, j, k, jacobi);

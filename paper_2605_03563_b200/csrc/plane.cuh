@@ -94,7 +94,7 @@ struct RowCoef<KIND_SPH, RPT> {
 };
 
 // Loader / epilogue concepts (see k_plane.cu for the instances):
-//   struct Ld { struct Raw; static bool PLAIN, SIDE; void prepare(); Raw load(size_t p) const; Raw load_own(size_t p) const;
+//   struct Ld { struct Raw; static bool PLAIN, SIDE, USES_DIAG (then: double2 form_own(const Raw&, double d0, double d1)); void prepare(); Raw load(size_t p) const; Raw load_own(size_t p) const;
 //               void side(const Raw&, size_t p) const;   (pointwise side effect on owned points, e.g. the CG x-update)
 //               double2 form(const Op&, const Raw&, int i, int j, int k) const;   (pair starting at column i)
 //               double at(const Op&, size_t p, int i, int j, int k) const; };
@@ -273,7 +273,23 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
             for (int r = 0; r < RPT; ++r) {
                 double2 fv;
                 if (act[r]) {
-                    fv = ld.form(op, s.o[r], i, jrow + r, s.kw);
+                    if constexpr (Ld::USES_DIAG) {
+                        // the row diagonals of the two owned points from the coefficients already in registers
+                        // (same expressions as stencil.cuh row_diag, so the quotients are the same bits)
+                        double d0, d1;
+                        if constexpr (KIND == KIND_SPH) {
+                            d0 = fma(rc.ir2[0], rc.dt[r], rc.dr[0]);
+                            d1 = fma(rc.ir2[1], rc.dt[r], rc.dr[1]);
+                        } else if constexpr (KIND == KIND_CART6) {
+                            d0 = d1 = rc.d;
+                        } else {
+                            d0 = rc.plain ? rc.d : row_diag<double, KIND_CART2>(op, i, jrow + r, s.kw);
+                            d1 = rc.plain ? rc.d : row_diag<double, KIND_CART2>(op, i + 1, jrow + r, s.kw);
+                        }
+                        fv = ld.form_own(s.o[r], d0, d1);
+                    } else {
+                        fv = ld.form(op, s.o[r], i, jrow + r, s.kw);
+                    }
                     if constexpr (Ld::SIDE) {
                         if (kk >= k0 && kk < k1) ld.side(s.o[r], (size_t)s.kw * plane + base0 + (size_t)r * n0);
                     }
