@@ -217,6 +217,19 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
         }
     }
 
+    // diagonals of this thread's halo points (spherical operator: fixed along the marching axis)
+    double hd0[NH], hd1[NH];
+#pragma unroll
+    for (int m = 0; m < NH; ++m) {
+        hd0[m] = hd1[m] = 1.0;
+        if constexpr (KIND == KIND_SPH) {
+            if (hcls[m] == 1) {
+                hd0[m] = row_diag<double, KIND_SPH>(op, hwi[m], hwj[m], 0);
+                hd1[m] = row_diag<double, KIND_SPH>(op, min(hwi[m] + 1, n0 - 1), hwj[m], 0);
+            }
+        }
+    }
+
     // ---- plane staging --------------------------------------------------------------------------------------------
     struct Staged {
         typename Ld::Raw o[RPT], h[NH];
@@ -302,7 +315,12 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
 #pragma unroll
             for (int m = 0; m < NH; ++m) {
                 if (hcls[m] == 1)
-                    st2(slot + hso[m], ld.form(op, s.h[m], hwi[m], hwj[m], s.kw));
+                {
+                    if constexpr (Ld::USES_DIAG && KIND == KIND_SPH)
+                        st2(slot + hso[m], ld.form_own(s.h[m], hd0[m], hd1[m]));  // spherical diagonal: no k dependence
+                    else
+                        st2(slot + hso[m], ld.form(op, s.h[m], hwi[m], hwj[m], s.kw));
+                }
                 else if (hcls[m] == 2)
                     st2(slot + hso[m], bpair(hi[m], hj[m], s.kw));
             }
