@@ -48,7 +48,7 @@ ROW_BYTES = {
     "multipole_bc": 8, "apply_laplacian": 16, "rbsor_sweep": 24, "mg_vcycle_f64": 75, "mg_vcycle_mixed": 66,
     "residual_norm": 16, "cg_iteration_19pt": 72, "multipole_bc_spherical": 8, "bicgstab_iteration": 136,
 }
-NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 320
+NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 250
 ROW_CITE = {
     "multipole_bc": "a6 PAPER.md:213-222", "apply_laplacian": "a1 PAPER.md:43-49", "rbsor_sweep": "a2 PAPER.md:59-63",
     "mg_vcycle_f64": "a5 PAPER.md:125-152", "mg_vcycle_mixed": "a5 PAPER.md:205", "residual_norm": "a7 PAPER.md:55",
@@ -356,8 +356,8 @@ def run_ours(args):
                "gpoint_updates_per_s": round(gpts, 3), "algorithmic_bytes_per_point": ROW_BYTES[name],
                "algorithmic_gbs": round(gbs, 1), "frac_of_hbm_peak": round(gbs / peak, 4), "bound": "hbm"}
         if name.startswith("multipole_bc"):
-            # lmax = 8 moments are bound by the plain fp64 ALUs, not HBM: 320 fp64-pipe instructions per point
-            # (ncu sm__inst_executed_pipe_fp64 of k_moments<8>); peak = SMs x 64 fp64 lanes x max SM clock (63 DFMA/clk/SM measured)
+            # lmax = 8 moments are bound by the plain fp64 ALUs, not HBM: ~250 fp64-pipe instructions per point
+            # (DMUL + DFMA + DADD of one point in the SASS of k_moments<8>); peak = SMs x 64 fp64 lanes x max SM clock
             alu_peak = NUM_SMS * 64 * FP64_CLOCK_HZ
             row.update(bound="alu", alu_dp_instr_per_point=MOMENTS_DP_INSTR,
                        alu_peak_dp_instr_per_s=alu_peak,

@@ -40,9 +40,17 @@ struct MpGeom {
     double r_ghost;
 };
 
+// One point's contribution to all moments, WITHOUT the normalisation N_lm (applied once per thread at the end).
+// Per (l, m): one multiply, one fma and one scaling for the recurrence, one fma (two for m > 0) for the sums; the
+// products (2l-1) z and k r^2 are formed once per point.
 template <int L>
 __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], double x, double y, double z, double w) {
     const double r2 = fma(z, z, fma(y, y, x * x));
+    double cz[L + 2], kr2[2 * L + 2];
+#pragma unroll
+    for (int l = 0; l <= L; ++l) cz[l] = (2 * l - 1) * z;
+#pragma unroll
+    for (int k = 0; k <= 2 * L; ++k) kr2[k] = k * r2;
     double A = 1.0, B = 0.0, dfact = 1.0;  // (x+iy)^m, (2m-1)!!
 #pragma unroll
     for (int m = 0; m <= L; ++m) {
@@ -54,15 +62,14 @@ __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], dou
             if (l == m)
                 ql = dfact;
             else if (l == m + 1)
-                ql = (2 * m + 1) * z * qm1;
+                ql = cz[l] * qm1;
             else
-                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) * (1.0 / (l - m));
+                ql = fma(cz[l], qm1, -(kr2[l + m - 1] * qm2)) * (1.0 / (l - m));
             if (m == 0) {
                 acc[l * l + l] = fma(wa, ql, acc[l * l + l]);
             } else {
-                const double nq = c_norm[l * l + l + m] * ql;
-                acc[l * l + l + m] = fma(wa, nq, acc[l * l + l + m]);
-                acc[l * l + l - m] = fma(wb, nq, acc[l * l + l - m]);
+                acc[l * l + l + m] = fma(wa, ql, acc[l * l + l + m]);
+                acc[l * l + l - m] = fma(wb, ql, acc[l * l + l - m]);
             }
             qm2 = qm1;
             qm1 = ql;
@@ -92,7 +99,8 @@ __global__ void __launch_bounds__(256, 1)
         const double d = p < n ? rho[p] : 0.0;
         if (__all_sync(0xffffffffu, d == 0.0)) continue;
         if (d == 0.0) continue;
-        const int k = (int)(p / plane), rem = (int)(p - (size_t)k * plane), j = rem / g.n[0], i = rem - j * g.n[0];
+        const int k = (int)(p / plane), rem = (int)(p - (size_t)k * plane);
+        const int j = rem / g.n[0], i = rem - j * g.n[0];
         double x, y, z, w;
         if (g.sph) {
             const double r = g.rc[i], rs = r * g.st[j];
@@ -108,6 +116,8 @@ __global__ void __launch_bounds__(256, 1)
         }
         accumulate<L>(acc, x, y, z, w);
     }
+#pragma unroll
+    for (int s = 0; s < NQ; ++s) acc[s] *= c_norm[s];  // N_lm, once per thread instead of once per point
     // block reduction: warp shuffles, then shared memory across the 8 warps
     __shared__ double sm[8][NQ];
     __shared__ int is_last;
