@@ -248,6 +248,28 @@ __global__ void __launch_bounds__(BX* BY)
     });
 }
 
+__device__ __forceinline__ void bicg_finish_iteration(KrylovCtl* ctl, double* hist, const double* tot) {
+    const double rr = tot[0];
+    finish_iteration(ctl, hist, rr);
+    ctl->rr = rr;
+    if (!isfinite(rr)) {
+        ctl->status = POISSON_BREAKDOWN;
+        ctl->done = 1;
+    } else if (!ctl->fixed && sqrt(rr) <= sqrt(ctl->tol2) * sqrt(ctl->rr0)) {
+        ctl->status = POISSON_OK;
+        ctl->done = 1;
+    } else if (!(fabs(ctl->omega) > 0.0)) {
+        ctl->status = POISSON_BREAKDOWN;
+        ctl->done = 1;
+    } else if (ctl->it >= ctl->max_it) {
+        ctl->done = 1;
+    } else {
+        const double rho_new = tot[1];
+        ctl->beta = (rho_new / ctl->rho) * (ctl->alpha / ctl->omega);
+        ctl->rho = rho_new;
+    }
+}
+
 template <int KIND>
 __global__ void __launch_bounds__(BX* BY)
     k_bicg_pass3(Op op, double* __restrict__ x, const double* __restrict__ p, const double* __restrict__ s,
@@ -273,27 +295,50 @@ __global__ void __launch_bounds__(BX* BY)
             a_r0r = fma(r0[q], rn, a_r0r);
         }
     double vals[2] = {a_rr, a_r0r};
-    grid_reduce<2>(vals, rb, [=](const double* tot) {
-        const double rr = tot[0];
-        finish_iteration(ctl, hist, rr);
-        ctl->rr = rr;
-        if (!isfinite(rr)) {
-            ctl->status = POISSON_BREAKDOWN;
-            ctl->done = 1;
-        } else if (!ctl->fixed && sqrt(rr) <= sqrt(ctl->tol2) * sqrt(ctl->rr0)) {
-            ctl->status = POISSON_OK;
-            ctl->done = 1;
-        } else if (!(fabs(ctl->omega) > 0.0)) {
-            ctl->status = POISSON_BREAKDOWN;
-            ctl->done = 1;
-        } else if (ctl->it >= ctl->max_it) {
-            ctl->done = 1;
-        } else {
-            const double rho_new = tot[1];
-            ctl->beta = (rho_new / ctl->rho) * (ctl->alpha / ctl->omega);
-            ctl->rho = rho_new;
+    grid_reduce<2>(vals, rb, [=](const double* tot) { bicg_finish_iteration(ctl, hist, tot); });
+}
+
+// Pair version for even n0: 16-byte accesses; the spherical diagonal does not depend on k, so it and its reciprocal are
+// formed once per column (the quotients by div_by stay correctly rounded, i.e. equal to p / D and s / D).
+template <int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_bicg_pass3_pair(Op op, double* __restrict__ x, const double* __restrict__ p, const double* __restrict__ s,
+                      const double* __restrict__ t, const double* __restrict__ r0, double* __restrict__ r,
+                      KrylovCtl* ctl, double* hist, int jacobi, int kc, RedBuf rb) {
+    if (ctl->done) return;
+    const double alpha = ctl->alpha, omega = ctl->omega;
+    const int i = 2 * (blockIdx.x * BX + threadIdx.x), j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    double a_rr = 0.0, a_r0r = 0.0;
+    if (i < op.n[0] && j < op.n[1]) {
+        double d0 = jac<KIND>(op, i, j, k0, jacobi), d1 = jac<KIND>(op, i + 1, j, k0, jacobi);
+        double rd0 = 1.0 / d0, rd1 = 1.0 / d1;
+        const size_t plane = (size_t)op.n[0] * op.n[1];
+        size_t q = gidx(op, i, j, k0);
+#pragma unroll 4
+        for (int k = k0; k < k1; ++k, q += plane) {
+            if (KIND != KIND_SPH) {
+                d0 = jac<KIND>(op, i, j, k, jacobi);
+                d1 = jac<KIND>(op, i + 1, j, k, jacobi);
+                rd0 = 1.0 / d0;
+                rd1 = 1.0 / d1;
+            }
+            const double2 pv = *reinterpret_cast<const double2*>(p + q), sv = *reinterpret_cast<const double2*>(s + q);
+            const double2 tv = *reinterpret_cast<const double2*>(t + q), zv = *reinterpret_cast<const double2*>(r0 + q);
+            double2 xv = *reinterpret_cast<const double2*>(x + q);
+            xv.x = fma(omega, div_by<double>(sv.x, d0, rd0), fma(alpha, div_by<double>(pv.x, d0, rd0), xv.x));
+            xv.y = fma(omega, div_by<double>(sv.y, d1, rd1), fma(alpha, div_by<double>(pv.y, d1, rd1), xv.y));
+            *reinterpret_cast<double2*>(x + q) = xv;
+            const double2 rn = make_double2(fma(-omega, tv.x, sv.x), fma(-omega, tv.y, sv.y));
+            *reinterpret_cast<double2*>(r + q) = rn;
+            a_rr = fma(rn.x, rn.x, a_rr);
+            a_r0r = fma(zv.x, rn.x, a_r0r);
+            a_rr = fma(rn.y, rn.y, a_rr);
+            a_r0r = fma(zv.y, rn.y, a_r0r);
         }
-    });
+    }
+    double vals[2] = {a_rr, a_r0r};
+    grid_reduce<2>(vals, rb, [=](const double* tot) { bicg_finish_iteration(ctl, hist, tot); });
 }
 
 // ---- launch wrappers --------------------------------------------------------------------------------------------------
@@ -388,10 +433,16 @@ int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double
                       const double* r0, double* r) {
     const Op& op = ctx->op;
     const int kc = pick_kc(op, ctx->num_sms);
-    const dim3 g = grid_for(op, kc), b(BX, BY);
     pre_launch(ctx, KID_BICG_PASS3);
-    KIND_SWITCH(ctx->kind, (k_bicg_pass3<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl, ctx->d_hist,
-                                                                        ctx->opt_jacobi, kc, ctx->red)));
+    if (op.n[0] % 2 == 0 && ctx->opt_path != 1) {
+        const dim3 g((op.n[0] / 2 + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + kc - 1) / kc), b(BX, BY);
+        KIND_SWITCH(ctx->kind, (k_bicg_pass3_pair<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl,
+                                                                                 ctx->d_hist, ctx->opt_jacobi, kc, ctx->red)));
+    } else {
+        const dim3 g = grid_for(op, kc), b(BX, BY);
+        KIND_SWITCH(ctx->kind, (k_bicg_pass3<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl, ctx->d_hist,
+                                                                            ctx->opt_jacobi, kc, ctx->red)));
+    }
     post_launch(ctx, KID_BICG_PASS3);
     return POISSON_OK;
 }
