@@ -198,6 +198,11 @@ int resid_restrict(poisson_ctx* ctx, const Op& fine, const Op& coarse, const dou
                    bool ug);
 int resid_restrict32(poisson_ctx* ctx, const Op& fine, const Op& coarse, const float* phi, const float* rhs, float* fc);
 
+// 7-point apply / residual with planes staged by bulk async copies (k_apply_bulk.cu), fp64
+bool apply_bulk_ok(const poisson_ctx* ctx, const Op& op);
+int apply_bulk(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32, int mode,
+               bool ug, bool reduce);
+
 // Plane-pipeline versions (k_plane.cu) for pair-aligned grids; same results, bit for bit
 int plane_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out,
                 float* out32, int mode, bool ug, bool reduce);

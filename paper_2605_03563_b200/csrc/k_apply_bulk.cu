@@ -1,0 +1,301 @@
+// k_apply_bulk.cu — 7-point Cartesian apply / residual (fp64, non-periodic) with the xy planes staged in shared memory
+// by the Tensor Memory Accelerator (cp.async.bulk.tensor, SASS UTMALDG) instead of by the threads:
+//   out = L v   or   out = rhs - L v   (+ fp32 copy, + sum(out^2), sum(out)).            PAPER.md:43-45 (Eq. 1), 55, 57.
+// A CTA of 64 x 4 threads owns a 128 x 8 tile and marches z; four such CTAs share an SM.  One thread issues, per plane,
+// ONE tensor copy of the (128+4) x (8+2) x 1 box (tile + halo; out-of-range parts are zero-filled by the hardware) into
+// a ring of NS planes and arms the plane's mbarrier with the byte count; copies run PF planes ahead of their use, so
+// ~4 x PF x 10 KB per SM are in flight without a staging register or an LSU load instruction.  Every thread owns a
+// 16-byte pair in two adjacent rows, keeps planes k-1, k, k+1 of them in registers (read once from the ring when a plane
+// lands) and takes the x / y neighbours of plane k from the ring; threads on a Dirichlet face take that neighbour from
+// the ghost-face array instead.  One __syncthreads per plane frees the oldest slot.  Arithmetic order = stencil.cuh
+// row_apply<KIND_CART2>, results bit-identical to the other apply kernels.
+// (A first version issued one 1 KB cp.async.bulk per tile row: 18 copies per plane cost ~3.6 k cycles of copy-engine
+// time per plane and ran at 140 Gpoint/s; the single tensor copy removes that.)
+#include <cuda.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstdlib>
+
+#include "pairq.cuh"
+
+namespace pb {
+
+namespace bulk {
+// Tile configuration: TX x TY points per CTA (64 x TY/2 ... threads: TX/2 pairs x TY/2 row pairs), NS ring slots, copies
+// PF planes ahead, MINB resident CTAs per SM asked of the compiler.
+template <int TX_, int TY_, int NS_, int PF_, int MINB_>
+struct Cfg {
+    static constexpr int TX = TX_, TY = TY_, NS = NS_, PF = PF_, MINB = MINB_;
+    static constexpr int SW = TX + 4, SH = TY + 2, NTX = TX / 2, NT = NTX * (TY / 2);
+    static constexpr int BOX_BYTES = SW * SH * 8;
+    static constexpr int SLOT = ((BOX_BYTES + 127) / 128) * 16;  // slot pitch in doubles, 128-byte aligned
+    static constexpr size_t SMEM = (size_t)NS * SLOT * sizeof(double) + NS * sizeof(uint64_t) + 128;
+};
+
+__device__ __forceinline__ uint32_t s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(s32(b)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_box(void* dst, const CUtensorMap* map, int x, int y, int z, uint64_t* b) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            s32(dst)),
+        "l"(map), "r"(x), "r"(y), "r"(z), "r"(s32(b))
+        : "memory");
+}
+}  // namespace bulk
+
+struct BulkGeom {
+    int ntx, nty;
+    long items;
+};
+
+template <class C, int MODE, bool RED, bool PLAIN>
+__global__ void __launch_bounds__(C::NT, C::MINB)
+    k_apply7_bulk(const Op op, const __grid_constant__ CUtensorMap vmap, const double* __restrict__ rhs,
+                  double* __restrict__ out, float* __restrict__ out32, const bool ug_in, const BulkGeom g, RedBuf rb,
+                  double* scal) {
+    using namespace bulk;
+    constexpr int TX = C::TX, TY = C::TY, SW = C::SW, NS = C::NS, PF = C::PF, SLOT = C::SLOT, BOX_BYTES = C::BOX_BYTES;
+    extern __shared__ unsigned char smraw0[];
+    unsigned char* const smraw = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smraw0) + 127) & ~uintptr_t(127));
+    double* const ring = reinterpret_cast<double*>(smraw);
+    uint64_t* const full = reinterpret_cast<uint64_t*>(ring + (size_t)NS * SLOT);
+    const int n0 = op.n[0], n1 = op.n[1], n2 = op.n[2];
+    const int tid = threadIdx.x, lx = tid % C::NTX, ty = tid / C::NTX;
+    const bool ug = ug_in && op.gamma == 0.0;
+    const double c0 = op.c[0], c1 = op.c[1], c2 = op.c[2];
+    const double dplain = 2.0 * ((c0 + c1) + c2);
+    const size_t plane = (size_t)n0 * n1;
+    // ghost-face arrays of the Dirichlet faces in use (nullptr: that neighbour is zero, which is what the copy delivers)
+    const double* gf[6];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) gf[f] = (ug && op.bc[f] == POISSON_BC_DIRICHLET_GHOST) ? op.ghost[f] : nullptr;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    unsigned issued = 0, used = 0;  // planes issued / consumed so far: slot = count % NS, parity = (count / NS) & 1
+    double s2 = 0.0, s1 = 0.0;
+
+    const long total = (long)g.ntx * g.nty * n2;
+    long pos = (long)blockIdx.x * g.items;
+    const long end = min(total, pos + g.items);
+    while (pos < end) {
+        const int t = (int)(pos / n2), k0 = (int)(pos % n2);
+        const int k1 = (int)min((long)n2, (long)k0 + (end - pos));
+        pos += k1 - k0;
+        const int i0 = (t % g.ntx) * TX, j0 = (t / g.ntx) * TY;
+        const int i = i0 + 2 * lx, jr = j0 + 2 * ty;  // this thread's pair (i, i+1) in rows jr, jr+1
+        const bool own0 = i < n0 && jr < n1, own1 = i < n0 && jr + 1 < n1;
+        const int kbeg = k0 - 1, kend = k1;
+        auto issue = [&](int kk) {  // thread 0: one tensor copy = tile + halo of plane kk (zero fill outside the array)
+            if (tid == 0) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                mbar_arrive_expect_tx(&full[issued % NS], (uint32_t)BOX_BYTES);
+                tma_box(ring + (size_t)(issued % NS) * SLOT, &vmap, i0 - 2, j0 - 1, kk, &full[issued % NS]);
+            }
+            ++issued;
+        };
+        double dx0 = dplain, dy0 = dplain, dx1 = dplain, dy1 = dplain;
+        if (!PLAIN) {
+            if (own0) { dx0 = a7_diag_xy<double>(op, i, jr); dy0 = a7_diag_xy<double>(op, i + 1, jr); }
+            if (own1) { dx1 = a7_diag_xy<double>(op, i, jr + 1); dy1 = a7_diag_xy<double>(op, i + 1, jr + 1); }
+        }
+        for (int m = 0; m < PF && kbeg + m <= kend; ++m) issue(kbeg + m);
+        const size_t cb0 = (size_t)jr * n0 + i, cb1 = cb0 + n0;
+        double2 qm0 = make_double2(0, 0), qc0 = qm0, qp0 = qm0, qm1 = qm0, qc1 = qm0, qp1 = qm0;
+        // right-hand side of planes kin-1 (a), kin (b), kin+1 (c) for the two owned rows: loaded two iterations ahead
+        double2 f0a = make_double2(0, 0), f0b = f0a, f0c = f0a, f1a = f0a, f1b = f0a, f1c = f0a;
+        const int so = (1 + 2 * ty) * SW + 2 + 2 * lx;  // own pair of row jr inside a slot; row jr+1 is SW further
+        const double* prev = ring;                       // slot of the previous plane
+        for (int kin = kbeg; kin <= kend; ++kin) {
+            const double* const cur = ring + (size_t)(used % NS) * SLOT;
+            mbar_wait(&full[used % NS], (used / NS) & 1u);
+            ++used;
+            qm0 = qc0; qc0 = qp0; qm1 = qc1; qc1 = qp1;
+            qp0 = *reinterpret_cast<const double2*>(cur + so);
+            qp1 = *reinterpret_cast<const double2*>(cur + so + SW);
+            if (kin < 0 || kin >= n2) {  // a z ghost plane: the copy delivered zeros; owned pairs come from the face array
+                const double* zf = kin < 0 ? gf[4] : gf[5];
+                if (zf && own0) qp0 = *reinterpret_cast<const double2*>(zf + cb0);
+                if (zf && own1) qp1 = *reinterpret_cast<const double2*>(zf + cb1);
+            }
+            f0a = f0b; f0b = f0c; f1a = f1b; f1b = f1c;
+            if (MODE != 0 && kin + 1 < k1) {  // rhs of plane kin + 1, used two iterations later
+                if (own0) f0c = *reinterpret_cast<const double2*>(rhs + (size_t)(kin + 1) * plane + cb0);
+                if (own1) f1c = *reinterpret_cast<const double2*>(rhs + (size_t)(kin + 1) * plane + cb1);
+            }
+            const int k = kin - 1;
+            if (k >= k0 && k < k1) {
+                const double* const P = prev + so;
+                double2 ya = *reinterpret_cast<const double2*>(P - SW), yb = *reinterpret_cast<const double2*>(P + 2 * SW);
+                double xl0 = P[-1], xr0 = P[2], xl1 = P[SW - 1], xr1 = P[SW + 2];
+                double2 below0 = qc1;  // neighbour of row jr in +y: own row jr+1 unless that is the ghost row
+                if (i == 0 && gf[0]) { xl0 = gf[0][(size_t)k * n1 + jr]; if (own1) xl1 = gf[0][(size_t)k * n1 + jr + 1]; }
+                if (i + 2 == n0 && gf[1]) { xr0 = gf[1][(size_t)k * n1 + jr]; if (own1) xr1 = gf[1][(size_t)k * n1 + jr + 1]; }
+                if (jr == 0 && gf[2] && own0) ya = *reinterpret_cast<const double2*>(gf[2] + (size_t)k * n0 + i);
+                if (jr + 2 == n1 && gf[3] && own0) yb = *reinterpret_cast<const double2*>(gf[3] + (size_t)k * n0 + i);
+                if (jr + 1 == n1 && gf[3] && own0) below0 = *reinterpret_cast<const double2*>(gf[3] + (size_t)k * n0 + i);
+                const double2 fa = f0a, fb = f1a;
+                double dz00 = dx0, dz01 = dy0, dz10 = dx1, dz11 = dy1;
+                if (!PLAIN && (k == 0 || k == n2 - 1)) {
+                    dz00 = a7_diag_z<double>(op, dz00, k); dz01 = a7_diag_z<double>(op, dz01, k);
+                    dz10 = a7_diag_z<double>(op, dz10, k); dz11 = a7_diag_z<double>(op, dz11, k);
+                }
+                const size_t po = (size_t)k * plane;
+                auto finish = [&](double lv0, double lv1, double2 f, size_t q) {
+                    const double o0 = MODE ? f.x - lv0 : lv0, o1 = MODE ? f.y - lv1 : lv1;
+                    if (out) *reinterpret_cast<double2*>(out + q) = make_double2(o0, o1);
+                    if (out32) *reinterpret_cast<float2*>(out32 + q) = make_float2((float)o0, (float)o1);
+                    if (RED) {
+                        s2 = fma(o0, o0, s2); s1 += o0;
+                        s2 = fma(o1, o1, s2); s1 += o1;
+                    }
+                };
+                if (own0) {  // row jr: y neighbours = ring row above (or ghost), row jr+1 (own, or ghost)
+                    double s = (xl0 + qc0.y) * c0;
+                    s = fma(ya.x + below0.x, c1, s);
+                    s = fma(qm0.x + qp0.x, c2, s);
+                    const double lv0 = fma(-dz00, qc0.x, s);
+                    s = (qc0.x + xr0) * c0;
+                    s = fma(ya.y + below0.y, c1, s);
+                    s = fma(qm0.y + qp0.y, c2, s);
+                    finish(lv0, fma(-dz01, qc0.y, s), fa, po + cb0);
+                }
+                if (own1) {  // row jr+1: y neighbours = own row jr, ring row below (or ghost)
+                    double s = (xl1 + qc1.y) * c0;
+                    s = fma(qc0.x + yb.x, c1, s);
+                    s = fma(qm1.x + qp1.x, c2, s);
+                    const double lv0 = fma(-dz10, qc1.x, s);
+                    s = (qc1.x + xr1) * c0;
+                    s = fma(qc0.y + yb.y, c1, s);
+                    s = fma(qm1.y + qp1.y, c2, s);
+                    finish(lv0, fma(-dz11, qc1.y, s), fb, po + cb1);
+                }
+            }
+            prev = cur;
+            __syncthreads();  // every reader is done with the planes before `cur`: their slots may be refilled
+            if (kin + PF <= kend) issue(kin + PF);
+        }
+    }
+    if (RED) {
+        double vals[2] = {s2, s1};
+        grid_reduce<2>(vals, rb, [=](const double* t) {
+            scal[0] = t[0];
+            scal[1] = t[1];
+        });
+    }
+}
+
+// ---- host side ----------------------------------------------------------------------------------------------------------
+bool apply_bulk_ok(const poisson_ctx* ctx, const Op& op) {
+    static const char* e = getenv("POISSON_APPLY_BULK");  // 0 = never, 1 = whenever eligible; default: large grids
+    const int mode = e ? atoi(e) : -1;
+    if (mode == 0 || ctx->opt_path == 1) return false;
+    if (op.coord != POISSON_CARTESIAN || op.order != 2 || op.n[0] % 2 != 0) return false;
+    for (int f = 0; f < 6; ++f)
+        if (op.bc[f] == POISSON_BC_PERIODIC) return false;
+    if (mode == 1) return true;
+    return op.n[0] >= 128 && (size_t)op.n[0] * op.n[1] * op.n[2] >= (size_t)1 << 21;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
+// 3-D fp64 tensor (n0, n1, n2), box = tile + halo of one plane, zero fill outside the array
+template <class C>
+static bool make_map(const Op& op, const double* v, CUtensorMap* map) {
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[3] = {(cuuint64_t)op.n[0], (cuuint64_t)op.n[1], (cuuint64_t)op.n[2]};
+    const cuuint64_t strides[2] = {(cuuint64_t)op.n[0] * 8, (cuuint64_t)op.n[0] * op.n[1] * 8};
+    const cuuint32_t box[3] = {(cuuint32_t)C::SW, (cuuint32_t)C::SH, 1};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(v), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <class C, int MODE, bool RED>
+static int bulk_launch(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32,
+                       bool ug) {
+    bool plain = op.gamma == 0.0;
+    for (int f = 0; f < 6; ++f) plain = plain && op.bc[f] != POISSON_BC_NEUMANN0;
+    BulkGeom g;
+    g.ntx = (op.n[0] + C::TX - 1) / C::TX;
+    g.nty = (op.n[1] + C::TY - 1) / C::TY;
+    const long total = (long)g.ntx * g.nty * op.n[2];
+    static int resident = 0;
+    CUtensorMap map;
+    if (!make_map<C>(op, v, &map)) return POISSON_UNSUPPORTED;  // the caller falls back to k_apply7
+    if (!resident) {
+        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
+        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_apply7_bulk<C, MODE, RED, true>, C::NT, C::SMEM));
+        if (resident < 1) resident = 1;
+    }
+    g.items = std::max(4L, (total + (long)ctx->num_sms * resident - 1) / ((long)ctx->num_sms * resident));
+    const int grid = (int)((total + g.items - 1) / g.items);
+    if (grid > kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");
+    if (plain)
+        PB_LAUNCH(ctx, KID_APPLY, (k_apply7_bulk<C, MODE, RED, true><<<grid, C::NT, C::SMEM, ctx->stream>>>(op, map, rhs, out, out32, ug, g, ctx->red, ctx->d_scal)));
+    else
+        PB_LAUNCH(ctx, KID_APPLY, (k_apply7_bulk<C, MODE, RED, false><<<grid, C::NT, C::SMEM, ctx->stream>>>(op, map, rhs, out, out32, ug, g, ctx->red, ctx->d_scal)));
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+// Tile choice, measured at 256^3 on B200 (us per apply, MODE 0): 128 x 8 tiles with 4 CTAs per SM 58; 3 CTAs 63;
+// 64 x 16 / 3 CTAs 66; 64 x 8 / 8 CTAs 64; 128 x 16 / 1 CTA of 512 threads 81 (= the thread-staged kernels): what pays
+// is MANY SMALL CTAs per SM, so that one CTA's per-plane barrier is hidden behind the others.  The residual variants
+// carry the right-hand side queue and the reduction and need the registers of the 3-CTA configuration.
+template <int MODE, bool RED>
+static int bulk_cfg(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32,
+                    bool ug) {
+    using C4 = bulk::Cfg<128, 8, 5, 3, 4>;  // 256 threads, ring of 5 planes, copies 3 planes ahead, four CTAs per SM
+    using C3 = bulk::Cfg<128, 8, 6, 4, 3>;  // 256 threads, ring of 6 planes, copies 4 planes ahead, three CTAs per SM
+    if (MODE == 0) return bulk_launch<C4, MODE, RED>(ctx, op, v, rhs, out, out32, ug);
+    return bulk_launch<C3, MODE, RED>(ctx, op, v, rhs, out, out32, ug);
+}
+
+int apply_bulk(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32, int mode,
+               bool ug, bool reduce) {
+    if (mode == 0) return bulk_cfg<0, false>(ctx, op, v, rhs, out, out32, ug);
+    if (!reduce) return bulk_cfg<1, false>(ctx, op, v, rhs, out, out32, ug);
+    return bulk_cfg<1, true>(ctx, op, v, rhs, out, out32, ug);
+}
+
+}  // namespace pb

@@ -91,6 +91,10 @@ static int apply_dispatch(poisson_ctx* ctx, const Op& op, const T* v, const T* r
 
 int launch_apply(poisson_ctx* ctx, const Op& op, int kind, const double* v, const double* rhs, double* out, int mode,
                  bool ug, bool reduce) {
+    if (kind == KIND_CART2 && apply_bulk_ok(ctx, op)) {
+        const int rc = apply_bulk(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
+        if (rc != POISSON_UNSUPPORTED) return rc;  // no tensor-map encoder in this driver: thread-staged kernel
+    }
     if (kind == KIND_CART2 && apply7_ok(ctx, op)) return apply7(ctx, op, v, rhs, out, nullptr, mode, ug, reduce);
     if (plane_ok(ctx, op)) return plane_apply(ctx, op, kind, v, rhs, out, nullptr, mode, ug, reduce);
     switch (kind) {
@@ -106,6 +110,10 @@ int launch_apply32(poisson_ctx* ctx, const Op& op, const float* v, const float* 
 }
 
 int launch_residual_to32(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, float* out32, bool ug) {
+    if (apply_bulk_ok(ctx, op)) {
+        const int rc = apply_bulk(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
+        if (rc != POISSON_UNSUPPORTED) return rc;
+    }
     if (apply7_ok(ctx, op)) return apply7(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
     if (plane_ok(ctx, op)) return plane_apply(ctx, op, KIND_CART2, v, rhs, nullptr, out32, 1, ug, true);
     return apply_dispatch<double, KIND_CART2>(ctx, op, v, rhs, nullptr, out32, 1, ug, true);
