@@ -3,6 +3,8 @@ import ctypes
 import os
 import re
 
+import pytest
+
 from paper_2605_03563_b200 import binding, build
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -43,3 +45,21 @@ def test_product_does_not_import_the_oracle():
                 s = open(os.path.join(dp, f)).read()
                 for needle in ("pyoracle", "liboracle", "import oracle", "from oracle", "oracle.build", "orc_"):
                     assert needle not in s, (f, needle)
+
+
+def test_tma_apply_kernel_is_compiled_to_tensor_copies():
+    """The TMA-staged apply kernel must really use the tensor copy engine: its SASS holds UTMALDG (cp.async.bulk.tensor)
+    and mbarrier instructions (SYNCS), for sm_100a."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    from paper_2605_03563_b200 import build as cuda_build
+    lib = cuda_build.build()
+    sass = subprocess.run([cuobjdump, "-sass", "-fun", "k_apply7_bulk", lib], capture_output=True, text=True).stdout
+    if "UTMALDG" not in sass:   # older cuobjdump: no substring match on -fun; scan the object file instead
+        obj = os.path.join(os.path.dirname(lib), "build", "k_apply_bulk.o")
+        sass = subprocess.run([cuobjdump, "-sass", obj], capture_output=True, text=True).stdout
+    assert "sm_100a" in sass or "SM100a" in sass or "sm_100" in sass
+    assert "UTMALDG" in sass and "SYNCS" in sass
