@@ -101,7 +101,13 @@ int poisson_cg_solve(poisson_t h, double* d_phi, const double* d_rhs, double rto
                      int* iters, double* relres);
 
 /* BiCGSTAB (Saad Alg. 7.7) with right Jacobi scaling, for the nonsymmetric spherical operator;
- * same stopping rule.  BREAKDOWN when rho, omega or r0^.v vanish or turn non-finite. */
+ * same stopping rule.  Near-breakdown restart (reading C4): when |r0^.r| <= 1e-12 |r0^| |r| at the beta
+ * step the shadow residual is replaced by r (rho = r.r, beta = 0); the environment variable
+ * POISSON_BICG_RESTART_EPS overrides the threshold, 0 disables the rule.  When the recurrence's residual meets rtol the
+ * true residual rhs - L phi is recomputed: OK (and *relres the true figure) only if it meets rtol as well, otherwise
+ * the iteration carries on from it; NOT_CONVERGED also after 30 such checks have failed (rtol below the attainable
+ * accuracy).  fixed_iters > 0 runs exactly that many iterations without any check.
+ * BREAKDOWN when rho, omega or r0^.v vanish or turn non-finite. */
 int poisson_bicgstab_solve(poisson_t h, double* d_phi, const double* d_rhs, double rtol, int max_iter,
                            int fixed_iters, int* iters, double* relres);
 

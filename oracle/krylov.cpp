@@ -84,6 +84,12 @@ int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, i
     return status;
 }
 
+// Restart threshold on |rho| / (||r^_0|| ||r||) (reading C4: Saad's Alg. 7.7 has no safeguard; on config 5 the
+// shadow residual and the residual become orthogonal to rounding level after ~10^3 iterations and the iteration
+// stagnates or breaks down, which of the two depends on the rounding of the dot products).
+static const double kBicgRestartEps = 1e-12;
+static const int kBicgMaxConfirm = 30;  // failed true-residual confirmations tolerated (C4)
+
 int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
              int* iters, double* relres, double* history) {
     const size_t n = g.size();
@@ -102,6 +108,8 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
     double rho = dot(g, r0.data(), r.data());
     const double rr0 = dot(g, r.data(), r.data());
     double rr = rr0;
+    double r0n2 = rr0;  // ||r^_0||^2
+    int nconf_failed = 0;  // true-residual confirmations that failed so far
     const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
     if (history) history[0] = 1.0;
     int it = 0, status = (fixed_iters > 0) ? ST_OK : ST_NOT_CONVERGED;
@@ -144,16 +152,45 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
                 break;
             }
             if (fixed_iters <= 0 && std::sqrt(rr) <= rtol * std::sqrt(rr0)) {
-                status = ST_OK;
-                break;
+                // The recursively updated r drifts away from b - A x over thousands of iterations (config 5: by a factor
+                // 40).  Confirm with the true residual; if that one is not there yet, carry on from it as from a fresh
+                // start (r^_0 := r, p := r), keeping the iteration count and ||r_0||.  DESIGN.md C4.
+                apply(g, x, v.data(), true);
+#pragma omp parallel for schedule(static)
+                for (size_t m = 0; m < n; ++m) r[m] = rhs[m] - v[m];
+                rr = dot(g, r.data(), r.data());
+                if (std::sqrt(rr) <= rtol * std::sqrt(rr0)) {
+                    status = ST_OK;
+                    break;
+                }
+                // rtol below the attainable accuracy: the recurrence keeps converging, the true residual never does
+                if (!std::isfinite(rr) || ++nconf_failed > kBicgMaxConfirm) {
+                    status = std::isfinite(rr) ? ST_NOT_CONVERGED : ST_BREAKDOWN;
+                    break;
+                }
+                r0 = r;
+                p = r;
+                r0n2 = rr;
+                rho = rr;
+                continue;
             }
             if (!(std::fabs(omega) > 0.0)) {
                 status = ST_BREAKDOWN;
                 break;
             }
             const double rho_new = dot(g, r0.data(), r.data());
-            const double beta = (rho_new / rho) * (alpha / omega);
-            rho = rho_new;
+            double beta;
+            if (std::fabs(rho_new) <= kBicgRestartEps * std::sqrt(r0n2 * rr)) {
+                // Near-breakdown: r has become orthogonal to the shadow residual up to rounding, the recurrences carry
+                // no information any more.  Restart with r^_0 := r (then rho = r.r, beta = 0, p = r).  DESIGN.md C4.
+                r0 = r;
+                r0n2 = rr;
+                rho = rr;
+                beta = 0.0;
+            } else {
+                beta = (rho_new / rho) * (alpha / omega);
+                rho = rho_new;
+            }
 #pragma omp parallel for schedule(static)
             for (size_t m = 0; m < n; ++m) p[m] = std::fma(beta, std::fma(-omega, v[m], p[m]), r[m]);
         }

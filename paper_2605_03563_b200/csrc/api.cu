@@ -435,6 +435,8 @@ static int krylov_setup(poisson_ctx* ctx, double rtol, int max_iter, int fixed_i
     c->project = project ? 1 : 0;
     c->record = ctx->opt_history;
     c->npoints = (double)ctx->npts;
+    c->eps_bd = ctx->opt_bicg_restart_eps;
+    if (const char* e = getenv("POISSON_BICG_RESTART_EPS")) c->eps_bd = atof(e);  // tuning aid
     if (ctx->opt_history) {
         if (ctx->hist_cap < nit + 1) {
             cudaFree(ctx->d_hist);
@@ -519,6 +521,7 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
     rc = launch_krylov_init(ctx, d_phi, d_rhs, r, true, r0);
     if (rc != POISSON_OK) return rc;
     const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    int nconfirm_failed = 0;
     for (int j = 0; j < nit;) {
         const int chunk = std::min(ctx->opt_poll, nit - j);
         for (int c = 0; c < chunk; ++c, ++j) {
@@ -531,7 +534,20 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
         if (fixed_iters <= 0) {
             rc = read_ctl(ctx);
             if (rc != POISSON_OK) return rc;
+            if (!ctx->h_ctl->done) continue;
+            if (ctx->h_ctl->status != POISSON_OK || !(ctx->h_ctl->rr0 > 0.0)) break;
+            // The recurrence says converged: confirm with the true residual r = rhs - L x (the recursively updated r
+            // drifts away from it over thousands of iterations); if it is not there yet the pass has restarted the
+            // iteration from it (r^_0 := r, p := r) and cleared done.  DESIGN.md reading C4.
+            static const int one = 1;
+            PB_CUDA_OK(cudaMemcpyAsync(&ctx->d_ctl->confirm, &one, sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
+            rc = launch_krylov_init(ctx, d_phi, d_rhs, r, true, r0);
+            if (rc != POISSON_OK) return rc;
+            rc = read_ctl(ctx);
+            if (rc != POISSON_OK) return rc;
             if (ctx->h_ctl->done) break;
+            nconfirm_failed += 1;
+            j = ctx->h_ctl->it;
         }
     }
     rc = read_ctl(ctx);
@@ -541,6 +557,10 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
     if (iters) *iters = c.it;
     if (relres) *relres = c.rr0 > 0 ? std::sqrt(c.rr / c.rr0) : 0.0;
     if (c.status == POISSON_NOT_CONVERGED) ctx->err = "BiCGSTAB: residual threshold not reached within max_iter";
+    if (getenv("POISSON_DEBUG"))
+        fprintf(stderr, "bicgstab ctl: it %d status %d rr %.6e rr0 %.6e rho %.6e r0v %.6e alpha %.6e omega %.6e ts %.6e tt %.6e beta %.6e\n",
+                c.it, c.status, c.rr, c.rr0, c.rho, c.r0v, c.alpha, c.omega, c.ts, c.tt, c.beta);
+    if (getenv("POISSON_DEBUG")) fprintf(stderr, "bicgstab restarts: %d, true-residual restarts: %d\n", c.nrestarts, nconfirm_failed);
     if (c.status == POISSON_BREAKDOWN) ctx->err = "BiCGSTAB: breakdown (rho, omega or r0.v vanished or is not finite)";
     return c.status;
 }

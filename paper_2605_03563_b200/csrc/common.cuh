@@ -58,12 +58,17 @@ enum KernelId {
 };
 
 // Device-resident scalars of the Krylov solvers: nothing crosses to the host inside an iteration.
+constexpr int kMaxBicgConfirm = 30;
+
 struct KrylovCtl {
     double rr, rr0, pq, alpha, beta, mu, rho, omega, r0v, ts, tt, tol2;
     double sum_x;
     int it, done, status, fixed;
-    int max_it, project, record, pad;
+    int max_it, project, record, restart;  // restart: BiCGSTAB takes r^_0 := r in the next pass 1 (near-breakdown)
     double npoints;
+    double r0n2, eps_bd;  // ||r^_0||^2 and the near-breakdown threshold on |rho| / (||r^_0|| ||r||)
+    int nconf_failed, pad3;  // true-residual confirmations that failed so far (at most kMaxBicgConfirm)
+    int nrestarts, confirm;                 // confirm: the next initial-residual pass re-checks convergence (BiCGSTAB)
 };
 
 struct RedBuf {
@@ -115,6 +120,7 @@ struct poisson_ctx {
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
     int opt_sor_nhs = 0;             // colour half-steps fused per HBM pass of the red-black kernel (2, 4; 0 = auto)
+    double opt_bicg_restart_eps = 1e-12;  // BiCGSTAB restart threshold (0 = never), reading C4
     int opt_fused_restrict = 0;      // V-cycle residual + restriction in one kernel: 0 auto (fp32 levels only), 1 always, 2 never
     void* sor_tmp = nullptr;         // ping-pong buffer of the fused red-black kernel
     size_t sor_tmp_bytes = 0;

@@ -49,22 +49,7 @@ __global__ void __launch_bounds__(BX* BY)
             s1 += o;
         }
     double vals[2] = {s2, s1};
-    grid_reduce<2>(vals, rb, [=](const double* t) {
-        const double mu = ctl->project ? t[1] / ctl->npoints : 0.0;
-        const double rr = ctl->project ? fma(-ctl->npoints * mu, mu, t[0]) : t[0];
-        ctl->mu = mu;
-        ctl->rr = rr;
-        ctl->rr0 = rr;
-        ctl->rho = rr;
-        ctl->alpha = 0.0;
-        ctl->beta = 0.0;
-        ctl->omega = 0.0;
-        ctl->it = 0;
-        const int trivially_done = (!ctl->fixed && !(rr > 0.0)) ? 1 : 0;
-        ctl->done = trivially_done;
-        ctl->status = (ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED;
-        if (ctl->record && hist) hist[0] = 1.0;
-    });
+    grid_reduce<2>(vals, rb, [=](const double* t) { krylov_init_finish(ctl, hist, t); });
 }
 
 // ---- CG ---------------------------------------------------------------------------------------------------------------
@@ -188,9 +173,11 @@ struct ShatLd {  // s = r - alpha v ; s^ = s / D
 template <int KIND>
 __global__ void __launch_bounds__(BX* BY)
     k_bicg_pass1(Op op, const double* __restrict__ r, const double* __restrict__ p_old,
-                 const double* __restrict__ v_old, const double* __restrict__ r0, double* __restrict__ p_new,
+                 const double* __restrict__ v_old, const double* r0, double* __restrict__ p_new,
                  double* __restrict__ v_new, KrylovCtl* ctl, int jacobi, int kc, RedBuf rb) {
     if (ctl->done) return;
+    const int restart = ctl->restart;
+    double* const r0w = const_cast<double*>(r0);
     const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
     const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
     const PhatLd<KIND> ld{op, r, p_old, v_old, ctl->beta, ctl->omega, jacobi};
@@ -201,7 +188,12 @@ __global__ void __launch_bounds__(BX* BY)
             const double vn = row_apply<double, KIND>(op, ld, i, j, k, false);
             p_new[p] = ld.pnew(p);
             v_new[p] = vn;
-            acc = fma(r0[p], vn, acc);
+            double r0p = r0[p];
+            if (restart) {  // r^_0 := r
+                r0p = r[p];
+                r0w[p] = r0p;
+            }
+            acc = fma(r0p, vn, acc);
         }
     double vals[1] = {acc};
     grid_reduce<1>(vals, rb, [=](const double* t) {
@@ -265,8 +257,18 @@ __device__ __forceinline__ void bicg_finish_iteration(KrylovCtl* ctl, double* hi
         ctl->done = 1;
     } else {
         const double rho_new = tot[1];
-        ctl->beta = (rho_new / ctl->rho) * (ctl->alpha / ctl->omega);
-        ctl->rho = rho_new;
+        if (fabs(rho_new) <= ctl->eps_bd * sqrt(ctl->r0n2 * rr)) {
+            // near-breakdown (r has become orthogonal to r^_0 up to rounding): restart with r^_0 := r, p := r
+            ctl->restart = 1;
+            ctl->nrestarts += 1;
+            ctl->beta = 0.0;
+            ctl->rho = rr;
+            ctl->r0n2 = rr;
+        } else {
+            ctl->restart = 0;
+            ctl->beta = (rho_new / ctl->rho) * (ctl->alpha / ctl->omega);
+            ctl->rho = rho_new;
+        }
     }
 }
 

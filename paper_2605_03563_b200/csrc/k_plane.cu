@@ -66,20 +66,24 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D; side effect on ow
     const double* p;
     const double* v;
     double* p_new;
+    double* r0w;  // r^_0, rewritten with r on a restart
     const KrylovCtl* ctl;
     int jacobi;
     double beta, omega;
+    int restart;
     struct Raw {
         double2 r, p, v;
     };
     __device__ __forceinline__ void prepare() {
         beta = ctl->beta;
         omega = ctl->omega;
+        restart = ctl->restart;
     }
     __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q), ld2(v + q)}; }
     __device__ __forceinline__ Raw load_own(size_t q) const { return load(q); }
     __device__ __forceinline__ void side(const Raw& w, size_t q) const {
         st2(p_new + q, mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x), fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y)));
+        if (restart) st2(r0w + q, w.r);  // r^_0 := r; the epilogue of this same thread reads it back for r^_0 . v
     }
     __device__ __forceinline__ double2 form(const Op& op, const Raw& w, int i, int j, int k) const {
         return mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x) / jac_<KIND>(op, i, j, k, jacobi),
@@ -185,22 +189,7 @@ struct EpInit {  // r = rhs - L x (ghosts included); r0^ = r; first scalars of t
         acc[0] = fma(o.y, o.y, acc[0]);
         acc[1] += o.y;
     }
-    __device__ __forceinline__ void finish(const double* t) const {
-        const double mu = ctl->project ? t[1] / ctl->npoints : 0.0;
-        const double rr = ctl->project ? fma(-ctl->npoints * mu, mu, t[0]) : t[0];
-        ctl->mu = mu;
-        ctl->rr = rr;
-        ctl->rr0 = rr;
-        ctl->rho = rr;
-        ctl->alpha = 0.0;
-        ctl->beta = 0.0;
-        ctl->omega = 0.0;
-        ctl->it = 0;
-        const int trivially_done = (!ctl->fixed && !(rr > 0.0)) ? 1 : 0;
-        ctl->done = trivially_done;
-        ctl->status = (ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED;
-        if (ctl->record && hist) hist[0] = 1.0;
-    }
+    __device__ __forceinline__ void finish(const double* t) const { krylov_init_finish(ctl, hist, t); }
 };
 
 struct EpCgA {  // stores p_new and q = L p_new, sum p.q -> alpha (the x-update rides on the loader, LdPnew::side)
@@ -337,7 +326,7 @@ int plane_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, con
                      double* p_new, double* v_new) {
     int rc = POISSON_OK;
     const EpBicg1 ep{r0, v_new, ctx->d_ctl};
-    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdPhat<K>{r, p_old, v_old, p_new, ctx->d_ctl, ctx->opt_jacobi, 0.0, 0.0},
+    KIND_SWITCH(ctx->kind, rc = launch_plane<K>(ctx, ctx->op, LdPhat<K>{r, p_old, v_old, p_new, const_cast<double*>(r0), ctx->d_ctl, ctx->opt_jacobi, 0.0, 0.0, 0},
                                                 ep, false, KID_BICG_PASS1));
     return rc;
 }

@@ -203,4 +203,39 @@ __device__ __forceinline__ void grid_reduce(double (&v)[NRED], RedBuf rb, Epi ep
     }
 }
 
+// Scalars after the initial-residual pass (t[0] = sum r^2, t[1] = sum r).  With ctl->confirm set the pass was the
+// true-residual check of a BiCGSTAB solution the recurrence calls converged: accept, or carry on from the true
+// residual as from a fresh start (r^_0 := r was stored by the pass, beta = 0 gives p := r), keeping it and rr0.
+__device__ __forceinline__ void krylov_init_finish(KrylovCtl* ctl, double* hist, const double* t) {
+    const double mu = ctl->project ? t[1] / ctl->npoints : 0.0;
+    const double rr = ctl->project ? fma(-ctl->npoints * mu, mu, t[0]) : t[0];
+    ctl->mu = mu;
+    ctl->rr = rr;
+    ctl->rho = rr;
+    ctl->r0n2 = rr;
+    ctl->restart = 0;
+    ctl->beta = 0.0;
+    if (ctl->confirm) {
+        ctl->confirm = 0;
+        const bool fin = isfinite(rr);
+        const bool ok = fin && sqrt(rr) <= sqrt(ctl->tol2) * sqrt(ctl->rr0);
+        // rtol below the attainable accuracy: the recurrence keeps converging, the true residual never does
+        if (!ok) ctl->nconf_failed += 1;
+        const bool stall = ctl->nconf_failed > kMaxBicgConfirm;
+        ctl->done = (ok || !fin || stall || ctl->it >= ctl->max_it) ? 1 : 0;
+        ctl->status = ok ? POISSON_OK : (fin ? POISSON_NOT_CONVERGED : POISSON_BREAKDOWN);
+        return;
+    }
+    ctl->rr0 = rr;
+    ctl->nconf_failed = 0;
+    ctl->nrestarts = 0;
+    ctl->alpha = 0.0;
+    ctl->omega = 0.0;
+    ctl->it = 0;
+    const int trivially_done = (!ctl->fixed && !(rr > 0.0)) ? 1 : 0;
+    ctl->done = trivially_done;
+    ctl->status = (ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED;
+    if (ctl->record && hist) hist[0] = 1.0;
+}
+
 }  // namespace pb

@@ -283,6 +283,29 @@ def test_bicgstab_on_cartesian_and_unscaled_variant():
         assert rel_l2(host(d_phi), phi_c) <= max(1e-10, 10 * sens)
 
 
+def test_bicgstab_true_residual_confirmation_and_attainable_accuracy():
+    # DESIGN.md reading C4: convergence is confirmed with the true residual; an rtol below the attainable accuracy ends
+    # with NOT_CONVERGED after 30 failed confirmations — same verdict and same solution on both sides
+    re, te, pe = wl.spherical_edges(8, 4, 8)
+    bc = (po.BC_NEUMANN0, po.BC_DIRICHLET_GHOST, po.BC_AXIS, po.BC_AXIS, po.BC_PERIODIC, po.BC_PERIODIC)
+    w = dict(shape=(8, 4, 8), edges=(re, te, pe), coord=po.SPHERICAL, bc=bc)
+    o, g = make_pair(w)
+    ghost = wl.hash_uniform(4, np.arange(o.face_len(1)))
+    set_faces(o, g, [None, ghost, None, None, None, None])
+    rhs = wl.random_field(w["shape"], 6)
+    b_norm = o.residual_norm(np.zeros_like(rhs), rhs)
+    for rtol, status in ((1e-11, pb.OK), (1e-13, pb.NOT_CONVERGED)):
+        phi_c = np.zeros_like(rhs)
+        d_phi = dev(phi_c)
+        res_c = o.bicgstab(phi_c, rhs, rtol=rtol, max_iter=2000)
+        res_g = g.bicgstab_solve(d_phi, dev(rhs), rtol=rtol, max_iter=2000)
+        assert res_c["status"] == status and res_g["status"] == status
+        assert res_g["iters"] < 400
+        true = o.residual_norm(host(d_phi), rhs) / b_norm
+        assert true == pytest.approx(res_g["relres"], rel=1e-3, abs=1e-14)     # the reported figure is the true one
+        assert true < 1e-11 and rel_l2(host(d_phi), phi_c) < 1e-9
+
+
 # ---- (a5) multigrid V-cycle -----------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n", [32, 64])
 @pytest.mark.parametrize("restriction", [0, 1])
