@@ -6,18 +6,17 @@
 // a ring of NS planes and arms the plane's mbarrier with the byte count; copies run PF planes ahead of their use, so
 // ~4 x PF x 10 KB per SM are in flight without a staging register or an LSU load instruction.  Every thread owns a
 // 16-byte pair in two adjacent rows, keeps planes k-1, k, k+1 of them in registers (read once from the ring when a plane
-// lands) and takes the x / y neighbours of plane k from the ring; threads on a Dirichlet face take that neighbour from
+// lands; the residual variants read the right-hand side from the tile that rides in the same slot) and takes the x / y neighbours of plane k from the ring; threads on a Dirichlet face take that neighbour from
 // the ghost-face array instead.  One __syncthreads per plane frees the oldest slot.  Arithmetic order = stencil.cuh
 // row_apply<KIND_CART2>, results bit-identical to the other apply kernels.
 // (A first version issued one 1 KB cp.async.bulk per tile row: 18 copies per plane cost ~3.6 k cycles of copy-engine
 // time per plane and ran at 140 Gpoint/s; the single tensor copy removes that.)
-#include <cuda.h>
-
 #include <algorithm>
 #include <cstdint>
 #include <cstdlib>
 
 #include "pairq.cuh"
+#include "tma.cuh"
 
 namespace pb {
 
@@ -30,33 +29,14 @@ struct Cfg {
     static constexpr int SW = TX + 4, SH = TY + 2, NTX = TX / 2, NT = NTX * (TY / 2);
     static constexpr int BOX_BYTES = SW * SH * 8;
     static constexpr int SLOT = ((BOX_BYTES + 127) / 128) * 16;  // slot pitch in doubles, 128-byte aligned
-    static constexpr size_t SMEM = (size_t)NS * SLOT * sizeof(double) + NS * sizeof(uint64_t) + 128;
+    static constexpr int RHS_BYTES = TX * TY * 8;  // residual variants: the tile of the right-hand side, no halo
+    // ring pitch in doubles: the box of v, then (residual variants) the right-hand side of the plane before it
+    __host__ __device__ static constexpr int pitch(bool with_rhs) { return SLOT + (with_rhs ? TX * TY : 0); }
+    __host__ __device__ static constexpr size_t smem(bool with_rhs) {
+        return (size_t)NS * pitch(with_rhs) * sizeof(double) + NS * sizeof(uint64_t) + 128;
+    }
 };
 
-__device__ __forceinline__ uint32_t s32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s32(b)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* b, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(s32(b)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(s32(b)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void tma_box(void* dst, const CUtensorMap* map, int x, int y, int z, uint64_t* b) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-            s32(dst)),
-        "l"(map), "r"(x), "r"(y), "r"(z), "r"(s32(b))
-        : "memory");
-}
 }  // namespace bulk
 
 struct BulkGeom {
@@ -66,11 +46,13 @@ struct BulkGeom {
 
 template <class C, int MODE, bool RED, bool PLAIN>
 __global__ void __launch_bounds__(C::NT, C::MINB)
-    k_apply7_bulk(const Op op, const __grid_constant__ CUtensorMap vmap, const double* __restrict__ rhs,
+    k_apply7_bulk(const Op op, const __grid_constant__ CUtensorMap vmap, const __grid_constant__ CUtensorMap fmap,
                   double* __restrict__ out, float* __restrict__ out32, const bool ug_in, const BulkGeom g, RedBuf rb,
                   double* scal) {
-    using namespace bulk;
-    constexpr int TX = C::TX, TY = C::TY, SW = C::SW, NS = C::NS, PF = C::PF, SLOT = C::SLOT, BOX_BYTES = C::BOX_BYTES;
+    using namespace tma;
+    constexpr int TX = C::TX, TY = C::TY, SW = C::SW, NS = C::NS, PF = C::PF, BOX_BYTES = C::BOX_BYTES;
+    constexpr int SLOT = C::pitch(MODE != 0), FOFF = C::SLOT;  // the right-hand side tile sits FOFF doubles into a slot
+    constexpr uint32_t TX_BYTES = BOX_BYTES + (MODE != 0 ? C::RHS_BYTES : 0);
     extern __shared__ unsigned char smraw0[];
     unsigned char* const smraw = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smraw0) + 127) & ~uintptr_t(127));
     double* const ring = reinterpret_cast<double*>(smraw);
@@ -108,8 +90,10 @@ __global__ void __launch_bounds__(C::NT, C::MINB)
         auto issue = [&](int kk) {  // thread 0: one tensor copy = tile + halo of plane kk (zero fill outside the array)
             if (tid == 0) {
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                mbar_arrive_expect_tx(&full[issued % NS], (uint32_t)BOX_BYTES);
+                mbar_arrive_expect_tx(&full[issued % NS], TX_BYTES);
                 tma_box(ring + (size_t)(issued % NS) * SLOT, &vmap, i0 - 2, j0 - 1, kk, &full[issued % NS]);
+                // the plane that is computed when v(kk) lands is kk - 1: its right-hand side rides in the same slot
+                if (MODE != 0) tma_box(ring + (size_t)(issued % NS) * SLOT + FOFF, &fmap, i0, j0, kk - 1, &full[issued % NS]);
             }
             ++issued;
         };
@@ -121,8 +105,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB)
         for (int m = 0; m < PF && kbeg + m <= kend; ++m) issue(kbeg + m);
         const size_t cb0 = (size_t)jr * n0 + i, cb1 = cb0 + n0;
         double2 qm0 = make_double2(0, 0), qc0 = qm0, qp0 = qm0, qm1 = qm0, qc1 = qm0, qp1 = qm0;
-        // right-hand side of planes kin-1 (a), kin (b), kin+1 (c) for the two owned rows: loaded two iterations ahead
-        double2 f0a = make_double2(0, 0), f0b = f0a, f0c = f0a, f1a = f0a, f1b = f0a, f1c = f0a;
+        const int fo = FOFF + (2 * ty) * TX + 2 * lx;   // own pair of row jr in the right-hand side tile; row jr+1 is TX further
         const int so = (1 + 2 * ty) * SW + 2 + 2 * lx;  // own pair of row jr inside a slot; row jr+1 is SW further
         const double* prev = ring;                       // slot of the previous plane
         for (int kin = kbeg; kin <= kend; ++kin) {
@@ -137,11 +120,6 @@ __global__ void __launch_bounds__(C::NT, C::MINB)
                 if (zf && own0) qp0 = *reinterpret_cast<const double2*>(zf + cb0);
                 if (zf && own1) qp1 = *reinterpret_cast<const double2*>(zf + cb1);
             }
-            f0a = f0b; f0b = f0c; f1a = f1b; f1b = f1c;
-            if (MODE != 0 && kin + 1 < k1) {  // rhs of plane kin + 1, used two iterations later
-                if (own0) f0c = *reinterpret_cast<const double2*>(rhs + (size_t)(kin + 1) * plane + cb0);
-                if (own1) f1c = *reinterpret_cast<const double2*>(rhs + (size_t)(kin + 1) * plane + cb1);
-            }
             const int k = kin - 1;
             if (k >= k0 && k < k1) {
                 const double* const P = prev + so;
@@ -153,7 +131,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB)
                 if (jr == 0 && gf[2] && own0) ya = *reinterpret_cast<const double2*>(gf[2] + (size_t)k * n0 + i);
                 if (jr + 2 == n1 && gf[3] && own0) yb = *reinterpret_cast<const double2*>(gf[3] + (size_t)k * n0 + i);
                 if (jr + 1 == n1 && gf[3] && own0) below0 = *reinterpret_cast<const double2*>(gf[3] + (size_t)k * n0 + i);
-                const double2 fa = f0a, fb = f1a;
+                double2 fa = make_double2(0, 0), fb = fa;
+                if (MODE != 0) {
+                    fa = *reinterpret_cast<const double2*>(cur + fo);
+                    fb = *reinterpret_cast<const double2*>(cur + fo + TX);
+                }
                 double dz00 = dx0, dz01 = dy0, dz10 = dx1, dz11 = dy1;
                 if (!PLAIN && (k == 0 || k == n2 - 1)) {
                     dz00 = a7_diag_z<double>(op, dz00, k); dz01 = a7_diag_z<double>(op, dz01, k);
@@ -216,39 +198,6 @@ bool apply_bulk_ok(const poisson_ctx* ctx, const Op& op) {
     return op.n[0] >= 128 && (size_t)op.n[0] * op.n[1] * op.n[2] >= (size_t)1 << 21;
 }
 
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static EncodeTiledFn encode_fn() {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (EncodeTiledFn)p;
-        cudaGetLastError();
-    }
-    return fn;
-}
-
-// 3-D fp64 tensor (n0, n1, n2), box = tile + halo of one plane, zero fill outside the array
-template <class C>
-static bool make_map(const Op& op, const double* v, CUtensorMap* map) {
-    EncodeTiledFn fn = encode_fn();
-    if (!fn) return false;
-    const cuuint64_t dims[3] = {(cuuint64_t)op.n[0], (cuuint64_t)op.n[1], (cuuint64_t)op.n[2]};
-    const cuuint64_t strides[2] = {(cuuint64_t)op.n[0] * 8, (cuuint64_t)op.n[0] * op.n[1] * 8};
-    const cuuint32_t box[3] = {(cuuint32_t)C::SW, (cuuint32_t)C::SH, 1};
-    const cuuint32_t estr[3] = {1, 1, 1};
-    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(v), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 template <class C, int MODE, bool RED>
 static int bulk_launch(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32,
                        bool ug) {
@@ -259,21 +208,24 @@ static int bulk_launch(poisson_ctx* ctx, const Op& op, const double* v, const do
     g.nty = (op.n[1] + C::TY - 1) / C::TY;
     const long total = (long)g.ntx * g.nty * op.n[2];
     static int resident = 0;
-    CUtensorMap map;
-    if (!make_map<C>(op, v, &map)) return POISSON_UNSUPPORTED;  // the caller falls back to k_apply7
+    CUtensorMap map, fmap;
+    if (!tma::make_map3(v, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, op.n, C::SW, C::SH, &map)) return POISSON_UNSUPPORTED;  // the caller falls back to k_apply7
+    fmap = map;
+    if (MODE != 0 && !tma::make_map3(rhs, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, op.n, C::TX, C::TY, &fmap)) return POISSON_UNSUPPORTED;
+    constexpr size_t SMEM = C::smem(MODE != 0);
     if (!resident) {
-        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM));
-        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_apply7_bulk<C, MODE, RED, true>, C::NT, C::SMEM));
+        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_apply7_bulk<C, MODE, RED, true>, C::NT, SMEM));
         if (resident < 1) resident = 1;
     }
     g.items = std::max(4L, (total + (long)ctx->num_sms * resident - 1) / ((long)ctx->num_sms * resident));
     const int grid = (int)((total + g.items - 1) / g.items);
     if (grid > kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");
     if (plain)
-        PB_LAUNCH(ctx, KID_APPLY, (k_apply7_bulk<C, MODE, RED, true><<<grid, C::NT, C::SMEM, ctx->stream>>>(op, map, rhs, out, out32, ug, g, ctx->red, ctx->d_scal)));
+        PB_LAUNCH(ctx, KID_APPLY, (k_apply7_bulk<C, MODE, RED, true><<<grid, C::NT, SMEM, ctx->stream>>>(op, map, fmap, out, out32, ug, g, ctx->red, ctx->d_scal)));
     else
-        PB_LAUNCH(ctx, KID_APPLY, (k_apply7_bulk<C, MODE, RED, false><<<grid, C::NT, C::SMEM, ctx->stream>>>(op, map, rhs, out, out32, ug, g, ctx->red, ctx->d_scal)));
+        PB_LAUNCH(ctx, KID_APPLY, (k_apply7_bulk<C, MODE, RED, false><<<grid, C::NT, SMEM, ctx->stream>>>(op, map, fmap, out, out32, ug, g, ctx->red, ctx->d_scal)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
@@ -281,12 +233,15 @@ static int bulk_launch(poisson_ctx* ctx, const Op& op, const double* v, const do
 // Tile choice, measured at 256^3 on B200 (us per apply, MODE 0): 128 x 8 tiles with 4 CTAs per SM 58; 3 CTAs 63;
 // 64 x 16 / 3 CTAs 66; 64 x 8 / 8 CTAs 64; 128 x 16 / 1 CTA of 512 threads 81 (= the thread-staged kernels): what pays
 // is MANY SMALL CTAs per SM, so that one CTA's per-plane barrier is hidden behind the others.  The residual variants
-// carry the right-hand side queue and the reduction and need the registers of the 3-CTA configuration.
+// stage the right-hand side tile of the plane being computed in the same slot, by a second tensor copy on the same
+// mbarrier (residual norm 68 us; with the threads loading it into a register queue one plane ahead it was 96 us: the
+// queue rotation waits for the load, which leaves one plane per DRAM latency per CTA).  Ring of 4 / 3 CTAs per SM and
+// ring of 3 / 4 CTAs measure the same; ring of 6 / 2 CTAs 82 us.
 template <int MODE, bool RED>
 static int bulk_cfg(poisson_ctx* ctx, const Op& op, const double* v, const double* rhs, double* out, float* out32,
                     bool ug) {
     using C4 = bulk::Cfg<128, 8, 5, 3, 4>;  // 256 threads, ring of 5 planes, copies 3 planes ahead, four CTAs per SM
-    using C3 = bulk::Cfg<128, 8, 6, 4, 3>;  // 256 threads, ring of 6 planes, copies 4 planes ahead, three CTAs per SM
+    using C3 = bulk::Cfg<128, 8, 4, 3, 3>;  // 256 threads, ring of 4 planes (+ rhs tiles), copies 3 planes ahead, three CTAs per SM
     if (MODE == 0) return bulk_launch<C4, MODE, RED>(ctx, op, v, rhs, out, out32, ug);
     return bulk_launch<C3, MODE, RED>(ctx, op, v, rhs, out, out32, ug);
 }

@@ -30,6 +30,11 @@ struct SorGeom {
     long items;     // (tile, plane) items per CTA
 };
 
+template <bool B>
+struct FastTag {
+    static constexpr bool value = B;
+};
+
 template <typename T>
 struct PairT {};
 template <>
@@ -228,6 +233,18 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
             if (kind == 1 && kk >= 0 && kk < n2) return *reinterpret_cast<const P2*>(prh);
             return PairT<T>::make((T)0, (T)0);
         };
+        // the same loads for a plane known to exist (FAST blocks)
+        auto loadv_in = [&]() -> P2 {
+            P2 v = PairT<T>::make((T)0, (T)0);
+            if (kind == 1 || kind == 4) v = *reinterpret_cast<const P2*>(vp);
+            else if (kind == 2) v.y = *vp;
+            else if (kind == 3) v.x = *vp;
+            return v;
+        };
+        auto loadr_in = [&]() -> P2 {
+            if (kind == 1) return *reinterpret_cast<const P2*>(prh);
+            return PairT<T>::make((T)0, (T)0);
+        };
         // register queues; the value of plane kin - m sits at index (m - u) mod D in unrolled iteration u
         T qA[D], qB[D], fA[D], fB[D];
 #pragma unroll
@@ -243,11 +260,15 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
             prh += plane;
         }
         __syncthreads();  // the previous segment's readers are done with the ring
-        for (int kin0 = kstart; kin0 <= kend; kin0 += D) {
+        // One block = D unrolled iterations.  FAST blocks lie strictly inside the z range (every plane touched exists,
+        // none is a boundary plane, every finished plane belongs to this run): no range tests, no z-closure of the
+        // diagonal — the same arithmetic with ~20 % fewer instructions; the lead-in / lead-out blocks take the full path.
+        auto block = [&](auto fast_tag, const int kin0) {
+            constexpr bool FAST = decltype(fast_tag)::value;
 #pragma unroll
             for (int u = 0; u < D; ++u) {
                 const int kin = kin0 + u;
-                if (kin > kend) break;
+                if (!FAST && kin > kend) break;
                 const int p0 = (D - u) % D;  // index of plane kin (m = 0)
                 const P2 nv = nvq[u % PF], nr = nrq[u % PF];
                 qA[p0] = cA ? nv.y : nv.x;
@@ -259,7 +280,10 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                     mine[u * SLOT + PXN] = nv.y;
                 }
                 pout += plane;
-                if (kin + PF <= kend) {
+                if (FAST) {
+                    nvq[u % PF] = loadv_in();
+                    nrq[u % PF] = loadr_in();
+                } else if (kin + PF <= kend) {
                     nvq[u % PF] = loadv(kin + PF);
                     nrq[u % PF] = loadr(kin + PF);
                 }
@@ -283,13 +307,13 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
 #pragma unroll
                 for (int h = 1; h <= NHS; ++h) {
                     const int kz = kin - h;
-                    const bool upd = col_in && kz >= 0 && kz < n2;
+                    const bool upd = FAST ? col_in : (col_in && kz >= 0 && kz < n2);
                     const int ph = (h - u + 2 * D) % D, pm = (h + 1 - u + 2 * D) % D, pp = (h - 1 - u + 2 * D) % D;
                     const T zp = actA ? qA[pp] : qB[pp], zm = actA ? qA[pm] : qB[pm];
                     const T old = actA ? qA[ph] : qB[ph];
                     const T f = actA ? fA[ph] : fB[ph];
                     T d = PLAIN ? dplain : (actA ? dA : dB), rd = PLAIN ? rdplain : (actA ? rdA : rdB);
-                    if (!PLAIN && (kz == 0 || kz == n2 - 1)) {
+                    if (!PLAIN && !FAST && (kz == 0 || kz == n2 - 1)) {
                         d = sor_diag_z<T>(op, d, kz);
                         rd = (T)1 / d;
                     }
@@ -302,11 +326,17 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                     }
                 }
                 const int ko = kin - NHS;
-                if (st_ok && ko >= k0 && ko < k1) {
+                if (FAST ? st_ok : (st_ok && ko >= k0 && ko < k1)) {
                     const int po = (NHS - u + 2 * D) % D;
                     *reinterpret_cast<P2*>(pout) = cA ? PairT<T>::make(qB[po], qA[po]) : PairT<T>::make(qA[po], qB[po]);
                 }
             }
+        };
+        for (int kin0 = kstart; kin0 <= kend; kin0 += D) {
+            const bool fast = kin0 - NHS >= 1 && kin0 + D - 1 + PF <= n2 - 1 && kin0 + D - 1 + PF <= kend &&
+                              kin0 - NHS >= k0 && kin0 + D - 1 - NHS < k1;
+            if (fast) block(FastTag<true>{}, kin0);
+            else block(FastTag<false>{}, kin0);
         }
     }
 }
