@@ -94,6 +94,8 @@ int orc_bicgstab(void* h, double* phi, const double* rhs, double rtol, int max_i
                  int* iters, double* relres, double* history) {
     return bicgstab(*(Grid*)h, phi, rhs, rtol, max_iter, fixed_iters, jacobi, iters, relres, history);
 }
+void orc_set_bicgstab_restart_eps(double eps) { set_bicgstab_restart_eps(eps); }
+void orc_bicgstab_stats(int* restarts, int* confirm_failed) { bicgstab_stats(restarts, confirm_failed); }
 int orc_vcycle(void* h, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, int coarsest_sweeps,
                int precision, int restriction, int ncycles, double* resnorms) {
     return vcycle(*(Grid*)h, phi, rhs, nu1, nu2, coarsest_n, coarsest_sweeps, precision, restriction, ncycles,

@@ -87,11 +87,19 @@ int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, i
 // Restart threshold on |rho| / (||r^_0|| ||r||) (reading C4: Saad's Alg. 7.7 has no safeguard; on config 5 the
 // shadow residual and the residual become orthogonal to rounding level after ~10^3 iterations and the iteration
 // stagnates or breaks down, which of the two depends on the rounding of the dot products).
-static const double kBicgRestartEps = 1e-12;
+static double kBicgRestartEps = 1e-12;  // tests may raise it to force the restart branch (set_bicgstab_restart_eps)
 static const int kBicgMaxConfirm = 30;  // failed true-residual confirmations tolerated (C4)
+
+static int g_restarts = 0, g_confirm_failed = 0;  // of the last bicgstab() call
+void set_bicgstab_restart_eps(double eps) { kBicgRestartEps = eps; }
+void bicgstab_stats(int* restarts, int* confirm_failed) {
+    *restarts = g_restarts;
+    *confirm_failed = g_confirm_failed;
+}
 
 int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
              int* iters, double* relres, double* history) {
+    g_restarts = g_confirm_failed = 0;
     const size_t n = g.size();
     std::vector<double> r(n), r0(n), p(n), v(n), s(n), t(n), ph(n), sh(n), dg(n);
     // D = diag(A) for right Jacobi scaling: p^ = D^-1 p, s^ = D^-1 s.  The system solved is L x = rhs as it
@@ -164,6 +172,7 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
                     break;
                 }
                 // rtol below the attainable accuracy: the recurrence keeps converging, the true residual never does
+                ++g_confirm_failed;
                 if (!std::isfinite(rr) || ++nconf_failed > kBicgMaxConfirm) {
                     status = std::isfinite(rr) ? ST_NOT_CONVERGED : ST_BREAKDOWN;
                     break;
@@ -187,6 +196,7 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
                 r0n2 = rr;
                 rho = rr;
                 beta = 0.0;
+                ++g_restarts;
             } else {
                 beta = (rho_new / rho) * (alpha / omega);
                 rho = rho_new;

@@ -159,6 +159,21 @@ class Oracle:
         return self._krylov(lib().orc_bicgstab, phi, rhs, rtol, max_iter, fixed_iters, want_history,
                             extra=(int(jacobi),))
 
+    @staticmethod
+    def set_bicgstab_restart_eps(eps):
+        """Near-breakdown threshold of BiCGSTAB (default 1e-12); tests raise it to force the restart branch."""
+        fn = lib().orc_set_bicgstab_restart_eps
+        fn.argtypes = [C.c_double]
+        fn.restype = None
+        fn(float(eps))
+
+    @staticmethod
+    def bicgstab_stats():
+        """(restarts, failed true-residual confirmations) of the last bicgstab call."""
+        a, b = C.c_int(0), C.c_int(0)
+        lib().orc_bicgstab_stats(C.byref(a), C.byref(b))
+        return a.value, b.value
+
     def vcycle(self, phi, rhs, nu1=2, nu2=2, coarsest_n=8, coarsest_sweeps=50, precision=0, restriction=0,
                ncycles=1):
         assert phi.dtype == np.float64 and phi.flags.c_contiguous

@@ -20,6 +20,10 @@ int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, i
 // BiCGSTAB, Saad Alg. 7.7 with right Jacobi scaling (jacobi != 0).  PAPER.md:105; reading C4/C10.
 int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
              int* iters, double* relres, double* history);
+// Near-breakdown threshold (default 1e-12; reading C4) and the counts of the last call: restarts taken,
+// true-residual confirmations that failed.
+void set_bicgstab_restart_eps(double eps);
+void bicgstab_stats(int* restarts, int* confirm_failed);
 
 // Geometric multigrid V-cycles (Eq. 11-13; reading C7).
 //   restriction: 0 = transpose of trilinear (1/8)[1 3 3 1]^3, 1 = mean of the 8 children

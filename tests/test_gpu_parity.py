@@ -306,6 +306,30 @@ def test_bicgstab_true_residual_confirmation_and_attainable_accuracy():
         assert true < 1e-11 and rel_l2(host(d_phi), phi_c) < 1e-9
 
 
+@pytest.mark.parametrize("path", PATHS)
+def test_bicgstab_restart_branch_parity(path, monkeypatch):
+    # the near-breakdown restart forced on both sides (threshold 0.1 instead of 1e-12): same restarts, same iterates
+    w = wl.config5(32, 16, 32)
+    o, g = make_pair(w, path)
+    o.multipole_bc(w["rho"], w["G"], w["lmax"])
+    g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
+    g.set_option(pb.OPT_RECORD_HISTORY, 1)
+    monkeypatch.setenv("POISSON_BICG_RESTART_EPS", "0.1")
+    try:
+        po.Oracle.set_bicgstab_restart_eps(0.1)
+        for fixed in (6, 12):
+            phi_c = np.zeros_like(w["rhs"])
+            d_phi = dev(phi_c)
+            res_c = o.bicgstab(phi_c, w["rhs"], fixed_iters=fixed, want_history=True)
+            restarts = po.Oracle.bicgstab_stats()[0]
+            g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=fixed)
+            assert restarts >= (1 if fixed == 6 else 3)
+            assert rel_l2(host(d_phi), phi_c) <= 1e-9
+            assert np.allclose(g.get_history(fixed + 1), res_c["history"], rtol=1e-6)
+    finally:
+        po.Oracle.set_bicgstab_restart_eps(1e-12)
+
+
 # ---- (a5) multigrid V-cycle -----------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n", [32, 64])
 @pytest.mark.parametrize("restriction", [0, 1])

@@ -185,3 +185,25 @@ def test_config5_64_reported_residual_is_the_true_one():
     true = o.residual_norm(phi, w["rhs"]) / r0
     assert res["status"] == 0 and res["relres"] <= 1e-8
     assert true == pytest.approx(res["relres"], rel=1e-6) and true <= 1e-8
+
+
+def test_bicgstab_restart_branch_forced_still_solves_the_system():
+    # DESIGN.md reading C4: the near-breakdown restart (r^_0 := r, rho := r.r, beta := 0) fires only at rounding level
+    # with the default threshold; raised to 0.3 it fires many times on the small spherical problem, and the restarted
+    # iteration must still reach the dense-LU solution — a wrong sign, a stale rho or a p that is not reset would not.
+    o = _sph_small()
+    A = dense_matrix(o)
+    rhs = wl.random_field(o.shape, 21)
+    exact = np.linalg.solve(A, rhs.reshape(-1)).reshape(rhs.shape)
+    try:
+        po.Oracle.set_bicgstab_restart_eps(0.3)
+        phi = np.zeros_like(rhs)
+        res = o.bicgstab(phi, rhs, rtol=1e-11, max_iter=4000)
+        restarts, _ = po.Oracle.bicgstab_stats()
+    finally:
+        po.Oracle.set_bicgstab_restart_eps(1e-12)
+    assert restarts >= 3 and res["status"] == 0
+    assert rel_l2(phi, exact) < 1e-9
+    phi2 = np.zeros_like(rhs)
+    o.bicgstab(phi2, rhs, rtol=1e-11, max_iter=4000)
+    assert po.Oracle.bicgstab_stats()[0] == 0 and rel_l2(phi2, exact) < 1e-9      # default threshold: no restart here
