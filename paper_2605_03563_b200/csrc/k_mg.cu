@@ -7,6 +7,17 @@
 namespace pb {
 
 template <typename T>
+struct Vec2 {};
+template <>
+struct Vec2<double> {
+    using type = double2;
+};
+template <>
+struct Vec2<float> {
+    using type = float2;
+};
+
+template <typename T>
 __global__ void __launch_bounds__(256)
     k_restrict(Op fine, Op coarse, const T* __restrict__ r, T* __restrict__ fc, int restriction) {
     const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
@@ -33,6 +44,43 @@ __global__ void __launch_bounds__(256)
     fc[gidx(coarse, I, J, K)] = acc;
 }
 
+// The same restriction ((1/8)[1 3 3 1]^3, terms added in the same order) for fine.n = 2 coarse.n and 32 x 8 thread
+// blocks: a warp is 32 consecutive coarse cells of one row, every thread loads the aligned fine pair (2I, 2I+1) of each
+// of the 16 fine rows it needs with one 16-byte access and takes r[2I-1] / r[2I+2] from its neighbour lanes (warp edges:
+// one extra scalar load) — 16 load instructions per coarse cell instead of 64 half-used ones.
+template <typename T>
+__global__ void __launch_bounds__(256)
+    k_restrict_v(Op fine, Op coarse, const T* __restrict__ r, T* __restrict__ fc) {
+    using V2 = typename Vec2<T>::type;
+    const int lane = threadIdx.x;
+    const int I = blockIdx.x * 32 + lane, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    const bool in = I < coarse.n[0] && J < coarse.n[1];
+    const bool has_l = 2 * I - 1 >= 0, has_r = 2 * I + 2 < fine.n[0];
+    const double W[4] = {0.125, 0.375, 0.375, 0.125};
+    T acc = 0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int j = 2 * J - 1 + b, k = 2 * K - 1 + c;
+            const bool row = in && j >= 0 && j < fine.n[1] && k >= 0 && k < fine.n[2];
+            V2 v;
+            v.x = v.y = (T)0;
+            const T* const p = r + gidx(fine, 2 * I, j, k);
+            if (row) v = *reinterpret_cast<const V2*>(p);
+            T left = __shfl_up_sync(0xffffffffu, v.y, 1), right = __shfl_down_sync(0xffffffffu, v.x, 1);
+            if (row && lane == 0 && has_l) left = p[-1];
+            if (row && lane == 31 && has_r) right = p[2];
+            if (row) {
+                if (has_l) acc += (T)(W[0] * W[b] * W[c]) * left;
+                acc += (T)(W[1] * W[b] * W[c]) * v.x;
+                acc += (T)(W[2] * W[b] * W[c]) * v.y;
+                if (has_r) acc += (T)(W[3] * W[b] * W[c]) * right;
+            }
+        }
+    if (in) fc[gidx(coarse, I, J, K)] = acc;
+}
+
 // coarse value with the ghost closure applied axis by axis: out-of-range index -> -gamma * clamped value
 template <typename T>
 __device__ __forceinline__ T coarse_val(const Op& c, const T* __restrict__ e, int I, int J, int K) {
@@ -44,17 +92,6 @@ __device__ __forceinline__ T coarse_val(const Op& c, const T* __restrict__ e, in
     return sgn * e[gidx(c, I, J, K)];
 }
 
-template <typename T>
-struct Vec2 {};
-template <>
-struct Vec2<double> {
-    using type = double2;
-};
-template <>
-struct Vec2<float> {
-    using type = float2;
-};
-
 // phi += P e_c (trilinear, "P = c R^T").  One thread per COARSE cell: it reads the 3 x 3 x 3 coarse
 // neighbourhood once (ghost closure applied by coarse_val) and updates its 8 fine children, two x-adjacent ones per
 // 16-byte (fp64) access.  Per fine point the arithmetic is exactly
@@ -65,17 +102,47 @@ __global__ void __launch_bounds__(256)
     using V2 = typename Vec2<T>::type;
     const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
     if (I >= coarse.n[0] || J >= coarse.n[1]) return;
+    // the four 16-byte pairs of phi this thread updates: loaded first, so that they are in flight during the interpolation
+    // (taking the x neighbours from the neighbour lanes by shuffles instead of loading them was measured slower)
+    V2* const q0 = reinterpret_cast<V2*>(phi + gidx(fine, 2 * I, 2 * J, 2 * K));
+    const size_t qsj = (size_t)fine.n[0] / 2, qsk = qsj * fine.n[1];  // strides in pairs
+    V2 w[2][2];
+#pragma unroll
+    for (int pk = 0; pk < 2; ++pk)
+#pragma unroll
+        for (int pj = 0; pj < 2; ++pj) w[pk][pj] = q0[pk * qsk + pj * qsj];
     T ex[2][3][3];  // [x parity][dJ][dK]
+    // Rows J +- 1 and planes K +- 1 all inside the coarse grid (true for whole warps, and for all but the boundary
+    // layers): no closure in y and z, and the x closure (clamped index, factor -gamma) is worked out once per thread —
+    // the same values as coarse_val delivers (1 * e and (-gamma) * e) with an eighth of its integer instructions.
+    const bool jk_inside = J >= 1 && J + 1 < coarse.n[1] && K >= 1 && K + 1 < coarse.n[2];
+    if (jk_inside) {
+        const T mg = (T)(-coarse.gamma);
+        const int Im = I > 0 ? I - 1 : 0, Ip = I + 1 < coarse.n[0] ? I + 1 : coarse.n[0] - 1;
+        const T sm = I > 0 ? (T)1 : mg, sp = I + 1 < coarse.n[0] ? (T)1 : mg;
+        const size_t sj = (size_t)coarse.n[0], sk = sj * coarse.n[1];
+        const T* const c0 = ec + gidx(coarse, 0, J - 1, K - 1);
 #pragma unroll
-    for (int dk = 0; dk < 3; ++dk)
+        for (int dk = 0; dk < 3; ++dk)
 #pragma unroll
-        for (int dj = 0; dj < 3; ++dj) {
-            const T em = coarse_val(coarse, ec, I - 1, J + dj - 1, K + dk - 1);
-            const T e0 = coarse_val(coarse, ec, I, J + dj - 1, K + dk - 1);
-            const T ep = coarse_val(coarse, ec, I + 1, J + dj - 1, K + dk - 1);
-            ex[0][dj][dk] = fma_((T)0.75, e0, (T)0.25 * em);
-            ex[1][dj][dk] = fma_((T)0.75, e0, (T)0.25 * ep);
-        }
+            for (int dj = 0; dj < 3; ++dj) {
+                const T* const row = c0 + dk * sk + dj * sj;
+                const T em = sm * row[Im], e0 = row[I], ep = sp * row[Ip];
+                ex[0][dj][dk] = fma_((T)0.75, e0, (T)0.25 * em);
+                ex[1][dj][dk] = fma_((T)0.75, e0, (T)0.25 * ep);
+            }
+    } else {
+#pragma unroll
+        for (int dk = 0; dk < 3; ++dk)
+#pragma unroll
+            for (int dj = 0; dj < 3; ++dj) {
+                const T em = coarse_val(coarse, ec, I - 1, J + dj - 1, K + dk - 1);
+                const T e0 = coarse_val(coarse, ec, I, J + dj - 1, K + dk - 1);
+                const T ep = coarse_val(coarse, ec, I + 1, J + dj - 1, K + dk - 1);
+                ex[0][dj][dk] = fma_((T)0.75, e0, (T)0.25 * em);
+                ex[1][dj][dk] = fma_((T)0.75, e0, (T)0.25 * ep);
+            }
+    }
 #pragma unroll
     for (int pk = 0; pk < 2; ++pk)
 #pragma unroll
@@ -89,11 +156,10 @@ __global__ void __launch_bounds__(256)
                 const T ey_far = fma_((T)0.75, ex[pi][1][fk], (T)0.25 * ex[pi][fj][fk]);
                 v[pi] = fma_((T)0.75, ey_near, (T)0.25 * ey_far);
             }
-            V2* q = reinterpret_cast<V2*>(phi + gidx(fine, 2 * I, 2 * J + pj, 2 * K + pk));
-            V2 w = *q;
-            w.x += v[0];
-            w.y += v[1];
-            *q = w;
+            V2 o = w[pk][pj];
+            o.x += v[0];
+            o.y += v[1];
+            q0[pk * qsk + pj * qsj] = o;
         }
 }
 
@@ -311,7 +377,11 @@ int launch_mg_bottom32(poisson_ctx* ctx, const Op* ops, int nlev, float* phi, co
 template <typename T>
 static int restrict_t(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T* r, T* fc, int restriction) {
     dim3 b(32, 8), g((coarse.n[0] + 31) / 32, (coarse.n[1] + 7) / 8, coarse.n[2]);
-    PB_LAUNCH(ctx, KID_MG_RESTRICT, (k_restrict<T><<<g, b, 0, ctx->stream>>>(fine, coarse, r, fc, restriction)));
+    const bool two_to_one = fine.n[0] == 2 * coarse.n[0] && fine.n[1] == 2 * coarse.n[1] && fine.n[2] == 2 * coarse.n[2];
+    if (restriction == 0 && two_to_one && ctx->opt_path != 1)
+        PB_LAUNCH(ctx, KID_MG_RESTRICT, (k_restrict_v<T><<<g, b, 0, ctx->stream>>>(fine, coarse, r, fc)));
+    else
+        PB_LAUNCH(ctx, KID_MG_RESTRICT, (k_restrict<T><<<g, b, 0, ctx->stream>>>(fine, coarse, r, fc, restriction)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
