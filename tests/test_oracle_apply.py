@@ -151,3 +151,44 @@ def test_spherical_second_order_on_r_cos_theta():
         errs.append(rel.max())
     assert errs[0] < 3e-2
     assert errs[0] / errs[1] == pytest.approx(4.0, rel=0.1)
+
+
+# ---- Cartesian zero-flux (Neumann) faces: the diagonal modification of oracle/grid.hpp diag() -------------------------
+N6 = (po.BC_NEUMANN0,) * 6
+
+
+def test_7pt_all_neumann_box_annihilates_constants_and_has_cosine_eigenvectors():
+    # PAPER.md:43-45 Eq. 1 with zero normal flux through every face (cell-centred: the mirror ghost equals the adjacent
+    # interior value, which removes one off-diagonal coefficient and lowers the diagonal by the same amount).  Then
+    # every row sums to zero (L 1 = 0 on ALL rows, faces/edges/corners included) and cos(m pi (i+1/2)/n) per axis is an
+    # exact eigenvector with eigenvalue -(4/h^2) sin^2(m pi/(2n)) (textbook DCT-II spectrum).  Dropping the `d -= c`
+    # on a face breaks both on that face's rows.
+    shape, h = (9, 6, 7), (0.2, 0.35, 0.15)
+    o = po.Oracle(shape, h, bc=N6)
+    out = o.apply(np.ones(o.npshape), use_ghost=False)
+    assert np.abs(out).max() <= 1e-12 * 2 * sum(1 / s ** 2 for s in h)
+    for m in ((1, 0, 0), (0, 2, 0), (0, 0, 3), (2, 1, 4), (8, 5, 6)):
+        cx = np.cos(m[0] * math.pi * (np.arange(shape[0]) + 0.5) / shape[0])
+        cy = np.cos(m[1] * math.pi * (np.arange(shape[1]) + 0.5) / shape[1])
+        cz = np.cos(m[2] * math.pi * (np.arange(shape[2]) + 0.5) / shape[2])
+        u = np.ascontiguousarray(cz[:, None, None] * cy[None, :, None] * cx[None, None, :])
+        lam = -sum((4 / h[a] ** 2) * math.sin(m[a] * math.pi / (2 * shape[a])) ** 2 for a in range(3))
+        assert np.abs(o.apply(u, use_ghost=False) - lam * u).max() <= 1e-12 * 2 * sum(1 / s ** 2 for s in h)
+
+
+def test_7pt_mixed_neumann_dirichlet_faces_dense_matrix():
+    # one Neumann face per axis (low x, high y, low z), ghost-Dirichlet on the others: still symmetric, and per axis the
+    # matrix is tridiag(1,-2,1)/h^2 with one -1 corner (mirror ghost on one side, ghost value at distance h on the
+    # other), whose eigenvalues are -(4/h^2) sin^2((2m+1) pi / (2(2n+1))), m = 0..n-1 (textbook Neumann-Dirichlet second
+    # difference).  The 3-D spectrum is the sum over the axes.
+    shape, h = (5, 4, 6), (0.3, 0.2, 0.25)
+    bc = (po.BC_NEUMANN0, po.BC_DIRICHLET_GHOST, po.BC_DIRICHLET_GHOST, po.BC_NEUMANN0, po.BC_NEUMANN0,
+          po.BC_DIRICHLET_GHOST)
+    o = po.Oracle(shape, h, bc=bc)
+    A = dense_matrix(o)
+    assert np.abs(A - A.T).max() == 0.0
+    ev = np.sort(np.linalg.eigvalsh(A))
+    ax = [np.array([-(4 / h[a] ** 2) * math.sin((2 * m + 1) * math.pi / (2 * (2 * shape[a] + 1))) ** 2
+                    for m in range(shape[a])]) for a in range(3)]
+    want = np.sort((ax[2][:, None, None] + ax[1][None, :, None] + ax[0][None, None, :]).ravel())
+    assert np.abs(ev - want).max() <= 1e-11 * np.abs(want).max()

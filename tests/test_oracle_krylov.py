@@ -207,3 +207,34 @@ def test_bicgstab_restart_branch_forced_still_solves_the_system():
     phi2 = np.zeros_like(rhs)
     o.bicgstab(phi2, rhs, rtol=1e-11, max_iter=4000)
     assert po.Oracle.bicgstab_stats()[0] == 0 and rel_l2(phi2, exact) < 1e-9      # default threshold: no restart here
+
+
+def test_bicgstab_restart_equals_a_fresh_warm_started_solve():
+    # DESIGN.md reading C4: a near-breakdown restart is "take r^_0 := r, rho := r.r, beta := 0 (p := r)", i.e. exactly what
+    # a NEW BiCGSTAB call warm-started from the current iterate does (it takes r = rhs - L x, which equals the recursively
+    # updated r up to round-off).  With the threshold raised to 10 the test |r^_0.r| <= eps ||r^_0|| ||r|| holds in every
+    # iteration (Cauchy-Schwarz), so k iterations of one call must equal k successive warm-started one-iteration calls.
+    # A stale rho (rho_new = r^_0_old . r kept instead of r.r), a p that is not reset, or an r^_0 that is not replaced
+    # gives a different alpha in the very next iteration and fails this at the 1e-2 level.
+    o = _sph_small()
+    rhs = wl.random_field(o.shape, 23)
+    k = 6
+    try:
+        po.Oracle.set_bicgstab_restart_eps(10.0)
+        a = np.zeros_like(rhs)
+        res = o.bicgstab(a, rhs, fixed_iters=k, want_history=True)
+        assert po.Oracle.bicgstab_stats()[0] >= k - 1
+    finally:
+        po.Oracle.set_bicgstab_restart_eps(1e-12)
+    b = np.zeros_like(rhs)
+    r0 = o.residual_norm(b, rhs)
+    hist = [1.0]
+    for _ in range(k):
+        o.bicgstab(b, rhs, fixed_iters=1)
+        hist.append(o.residual_norm(b, rhs) / r0)
+    assert rel_l2(a, b) < 1e-11
+    assert np.allclose(res["history"], hist, rtol=1e-9)
+    # and the restarted run is NOT what the unrestarted recurrence produces (the test bites)
+    c = np.zeros_like(rhs)
+    o.bicgstab(c, rhs, fixed_iters=k)
+    assert rel_l2(c, a) > 1e-3

@@ -142,3 +142,25 @@ def test_vcycle_fixed_point_is_discrete_solution():
         phi = np.zeros_like(rhs)
         o.vcycle(phi, rhs, coarsest_n=4, coarsest_sweeps=50, restriction=restriction, ncycles=25)
         assert rel_l2(phi, exact) < 1e-12
+
+
+def test_coarsest_level_sor_uses_omega_opt_of_the_8cubed_operator():
+    # DESIGN.md reading C7 / PAPER.md:65-76 Eq. 3-4: the coarsest level is solved by SOR sweeps at omega_opt =
+    # 2/(1+sin(pi/(n+1))) of an n-unknowns-per-axis Dirichlet operator (r_J = cos(pi/(n+1))).  At omega_opt every
+    # eigenvalue of the SOR iteration matrix has modulus omega_opt - 1 (Young's theory; the red-black ordering is
+    # consistently ordered), so the residual contracts asymptotically like k (omega_opt-1)^k: between 30 and 50 sweeps
+    # the mean factor per sweep is (50/30)^(1/20) (omega_opt - 1) = 1.026 * 0.4903 = 0.503.  With pi/n instead of
+    # pi/(n+1) (omega = 1.4465 < omega_opt) the spectral radius is ((omega r_J + sqrt(omega^2 r_J^2 - 4(omega-1)))/2)^2
+    # = 0.646, far outside the band.  On a single-level hierarchy (grid == coarsest grid) a "V-cycle" is exactly that solve.
+    n = 8
+    h = 2.0 / n
+    o = po.Oracle((n,) * 3, (h,) * 3, origin=(-1 + h / 2,) * 3, bc=D6)
+    rhs = wl.random_field((n,) * 3, 43)
+    res = {}
+    for sweeps in (30, 50):
+        phi = np.zeros_like(rhs)
+        res[sweeps] = o.vcycle(phi, rhs, coarsest_n=n, coarsest_sweeps=sweeps, ncycles=1)["resnorms"][1]
+    factor = (res[50] / res[30]) ** (1 / 20)
+    w_opt = 2 / (1 + math.sin(math.pi / (n + 1)))
+    assert factor == pytest.approx((50 / 30) ** (1 / 20) * (w_opt - 1), rel=0.03)
+    assert factor < 0.53
