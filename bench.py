@@ -45,7 +45,8 @@ UNIT = "Gpoint-updates/s"
 
 # Algorithmic bytes per point per unit.
 ROW_BYTES = {
-    "multipole_bc": 8, "apply_laplacian": 16, "rbsor_sweep": 24, "mg_vcycle_f64": 75, "mg_vcycle_mixed": 66,
+    "multipole_bc": 8, "apply_laplacian": 16, "rbsor_sweep": 12,   # 24/T, T = 2 sweeps per HBM pass (NHS = 4) on grids >= 2^21 points
+    "mg_vcycle_f64": 75, "mg_vcycle_mixed": 66,
     "residual_norm": 16, "cg_iteration_19pt": 72, "multipole_bc_spherical": 8, "bicgstab_iteration": 136,
 }
 NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 250
@@ -225,6 +226,13 @@ def run_ours(args):
     omega3 = 2.0 / (1.0 + math.sin(math.pi / (p["n3"] + 1)))
     row_names = [u[0] for u in units]
 
+    def krylov_ok(what, res, fixed):
+        # a BREAKDOWN in fixed mode sets the device `done` flag and every later pass returns at once: that would time
+        # empty launches.  A timed solve must have run all its iterations.
+        if res["status"] != pb.OK or res["iters"] != fixed:
+            raise SystemExit("bench: %s ended with status %d after %d of %d iterations — timing would be invalid"
+                             % (what, res["status"], res["iters"], fixed))
+
     def _apply():
         for _ in range(p["apply"]):
             g3.apply_laplacian(d["phi3"], d["out3"])
@@ -242,9 +250,10 @@ def run_ours(args):
         "mg_vcycle_mixed": lambda: g3.mg_vcycle(d["mx3"], d["rhs3"], ncycles=p["vcmx"], precision=pb.MIXED,
                                                 want_resnorms=False),
         "residual_norm": _resn,
-        "cg_iteration_19pt": lambda: g4.cg_solve(d["phi4"], d["rhs4"], fixed_iters=p["cg"]),
+        "cg_iteration_19pt": lambda: krylov_ok("CG", g4.cg_solve(d["phi4"], d["rhs4"], fixed_iters=p["cg"]), p["cg"]),
         "multipole_bc_spherical": lambda: g5.multipole_bc(d["rho5"], 1.0, 8, want_moments=False),
-        "bicgstab_iteration": lambda: g5.bicgstab_solve(d["phi5"], d["rhs5"], fixed_iters=p["bicg"]),
+        "bicgstab_iteration": lambda: krylov_ok("BiCGSTAB", g5.bicgstab_solve(d["phi5"], d["rhs5"],
+                                                                             fixed_iters=p["bicg"]), p["bicg"]),
     }
 
     def step_device(ev=None):
@@ -271,13 +280,16 @@ def run_ours(args):
                                                       want_resnorms=False), 2 * n3b, n3b),
         # residual norm of host data: zero sweeps + the norm
         "residual_norm": (lambda: g3.rbsor_sweep_host(h["phi3"], h["rhs3"], 1.0, 0, want_resnorm=True), 2 * n3b, n3b),
-        "cg_iteration_19pt": (lambda: g4.cg_solve_host(h["phi4"], h["rhs4"], fixed_iters=p["cg"]), 2 * n4b, n4b),
+        "cg_iteration_19pt": (lambda: krylov_ok("CG (host)", g4.cg_solve_host(h["phi4"], h["rhs4"],
+                                                                             fixed_iters=p["cg"]), p["cg"]), 2 * n4b, n4b),
         "multipole_bc_spherical": (lambda: g5.multipole_bc_host(h["rho5"], 1.0, 8, want_moments=False), n5b, 0),
-        "bicgstab_iteration": (lambda: g5.bicgstab_solve_host(h["phi5"], h["rhs5"], fixed_iters=p["bicg"]),
-                               2 * n5b, n5b),
+        "bicgstab_iteration": (lambda: krylov_ok("BiCGSTAB (host)", g5.bicgstab_solve_host(
+            h["phi5"], h["rhs5"], fixed_iters=p["bicg"]), p["bicg"]), 2 * n5b, n5b),
     }
 
     def step_host():
+        for k in ("phi3", "phi4", "phi5"):
+            h[k].zero_()
         for name in row_names:
             host_fn[name][0]()
 
@@ -310,6 +322,7 @@ def run_ours(args):
     t0.record()
     for _ in range(args.steps):
         ev = []
+        zero_state()   # every timed step starts from the same cold state (phi = 0) as the warm-up steps
         step_device(ev)
         evs.append(ev)
     t1.record()

@@ -62,20 +62,31 @@ enum {
     POISSON_OPT_FUSED_RESTRICT = 7,/* V-cycle: residual + restriction fused into one pass over the level (no fine residual
                                       in memory): 0 = automatic (fp32 levels of the mixed cycle), 1 = always, 2 = never;
                                       the results do not depend on it */
-    POISSON_OPT_TIME_KERNELS = 5   /* bracket every launch of one kernel class (0..poisson_kernel_classes()-1) with
+    POISSON_OPT_TIME_KERNELS = 5,  /* bracket every launch of one kernel class (0..poisson_kernel_classes()-1) with
                                       CUDA events on the handle's stream; -2 = every class, -1 = off (default) */
+    /* tuning overrides for measurements; the results do not depend on them; -1 = automatic (default) */
+    POISSON_OPT_TILE_CFG = 9,      /* index of the compiled tile configuration of the fused SOR / lean apply kernels */
+    POISSON_OPT_PLANE_SPLIT = 10,  /* plane engine: 1 = always split the (tile, plane) items linearly, 0 = never */
+    POISSON_OPT_APPLY_BULK = 11,   /* TMA-staged 7-point apply: 1 = whenever eligible, 0 = never */
+    /* floating-point options (poisson_set_option_f64) */
+    POISSON_OPT_BICG_RESTART_EPS = 8 /* BiCGSTAB near-breakdown restart threshold on |r0^.r| / (|r0^| |r|); default
+                                      1e-12 (reading C4), 0 = never restart */
 };
 
 /* Create a solver context for one grid + operator ("uniform and nonuniform grids in spherical and
  * Cartesian coordinates"; 41-57).
  *   shape[3], spacing[3], origin[3]: Cartesian geometry (spacing/origin ignored for spherical).
- *   edges: NULL for Cartesian; for spherical three HOST arrays of shape[a]+1 cell-edge coordinates (r, theta, phi).
- *          Radial centres are the geometric means of the edges.
+ *   edges: NULL for Cartesian; for spherical three HOST arrays of shape[a]+1 strictly increasing cell-edge
+ *          coordinates (r, theta, phi), r_in > 0, theta within [0, pi].  Only r may be nonuniform (radial centres are
+ *          the geometric means of the edges); theta and phi edges must be uniform (UNSUPPORTED
+ *          otherwise) and a BC_AXIS face must lie on the polar axis (theta edge 0 or pi).
  *   coord_system: POISSON_CARTESIAN | POISSON_SPHERICAL.
  *   stencil_order: 2 (7-point, radius 1) or 6 (19-point star, radius 3; Cartesian only) — PAPER.md:172.
  *   bc[6]: boundary type per face.
  *   cuda_stream: a cudaStream_t (NULL = default stream).
- * Errors: INVALID_ARG (bad shape/order/bc), UNSUPPORTED, OUT_OF_MEMORY, CUDA_ERROR. */
+ * The handle is bound to the CUDA device that is current at create time (every call runs there whatever the
+ * caller's current device is) and must not be used from two threads at once.
+ * Errors: INVALID_ARG (bad shape/order/bc/edges), UNSUPPORTED, OUT_OF_MEMORY, CUDA_ERROR. */
 int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], const double origin[3],
                    const double* const edges[3], int coord_system, int stencil_order, const int bc[6],
                    void* cuda_stream);
@@ -83,6 +94,7 @@ int poisson_destroy(poisson_t h);
 /* Static string describing the last error of this handle (or of create when h is NULL). */
 const char* poisson_last_error(poisson_t h);
 int poisson_set_option(poisson_t h, int option, int value);
+int poisson_set_option_f64(poisson_t h, int option, double value);
 
 /* out = L_h phi with the handle's ghost values on Dirichlet faces.  d_out must not alias d_phi. */
 int poisson_apply_laplacian(poisson_t h, const double* d_phi, double* d_out);
@@ -102,8 +114,8 @@ int poisson_cg_solve(poisson_t h, double* d_phi, const double* d_rhs, double rto
 
 /* BiCGSTAB (Saad Alg. 7.7) with right Jacobi scaling, for the nonsymmetric spherical operator;
  * same stopping rule.  Near-breakdown restart (reading C4): when |r0^.r| <= 1e-12 |r0^| |r| at the beta
- * step the shadow residual is replaced by r (rho = r.r, beta = 0); the environment variable
- * POISSON_BICG_RESTART_EPS overrides the threshold, 0 disables the rule.  When the recurrence's residual meets rtol the
+ * step the shadow residual is replaced by r (rho = r.r, beta = 0); POISSON_OPT_BICG_RESTART_EPS overrides the
+ * threshold, 0 disables the rule.  When the recurrence's residual meets rtol the
  * true residual rhs - L phi is recomputed: OK (and *relres the true figure) only if it meets rtol as well, otherwise
  * the iteration carries on from it; NOT_CONVERGED also after 30 such checks have failed (rtol below the attainable
  * accuracy).  fixed_iters > 0 runs exactly that many iterations without any check.
@@ -111,9 +123,12 @@ int poisson_cg_solve(poisson_t h, double* d_phi, const double* d_rhs, double rto
 int poisson_bicgstab_solve(poisson_t h, double* d_phi, const double* d_rhs, double rtol, int max_iter,
                            int fixed_iters, int* iters, double* relres);
 
-/* ncycles geometric-multigrid V-cycles (Eq. 11-13): nu1/nu2 red-black Gauss-Seidel sweeps,
- * full-weighting restriction, trilinear prolongation, 2:1 cell-centred coarsening down to coarsest_n points per
- * axis, coarsest level by coarsest_sweeps SOR sweeps.  precision = POISSON_F64 or POISSON_MIXED (fp64 residual
+/* ncycles geometric-multigrid V-cycles (Eq. 11-12) in the CELL-CENTRED variant BASELINE.json config 3
+ * fixes (reading C7) — not the paper's own vertex-centred Eq. 13-14 operators, for which see
+ * poisson_mgv_vcycle below: nu1/nu2 red-black Gauss-Seidel sweeps, restriction = transpose of trilinear
+ * (1/8)[1 3 3 1]^3 ("full weighting" for cell centres; P = 8 R^T), trilinear prolongation, 7-point
+ * rediscretisation on 2:1 coarsened cells down to coarsest_n points per axis, coarsest level by coarsest_sweeps SOR
+ * sweeps at omega_opt of Eq. 3-4.  precision = POISSON_F64 or POISSON_MIXED (fp64 residual
  * and correction, fp32 error-equation cycle).  Cartesian, order 2, Dirichlet faces only.
  * h_resnorms (nullable, ncycles+1): ||rhs - L phi||_2 before the first and after every cycle. */
 int poisson_mg_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
@@ -136,6 +151,8 @@ long poisson_face_len(poisson_t h, int face);
 int poisson_residual_norm(poisson_t h, const double* d_phi, const double* d_rhs, double* h_norm);
 /* Relative residual history of the last Krylov solve (needs POISSON_OPT_RECORD_HISTORY): h_out[0..n-1]. */
 int poisson_get_history(poisson_t h, double* h_out, int n);
+/* Near-breakdown restarts taken and true-residual confirmations that failed in the last BiCGSTAB solve (nullable). */
+int poisson_bicgstab_stats(poisson_t h, int* restarts, int* confirm_failed);
 /* Number of kernels this handle has launched so far (bench bookkeeping). */
 long poisson_kernel_launches(poisson_t h);
 

@@ -48,7 +48,9 @@ int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, i
     const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
     if (history) history[0] = 1.0;
     int it = 0, status = (fixed_iters > 0) ? ST_OK : ST_NOT_CONVERGED;
-    if (fixed_iters <= 0 && (rr0 == 0.0)) {
+    if (!std::isfinite(rr0)) {
+        status = ST_BREAKDOWN;  // NaN/Inf in rhs or in the initial guess (include/poisson.h "BREAKDOWN"); no iteration
+    } else if (fixed_iters <= 0 && (rr0 == 0.0)) {
         status = ST_OK;
     } else {
         for (it = 0; it < nit;) {
@@ -121,7 +123,9 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
     const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
     if (history) history[0] = 1.0;
     int it = 0, status = (fixed_iters > 0) ? ST_OK : ST_NOT_CONVERGED;
-    if (fixed_iters <= 0 && rr0 == 0.0) {
+    if (!std::isfinite(rr0)) {
+        status = ST_BREAKDOWN;  // NaN/Inf in rhs or in the initial guess; no iteration
+    } else if (fixed_iters <= 0 && rr0 == 0.0) {
         status = ST_OK;
     } else {
         for (it = 0; it < nit;) {

@@ -16,11 +16,13 @@ F64, MIXED = 0, 1
 OK, NOT_CONVERGED, BREAKDOWN = 0, 1, 2
 INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY = -1, -2, -3, -4
 OPT_KERNEL_PATH, OPT_RESTRICTION, OPT_POLL_INTERVAL, OPT_JACOBI, OPT_RECORD_HISTORY, OPT_TIME_KERNELS = 0, 1, 2, 3, 4, 5
-OPT_SOR_HALFSTEPS, OPT_FUSED_RESTRICT = 6, 7
+OPT_SOR_HALFSTEPS, OPT_FUSED_RESTRICT, OPT_BICG_RESTART_EPS = 6, 7, 8
+OPT_TILE_CFG, OPT_PLANE_SPLIT, OPT_APPLY_BULK = 9, 10, 11
 PATH_AUTO, PATH_GENERIC, PATH_PLANE = 0, 1, 2
 
 SYMBOLS = [
-    "poisson_create", "poisson_destroy", "poisson_last_error", "poisson_set_option", "poisson_apply_laplacian",
+    "poisson_create", "poisson_destroy", "poisson_last_error", "poisson_set_option", "poisson_set_option_f64",
+    "poisson_bicgstab_stats", "poisson_apply_laplacian",
     "poisson_rbsor_sweep", "poisson_cg_solve", "poisson_bicgstab_solve", "poisson_mg_vcycle", "poisson_multipole_bc",
     "poisson_set_ghost_faces", "poisson_get_ghost_face", "poisson_face_len", "poisson_residual_norm",
     "poisson_get_history", "poisson_kernel_launches", "poisson_kernel_classes", "poisson_kernel_name",
@@ -126,6 +128,15 @@ class Poisson:
 
     def set_option(self, option, value):
         self._check(lib().poisson_set_option(self.h, int(option), int(value)))
+
+    def set_option_f64(self, option, value):
+        self._check(lib().poisson_set_option_f64(self.h, int(option), C.c_double(value)))
+
+    def bicgstab_stats(self):
+        """(near-breakdown restarts, failed true-residual confirmations) of the last BiCGSTAB solve."""
+        a, b = C.c_int(0), C.c_int(0)
+        self._check(lib().poisson_bicgstab_stats(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def kernel_launches(self):
         return int(lib().poisson_kernel_launches(self.h))

@@ -182,6 +182,7 @@ extern "C" {
 const char* poisson_last_error(poisson_t h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
 int poisson_destroy(poisson_t ctx) {
+    const DeviceGuard on_device(ctx);
     if (!ctx) return POISSON_INVALID_ARG;
     cudaStreamSynchronize(ctx->stream);
     free_levels(ctx);
@@ -237,10 +238,29 @@ int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], 
     } else {
         if (!edges || !edges[0] || !edges[1] || !edges[2])
             return fail(nullptr, POISSON_INVALID_ARG, "spherical grids need edges[3]");
+        for (int a = 0; a < 3; ++a)
+            for (int i = 0; i < shape[a]; ++i)
+                if (!(edges[a][i + 1] > edges[a][i]))
+                    return fail(nullptr, POISSON_INVALID_ARG, "cell edges must increase strictly");
+        if (!(edges[0][0] > 0.0)) return fail(nullptr, POISSON_INVALID_ARG, "spherical grids need r_in > 0");
+        if (edges[1][0] < -1e-12 || edges[1][shape[1]] > M_PI + 1e-12)
+            return fail(nullptr, POISSON_INVALID_ARG, "theta edges must lie in [0, pi]");
+        // the theta and phi differences are taken with one cell width (reading C5): uniform angles only
+        for (int a = 1; a < 3; ++a) {
+            const double w0 = (edges[a][shape[a]] - edges[a][0]) / shape[a];
+            for (int i = 0; i < shape[a]; ++i)
+                if (std::fabs((edges[a][i + 1] - edges[a][i]) - w0) > 1e-10 * w0)
+                    return fail(nullptr, POISSON_UNSUPPORTED, "nonuniform theta / phi edges are not supported (only r may be nonuniform)");
+        }
+        if (bc[2] == POISSON_BC_AXIS && std::fabs(edges[1][0]) > 1e-12)
+            return fail(nullptr, POISSON_INVALID_ARG, "BC_AXIS on the low theta face needs theta_edge[0] = 0");
+        if (bc[3] == POISSON_BC_AXIS && std::fabs(edges[1][shape[1]] - M_PI) > 1e-12)
+            return fail(nullptr, POISSON_INVALID_ARG, "BC_AXIS on the high theta face needs theta_edge[n] = pi");
+        if (bc[0] == POISSON_BC_AXIS || bc[1] == POISSON_BC_AXIS || bc[4] == POISSON_BC_AXIS || bc[5] == POISSON_BC_AXIS)
+            return fail(nullptr, POISSON_INVALID_ARG, "BC_AXIS applies to the theta faces only");
     }
     poisson_ctx* ctx = new poisson_ctx;
     ctx->stream = (cudaStream_t)cuda_stream;
-    if (const char* e = getenv("POISSON_SOR_HALFSTEPS")) ctx->opt_sor_nhs = atoi(e) == 4 ? 4 : (atoi(e) == 2 ? 2 : 0);  // tuning aid
     Op& op = ctx->op;
     std::memset(&op, 0, sizeof(op));
     ctx->npts = 1;
@@ -258,6 +278,7 @@ int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], 
     ctx->kind = coord_system == POISSON_SPHERICAL ? KIND_SPH : (stencil_order == 6 ? KIND_CART6 : KIND_CART2);
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
+    ctx->device = dev;
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) {
         int rc = fail_cuda(nullptr, e, "cudaGetDevice", __FILE__, __LINE__);
@@ -334,12 +355,39 @@ int poisson_set_option(poisson_t ctx, int option, int value) {
             if (value < 0 || value > 2) return fail(ctx, POISSON_INVALID_ARG, "fused restriction must be 0, 1 or 2");
             ctx->opt_fused_restrict = value;
             return POISSON_OK;
+        case POISSON_OPT_TILE_CFG:
+            ctx->opt_tile_cfg = value < 0 ? -1 : value;
+            return POISSON_OK;
+        case POISSON_OPT_PLANE_SPLIT:
+            ctx->opt_plane_split = value < 0 ? -1 : (value ? 1 : 0);
+            return POISSON_OK;
+        case POISSON_OPT_APPLY_BULK:
+            ctx->opt_apply_bulk = value < 0 ? -1 : (value ? 1 : 0);
+            return POISSON_OK;
         case POISSON_OPT_TIME_KERNELS:
             if (value < -2 || value >= KID_COUNT) return fail(ctx, POISSON_INVALID_ARG, "bad kernel class");
             ctx->time_kid = value;
             return POISSON_OK;
     }
     return fail(ctx, POISSON_INVALID_ARG, "unknown option");
+}
+
+int poisson_set_option_f64(poisson_t ctx, int option, double value) {
+    if (!ctx) return POISSON_INVALID_ARG;
+    switch (option) {
+        case POISSON_OPT_BICG_RESTART_EPS:
+            if (!(value >= 0.0)) return fail(ctx, POISSON_INVALID_ARG, "restart threshold must be >= 0");
+            ctx->opt_bicg_restart_eps = value;
+            return POISSON_OK;
+    }
+    return fail(ctx, POISSON_INVALID_ARG, "unknown floating-point option");
+}
+
+int poisson_bicgstab_stats(poisson_t ctx, int* restarts, int* confirm_failed) {
+    if (!ctx) return POISSON_INVALID_ARG;
+    if (restarts) *restarts = ctx->last_restarts;
+    if (confirm_failed) *confirm_failed = ctx->last_confirm_failed;
+    return POISSON_OK;
 }
 
 long poisson_face_len(poisson_t ctx, int face) { return (ctx && face >= 0 && face < 6) ? ctx->face_len[face] : -1; }
@@ -353,6 +401,7 @@ long poisson_kernel_class_launches(poisson_t ctx, int kernel_class) {
     return (ctx && kernel_class >= 0 && kernel_class < KID_COUNT) ? ctx->launches_by_kid[kernel_class] : -1;
 }
 int poisson_kernel_time(poisson_t ctx, int kernel_class, double* h_ms_total, long* h_count) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || kernel_class < 0 || kernel_class >= KID_COUNT) return POISSON_INVALID_ARG;
     PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
     double tot = 0;
@@ -369,6 +418,7 @@ int poisson_kernel_time(poisson_t ctx, int kernel_class, double* h_ms_total, lon
     return POISSON_OK;
 }
 int poisson_reset_kernel_times(poisson_t ctx) {
+    const DeviceGuard on_device(ctx);
     if (!ctx) return POISSON_INVALID_ARG;
     PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
     ctx->ev_used = 0;
@@ -376,6 +426,7 @@ int poisson_reset_kernel_times(poisson_t ctx) {
 }
 
 int poisson_set_ghost_faces(poisson_t ctx, const double* const d_faces[6]) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_faces) return POISSON_INVALID_ARG;
     for (int f = 0; f < 6; ++f) {
         if (!d_faces[f]) continue;
@@ -388,6 +439,7 @@ int poisson_set_ghost_faces(poisson_t ctx, const double* const d_faces[6]) {
 }
 
 int poisson_get_ghost_face(poisson_t ctx, int face, double* d_out) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || face < 0 || face > 5 || !d_out) return POISSON_INVALID_ARG;
     if (!ctx->d_ghost[face]) return fail(ctx, POISSON_INVALID_ARG, "not a Dirichlet face");
     PB_CUDA_OK(cudaMemcpyAsync(d_out, ctx->d_ghost[face], ctx->face_len[face] * sizeof(double),
@@ -396,6 +448,7 @@ int poisson_get_ghost_face(poisson_t ctx, int face, double* d_out) {
 }
 
 int poisson_apply_laplacian(poisson_t ctx, const double* d_phi, double* d_out) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_phi || !d_out || d_phi == d_out) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     return launch_apply(ctx, ctx->op, ctx->kind, d_phi, nullptr, d_out, 0, true, false);
 }
@@ -410,12 +463,14 @@ static int residual_norm_sync(poisson_ctx* ctx, const double* d_phi, const doubl
 }
 
 int poisson_residual_norm(poisson_t ctx, const double* d_phi, const double* d_rhs, double* h_norm) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_phi || !d_rhs || !h_norm) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     return residual_norm_sync(ctx, d_phi, d_rhs, h_norm);
 }
 
 int poisson_rbsor_sweep(poisson_t ctx, double* d_phi, const double* d_rhs, double omega, int nsweeps,
                         double* h_resnorm) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_phi || !d_rhs || nsweeps < 0) return fail(ctx, POISSON_INVALID_ARG, "bad arguments");
     if (!(omega > 0.0 && omega < 2.0)) return fail(ctx, POISSON_INVALID_ARG, "omega must lie in (0,2) (PAPER.md:63)");
     int rc = launch_rbsor(ctx, ctx->op, ctx->kind, d_phi, d_rhs, omega, nsweeps, true);
@@ -436,7 +491,6 @@ static int krylov_setup(poisson_ctx* ctx, double rtol, int max_iter, int fixed_i
     c->record = ctx->opt_history;
     c->npoints = (double)ctx->npts;
     c->eps_bd = ctx->opt_bicg_restart_eps;
-    if (const char* e = getenv("POISSON_BICG_RESTART_EPS")) c->eps_bd = atof(e);  // tuning aid
     if (ctx->opt_history) {
         if (ctx->hist_cap < nit + 1) {
             cudaFree(ctx->d_hist);
@@ -464,6 +518,7 @@ static bool all_periodic(const poisson_ctx* ctx) {
 
 int poisson_cg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,
                      int* iters, double* relres) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     if (fixed_iters <= 0 && (max_iter < 1 || !(rtol > 0))) return fail(ctx, POISSON_INVALID_ARG, "bad rtol/max_iter");
     if (ctx->kind == KIND_SPH)
@@ -481,8 +536,8 @@ int poisson_cg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double r
     for (int j = 0; j < nit;) {
         const int chunk = std::min(ctx->opt_poll, nit - j);
         for (int c = 0; c < chunk; ++c, ++j) {
-            launch_cg_passA(ctx, r, P[j & 1], P[(j + 1) & 1], q, d_phi);
-            launch_cg_passB(ctx, r, q);
+            if ((rc = launch_cg_passA(ctx, r, P[j & 1], P[(j + 1) & 1], q, d_phi)) != POISSON_OK) return rc;
+            if ((rc = launch_cg_passB(ctx, r, q)) != POISSON_OK) return rc;
         }
         PB_CUDA_OK(cudaGetLastError());
         if (fixed_iters <= 0) {
@@ -510,6 +565,7 @@ int poisson_cg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double r
 
 int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter,
                            int fixed_iters, int* iters, double* relres) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     if (fixed_iters <= 0 && (max_iter < 1 || !(rtol > 0))) return fail(ctx, POISSON_INVALID_ARG, "bad rtol/max_iter");
     double *r = scratch(ctx, 0), *r0 = scratch(ctx, 1), *P[2] = {scratch(ctx, 2), scratch(ctx, 3)},
@@ -526,9 +582,9 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
         const int chunk = std::min(ctx->opt_poll, nit - j);
         for (int c = 0; c < chunk; ++c, ++j) {
             const int o = j & 1, n = (j + 1) & 1;
-            launch_bicg_pass1(ctx, r, P[o], V[o], r0, P[n], V[n]);
-            launch_bicg_pass2(ctx, r, V[n], s, t);
-            launch_bicg_pass3(ctx, d_phi, P[n], s, t, r0, r);
+            if ((rc = launch_bicg_pass1(ctx, r, P[o], V[o], r0, P[n], V[n])) != POISSON_OK) return rc;
+            if ((rc = launch_bicg_pass2(ctx, r, V[n], s, t)) != POISSON_OK) return rc;
+            if ((rc = launch_bicg_pass3(ctx, d_phi, P[n], s, t, r0, r)) != POISSON_OK) return rc;
         }
         PB_CUDA_OK(cudaGetLastError());
         if (fixed_iters <= 0) {
@@ -557,15 +613,14 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
     if (iters) *iters = c.it;
     if (relres) *relres = c.rr0 > 0 ? std::sqrt(c.rr / c.rr0) : 0.0;
     if (c.status == POISSON_NOT_CONVERGED) ctx->err = "BiCGSTAB: residual threshold not reached within max_iter";
-    if (getenv("POISSON_DEBUG"))
-        fprintf(stderr, "bicgstab ctl: it %d status %d rr %.6e rr0 %.6e rho %.6e r0v %.6e alpha %.6e omega %.6e ts %.6e tt %.6e beta %.6e\n",
-                c.it, c.status, c.rr, c.rr0, c.rho, c.r0v, c.alpha, c.omega, c.ts, c.tt, c.beta);
-    if (getenv("POISSON_DEBUG")) fprintf(stderr, "bicgstab restarts: %d, true-residual restarts: %d\n", c.nrestarts, nconfirm_failed);
+    ctx->last_restarts = c.nrestarts;
+    ctx->last_confirm_failed = nconfirm_failed;
     if (c.status == POISSON_BREAKDOWN) ctx->err = "BiCGSTAB: breakdown (rho, omega or r0.v vanished or is not finite)";
     return c.status;
 }
 
 int poisson_get_history(poisson_t ctx, double* h_out, int n) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_out || n < 0) return POISSON_INVALID_ARG;
     if (!ctx->d_hist || n > ctx->hist_cap) return fail(ctx, POISSON_INVALID_ARG, "no history recorded / n too large");
     PB_CUDA_OK(cudaMemcpyAsync(h_out, ctx->d_hist, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
@@ -703,6 +758,7 @@ static int cycle32(poisson_ctx* ctx, size_t l, int nu1, int nu2, int csweeps, fl
 
 int poisson_mg_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
                       int coarsest_sweeps, int precision, int ncycles, double* h_resnorms) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     if (nu1 < 0 || nu2 < 0 || coarsest_n < 1 || coarsest_sweeps < 0 || ncycles < 0 ||
         (precision != POISSON_F64 && precision != POISSON_MIXED))
@@ -754,6 +810,7 @@ int poisson_mg_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1
 
 // ---- multipole boundary -------------------------------------------------------------------------------------------------
 int poisson_multipole_bc(poisson_t ctx, const double* d_rho, double G, int lmax, double* h_moments) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !d_rho) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     double* d_q = ctx->d_scal + 128;
@@ -793,6 +850,7 @@ static int unstage(poisson_ctx* ctx, int slot, double* h_dst) {
     } while (0)
 
 int poisson_apply_laplacian_host(poisson_t ctx, const double* h_phi, double* h_out) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_phi || !h_out) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     STAGE_OK(stage(ctx, 0, h_phi));
     STAGE_OK(stage(ctx, 1, nullptr));
@@ -803,6 +861,7 @@ int poisson_apply_laplacian_host(poisson_t ctx, const double* h_phi, double* h_o
 
 int poisson_rbsor_sweep_host(poisson_t ctx, double* h_phi, const double* h_rhs, double omega, int nsweeps,
                              double* h_resnorm) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     STAGE_OK(stage(ctx, 0, h_phi));
     STAGE_OK(stage(ctx, 1, h_rhs));
@@ -813,6 +872,7 @@ int poisson_rbsor_sweep_host(poisson_t ctx, double* h_phi, const double* h_rhs, 
 
 int poisson_cg_solve_host(poisson_t ctx, double* h_phi, const double* h_rhs, double rtol, int max_iter,
                           int fixed_iters, int* iters, double* relres) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     STAGE_OK(stage(ctx, 0, h_phi));
     STAGE_OK(stage(ctx, 1, h_rhs));
@@ -824,6 +884,7 @@ int poisson_cg_solve_host(poisson_t ctx, double* h_phi, const double* h_rhs, dou
 
 int poisson_bicgstab_solve_host(poisson_t ctx, double* h_phi, const double* h_rhs, double rtol, int max_iter,
                                 int fixed_iters, int* iters, double* relres) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     STAGE_OK(stage(ctx, 0, h_phi));
     STAGE_OK(stage(ctx, 1, h_rhs));
@@ -836,6 +897,7 @@ int poisson_bicgstab_solve_host(poisson_t ctx, double* h_phi, const double* h_rh
 
 int poisson_mg_vcycle_host(poisson_t ctx, double* h_phi, const double* h_rhs, int nu1, int nu2, int coarsest_n,
                            int coarsest_sweeps, int precision, int ncycles, double* h_resnorms) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     STAGE_OK(stage(ctx, 0, h_phi));
     STAGE_OK(stage(ctx, 1, h_rhs));
@@ -846,6 +908,7 @@ int poisson_mg_vcycle_host(poisson_t ctx, double* h_phi, const double* h_rhs, in
 }
 
 int poisson_multipole_bc_host(poisson_t ctx, const double* h_rho, double G, int lmax, double* h_moments) {
+    const DeviceGuard on_device(ctx);
     if (!ctx || !h_rho) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     STAGE_OK(stage(ctx, 1, h_rho));
     const int rc = poisson_multipole_bc(ctx, ctx->d_stage[1], G, lmax, h_moments);

@@ -6,6 +6,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "../../include/poisson.h"
@@ -132,6 +133,12 @@ struct poisson_ctx {
     std::vector<int> ev_kid;                    // kernel class of pair i
     size_t ev_used = 0;
     int num_sms = 148;
+    int device = 0;                  // the device the handle was created on; every entry point runs on it
+    // kernels whose dynamic shared-memory limit has been raised on this handle's device -> resident CTAs per SM
+    std::unordered_map<const void*, int> kern_resident;
+    // tuning overrides (poisson_set_option): -1 = automatic
+    int opt_tile_cfg = -1, opt_plane_split = -1, opt_apply_bulk = -1;
+    int last_restarts = 0, last_confirm_failed = 0;  // of the last BiCGSTAB solve (poisson_bicgstab_stats)
     std::string err;
     // pinned staging for the host-buffer entry points
     double* d_stage[2] = {nullptr, nullptr};
@@ -144,6 +151,35 @@ int fail_cuda(poisson_ctx* ctx, cudaError_t e, const char* what, const char* fil
 double* scratch(poisson_ctx* ctx, int slot);  // lazily allocated npts-sized vector; nullptr on OOM
 void pre_launch(poisson_ctx* ctx, int kid);
 void post_launch(poisson_ctx* ctx, int kid);
+
+// Raise the kernel's dynamic shared-memory limit (a per-device attribute) once per handle and report how many CTAs of
+// it fit on an SM.  Handles are bound to one device and are not thread-safe, so the cache lives in the handle.
+template <class K>
+inline int kernel_ready(poisson_ctx* ctx, K kern, int nthreads, size_t smem, int* resident = nullptr) {
+    const void* key = reinterpret_cast<const void*>(kern);
+    auto it = ctx->kern_resident.find(key);
+    if (it == ctx->kern_resident.end()) {
+        PB_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int r = 0;
+        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&r, kern, nthreads, smem));
+        it = ctx->kern_resident.emplace(key, r).first;
+    }
+    if (resident) *resident = it->second;
+    return POISSON_OK;
+}
+
+// Entry points run on the handle's device whatever the caller's current device is.
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const poisson_ctx* ctx) {
+        if (!ctx) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) switched = cudaSetDevice(ctx->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 // Every kernel launch of the library goes through this: counts it and, when asked, brackets it with CUDA events.
 #define PB_LAUNCH(ctx, kid, ...)       \

@@ -203,27 +203,15 @@ static int apply7_launch(poisson_ctx* ctx, const Op& op, const T* v, const T* rh
     const int grid = (int)((total + g.items - 1) / g.items);
     if (grid > kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");
     const size_t smem = (size_t)Cfg::NS * Cfg::SLOT * sizeof(T);
-    static bool attr_set = false;
-    if (!attr_set) {
-        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7<T, Cfg, MODE, RED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7<T, Cfg, MODE, RED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    int rc = kernel_ready(ctx, k_apply7<T, Cfg, MODE, RED, true>, Cfg::NT, smem);
+    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_apply7<T, Cfg, MODE, RED, false>, Cfg::NT, smem);
+    if (rc != POISSON_OK) return rc;
     if (plain)
         PB_LAUNCH(ctx, KID_APPLY, (k_apply7<T, Cfg, MODE, RED, true><<<grid, Cfg::NT, smem, ctx->stream>>>(op, v, rhs, out, out32, ug, g, ctx->red, ctx->d_scal)));
     else
         PB_LAUNCH(ctx, KID_APPLY, (k_apply7<T, Cfg, MODE, RED, false><<<grid, Cfg::NT, smem, ctx->stream>>>(op, v, rhs, out, out32, ug, g, ctx->red, ctx->d_scal)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
-}
-
-static int a7_cfg_override() {
-    static int v = -2;
-    if (v == -2) {
-        const char* e = getenv("POISSON_A7_CFG");
-        v = e ? atoi(e) : -1;
-    }
-    return v;
 }
 
 template <typename T, int MODE, bool RED>
@@ -233,7 +221,7 @@ static int apply7_cfg(poisson_ctx* ctx, const Op& op, const T* v, const T* rhs, 
     using CA = A7Tile<34, 18, 1, 3>;  // 64 x 16 valid, 612 threads, one CTA per SM
     using CC = A7Tile<18, 14, 4>;     // 32 x 12 valid, 252 threads (small grids)
     int c = (size_t)op.n[0] * op.n[1] * op.n[2] >= ((size_t)1 << 21) ? 0 : 2;
-    const int ov = a7_cfg_override();
+    const int ov = ctx->opt_tile_cfg;
     if (ov >= 0 && ov < 3) c = ov;
     switch (c) {
         case 0: return apply7_launch<T, CE, MODE, RED>(ctx, op, v, rhs, out, out32, ug, 2);

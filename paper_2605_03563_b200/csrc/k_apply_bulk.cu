@@ -188,8 +188,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB)
 
 // ---- host side ----------------------------------------------------------------------------------------------------------
 bool apply_bulk_ok(const poisson_ctx* ctx, const Op& op) {
-    static const char* e = getenv("POISSON_APPLY_BULK");  // 0 = never, 1 = whenever eligible; default: large grids
-    const int mode = e ? atoi(e) : -1;
+    const int mode = ctx->opt_apply_bulk;  // POISSON_OPT_APPLY_BULK: 0 = never, 1 = whenever eligible; -1: large grids
     if (mode == 0 || ctx->opt_path == 1) return false;
     if (op.coord != POISSON_CARTESIAN || op.order != 2 || op.n[0] % 2 != 0) return false;
     for (int f = 0; f < 6; ++f)
@@ -207,18 +206,16 @@ static int bulk_launch(poisson_ctx* ctx, const Op& op, const double* v, const do
     g.ntx = (op.n[0] + C::TX - 1) / C::TX;
     g.nty = (op.n[1] + C::TY - 1) / C::TY;
     const long total = (long)g.ntx * g.nty * op.n[2];
-    static int resident = 0;
+    int resident = 0;
     CUtensorMap map, fmap;
     if (!tma::make_map3(v, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, op.n, C::SW, C::SH, &map)) return POISSON_UNSUPPORTED;  // the caller falls back to k_apply7
     fmap = map;
     if (MODE != 0 && !tma::make_map3(rhs, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 8, op.n, C::TX, C::TY, &fmap)) return POISSON_UNSUPPORTED;
     constexpr size_t SMEM = C::smem(MODE != 0);
-    if (!resident) {
-        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-        PB_CUDA_OK(cudaFuncSetAttribute(k_apply7_bulk<C, MODE, RED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, k_apply7_bulk<C, MODE, RED, true>, C::NT, SMEM));
-        if (resident < 1) resident = 1;
-    }
+    int rc = kernel_ready(ctx, k_apply7_bulk<C, MODE, RED, false>, C::NT, SMEM);
+    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_apply7_bulk<C, MODE, RED, true>, C::NT, SMEM, &resident);
+    if (rc != POISSON_OK) return rc;
+    if (resident < 1) resident = 1;
     g.items = std::max(4L, (total + (long)ctx->num_sms * resident - 1) / ((long)ctx->num_sms * resident));
     const int grid = (int)((total + g.items - 1) / g.items);
     if (grid > kMaxRedBlocks) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");

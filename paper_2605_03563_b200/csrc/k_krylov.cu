@@ -8,6 +8,8 @@
 //             pass 3: x += alpha D^-1 p + omega D^-1 s ; r = s - omega t ; sum r.r, r0^.r     -> beta, convergence
 // Vectors whose stencil is taken in the pass that forms them (p, v, s) are recomputed in the halo from read-only
 // inputs and written to a different buffer (ping-pong), so no block reads what another block is writing.
+#include <algorithm>
+
 #include "stencil.cuh"
 
 namespace pb {
@@ -20,8 +22,14 @@ static inline int pick_kc(const Op& op, int sms) {
     while (kc > 8 && cols * ((op.n[2] + kc - 1) / kc) < 8L * sms) kc = (kc + 1) / 2;
     return kc;
 }
-static dim3 grid_for(const Op& op, int kc) {
-    return dim3((op.n[0] + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + kc - 1) / kc);
+// The reduction buffer holds one set of partials per block: lengthen the z chunks until the grid fits, or refuse.
+static int fit_grid(poisson_ctx* ctx, const Op& op, int nx_eff, int* kc, dim3* g) {
+    for (;;) {
+        *g = dim3((nx_eff + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + *kc - 1) / *kc);
+        if ((size_t)g->x * g->y * g->z <= (size_t)kMaxRedBlocks) return POISSON_OK;
+        if (*kc >= op.n[2]) return fail(ctx, POISSON_UNSUPPORTED, "grid too large for the reduction buffer");
+        *kc = std::min(op.n[2], *kc * 2);
+    }
 }
 
 __device__ __forceinline__ void finish_iteration(KrylovCtl* c, double* hist, double rr_new) {
@@ -362,8 +370,11 @@ static int stream_blocks(poisson_ctx* ctx, size_t n) {
 int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, double* r, bool bicg, double* r0hat) {
     const Op& op = ctx->op;
     if (plane_ok(ctx, op)) return plane_krylov_init(ctx, x, rhs, r, bicg ? r0hat : nullptr);
-    const int kc = pick_kc(op, ctx->num_sms);
-    const dim3 g = grid_for(op, kc), b(BX, BY);
+    int kc = pick_kc(op, ctx->num_sms);
+    dim3 g;
+    const dim3 b(BX, BY);
+    const int rcg = fit_grid(ctx, op, op.n[0], &kc, &g);
+    if (rcg != POISSON_OK) return rcg;
     pre_launch(ctx, KID_KRYLOV_INIT);
     KIND_SWITCH(ctx->kind, (k_krylov_init<K><<<g, b, 0, ctx->stream>>>(op, x, rhs, r, bicg ? r0hat : nullptr, ctx->d_ctl,
                                                                          ctx->d_hist, kc, ctx->red)));
@@ -375,8 +386,11 @@ int launch_krylov_init(poisson_ctx* ctx, const double* x, const double* rhs, dou
 int launch_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, double* p_new, double* q, double* x) {
     const Op& op = ctx->op;
     if (plane_ok(ctx, op)) return plane_cg_passA(ctx, r, p_old, p_new, q, x);
-    const int kc = pick_kc(op, ctx->num_sms);
-    const dim3 g = grid_for(op, kc), b(BX, BY);
+    int kc = pick_kc(op, ctx->num_sms);
+    dim3 g;
+    const dim3 b(BX, BY);
+    const int rcg = fit_grid(ctx, op, op.n[0], &kc, &g);
+    if (rcg != POISSON_OK) return rcg;
     pre_launch(ctx, KID_CG_PASS_A);
     KIND_SWITCH(ctx->kind,
                 (k_cg_passA<K><<<g, b, 0, ctx->stream>>>(op, r, p_old, p_new, q, x, ctx->d_ctl, kc, ctx->red)));
@@ -410,8 +424,11 @@ int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, co
                       double* p_new, double* v_new) {
     const Op& op = ctx->op;
     if (plane_ok(ctx, op)) return plane_bicg_pass1(ctx, r, p_old, v_old, r0, p_new, v_new);
-    const int kc = pick_kc(op, ctx->num_sms);
-    const dim3 g = grid_for(op, kc), b(BX, BY);
+    int kc = pick_kc(op, ctx->num_sms);
+    dim3 g;
+    const dim3 b(BX, BY);
+    const int rcg = fit_grid(ctx, op, op.n[0], &kc, &g);
+    if (rcg != POISSON_OK) return rcg;
     pre_launch(ctx, KID_BICG_PASS1);
     KIND_SWITCH(ctx->kind, (k_bicg_pass1<K><<<g, b, 0, ctx->stream>>>(op, r, p_old, v_old, r0, p_new, v_new, ctx->d_ctl,
                                                                         ctx->opt_jacobi, kc, ctx->red)));
@@ -422,8 +439,11 @@ int launch_bicg_pass1(poisson_ctx* ctx, const double* r, const double* p_old, co
 int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double* s, double* t) {
     const Op& op = ctx->op;
     if (plane_ok(ctx, op)) return plane_bicg_pass2(ctx, r, v, s, t);
-    const int kc = pick_kc(op, ctx->num_sms);
-    const dim3 g = grid_for(op, kc), b(BX, BY);
+    int kc = pick_kc(op, ctx->num_sms);
+    dim3 g;
+    const dim3 b(BX, BY);
+    const int rcg = fit_grid(ctx, op, op.n[0], &kc, &g);
+    if (rcg != POISSON_OK) return rcg;
     pre_launch(ctx, KID_BICG_PASS2);
     KIND_SWITCH(ctx->kind, (k_bicg_pass2<K><<<g, b, 0, ctx->stream>>>(op, r, v, s, t, ctx->d_ctl, ctx->opt_jacobi, kc,
                                                                         ctx->red)));
@@ -434,14 +454,17 @@ int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double
 int launch_bicg_pass3(poisson_ctx* ctx, double* x, const double* p, const double* s, const double* t,
                       const double* r0, double* r) {
     const Op& op = ctx->op;
-    const int kc = pick_kc(op, ctx->num_sms);
+    int kc = pick_kc(op, ctx->num_sms);
+    const bool pair = op.n[0] % 2 == 0 && ctx->opt_path != 1;
+    dim3 g;
+    const dim3 b(BX, BY);
+    const int rcg = fit_grid(ctx, op, pair ? op.n[0] / 2 : op.n[0], &kc, &g);
+    if (rcg != POISSON_OK) return rcg;
     pre_launch(ctx, KID_BICG_PASS3);
-    if (op.n[0] % 2 == 0 && ctx->opt_path != 1) {
-        const dim3 g((op.n[0] / 2 + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + kc - 1) / kc), b(BX, BY);
+    if (pair) {
         KIND_SWITCH(ctx->kind, (k_bicg_pass3_pair<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl,
                                                                                  ctx->d_hist, ctx->opt_jacobi, kc, ctx->red)));
     } else {
-        const dim3 g = grid_for(op, kc), b(BX, BY);
         KIND_SWITCH(ctx->kind, (k_bicg_pass3<K><<<g, b, 0, ctx->stream>>>(op, x, p, s, t, r0, r, ctx->d_ctl, ctx->d_hist,
                                                                             ctx->opt_jacobi, kc, ctx->red)));
     }

@@ -356,11 +356,8 @@ static int bottom_t(poisson_ctx* ctx, const Op* ops, int nlev, T* phi, const T* 
     a.csweeps = csweeps;
     a.restriction = ctx->opt_restriction;
     a.omega_c = omega_c;
-    static bool attr_set = false;
-    if (!attr_set) {
-        PB_CUDA_OK(cudaFuncSetAttribute(k_mg_bottom<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    const int rc = kernel_ready(ctx, k_mg_bottom<T>, 1024, 200 * 1024);
+    if (rc != POISSON_OK) return rc;
     PB_LAUNCH(ctx, KID_MG_COARSE, (k_mg_bottom<T><<<1, 1024, bytes, ctx->stream>>>(a, phi, rhs)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;

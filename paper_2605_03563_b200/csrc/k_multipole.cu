@@ -12,12 +12,11 @@
 
 namespace pb {
 
-__constant__ double c_norm[(kMaxLmax + 1) * (kMaxLmax + 1)];  // N_lm at index l*l + l + m (m >= 0); 1 for m = 0
-static bool g_norm_ready = false;
+constexpr int kNQ = (kMaxLmax + 1) * (kMaxLmax + 1);
 
-static void init_norm() {
-    if (g_norm_ready) return;
-    double h[(kMaxLmax + 1) * (kMaxLmax + 1)] = {0};
+// N_lm at index l*l + l + m (both signs of m); 1 for m = 0.  Travels in the kernel parameters (constant bank), so
+// there is no per-process or per-device state.
+static void fill_norm(double* h) {
     for (int l = 0; l <= kMaxLmax; ++l) {
         h[l * l + l] = 1.0;
         for (int m = 1; m <= l; ++m) {
@@ -27,11 +26,10 @@ static void init_norm() {
             h[l * l + l - m] = h[l * l + l + m];
         }
     }
-    cudaMemcpyToSymbol(c_norm, h, sizeof(h));
-    g_norm_ready = true;
 }
 
 struct MpGeom {
+    double norm[kNQ];
     int sph;
     int n[3];
     double origin[3], h[3];
@@ -117,7 +115,7 @@ __global__ void __launch_bounds__(256, 1)
         accumulate<L>(acc, x, y, z, w);
     }
 #pragma unroll
-    for (int s = 0; s < NQ; ++s) acc[s] *= c_norm[s];  // N_lm, once per thread instead of once per point
+    for (int s = 0; s < NQ; ++s) acc[s] *= g.norm[s];  // N_lm, once per thread instead of once per point
     // block reduction: warp shuffles, then shared memory across the 8 warps
     __shared__ double sm[8][NQ];
     __shared__ int is_last;
@@ -149,8 +147,8 @@ __global__ void __launch_bounds__(256, 1)
 }
 
 // Phi at one exterior point from the moments.
-__device__ __forceinline__ double expansion(const double* __restrict__ q, int lmax, double G, double x, double y,
-                                            double z) {
+__device__ __forceinline__ double expansion(const double* __restrict__ norm, const double* __restrict__ q, int lmax,
+                                            double G, double x, double y, double z) {
     const double r2 = fma(z, z, fma(y, y, x * x));
     const double rinv = 1.0 / sqrt(r2), rinv2 = rinv * rinv;
     double A = 1.0, B = 0.0, dfact = 1.0, acc = 0.0;
@@ -168,7 +166,7 @@ __device__ __forceinline__ double expansion(const double* __restrict__ q, int lm
             if (m == 0)
                 acc = fma(q[l * l + l] * ql, pw, acc);
             else {
-                const double nq = c_norm[l * l + l + m] * ql;
+                const double nq = norm[l * l + l + m] * ql;
                 acc = fma((q[l * l + l + m] * A + q[l * l + l - m] * B) * nq, pw, acc);
             }
             qm2 = qm1;
@@ -206,11 +204,12 @@ __global__ void __launch_bounds__(256)
         y = fma((double)id[1], g.h[1], g.origin[1]);
         z = fma((double)id[2], g.h[2], g.origin[2]);
     }
-    out[t] = expansion(q, lmax, G, x, y, z);
+    out[t] = expansion(g.norm, q, lmax, G, x, y, z);
 }
 
 static MpGeom make_geom(poisson_ctx* ctx) {
     MpGeom g{};
+    fill_norm(g.norm);
     g.sph = ctx->op.coord == POISSON_SPHERICAL;
     for (int a = 0; a < 3; ++a) {
         g.n[a] = ctx->op.n[a];
@@ -240,7 +239,6 @@ static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho,
 
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
-    init_norm();
     const MpGeom g = make_geom(ctx);
     int blocks = ctx->num_sms * 2;
     const size_t maxb = (ctx->npts + 255) / 256;
@@ -264,7 +262,6 @@ int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
 }
 
 int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, double G, int lmax) {
-    init_norm();
     const MpGeom g = make_geom(ctx);
     for (int f = 0; f < 6; ++f) {
         if (ctx->op.bc[f] != POISSON_BC_DIRICHLET_GHOST || !ctx->d_ghost[f]) continue;

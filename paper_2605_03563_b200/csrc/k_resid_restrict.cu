@@ -234,12 +234,9 @@ static int rr_launch(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T
     g.items = std::max(2L, (total + ctx->num_sms - 1) / ctx->num_sms);
     const int grid = (int)((total + g.items - 1) / g.items);
     const size_t smem = (size_t)7 * Cfg::SLOT * sizeof(T);
-    static bool attr_set = false;
-    if (!attr_set) {
-        PB_CUDA_OK(cudaFuncSetAttribute(k_resid_restrict<T, Cfg, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        PB_CUDA_OK(cudaFuncSetAttribute(k_resid_restrict<T, Cfg, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    int rc = kernel_ready(ctx, k_resid_restrict<T, Cfg, true>, Cfg::NT, smem);
+    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_resid_restrict<T, Cfg, false>, Cfg::NT, smem);
+    if (rc != POISSON_OK) return rc;
     if (plain)
         PB_LAUNCH(ctx, KID_MG_RESTRICT, (k_resid_restrict<T, Cfg, true><<<grid, Cfg::NT, smem, ctx->stream>>>(fine, coarse, phi, rhs, fc, ug, ctx->opt_restriction, g)));
     else

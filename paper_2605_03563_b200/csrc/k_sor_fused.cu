@@ -371,12 +371,9 @@ static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, c
     bool plain = op.gamma == 0.0;
     for (int f = 0; f < 6; ++f) plain = plain && op.bc[f] != POISSON_BC_NEUMANN0;
     const size_t smem = (size_t)Cfg::D * Cfg::SLOT * sizeof(T);
-    static bool attr_set = false;
-    if (!attr_set) {
-        PB_CUDA_OK(cudaFuncSetAttribute(k_sor_fused<T, Cfg, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        PB_CUDA_OK(cudaFuncSetAttribute(k_sor_fused<T, Cfg, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    int rc = kernel_ready(ctx, k_sor_fused<T, Cfg, true>, Cfg::NT, smem);
+    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_sor_fused<T, Cfg, false>, Cfg::NT, smem);
+    if (rc != POISSON_OK) return rc;
     if (plain)
         PB_LAUNCH(ctx, KID_RBSOR, (k_sor_fused<T, Cfg, true><<<grid, Cfg::NT, smem, ctx->stream>>>(op, in, out, rhs, omega, ug, g)));
     else
@@ -384,16 +381,7 @@ static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, c
     return POISSON_OK;
 }
 
-static int sor_cfg_override() {
-    static int v = -2;
-    if (v == -2) {
-        const char* e = getenv("POISSON_SOR_CFG");
-        v = e ? atoi(e) : -1;
-    }
-    return v;
-}
-
-// Tile choice: the compiled configuration with the smallest estimated pass time (POISSON_SOR_CFG=<n> overrides).
+// Tile choice: the compiled configuration with the smallest estimated pass time (POISSON_OPT_TILE_CFG overrides).
 template <typename T, int NHS>
 static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, T omega, bool ug) {
     using C0 = SorTile<NHS, 32 + NHS, 14 + 2 * NHS>;   // 64 x 14 valid, 612 threads at NHS = 2 (best at 256^3 on B200)
@@ -407,7 +395,7 @@ static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, c
     int best = 0;
     for (int c = 1; c < 4; ++c)
         if (cost[c] < cost[best]) best = c;
-    const int ov = sor_cfg_override();
+    const int ov = ctx->opt_tile_cfg;
     if (ov >= 0 && ov < 4) best = ov;
     switch (best) {
         case 0: return sor_launch_cfg<T, C0>(ctx, op, in, out, rhs, omega, ug, g[0], grid[0]);

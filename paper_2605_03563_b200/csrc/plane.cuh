@@ -512,13 +512,12 @@ struct PlanePlan {
 // neighbouring tiles drift apart in z and their halos come from HBM again: measured +22 % DRAM traffic on the 512^3
 // 19-point CG pass).  The linear split therefore carries a penalty and wins only when chunks leave SMs idle.
 template <class G>
-static PlanePlan plane_plan(const Op& op, long slots) {
+static PlanePlan plane_plan(const Op& op, long slots, int force_split /* POISSON_OPT_PLANE_SPLIT: 1 always, 0 never, -1 auto */) {
     PlanePlan pl;
     pl.ntx = (op.n[0] + G::TX - 1) / G::TX;
     const int nty = (op.n[1] + G::TY - 1) / G::TY;
     const long total = (long)pl.ntx * nty * op.n[2];
-    static const char* force_split = getenv("POISSON_PLANE_SPLIT");  // tuning aid: 1 = always split, 0 = never
-    const double halo_pen = force_split ? (atoi(force_split) ? 1e-3 : 1e3) : 1.0 + 0.15 * G::R;
+    const double halo_pen = force_split >= 0 ? (force_split ? 1e-3 : 1e3) : 1.0 + 0.15 * G::R;
     pl.items = std::max(4L, (total + slots - 1) / slots);
     pl.nctas = (total + pl.items - 1) / pl.items;
     pl.per_tile = 0;
@@ -543,12 +542,10 @@ template <int KIND, class Cfg, class Ld, class Ep>
 static int plane_resident(poisson_ctx* ctx, int* out) {
     using G = PlaneGeom<KIND, Cfg>;
     auto kern = k_plane<KIND, Cfg, Ld, Ep>;
-    static int resident = 0;
-    if (!resident) {
-        PB_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-        PB_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, G::NT, G::SMEM));
-        if (resident < 1) return fail(ctx, POISSON_CUDA_ERROR, "plane kernel does not fit on an SM");
-    }
+    int resident = 0;
+    const int rc = kernel_ready(ctx, kern, G::NT, G::SMEM, &resident);
+    if (rc != POISSON_OK) return rc;
+    if (resident < 1) return fail(ctx, POISSON_CUDA_ERROR, "plane kernel does not fit on an SM");
     *out = resident;
     return POISSON_OK;
 }
@@ -573,7 +570,7 @@ template <int KIND, class Ld, class Ep>
 static int launch_plane(poisson_ctx* ctx, const Op& op, const Ld& ld, const Ep& ep, bool ug, int kid) {
     int ra = 0, rc;
     if ((rc = plane_resident<KIND, CfgA, Ld, Ep>(ctx, &ra)) != POISSON_OK) return rc;
-    const PlanePlan pa = plane_plan<PlaneGeom<KIND, CfgA>>(op, (long)ctx->num_sms * ra);
+    const PlanePlan pa = plane_plan<PlaneGeom<KIND, CfgA>>(op, (long)ctx->num_sms * ra, ctx->opt_plane_split);
     return plane_run<KIND, CfgA, Ld, Ep>(ctx, op, ld, ep, ug, kid, pa);
 }
 

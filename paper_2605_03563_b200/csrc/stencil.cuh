@@ -232,9 +232,12 @@ __device__ __forceinline__ void krylov_init_finish(KrylovCtl* ctl, double* hist,
     ctl->alpha = 0.0;
     ctl->omega = 0.0;
     ctl->it = 0;
-    const int trivially_done = (!ctl->fixed && !(rr > 0.0)) ? 1 : 0;
-    ctl->done = trivially_done;
-    ctl->status = (ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED;
+    // a zero initial residual is convergence; a non-finite one (NaN/Inf in rhs or in the initial guess) is BREAKDOWN in
+    // both modes — `!(rr > 0)` would call NaN converged
+    const bool fin = isfinite(rr);
+    const int trivially_done = (!ctl->fixed && rr == 0.0) ? 1 : 0;
+    ctl->done = (trivially_done || !fin) ? 1 : 0;
+    ctl->status = !fin ? POISSON_BREAKDOWN : ((ctl->fixed || trivially_done) ? POISSON_OK : POISSON_NOT_CONVERGED);
     if (ctl->record && hist) hist[0] = 1.0;
 }
 

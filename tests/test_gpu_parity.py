@@ -95,18 +95,30 @@ def test_rbsor_with_ghosts_and_odd_shapes(path, shape):
         o.rbsor(phi_c, rhs, 1.3, nsw)
         g.rbsor_sweep(d_phi, d_rhs, 1.3, nsw)
         assert pointwise_scaled(host(d_phi), phi_c, stencil_scale(phi_c, rhs * 0.003)) <= 1e-13
+    before = host(d_phi).copy()
     g.rbsor_sweep(d_phi, d_rhs, 1.3, 0)  # zero sweeps: a no-op
-    assert np.array_equal(host(d_phi), host(d_phi))
+    assert np.array_equal(host(d_phi), before)
 
 
 # ---- (a6) multipole boundary ----------------------------------------------------------------------------------------
+def _assert_moments_per_l(q_g, q_c, lmax):
+    """|dq_lm| <= 1e-12 max_m |q_lm| for every l separately (the high moments are ~1e-9 of q_00 on config 2), with an
+    absolute floor at the rounding level of the sum itself: 1e-12 * sum |rho| r^l dV would be the sharp one; the
+    monopole-scaled 1e-16 r_max^l is a bound for it on these grids."""
+    q_g, q_c = np.asarray(q_g), np.asarray(q_c)
+    for l in range(lmax + 1):
+        sl = slice(l * l, (l + 1) * (l + 1))
+        scale = np.abs(q_c[sl]).max()
+        assert np.abs(q_g[sl] - q_c[sl]).max() <= 1e-12 * scale + 1e-16 * abs(q_c[0]), "l = %d" % l
+
+
 @pytest.mark.parametrize("lmax", [0, 2, 4, 8])
 def test_multipole_cartesian(lmax):
     w = wl.config2(32)
     o, g = make_pair(w)
     q_c = o.multipole_bc(w["rho"], 1.0, lmax)
     q_g = np.array(g.multipole_bc(dev(w["rho"]), 1.0, lmax))
-    assert np.abs(q_g - q_c).max() <= 1e-12 * np.abs(q_c).max()
+    _assert_moments_per_l(q_g, q_c, lmax)
     for f in range(6):
         buf = torch.empty(g.face_len(f), device="cuda", dtype=torch.float64)
         g.get_ghost_face(f, buf)
@@ -119,7 +131,7 @@ def test_multipole_spherical():
     o, g = make_pair(w)
     q_c = o.multipole_bc(w["rho"], 1.0, 8)
     q_g = np.array(g.multipole_bc(dev(w["rho"]), 1.0, 8))
-    assert np.abs(q_g - q_c).max() <= 1e-12 * np.abs(q_c).max()
+    _assert_moments_per_l(q_g, q_c, 8)
     buf = torch.empty(g.face_len(1), device="cuda", dtype=torch.float64)
     g.get_ghost_face(1, buf)
     want = o.get_ghost_face(1)
@@ -186,6 +198,15 @@ def _oracle_rounding_sensitivity(w, o, fixed, solver="cg"):
     return rel_l2(x2, x1), float(np.max(np.abs(h2 - h1) / h1))
 
 
+SENS_CAP = 1e-6   # a sensitivity-based tolerance never widens beyond this (north_star's 1e-10 is the floor)
+
+
+def _sens_tol(floor, sens, what):
+    tol = min(max(floor, 10 * sens), SENS_CAP)
+    print("%s: oracle 1-ulp sensitivity %.2e -> tolerance %.2e" % (what, sens, tol))
+    return tol
+
+
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("n", [32, 64])
 def test_config4_periodic_cg6(path, n):
@@ -195,12 +216,14 @@ def test_config4_periodic_cg6(path, n):
     phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, fixed_iters=5)
     assert rel_l2(phi_g, phi_c) <= 1e-10
     assert abs(phi_g.mean()) <= 1e-13 * np.abs(phi_g).max()
-    # 25 iterations: within the oracle's own sensitivity to a 1-ulp perturbation of the input
-    phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, fixed_iters=25)
-    sens_x, sens_hist = _oracle_rounding_sensitivity(w, o, 25)
-    assert rel_l2(phi_g, phi_c) <= max(1e-10, 10 * sens_x)
-    hist = np.array(g.get_history(26))
-    assert np.allclose(hist, res_c["history"], rtol=max(1e-8, 10 * sens_hist))
+    # 10 iterations: within the oracle's own sensitivity to a 1-ulp perturbation of the input, capped at 1e-6 (the
+    # band-limited right-hand side lets the CG polynomial grow on the unexcited high modes: at 25 iterations that
+    # sensitivity is already 1e-3, which would test nothing — the white-noise test below covers 25 iterations at 1e-10)
+    phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, fixed_iters=10)
+    sens_x, sens_hist = _oracle_rounding_sensitivity(w, o, 10)
+    assert rel_l2(phi_g, phi_c) <= _sens_tol(1e-10, sens_x, "config 4 n=%d x after 10 its" % n)
+    hist = np.array(g.get_history(11))
+    assert np.allclose(hist, res_c["history"], rtol=_sens_tol(1e-8, sens_hist, "config 4 n=%d history" % n))
     assert np.allclose(hist[:6], res_c["history"][:6], rtol=1e-9)
     phi_c, phi_g, res_c, res_g = _cg_both(w, o, g, rtol=1e-10, max_iter=3000)
     assert res_g["status"] == pb.OK and abs(res_g["iters"] - res_c["iters"]) <= 2
@@ -253,8 +276,9 @@ def test_config5_bicgstab(path):
         # north_star's 1e-10 while rounding differences are not yet amplified; beyond that the oracle's own
         # sensitivity to a 1-ulp perturbation of its input bounds what any correct implementation can match
         sens_x, sens_h = (0.0, 0.0) if fixed == 3 else _oracle_rounding_sensitivity(w, o, fixed, "bicgstab")
-        assert rel_l2(host(d_phi), phi_c) <= max(1e-10, 10 * sens_x)
-        assert np.allclose(g.get_history(fixed + 1), res_c["history"], rtol=max(1e-7, 10 * sens_h))
+        assert rel_l2(host(d_phi), phi_c) <= _sens_tol(1e-10, sens_x, "config 5 x after %d its" % fixed)
+        assert np.allclose(g.get_history(fixed + 1), res_c["history"],
+                           rtol=_sens_tol(1e-7, sens_h, "config 5 history after %d its" % fixed))
     phi_c = np.zeros_like(w["rhs"])
     d_phi = dev(phi_c)
     res_c = o.bicgstab(phi_c, w["rhs"], rtol=1e-8, max_iter=3000)
@@ -280,7 +304,7 @@ def test_bicgstab_on_cartesian_and_unscaled_variant():
             eps = np.finfo(np.float64).eps * np.abs(w["rhs"]).max()
             o.bicgstab(x2, w["rhs"] + eps * wl.random_field(w["shape"], 77), fixed_iters=fixed, jacobi=0)
             sens = rel_l2(x2, phi_c)
-        assert rel_l2(host(d_phi), phi_c) <= max(1e-10, 10 * sens)
+        assert rel_l2(host(d_phi), phi_c) <= _sens_tol(1e-10, sens, "unscaled BiCGSTAB x after %d its" % fixed)
 
 
 def test_bicgstab_true_residual_confirmation_and_attainable_accuracy():
@@ -307,14 +331,14 @@ def test_bicgstab_true_residual_confirmation_and_attainable_accuracy():
 
 
 @pytest.mark.parametrize("path", PATHS)
-def test_bicgstab_restart_branch_parity(path, monkeypatch):
+def test_bicgstab_restart_branch_parity(path):
     # the near-breakdown restart forced on both sides (threshold 0.1 instead of 1e-12): same restarts, same iterates
     w = wl.config5(32, 16, 32)
     o, g = make_pair(w, path)
     o.multipole_bc(w["rho"], w["G"], w["lmax"])
     g.multipole_bc(dev(w["rho"]), w["G"], w["lmax"], want_moments=False)
     g.set_option(pb.OPT_RECORD_HISTORY, 1)
-    monkeypatch.setenv("POISSON_BICG_RESTART_EPS", "0.1")
+    g.set_option_f64(pb.OPT_BICG_RESTART_EPS, 0.1)
     try:
         po.Oracle.set_bicgstab_restart_eps(0.1)
         for fixed in (6, 12):
@@ -323,7 +347,7 @@ def test_bicgstab_restart_branch_parity(path, monkeypatch):
             res_c = o.bicgstab(phi_c, w["rhs"], fixed_iters=fixed, want_history=True)
             restarts = po.Oracle.bicgstab_stats()[0]
             g.bicgstab_solve(d_phi, dev(w["rhs"]), fixed_iters=fixed)
-            assert restarts >= (1 if fixed == 6 else 3)
+            assert restarts >= (1 if fixed == 6 else 3) and g.bicgstab_stats()[0] == restarts
             assert rel_l2(host(d_phi), phi_c) <= 1e-9
             assert np.allclose(g.get_history(fixed + 1), res_c["history"], rtol=1e-6)
     finally:
@@ -381,3 +405,41 @@ def test_error_codes():
         g6.mg_vcycle(x, x.clone())
     assert e.value.code == pb.UNSUPPORTED
     assert g.kernel_launches() >= 0
+
+
+def test_spherical_edges_are_validated():
+    re, te, pe = wl.spherical_edges(8, 4, 8)
+    bc = (po.BC_NEUMANN0, po.BC_DIRICHLET_GHOST, po.BC_AXIS, po.BC_AXIS, po.BC_PERIODIC, po.BC_PERIODIC)
+    mk = lambda r, t, p, b=bc: pb.Poisson((8, 4, 8), edges=(r, t, p), coord=pb.SPHERICAL, bc=b)
+    mk(re, te, pe)
+    bad_r = re.copy(); bad_r[3] = bad_r[2]
+    for args, code in (((bad_r, te, pe), pb.INVALID_ARG),                              # not increasing
+                       ((re - re[0], te, pe), pb.INVALID_ARG),                         # r_in = 0
+                       ((re, te * 1.1, pe), pb.INVALID_ARG),                           # theta beyond pi
+                       ((re, te ** 1.2 / te[-1] ** 0.2, pe), pb.UNSUPPORTED),          # nonuniform theta
+                       ((re, te, pe ** 1.1 / pe[-1] ** 0.1), pb.UNSUPPORTED),          # nonuniform phi
+                       ((re, 0.1 + 0.9 * te, pe), pb.INVALID_ARG)):                    # axis face off the axis
+        with pytest.raises(pb.PoissonError) as e:
+            mk(*args)
+        assert e.value.code == code, str(e.value)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_non_finite_input_is_breakdown_not_convergence(path):
+    # include/poisson.h: BREAKDOWN on non-finite values; a NaN initial residual must never read as "converged"
+    w = wl.config2(32)
+    o, g = make_pair(w, path)
+    rhs = w["rhs"].copy()
+    rhs[3, 4, 5] = np.nan
+    for fixed in (0, 4):
+        phi_c = np.zeros_like(rhs)
+        res_c = o.cg(phi_c, rhs, rtol=1e-8, max_iter=20, fixed_iters=fixed)
+        res_g = g.cg_solve(dev(np.zeros_like(rhs)), dev(rhs), rtol=1e-8, max_iter=20, fixed_iters=fixed)
+        assert res_c["status"] == po_status_breakdown() and res_g["status"] == pb.BREAKDOWN and res_g["iters"] == 0
+        res_c = o.bicgstab(phi_c, rhs, rtol=1e-8, max_iter=20, fixed_iters=fixed)
+        res_g = g.bicgstab_solve(dev(np.zeros_like(rhs)), dev(rhs), rtol=1e-8, max_iter=20, fixed_iters=fixed)
+        assert res_c["status"] == po_status_breakdown() and res_g["status"] == pb.BREAKDOWN and res_g["iters"] == 0
+
+
+def po_status_breakdown():
+    return 2   # orc::ST_BREAKDOWN (oracle/solvers.hpp)
