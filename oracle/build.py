@@ -7,7 +7,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["apply.cpp", "rbsor.cpp", "krylov.cpp", "vcycle.cpp", "multipole.cpp", "capi.cpp"]
+SOURCES = ["apply.cpp", "rbsor.cpp", "krylov.cpp", "vcycle.cpp", "mgv.cpp", "multipole.cpp", "capi.cpp"]
 HEADERS = ["grid.hpp", "solvers.hpp"]
 LIB = os.path.join(HERE, "liboracle.so")
 

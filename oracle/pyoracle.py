@@ -14,6 +14,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CARTESIAN, SPHERICAL = 0, 1
 BC_DIRICHLET_GHOST, BC_PERIODIC, BC_NEUMANN0, BC_AXIS = 0, 1, 2, 3
 
+# PAPER.md:176-182 Table 1, row "Order 2": omega, alpha, beta, gamma, delta of the SPAI smoother (Eq. 15-16)
+SPAI_ORDER2 = (1.3699, 0.1432, 0.0284, 0.0081, 0.0025)
+
 _lib = None
 
 
@@ -193,6 +196,41 @@ class Oracle:
         assert phi.dtype == np.float64 and phi.flags.c_contiguous
         ec = _f64(ec)
         lib().orc_prolong_add(self.h, _p(ec), _p(phi), C.c_double(coarse_gamma))
+
+    # ---- the paper's own multigrid (oracle/mgv.cpp) ----
+    def spai_smooth(self, phi, rhs, spai=SPAI_ORDER2, nsteps=1):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs, sp = _f64(rhs), _f64(np.array(spai))
+        lib().orc_spai_smooth(self.h, _p(phi), _p(rhs), _p(sp), int(nsteps))
+
+    def mgv_vcycle(self, phi, rhs, nu1=1, nu2=1, coarsest_n=3, spai=SPAI_ORDER2, cg_rtol=1e-3, storage_f32=False,
+                   ncycles=1):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs, sp = _f64(rhs), _f64(np.array(spai))
+        rn = np.zeros(ncycles + 1)
+        fn = lib().orc_mgv_vcycle
+        fn.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_double, C.c_int,
+                       C.c_int, C.c_void_p]
+        st = fn(self.h, phi.ctypes.data, rhs.ctypes.data, int(nu1), int(nu2), int(coarsest_n), sp.ctypes.data,
+                float(cg_rtol), int(bool(storage_f32)), int(ncycles), rn.ctypes.data)
+        return dict(status=int(st), resnorms=rn)
+
+    def mgv_galerkin_stencil(self, level, I, J, K):
+        out = np.zeros(27)
+        rc = lib().orc_mgv_galerkin_stencil(self.h, int(level), int(I), int(J), int(K), _p(out))
+        assert rc == 0
+        return out.reshape(3, 3, 3)
+
+    def mgv_restrict(self, r):
+        r = _f64(r)
+        bc = np.zeros(tuple((s - 1) // 2 for s in self.npshape))
+        lib().orc_mgv_restrict(self.h, _p(r), _p(bc))
+        return bc
+
+    def mgv_prolong_add(self, ec, x):
+        assert x.dtype == np.float64 and x.flags.c_contiguous
+        ec = _f64(ec)
+        lib().orc_mgv_prolong_add(self.h, _p(ec), _p(x))
 
     def multipole_moments(self, rho, lmax):
         rho = _f64(rho)

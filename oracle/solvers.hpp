@@ -38,6 +38,15 @@ template <typename T>
 void prolong_add(const Grid& fine, const Grid& coarse, const T* ec, T* phi);
 Grid coarsen(const Grid& fine, int level_of_coarse);
 
+// ---- the paper's own multigrid (mgv.cpp): vertex-centred, Galerkin, SPAI smoother, CG coarsest; PAPER.md:125-205 -------
+// spai[5] = {omega, alpha, beta, gamma, delta} of Eq. 15-16 (Table 1).
+void spai_smooth(const Grid& g, double* phi, const double* rhs, const double spai[5], int nsteps);
+int mgv_vcycle(const Grid& g, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, const double spai[5],
+               double cg_rtol, int storage_f32, int ncycles, double* resnorms /* nullable, ncycles+1 */);
+int mgv_galerkin_stencil(const Grid& g, int level, int I, int J, int K, double* out27);
+void mgv_restrict(const Grid& g, const double* r, double* bc);
+void mgv_prolong_add(const Grid& g, const double* ec, double* x);
+
 // Multipole boundary condition, Eq. 19-20.  Fills g.ghost[] on Dirichlet faces.
 void multipole_moments(const Grid& g, const double* rho, int lmax, double* q /* (lmax+1)^2, index l*l+l+m */);
 double multipole_potential(const double* q, int lmax, double G, double x, double y, double z);
