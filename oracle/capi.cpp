@@ -94,6 +94,30 @@ int orc_bicgstab(void* h, double* phi, const double* rhs, double rtol, int max_i
                  int* iters, double* relres, double* history) {
     return bicgstab(*(Grid*)h, phi, rhs, rtol, max_iter, fixed_iters, jacobi, iters, relres, history);
 }
+int orc_pcg(void* h, double* phi, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
+            double* relres, double* history) {
+    return pcg(*(Grid*)h, phi, rhs, rtol, max_iter, fixed_iters, iters, relres, history);
+}
+void orc_gs_precond(void* h, const double* v, double* z, int sign, int symmetric) {
+    gs_precond(*(Grid*)h, v, z, sign, symmetric != 0);
+}
+double orc_jacobi_radius(void* h) { return jacobi_radius(*(Grid*)h); }
+double orc_local_jacobi_radius(void* h, int i, int j) { return local_jacobi_radius(*(Grid*)h, i, j); }
+void orc_rbsor_cheby(void* h, double* phi, const double* rhs, double rJ, int nsweeps, int start_n, double* omegas) {
+    rbsor_cheby(*(Grid*)h, phi, rhs, rJ, nsweeps, start_n, true, omegas);
+}
+void orc_rbsor_local(void* h, double* phi, const double* rhs, int nsweeps, int start_n) {
+    rbsor_local(*(Grid*)h, phi, rhs, nsweeps, start_n, true);
+}
+void orc_multipole_bc2(void* h, const double* rho, double G, int lmax, double* moments, double* inner_moments) {
+    multipole_bc(*(Grid*)h, rho, G, lmax, moments, inner_moments);
+}
+void orc_multipole_inner_moments(void* h, const double* rho, int lmax, double* qbar) {
+    multipole_inner_moments(*(Grid*)h, rho, lmax, qbar);
+}
+double orc_multipole_inner_potential(const double* qbar, int lmax, double G, double x, double y, double z) {
+    return multipole_inner_potential(qbar, lmax, G, x, y, z);
+}
 void orc_set_bicgstab_restart_eps(double eps) { set_bicgstab_restart_eps(eps); }
 void orc_bicgstab_stats(int* restarts, int* confirm_failed) { bicgstab_stats(restarts, confirm_failed); }
 int orc_vcycle(void* h, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, int coarsest_sweeps,

@@ -86,6 +86,79 @@ int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, i
     return status;
 }
 
+// ---- multi-colour Gauss-Seidel preconditioning (Eq. 9-10) -------------------------
+// Two colours for the radius-1 stencils.  With the unknowns ordered red then black the matrix is
+// [[D_R, N_RB], [N_BR, D_B]] (Eq. 9) and B = [[D_R, 0], [N_BR, D_B]] (Eq. 10); "the required systems can now be solved
+// directly block-wise in a number of steps equal to the number of colors": z_R = D_R^-1 v_R, z_B = D_B^-1 (v_B - N_BR z_R)
+// — which is one red-black Gauss-Seidel sweep on (matrix) z = v started from z = 0.  sign = +1: the matrix is L_h,
+// sign = -1: the matrix is A = -L_h (then L_h z = -v).  symmetric: a third half-sweep (red again) turns B^-1 into the
+// symmetric Gauss-Seidel preconditioner (red, black | black, red with the repeated black step being idempotent), which
+// is what a CG iteration needs (Saad §10.2); reading C15.
+void gs_precond(const Grid& g, const double* v, double* z, int sign, bool symmetric) {
+    const size_t n = g.size();
+    std::vector<double> f(n);
+#pragma omp parallel for schedule(static)
+    for (size_t m = 0; m < n; ++m) {
+        f[m] = sign > 0 ? v[m] : -v[m];
+        z[m] = 0.0;
+    }
+    rbsor_half(g, z, f.data(), 1.0, 0, false);
+    rbsor_half(g, z, f.data(), 1.0, 1, false);
+    if (symmetric) rbsor_half(g, z, f.data(), 1.0, 0, false);
+}
+
+// Preconditioned CG, Saad Alg. 9.1, on A = -L_h, b = -rhs, M^-1 = symmetric red-black Gauss-Seidel.  Convergence is
+// tested on the unpreconditioned residual ||r_k|| / ||r_0|| like cg() ("residual reduction").
+int pcg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
+        double* relres, double* history) {
+    const size_t n = g.size();
+    std::vector<double> r(n), z(n), p(n), q(n);
+    apply(g, x, q.data(), true);
+#pragma omp parallel for schedule(static)
+    for (size_t m = 0; m < n; ++m) r[m] = q[m] - rhs[m];  // b - A x = -rhs + L x
+    gs_precond(g, r.data(), z.data(), -1, true);
+    p = z;
+    double rz = dot(g, r.data(), z.data());
+    double rr = dot(g, r.data(), r.data());
+    const double rr0 = rr;
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    if (history) history[0] = 1.0;
+    int it = 0, status = (fixed_iters > 0) ? ST_OK : ST_NOT_CONVERGED;
+    if (!std::isfinite(rr0)) {
+        status = ST_BREAKDOWN;
+    } else if (fixed_iters <= 0 && rr0 == 0.0) {
+        status = ST_OK;
+    } else {
+        for (it = 0; it < nit;) {
+            apply(g, p.data(), q.data(), false);
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) q[m] = -q[m];
+            const double alpha = rz / dot(g, p.data(), q.data());
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) {
+                x[m] = std::fma(alpha, p[m], x[m]);
+                r[m] = std::fma(-alpha, q[m], r[m]);
+            }
+            rr = dot(g, r.data(), r.data());
+            ++it;
+            if (history) history[it] = std::sqrt(rr / rr0);
+            if (fixed_iters <= 0 && std::sqrt(rr) <= rtol * std::sqrt(rr0)) {
+                status = ST_OK;
+                break;
+            }
+            gs_precond(g, r.data(), z.data(), -1, true);
+            const double rz_new = dot(g, r.data(), z.data());
+            const double beta = rz_new / rz;
+            rz = rz_new;
+#pragma omp parallel for schedule(static)
+            for (size_t m = 0; m < n; ++m) p[m] = std::fma(beta, p[m], z[m]);
+        }
+    }
+    if (iters) *iters = it;
+    if (relres) *relres = (rr0 > 0) ? std::sqrt(rr / rr0) : 0.0;
+    return status;
+}
+
 // Restart threshold on |rho| / (||r^_0|| ||r||) (reading C4: Saad's Alg. 7.7 has no safeguard; on config 5 the
 // shadow residual and the residual become orthogonal to rounding level after ~10^3 iterations and the iteration
 // stagnates or breaks down, which of the two depends on the rounding of the dot products).
@@ -108,7 +181,7 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
     // stands (A = L, nonsymmetric); its diagonal is -d.
     for (int k = 0; k < g.n[2]; ++k)
         for (int j = 0; j < g.n[1]; ++j)
-            for (int i = 0; i < g.n[0]; ++i) dg[g.idx(i, j, k)] = jacobi ? -diag<double>(g, i, j, k) : 1.0;
+            for (int i = 0; i < g.n[0]; ++i) dg[g.idx(i, j, k)] = jacobi == 1 ? -diag<double>(g, i, j, k) : 1.0;
     // r0 = b - A x0 (ghosts included)
     apply(g, x, v.data(), true);
 #pragma omp parallel for schedule(static)
@@ -129,8 +202,12 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
         status = ST_OK;
     } else {
         for (it = 0; it < nit;) {
+            if (jacobi == 2) {
+                gs_precond(g, p.data(), ph.data(), +1, false);  // p^ = B^-1 p, Eq. 10
+            } else {
 #pragma omp parallel for schedule(static)
-            for (size_t m = 0; m < n; ++m) ph[m] = p[m] / dg[m];
+                for (size_t m = 0; m < n; ++m) ph[m] = p[m] / dg[m];
+            }
             apply(g, ph.data(), v.data(), false);  // v = A p^
             const double r0v = dot(g, r0.data(), v.data());
             if (!(std::fabs(r0v) > 0.0) || !std::isfinite(r0v) || !(std::fabs(rho) > 0.0)) {
@@ -143,6 +220,7 @@ int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_i
                 s[m] = std::fma(-alpha, v[m], r[m]);
                 sh[m] = s[m] / dg[m];
             }
+            if (jacobi == 2) gs_precond(g, s.data(), sh.data(), +1, false);  // s^ = B^-1 s
             apply(g, sh.data(), t.data(), false);  // t = A s^
             const double ts = dot(g, t.data(), s.data());
             const double tt = dot(g, t.data(), t.data());

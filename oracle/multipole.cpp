@@ -109,13 +109,76 @@ double multipole_potential(const double* q, int lmax, double G, double x, double
     return (double)(-(long double)G * acc);
 }
 
+// Inner multipoles, Eq. 22: qbar_lm = sum_cells rho r'^-(l+1) S_lm dV (spherical grids with r_in > 0).
+void multipole_inner_moments(const Grid& g, const double* rho, int lmax, double* qbar) {
+    const int nq = (lmax + 1) * (lmax + 1);
+    std::vector<std::vector<long double>> part(g.n[2], std::vector<long double>(nq, 0.0L));
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g.n[2]; ++k) {
+        long double S[(LMAX_CAP + 1) * (LMAX_CAP + 1)];
+        for (int j = 0; j < g.n[1]; ++j)
+            for (int i = 0; i < g.n[0]; ++i) {
+                long double r, ct, st, ph, dV;
+                if (g.coord == CARTESIAN) {
+                    to_spherical(g.coordinate(0, i), g.coordinate(1, j), g.coordinate(2, k), r, ct, st, ph);
+                    dV = (long double)g.h[0] * g.h[1] * g.h[2];
+                } else {
+                    r = g.ctr[0][i];
+                    ct = cosl((long double)g.ctr[1][j]);
+                    st = sinl((long double)g.ctr[1][j]);
+                    ph = g.ctr[2][k];
+                    long double r0 = g.edge[0][i], r1 = g.edge[0][i + 1];
+                    dV = (r1 * r1 * r1 - r0 * r0 * r0) / 3.0L *
+                         (cosl((long double)g.edge[1][j]) - cosl((long double)g.edge[1][j + 1])) *
+                         ((long double)g.edge[2][k + 1] - (long double)g.edge[2][k]);
+                }
+                if (rho[g.idx(i, j, k)] == 0.0 || r == 0) continue;
+                real_harmonics(lmax, ct, st, ph, S);
+                long double w = (long double)rho[g.idx(i, j, k)] * dV, rl = 1 / r;  // r^-(l+1)
+                for (int l = 0; l <= lmax; ++l) {
+                    for (int m = -l; m <= l; ++m) part[k][l * l + l + m] += w * rl * S[l * l + l + m];
+                    rl /= r;
+                }
+            }
+    }
+    for (int s = 0; s < nq; ++s) {
+        long double tot = 0;
+        for (int k = 0; k < g.n[2]; ++k) tot += part[k][s];
+        qbar[s] = (double)tot;
+    }
+}
+
+// Eq. 21: Phi(x) = -G sum_lm qbar_lm r^l S_lm(x), valid inside all the mass.
+double multipole_inner_potential(const double* qbar, int lmax, double G, double x, double y, double z) {
+    long double r, ct, st, ph;
+    to_spherical(x, y, z, r, ct, st, ph);
+    long double S[(LMAX_CAP + 1) * (LMAX_CAP + 1)];
+    real_harmonics(lmax, ct, st, ph, S);
+    long double acc = 0, rp = 1;  // r^l
+    for (int l = 0; l <= lmax; ++l) {
+        long double sl = 0;
+        for (int m = -l; m <= l; ++m) sl += (long double)qbar[l * l + l + m] * S[l * l + l + m];
+        acc += sl * rp;
+        rp *= r;
+    }
+    return (double)(-(long double)G * acc);
+}
+
 // Fill the ghost zones of every Dirichlet face with Eq. 19 ("We use this formula for all
 // boundaries in Cartesian coordinates, and for the outer boundary r = r_out in spherical coordinates").
-void multipole_bc(Grid& g, const double* rho, double G, int lmax, double* moments) {
-    std::vector<double> q((lmax + 1) * (lmax + 1));
+void multipole_bc(Grid& g, const double* rho, double G, int lmax, double* moments, double* inner_moments) {
+    std::vector<double> q((lmax + 1) * (lmax + 1)), qbar;
     multipole_moments(g, rho, lmax, q.data());
     if (moments)
         for (size_t s = 0; s < q.size(); ++s) moments[s] = q[s];
+    // a spherical grid whose inner radial face is a ghost-Dirichlet face also needs the inner expansion, Eq. 21-22
+    const bool inner = g.coord == SPHERICAL && g.bc[0] == BC_DIRICHLET_GHOST;
+    if (inner) {
+        qbar.resize(q.size());
+        multipole_inner_moments(g, rho, lmax, qbar.data());
+        if (inner_moments)
+            for (size_t s = 0; s < qbar.size(); ++s) inner_moments[s] = qbar[s];
+    }
     for (int f = 0; f < 6; ++f) {
         if (g.bc[f] != BC_DIRICHLET_GHOST) continue;
         int a = f / 2, a1 = (a == 0) ? 1 : 0, a2 = (a == 2) ? 1 : 2;
@@ -133,14 +196,17 @@ void multipole_bc(Grid& g, const double* rho, double G, int lmax, double* moment
                         y = g.coordinate(1, id[1]);
                         z = g.coordinate(2, id[2]);
                     } else {
-                        if (f != 1) continue;  // only the outer radial shell carries Eq. 19
-                        double r = g.r_ghost_out, th = g.ctr[1][q1], ph = g.ctr[2][q2];
+                        if (f > 1) continue;  // only the radial shells carry Eq. 19 / Eq. 21
+                        // ghost shell centres continue the geometric progression of the radial centres
+                        double r = f == 1 ? g.r_ghost_out : g.edge[0][0] * std::sqrt(g.edge[0][0] / g.edge[0][1]);
+                        double th = g.ctr[1][q1], ph = g.ctr[2][q2];
                         x = r * std::sin(th) * std::cos(ph);
                         y = r * std::sin(th) * std::sin(ph);
                         z = r * std::cos(th);
                     }
                     g.ghost[f][((size_t)layer * g.n[a2] + q2) * g.n[a1] + q1] =
-                        multipole_potential(q.data(), lmax, G, x, y, z);
+                        (inner && f == 0) ? multipole_inner_potential(qbar.data(), lmax, G, x, y, z)
+                                          : multipole_potential(q.data(), lmax, G, x, y, z);
                 }
     }
 }

@@ -32,6 +32,9 @@ def lib():
         _lib.orc_multipole_potential.restype = C.c_double
         _lib.orc_r_ghost_out.restype = C.c_double
         _lib.orc_face_len.restype = C.c_long
+        _lib.orc_jacobi_radius.restype = C.c_double
+        _lib.orc_local_jacobi_radius.restype = C.c_double
+        _lib.orc_multipole_inner_potential.restype = C.c_double
     return _lib
 
 
@@ -162,6 +165,50 @@ class Oracle:
         return self._krylov(lib().orc_bicgstab, phi, rhs, rtol, max_iter, fixed_iters, want_history,
                             extra=(int(jacobi),))
 
+    def pcg(self, phi, rhs, rtol=1e-8, max_iter=10000, fixed_iters=0, want_history=False):
+        """CG preconditioned by the symmetrised red-black Gauss-Seidel sweep (row f3)."""
+        return self._krylov(lib().orc_pcg, phi, rhs, rtol, max_iter, fixed_iters, want_history)
+
+    def gs_precond(self, v, sign=-1, symmetric=True):
+        v = _f64(v)
+        z = np.zeros_like(v)
+        lib().orc_gs_precond(self.h, _p(v), _p(z), int(sign), int(bool(symmetric)))
+        return z
+
+    def jacobi_radius(self):
+        return float(lib().orc_jacobi_radius(self.h))
+
+    def local_jacobi_radius(self, i, j):
+        return float(lib().orc_local_jacobi_radius(self.h, int(i), int(j)))
+
+    def rbsor_cheby(self, phi, rhs, nsweeps, rJ=None, start_n=1):
+        """Chebyshev-accelerated omega sequence (Eq. 6), one omega per colour half-sweep; returns the omegas used."""
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs = _f64(rhs)
+        om = np.zeros(2 * nsweeps)
+        rJ = self.jacobi_radius() if rJ is None else rJ
+        lib().orc_rbsor_cheby(self.h, _p(phi), _p(rhs), C.c_double(rJ), int(nsweeps), int(start_n), _p(om))
+        return om
+
+    def rbsor_local(self, phi, rhs, nsweeps, start_n=1):
+        assert phi.dtype == np.float64 and phi.flags.c_contiguous
+        rhs = _f64(rhs)
+        lib().orc_rbsor_local(self.h, _p(phi), _p(rhs), int(nsweeps), int(start_n))
+
+    def multipole_bc2(self, rho, G, lmax):
+        """(outer moments, inner moments): fills the outer and — on a spherical grid with a Dirichlet inner face — the
+        inner ghost shell (Eq. 19-22)."""
+        rho = _f64(rho)
+        q, qb = np.zeros((lmax + 1) ** 2), np.zeros((lmax + 1) ** 2)
+        lib().orc_multipole_bc2(self.h, _p(rho), C.c_double(G), int(lmax), _p(q), _p(qb))
+        return q, qb
+
+    def multipole_inner_moments(self, rho, lmax):
+        rho = _f64(rho)
+        q = np.zeros((lmax + 1) ** 2)
+        lib().orc_multipole_inner_moments(self.h, _p(rho), int(lmax), _p(q))
+        return q
+
     @staticmethod
     def set_bicgstab_restart_eps(eps):
         """Near-breakdown threshold of BiCGSTAB (default 1e-12); tests raise it to force the restart branch."""
@@ -251,6 +298,12 @@ class Oracle:
 
     def r_ghost_out(self):
         return float(lib().orc_r_ghost_out(self.h))
+
+
+def multipole_inner_potential(qbar, lmax, G, x, y, z):
+    qbar = _f64(qbar)
+    return float(lib().orc_multipole_inner_potential(_p(qbar), int(lmax), C.c_double(G), C.c_double(x), C.c_double(y),
+                                                     C.c_double(z)))
 
 
 def multipole_potential(q, lmax, G, x, y, z):

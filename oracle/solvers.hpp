@@ -13,11 +13,27 @@ void rbsor_half(const Grid& g, T* phi, const T* rhs, T omega, int colour, bool u
 template <typename T>
 void rbsor(const Grid& g, T* phi, const T* rhs, T omega, int nsweeps, bool use_ghost);
 
+// Row f4 (Eq. 6-7): Chebyshev-accelerated omega sequence and its position-dependent variant.
+double jacobi_radius(const Grid& g);
+double local_jacobi_radius(const Grid& g, int i, int j);
+double cheby_next(double rJ, int n_next, double omega_n);
+void rbsor_cheby(const Grid& g, double* phi, const double* rhs, double rJ, int nsweeps, int start_n, bool use_ghost,
+                 double* omegas /* nullable, 2 nsweeps */);
+void rbsor_local(const Grid& g, double* phi, const double* rhs, int nsweeps, int start_n, bool use_ghost);
+
 // Conjugate gradient, Saad Alg. 6.18 on A = -L_h (SPD), b = -rhs.  PAPER.md:95-105.
 int cg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
        double* relres, double* history /* nullable, max_iter+1 relative residuals */);
 
-// BiCGSTAB, Saad Alg. 7.7 with right Jacobi scaling (jacobi != 0).  PAPER.md:105; reading C4/C10.
+// Row f3 (Eq. 9-10): z = B^-1 v with B the colour-block lower-triangular part of the operator
+// (sign = +1: of L_h; -1: of A = -L_h), i.e. one red-black Gauss-Seidel sweep from zero; symmetric: red, black, red.
+void gs_precond(const Grid& g, const double* v, double* z, int sign, bool symmetric);
+// Preconditioned CG (Saad Alg. 9.1) on A = -L_h with M^-1 = the symmetrised red-black Gauss-Seidel sweep.
+int pcg(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int* iters,
+        double* relres, double* history);
+
+// BiCGSTAB, Saad Alg. 7.7, right-preconditioned: jacobi = 0 none, 1 Jacobi scaling (reading C4/C10),
+// 2 the red-black Gauss-Seidel preconditioner of Eq. 10.  PAPER.md:105, 107-123.
 int bicgstab(const Grid& g, double* x, const double* rhs, double rtol, int max_iter, int fixed_iters, int jacobi,
              int* iters, double* relres, double* history);
 // Near-breakdown threshold (default 1e-12; reading C4) and the counts of the last call: restarts taken,
@@ -50,6 +66,10 @@ void mgv_prolong_add(const Grid& g, const double* ec, double* x);
 // Multipole boundary condition, Eq. 19-20.  Fills g.ghost[] on Dirichlet faces.
 void multipole_moments(const Grid& g, const double* rho, int lmax, double* q /* (lmax+1)^2, index l*l+l+m */);
 double multipole_potential(const double* q, int lmax, double G, double x, double y, double z);
-void multipole_bc(Grid& g, const double* rho, double G, int lmax, double* moments /* nullable */);
+void multipole_bc(Grid& g, const double* rho, double G, int lmax, double* moments /* nullable */,
+                  double* inner_moments = nullptr /* nullable */);
+// Inner expansion for a spherical grid with r_in > 0 (Eq. 21-22).
+void multipole_inner_moments(const Grid& g, const double* rho, int lmax, double* qbar);
+double multipole_inner_potential(const double* qbar, int lmax, double G, double x, double y, double z);
 
 }  // namespace orc
