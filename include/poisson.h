@@ -134,6 +134,26 @@ int poisson_bicgstab_solve(poisson_t h, double* d_phi, const double* d_rhs, doub
 int poisson_mg_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
                       int coarsest_sweeps, int precision, int ncycles, double* h_resnorms);
 
+/* The paper's own multigrid ingredients, for vertex-centred grids of 2^N k - 1 points per
+ * axis with isotropic spacing and Dirichlet (ghost) faces, 7-point operator.
+ *
+ * poisson_spai_smooth: nsteps steps of the SPAI smoother  x <- x + omega M (b - A x)  (Eq. 15) on
+ *   A = -L_h, b = -rhs, with M = h^2 {alpha at the centre, beta on the 6 faces, gamma on the 12 edges, delta on the
+ *   8 corners} (Eq. 16).  spai = {omega, alpha, beta, gamma, delta}; NULL = Table 1, order 2:
+ *   {1.3699, 0.1432, 0.0284, 0.0081, 0.0025}.  Works on any shape (it is level 0 of the hierarchy below).
+ *
+ * poisson_mgv_vcycle: ncycles V-cycles (Eq. 11-12) with nu1/nu2 SPAI steps, full-weighting restriction
+ *   R = (1/4 [1 2 1])^(x)3 (Eq. 13), prolongation P = 8 R^T (trilinear, "c adjusted such that P preserves constant
+ *   functions"), Galerkin coarse operators R A P (Eq. 14; reading C13 on the constant), coarsening while
+ *   every axis is odd and the coarse level keeps >= coarsest_n points per axis (coarsest_n = 3 gives the paper's seven
+ *   coarse levels at 511^3), coarsest level by CG to relative residual cg_rtol (at most 15^3 unknowns).
+ *   precision = POISSON_F64, or POISSON_MIXED = the paper's mixed precision: all coarse-level data stored
+ *   in fp32, all arithmetic in fp64.  UNSUPPORTED when the grid admits no coarse level.
+ *   h_resnorms (nullable, ncycles+1): ||rhs - L phi||_2 before the first and after every cycle (for Eq. 18). */
+int poisson_spai_smooth(poisson_t h, double* d_phi, const double* d_rhs, const double* spai, int nsteps);
+int poisson_mgv_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
+                       const double* spai, double cg_rtol, int precision, int ncycles, double* h_resnorms);
+
 /* Multipole-expansion open boundary (Eq. 19-20): moments q_lm = sum_cells rho r^l S_lm dV for
  * 0 <= l <= lmax (<= 8), |m| <= l in one fused reduction over d_rho, then Phi_ghost = -G sum q_lm S_lm / r^(l+1)
  * written into the handle's ghost faces (all Dirichlet faces in Cartesian, the outer radial shell in spherical).
@@ -178,6 +198,8 @@ int poisson_bicgstab_solve_host(poisson_t h, double* h_phi, const double* h_rhs,
 int poisson_mg_vcycle_host(poisson_t h, double* h_phi, const double* h_rhs, int nu1, int nu2, int coarsest_n,
                            int coarsest_sweeps, int precision, int ncycles, double* h_resnorms);
 int poisson_multipole_bc_host(poisson_t h, const double* h_rho, double G, int lmax, double* h_moments);
+int poisson_mgv_vcycle_host(poisson_t h, double* h_phi, const double* h_rhs, int nu1, int nu2, int coarsest_n,
+                            const double* spai, double cg_rtol, int precision, int ncycles, double* h_resnorms);
 
 #ifdef __cplusplus
 }

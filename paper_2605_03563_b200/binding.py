@@ -29,6 +29,7 @@ SYMBOLS = [
     "poisson_kernel_class_launches", "poisson_kernel_time", "poisson_reset_kernel_times",
     "poisson_apply_laplacian_host", "poisson_rbsor_sweep_host", "poisson_cg_solve_host",
     "poisson_bicgstab_solve_host", "poisson_mg_vcycle_host", "poisson_multipole_bc_host",
+    "poisson_spai_smooth", "poisson_mgv_vcycle", "poisson_mgv_vcycle_host",
 ]
 
 _lib = None
@@ -218,6 +219,22 @@ class Poisson:
                                                       int(coarsest_n), int(coarsest_sweeps), int(precision),
                                                       int(ncycles), buf if want_resnorms else None))
         return dict(status=rc, resnorms=list(buf) if want_resnorms else None)
+
+    def spai_smooth(self, d_phi, d_rhs, spai=None, nsteps=1):
+        sp = (C.c_double * 5)(*spai) if spai is not None else None
+        self._check(lib().poisson_spai_smooth(self.h, _ptr(d_phi), _ptr(d_rhs), sp, int(nsteps)))
+
+    def mgv_vcycle(self, d_phi, d_rhs, nu1=1, nu2=1, coarsest_n=3, spai=None, cg_rtol=1e-3, precision=F64, ncycles=1,
+                   want_resnorms=True, _fn=None):
+        sp = (C.c_double * 5)(*spai) if spai is not None else None
+        buf = (C.c_double * (ncycles + 1))()
+        fn = _fn or lib().poisson_mgv_vcycle
+        rc = self._check(fn(self.h, _ptr(d_phi), _ptr(d_rhs), int(nu1), int(nu2), int(coarsest_n), sp,
+                            C.c_double(cg_rtol), int(precision), int(ncycles), buf if want_resnorms else None))
+        return dict(status=rc, resnorms=list(buf) if want_resnorms else None)
+
+    def mgv_vcycle_host(self, h_phi, h_rhs, **kw):
+        return self.mgv_vcycle(h_phi, h_rhs, _fn=lib().poisson_mgv_vcycle_host, **kw)
 
     def multipole_bc(self, d_rho, G, lmax, want_moments=True, _fn=None):
         nq = (lmax + 1) ** 2

@@ -88,7 +88,8 @@ void post_launch(poisson_ctx* ctx, int kid) {
 
 static const char* const kKernelNames[pb::KID_COUNT] = {
     "apply", "rbsor", "krylov_init", "cg_pass_a", "cg_pass_b", "cg_final", "bicg_pass1", "bicg_pass2", "bicg_pass3",
-    "mg_restrict", "mg_prolong", "mg_coarse", "mg_axpy", "mp_moments", "mp_ghosts"};
+    "mg_restrict", "mg_prolong", "mg_coarse", "mg_axpy", "mp_moments", "mp_ghosts",
+    "mgv_smooth", "mgv_restrict", "mgv_prolong", "mgv_coarse", "mgv_setup", "pcg_precond"};
 
 static void free_levels(poisson_ctx* ctx) {
     for (auto& L : ctx->levels) {
@@ -186,6 +187,7 @@ int poisson_destroy(poisson_t ctx) {
     if (!ctx) return POISSON_INVALID_ARG;
     cudaStreamSynchronize(ctx->stream);
     free_levels(ctx);
+    mgv_destroy(ctx);
     for (double* v : ctx->vec) cudaFree(v);
     for (int f = 0; f < 6; ++f) cudaFree(ctx->d_ghost[f]);
     cudaFree(ctx->sor_tmp);
@@ -808,6 +810,42 @@ int poisson_mg_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1
     return POISSON_OK;
 }
 
+// ---- the paper's own multigrid: SPAI smoother, vertex-centred Galerkin hierarchy (rows f1, f2) -------------------------------
+int poisson_spai_smooth(poisson_t ctx, double* d_phi, const double* d_rhs, const double* spai, int nsteps) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !d_phi || !d_rhs || nsteps < 0) return fail(ctx, POISSON_INVALID_ARG, "bad arguments");
+    return mgv_spai_smooth(ctx, d_phi, d_rhs, spai, nsteps);
+}
+
+int poisson_mgv_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
+                       const double* spai, double cg_rtol, int precision, int ncycles, double* h_resnorms) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (nu1 < 0 || nu2 < 0 || coarsest_n < 1 || ncycles < 0 || ncycles + 1 > 200 || !(cg_rtol > 0) ||
+        (precision != POISSON_F64 && precision != POISSON_MIXED))
+        return fail(ctx, POISSON_INVALID_ARG, "bad V-cycle parameters");
+    auto record_norm = [&](int slot) -> int {
+        if (!h_resnorms) return POISSON_OK;
+        int r2 = launch_apply(ctx, ctx->op, ctx->kind, d_phi, d_rhs, nullptr, 1, true, true);
+        if (r2 != POISSON_OK) return r2;
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->d_scal + 16 + slot, ctx->d_scal, sizeof(double), cudaMemcpyDeviceToDevice,
+                                   ctx->stream));
+        return POISSON_OK;
+    };
+    int rc = record_norm(0);
+    if (rc != POISSON_OK) return rc;
+    rc = mgv_vcycles(ctx, d_phi, d_rhs, nu1, nu2, coarsest_n, spai, cg_rtol, precision == POISSON_MIXED, ncycles,
+                     record_norm);
+    if (rc != POISSON_OK) return rc;
+    if (h_resnorms) {
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->h_scal, ctx->d_scal + 16, (ncycles + 1) * sizeof(double),
+                                   cudaMemcpyDeviceToHost, ctx->stream));
+        PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+        for (int c = 0; c <= ncycles; ++c) h_resnorms[c] = std::sqrt(ctx->h_scal[c]);
+    }
+    return POISSON_OK;
+}
+
 // ---- multipole boundary -------------------------------------------------------------------------------------------------
 int poisson_multipole_bc(poisson_t ctx, const double* d_rho, double G, int lmax, double* h_moments) {
     const DeviceGuard on_device(ctx);
@@ -903,6 +941,18 @@ int poisson_mg_vcycle_host(poisson_t ctx, double* h_phi, const double* h_rhs, in
     STAGE_OK(stage(ctx, 1, h_rhs));
     const int rc = poisson_mg_vcycle(ctx, ctx->d_stage[0], ctx->d_stage[1], nu1, nu2, coarsest_n, coarsest_sweeps,
                                      precision, ncycles, h_resnorms);
+    if (rc < 0) return rc;
+    return unstage(ctx, 0, h_phi);
+}
+
+int poisson_mgv_vcycle_host(poisson_t ctx, double* h_phi, const double* h_rhs, int nu1, int nu2, int coarsest_n,
+                            const double* spai, double cg_rtol, int precision, int ncycles, double* h_resnorms) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !h_phi || !h_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    STAGE_OK(stage(ctx, 0, h_phi));
+    STAGE_OK(stage(ctx, 1, h_rhs));
+    const int rc = poisson_mgv_vcycle(ctx, ctx->d_stage[0], ctx->d_stage[1], nu1, nu2, coarsest_n, spai, cg_rtol,
+                                      precision, ncycles, h_resnorms);
     if (rc < 0) return rc;
     return unstage(ctx, 0, h_phi);
 }

@@ -5,6 +5,7 @@
 
 #include <cstdint>
 #include <cstdio>
+#include <functional>
 #include <string>
 #include <unordered_map>
 #include <vector>
@@ -55,6 +56,12 @@ enum KernelId {
     KID_MG_AXPY,        // mixed path: phi += (double) e32
     KID_MP_MOMENTS,     // multipole moments (a6)
     KID_MP_GHOSTS,      // ghost-zone evaluation (a6)
+    KID_MGV_SMOOTH,     // SPAI smoothing step (f1)
+    KID_MGV_RESTRICT,   // vertex-centred residual + full weighting (f2)
+    KID_MGV_PROLONG,    // vertex-centred trilinear prolongation + correction (f2)
+    KID_MGV_COARSE,     // coarsest-level CG (f2)
+    KID_MGV_SETUP,      // Galerkin stencils, boundary folding (f2)
+    KID_PCG_PRECOND,    // red-black Gauss-Seidel preconditioner sweeps (f3)
     KID_COUNT
 };
 
@@ -92,6 +99,14 @@ struct MgLevel {
     float* alt32 = nullptr;
 };
 
+// One level of the vertex-centred Galerkin hierarchy (k_mgv.cu): constant symmetric 27-point operator, spacing h.
+struct MgvLevel {
+    int n[3] = {0, 0, 0};
+    double h = 0.0;
+    size_t npts = 0;
+    void *x = nullptr, *b = nullptr, *t = nullptr;  // x: two buffers (coarse levels); b; t: fp64 residual / ping-pong
+};
+
 }  // namespace pb
 
 struct poisson_ctx {
@@ -118,6 +133,9 @@ struct poisson_ctx {
     double* h_scal = nullptr;        // pinned
     std::vector<pb::MgLevel> levels;
     int mg_coarsest_n = -1;
+    std::vector<pb::MgvLevel> vlevels;  // the paper's vertex-centred hierarchy
+    double* v_sten = nullptr;           // 4 stencil coefficients per level (device)
+    int v_key[2] = {-1, -1};            // (coarsest_n, fp32 storage) the hierarchy was built for
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
     int opt_sor_nhs = 0;             // colour half-steps fused per HBM pass of the red-black kernel (2, 4; 0 = auto)
@@ -268,6 +286,12 @@ int launch_mg_bottom(poisson_ctx* ctx, const Op* ops, int nlev, double* phi, con
                      int csweeps, double omega_c);
 int launch_mg_bottom32(poisson_ctx* ctx, const Op* ops, int nlev, float* phi, const float* rhs, int nu1, int nu2,
                        int csweeps, double omega_c);
+
+// The paper's own multigrid (k_mgv.cu): SPAI smoother, vertex-centred transfers, Galerkin stencils, CG coarsest
+int mgv_spai_smooth(poisson_ctx* ctx, double* phi, const double* rhs, const double* spai, int nsteps);
+int mgv_vcycles(poisson_ctx* ctx, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, const double* spai,
+                double cg_rtol, int storage_f32, int ncycles, const std::function<int(int)>& record);
+void mgv_destroy(poisson_ctx* ctx);
 
 // Multipole
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q);
