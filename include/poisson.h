@@ -104,6 +104,30 @@ int poisson_apply_laplacian(poisson_t h, const double* d_phi, double* d_out);
 int poisson_rbsor_sweep(poisson_t h, double* d_phi, const double* d_rhs, double omega, int nsweeps,
                         double* h_resnorm);
 
+/* Red-black SOR with the Chebyshev-accelerated sequence of PAPER.md:81-88 Eq. 6 instead of a fixed omega:
+ *   omega_0 = 1, omega_1 = 1/(1 - rJ^2/2), omega_{n+1} = 1/(1 - rJ^2 omega_n/4)  ->  omega_opt of Eq. 3,
+ * one member per colour half-sweep (Press et al. Eq. 20.5.30, as cited there): half-sweep m = 0, 1, 2, ... (red, black,
+ * red, ...) uses omega_{m + start_n}; start_n = 1 is the variant the paper uses ("starting from n = 1").
+ * r_jacobi: spectral radius of the Jacobi iteration; <= 0 selects Eq. 4 with N = n + 1 intervals (Cartesian grids).
+ * Each call starts the sequence afresh.  h_resnorm as in poisson_rbsor_sweep. */
+int poisson_rbsor_cheby(poisson_t h, double* d_phi, const double* d_rhs, double r_jacobi, int nsweeps, int start_n,
+                        double* h_resnorm);
+
+/* The position-dependent variant for spherical (and nonuniform) grids, Eq. 7: every point (i,j) runs
+ * the sequence of Eq. 6 with its own local Jacobi radius
+ *   rJ(i,j) = [cos(pi/Nr) dr_i^-2 + cos(pi/Nth) (r_i dth)^-2 + cos(pi/Nph) (r_i sin th_j dph)^-2] / [sum of the three],
+ * advanced after every colour half-sweep.  On a Cartesian grid rJ is that of Eq. 4 everywhere. */
+int poisson_rbsor_local(poisson_t h, double* d_phi, const double* d_rhs, int nsweeps, int start_n, double* h_resnorm);
+
+/* Conjugate gradient preconditioned by the multi-colour Gauss-Seidel preconditioner of PAPER.md:107-123 Eq. 9-10
+ * (two colours for the 7-point operator): z = M^-1 r is one red-black Gauss-Seidel sweep on L_h z = r from z = 0 —
+ * the block lower-triangular solve B^-1 of Eq. 10 — followed by a second red half-sweep, which makes M the symmetric
+ * Gauss-Seidel splitting a CG iteration needs (reading C15); Saad Alg. 9.1.  The sweep is ONE fused pass
+ * over HBM.  Same stopping rule (on the unpreconditioned residual), statuses and outputs as poisson_cg_solve.
+ * Cartesian 7-point operator, non-periodic faces. */
+int poisson_pcg_solve(poisson_t h, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,
+                      int* iters, double* relres);
+
 /* Unpreconditioned conjugate gradient on A = -L_h (Saad Alg. 6.18), fused as
  * {p-update + matvec + p.Ap} and {r-update + ||r||^2}.  Stops when ||r_k|| <= rtol ||r_0|| (r_0 from the initial
  * guess) or after max_iter iterations (-> NOT_CONVERGED).  fixed_iters > 0 runs exactly that many iterations.
@@ -160,6 +184,10 @@ int poisson_mgv_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1,
  * Expansion centre = coordinate origin.  h_moments (nullable): (lmax+1)^2 values, index l*l + l + m, cosine
  * harmonics m >= 0, sine harmonics m < 0. */
 int poisson_multipole_bc(poisson_t h, const double* d_rho, double G, int lmax, double* h_moments);
+/* Spherical grids whose inner radial face (face 0) is POISSON_BC_DIRICHLET_GHOST: poisson_multipole_bc also forms the
+ * inner multipoles qbar_lm = sum_cells rho r^-(l+1) S_lm dV and writes Phi = -G sum qbar_lm r^l S_lm into the inner
+ * ghost shell (Eq. 21-22).  This call returns those moments, (lmax+1)^2 values, same indexing. */
+int poisson_multipole_inner_moments(poisson_t h, double* h_qbar, int lmax);
 
 /* Helpers. */
 /* Copy caller-supplied ghost values (DEVICE arrays, layout above; NULL entries = leave that face) into the handle. */

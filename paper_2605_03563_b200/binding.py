@@ -30,6 +30,7 @@ SYMBOLS = [
     "poisson_apply_laplacian_host", "poisson_rbsor_sweep_host", "poisson_cg_solve_host",
     "poisson_bicgstab_solve_host", "poisson_mg_vcycle_host", "poisson_multipole_bc_host",
     "poisson_spai_smooth", "poisson_mgv_vcycle", "poisson_mgv_vcycle_host",
+    "poisson_rbsor_cheby", "poisson_rbsor_local", "poisson_pcg_solve", "poisson_multipole_inner_moments",
 ]
 
 _lib = None
@@ -180,6 +181,26 @@ class Poisson:
         self._check(lib().poisson_rbsor_sweep_host(self.h, _ptr(h_phi), _ptr(h_rhs), C.c_double(omega), int(nsweeps),
                                                    C.byref(out) if want_resnorm else None))
         return out.value if want_resnorm else None
+
+    def rbsor_cheby(self, d_phi, d_rhs, nsweeps, r_jacobi=0.0, start_n=1, want_resnorm=False):
+        out = C.c_double(0.0)
+        self._check(lib().poisson_rbsor_cheby(self.h, _ptr(d_phi), _ptr(d_rhs), C.c_double(r_jacobi), int(nsweeps),
+                                              int(start_n), C.byref(out) if want_resnorm else None))
+        return out.value if want_resnorm else None
+
+    def rbsor_local(self, d_phi, d_rhs, nsweeps, start_n=1, want_resnorm=False):
+        out = C.c_double(0.0)
+        self._check(lib().poisson_rbsor_local(self.h, _ptr(d_phi), _ptr(d_rhs), int(nsweeps), int(start_n),
+                                              C.byref(out) if want_resnorm else None))
+        return out.value if want_resnorm else None
+
+    def pcg_solve(self, d_phi, d_rhs, rtol=1e-8, max_iter=10000, fixed_iters=0):
+        return self._krylov(lib().poisson_pcg_solve, d_phi, d_rhs, rtol, max_iter, fixed_iters)
+
+    def multipole_inner_moments(self, lmax):
+        buf = (C.c_double * ((lmax + 1) ** 2))()
+        self._check(lib().poisson_multipole_inner_moments(self.h, buf, int(lmax)))
+        return list(buf)
 
     def _krylov(self, fn, d_phi, d_rhs, rtol, max_iter, fixed_iters):
         it, rr = C.c_int(0), C.c_double(0.0)

@@ -193,6 +193,7 @@ int poisson_destroy(poisson_t ctx) {
     cudaFree(ctx->sor_tmp);
     cudaFree(ctx->d_coef);
     cudaFree(ctx->d_ctr);
+    cudaFree(ctx->d_rj);
     cudaFree(ctx->red.partials);
     cudaFree(ctx->red.counter);
     cudaFree(ctx->d_ctl);
@@ -311,9 +312,9 @@ int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], 
     CREATE_OK(cudaMalloc((void**)&ctx->d_ctl, sizeof(KrylovCtl)));
     CREATE_OK(cudaMemset(ctx->d_ctl, 0, sizeof(KrylovCtl)));
     CREATE_OK(cudaMallocHost((void**)&ctx->h_ctl, sizeof(KrylovCtl)));
-    CREATE_OK(cudaMalloc((void**)&ctx->d_scal, 256 * sizeof(double)));
-    CREATE_OK(cudaMemset(ctx->d_scal, 0, 256 * sizeof(double)));
-    CREATE_OK(cudaMallocHost((void**)&ctx->h_scal, 256 * sizeof(double)));
+    CREATE_OK(cudaMalloc((void**)&ctx->d_scal, 512 * sizeof(double)));
+    CREATE_OK(cudaMemset(ctx->d_scal, 0, 512 * sizeof(double)));
+    CREATE_OK(cudaMallocHost((void**)&ctx->h_scal, 512 * sizeof(double)));
     if (coord_system == POISSON_SPHERICAL) {
         for (int a = 0; a < 3; ++a) ctx->edges[a].assign(edges[a], edges[a] + shape[a] + 1);
         int rc = setup_spherical(ctx);
@@ -482,7 +483,7 @@ int poisson_rbsor_sweep(poisson_t ctx, double* d_phi, const double* d_rhs, doubl
 }
 
 // ---- Krylov drivers ---------------------------------------------------------------------------------------------------
-static int krylov_setup(poisson_ctx* ctx, double rtol, int max_iter, int fixed_iters, bool project) {
+static int krylov_setup(poisson_ctx* ctx, double rtol, int max_iter, int fixed_iters, bool project, bool pcg = false) {
     const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
     KrylovCtl* c = ctx->h_ctl;
     std::memset(c, 0, sizeof(*c));
@@ -493,6 +494,7 @@ static int krylov_setup(poisson_ctx* ctx, double rtol, int max_iter, int fixed_i
     c->record = ctx->opt_history;
     c->npoints = (double)ctx->npts;
     c->eps_bd = ctx->opt_bicg_restart_eps;
+    c->pcg = pcg ? 1 : 0;
     if (ctx->opt_history) {
         if (ctx->hist_cap < nit + 1) {
             cudaFree(ctx->d_hist);
@@ -852,9 +854,16 @@ int poisson_multipole_bc(poisson_t ctx, const double* d_rho, double G, int lmax,
     if (!ctx || !d_rho) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     double* d_q = ctx->d_scal + 128;
-    int rc = launch_moments(ctx, d_rho, lmax, d_q);
+    int rc = launch_moments(ctx, d_rho, lmax, d_q, false);
     if (rc != POISSON_OK) return rc;
-    rc = launch_ghost_eval(ctx, d_q, G, lmax);
+    // a spherical grid whose inner radial face is a Dirichlet face also takes the inner expansion (Eq. 21-22)
+    double* d_qbar = nullptr;
+    if (ctx->op.coord == POISSON_SPHERICAL && ctx->op.bc[0] == POISSON_BC_DIRICHLET_GHOST) {
+        d_qbar = ctx->d_scal + 300;
+        if ((rc = launch_moments(ctx, d_rho, lmax, d_qbar, true)) != POISSON_OK) return rc;
+    }
+    ctx->inner_lmax = d_qbar ? lmax : -1;
+    rc = launch_ghost_eval(ctx, d_q, d_qbar, G, lmax);
     if (rc != POISSON_OK) return rc;
     ctx->ghost_nonzero = true;
     if (h_moments) {
@@ -864,6 +873,141 @@ int poisson_multipole_bc(poisson_t ctx, const double* d_rho, double G, int lmax,
         std::memcpy(h_moments, ctx->h_scal + 128, nq * sizeof(double));
     }
     return POISSON_OK;
+}
+
+int poisson_multipole_inner_moments(poisson_t ctx, double* h_qbar, int lmax) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !h_qbar) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (ctx->inner_lmax < 0 || lmax != ctx->inner_lmax)
+        return fail(ctx, POISSON_INVALID_ARG, "no inner moments of this order: call poisson_multipole_bc on a spherical grid "
+                                              "with a Dirichlet inner face first");
+    const int nq = (lmax + 1) * (lmax + 1);
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->h_scal + 300, ctx->d_scal + 300, nq * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    std::memcpy(h_qbar, ctx->h_scal + 300, nq * sizeof(double));
+    return POISSON_OK;
+}
+
+// ---- rows f3, f4: omega sequences, position-dependent omega, Gauss-Seidel-preconditioned CG ------------------------------
+// Eq. 4 with N = n + 1 intervals (exact for ghost-Dirichlet faces; reading C0).
+static double jacobi_radius_eq4(const poisson_ctx* ctx) {
+    double num = 0.0, den = 0.0;
+    for (int a = 0; a < 3; ++a) {
+        num += ctx->op.c[a] * std::cos(M_PI / (ctx->op.n[a] + 1));
+        den += ctx->op.c[a];
+    }
+    return num / den;
+}
+
+int poisson_rbsor_cheby(poisson_t ctx, double* d_phi, const double* d_rhs, double r_jacobi, int nsweeps, int start_n,
+                        double* h_resnorm) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !d_phi || !d_rhs || nsweeps < 0 || start_n < 0) return fail(ctx, POISSON_INVALID_ARG, "bad arguments");
+    if (!(r_jacobi > 0.0)) {
+        if (ctx->kind != KIND_CART2) return fail(ctx, POISSON_INVALID_ARG, "r_jacobi must be given on this grid (Eq. 4 is Cartesian)");
+        r_jacobi = jacobi_radius_eq4(ctx);
+    }
+    if (!(r_jacobi < 1.0)) return fail(ctx, POISSON_INVALID_ARG, "the Jacobi spectral radius must lie in (0,1)");
+    // Eq. 6: omega_0 = 1, omega_1 = 1/(1 - rJ^2/2), omega_{n+1} = 1/(1 - rJ^2 omega_n/4); half-sweep m uses omega_{m+start_n}
+    std::vector<double> om((size_t)2 * nsweeps);
+    double w = 1.0;
+    for (int n = 1; n <= start_n; ++n) w = n == 1 ? 1.0 / (1.0 - 0.5 * r_jacobi * r_jacobi) : 1.0 / (1.0 - 0.25 * r_jacobi * r_jacobi * w);
+    for (int m = 0; m < 2 * nsweeps; ++m) {
+        om[m] = w;
+        const int nn = m + start_n + 1;
+        w = nn == 1 ? 1.0 / (1.0 - 0.5 * r_jacobi * r_jacobi) : 1.0 / (1.0 - 0.25 * r_jacobi * r_jacobi * w);
+    }
+    int rc = launch_rbsor_seq(ctx, ctx->op, ctx->kind, d_phi, d_rhs, om.data(), nsweeps, true);
+    if (rc != POISSON_OK) return rc;
+    if (h_resnorm) return residual_norm_sync(ctx, d_phi, d_rhs, h_resnorm);
+    return POISSON_OK;
+}
+
+int poisson_rbsor_local(poisson_t ctx, double* d_phi, const double* d_rhs, int nsweeps, int start_n, double* h_resnorm) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !d_phi || !d_rhs || nsweeps < 0 || start_n < 0) return fail(ctx, POISSON_INVALID_ARG, "bad arguments");
+    if (ctx->kind == KIND_CART6) return fail(ctx, POISSON_UNSUPPORTED, "red-black sweeps need a radius-1 stencil");
+    const int n0 = ctx->op.n[0], n1 = ctx->op.n[1];
+    const size_t n2d = (size_t)n0 * n1;
+    if (!ctx->d_rj) {
+        // Eq. 7: the local Jacobi radius from the grid metric (a coefficient array like those of setup_spherical)
+        std::vector<double> rj(n2d);
+        for (int j = 0; j < n1; ++j)
+            for (int i = 0; i < n0; ++i) {
+                if (ctx->kind == KIND_SPH) {
+                    const double dr = ctx->edges[0][i + 1] - ctx->edges[0][i], dth = ctx->edges[1][j + 1] - ctx->edges[1][j];
+                    const double dph = ctx->edges[2][1] - ctx->edges[2][0];
+                    const double r = ctx->ctr[0][i], st = std::sin(ctx->ctr[1][j]);
+                    const double a = 1.0 / (dr * dr), b = 1.0 / ((r * dth) * (r * dth)), c = 1.0 / ((r * st * dph) * (r * st * dph));
+                    rj[(size_t)j * n0 + i] = (std::cos(M_PI / n0) * a + std::cos(M_PI / n1) * b + std::cos(M_PI / ctx->op.n[2]) * c) / (a + b + c);
+                } else {
+                    rj[(size_t)j * n0 + i] = jacobi_radius_eq4(ctx);
+                }
+            }
+        PB_CUDA_OK(cudaMalloc((void**)&ctx->d_rj, 2 * n2d * sizeof(double)));
+        PB_CUDA_OK(cudaMemcpy(ctx->d_rj, rj.data(), n2d * sizeof(double), cudaMemcpyHostToDevice));
+    }
+    int rc = launch_rbsor_local(ctx, ctx->op, ctx->kind, d_phi, d_rhs, ctx->d_rj, ctx->d_rj + n2d, nsweeps, start_n, true);
+    if (rc != POISSON_OK) return rc;
+    if (h_resnorm) return residual_norm_sync(ctx, d_phi, d_rhs, h_resnorm);
+    return POISSON_OK;
+}
+
+// z = M^-1 r: the symmetrised red-black Gauss-Seidel sweep (red, black, red) on L z = r from z = 0.
+static int gs_precond(poisson_ctx* ctx, const double* r, double* z, const double* zeros) {
+    if (sor_fused_ok(ctx, ctx->op)) return sor_fused_precond(ctx, ctx->op, zeros, z, r, true);
+    PB_CUDA_OK(cudaMemsetAsync(z, 0, ctx->npts * sizeof(double), ctx->stream));
+    for (int colour : {0, 1, 0}) {
+        const int rc = launch_rbsor_half(ctx, ctx->op, ctx->kind, z, r, 1.0, colour, false, KID_PCG_PRECOND);
+        if (rc != POISSON_OK) return rc;
+    }
+    return POISSON_OK;
+}
+
+int poisson_pcg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,
+                      int* iters, double* relres) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !d_phi || !d_rhs) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (fixed_iters <= 0 && (max_iter < 1 || !(rtol > 0))) return fail(ctx, POISSON_INVALID_ARG, "bad rtol/max_iter");
+    if (ctx->kind != KIND_CART2)
+        return fail(ctx, POISSON_UNSUPPORTED, "Gauss-Seidel-preconditioned CG: Cartesian 7-point operator (two colours, PAPER.md:113)");
+    for (int f = 0; f < 6; ++f)
+        if (ctx->op.bc[f] == POISSON_BC_PERIODIC)
+            return fail(ctx, POISSON_UNSUPPORTED, "Gauss-Seidel-preconditioned CG: non-periodic faces only");
+    double *r = scratch(ctx, 0), *P[2] = {scratch(ctx, 1), scratch(ctx, 2)}, *q = scratch(ctx, 3), *z = scratch(ctx, 4),
+           *zeros = scratch(ctx, 5);
+    if (!r || !P[0] || !P[1] || !q || !z || !zeros) return POISSON_OUT_OF_MEMORY;
+    int rc = krylov_setup(ctx, rtol, max_iter, fixed_iters, false, true);
+    if (rc != POISSON_OK) return rc;
+    for (double* v : {P[0], P[1], zeros}) PB_CUDA_OK(cudaMemsetAsync(v, 0, ctx->npts * sizeof(double), ctx->stream));
+    if ((rc = launch_krylov_init(ctx, d_phi, d_rhs, r, false, nullptr)) != POISSON_OK) return rc;
+    if ((rc = gs_precond(ctx, r, z, zeros)) != POISSON_OK) return rc;
+    if ((rc = launch_pcg_dot(ctx, r, z)) != POISSON_OK) return rc;
+    const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
+    for (int j = 0; j < nit;) {
+        const int chunk = std::min(ctx->opt_poll, nit - j);
+        for (int c = 0; c < chunk; ++c, ++j) {
+            // pass A with z in the place of r: p = z + beta p_old, q = L p, alpha = r.z / p.q (+ deferred x-update)
+            if ((rc = launch_cg_passA(ctx, z, P[j & 1], P[(j + 1) & 1], q, d_phi)) != POISSON_OK) return rc;
+            if ((rc = launch_cg_passB(ctx, r, q)) != POISSON_OK) return rc;
+            if ((rc = gs_precond(ctx, r, z, zeros)) != POISSON_OK) return rc;
+            if ((rc = launch_pcg_dot(ctx, r, z)) != POISSON_OK) return rc;
+        }
+        PB_CUDA_OK(cudaGetLastError());
+        if (fixed_iters <= 0) {
+            if ((rc = read_ctl(ctx)) != POISSON_OK) return rc;
+            if (ctx->h_ctl->done) break;
+        }
+    }
+    if ((rc = read_ctl(ctx)) != POISSON_OK) return rc;
+    const KrylovCtl c = *ctx->h_ctl;
+    if ((rc = launch_cg_final(ctx, d_phi, P[c.it & 1])) != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));
+    ctx->hist_len = c.it + 1;
+    if (iters) *iters = c.it;
+    if (relres) *relres = c.rr0 > 0 ? std::sqrt(c.rr / c.rr0) : 0.0;
+    if (c.status == POISSON_NOT_CONVERGED) ctx->err = "PCG: residual threshold not reached within max_iter iterations";
+    return c.status;
 }
 
 // ---- end-to-end with host buffers -----------------------------------------------------------------------------------------

@@ -77,6 +77,8 @@ struct KrylovCtl {
     double r0n2, eps_bd;  // ||r^_0||^2 and the near-breakdown threshold on |rho| / (||r^_0|| ||r||)
     int nconf_failed, pad3;  // true-residual confirmations that failed so far (at most kMaxBicgConfirm)
     int nrestarts, confirm;                 // confirm: the next initial-residual pass re-checks convergence (BiCGSTAB)
+    double rz;                              // preconditioned CG: r . M^-1 r
+    int pcg, pad4;                          // pcg: alpha = rz / p.q and beta = rz_new / rz_old (Saad Alg. 9.1)
 };
 
 struct RedBuf {
@@ -119,9 +121,11 @@ struct poisson_ctx {
     double r_ghost_out = 0;
     double* d_coef = nullptr;       // spherical coefficient arrays, one allocation
     double* d_ctr = nullptr;        // spherical centres + cos/sin tables for the multipole kernels
+    double* d_rj = nullptr;         // local Jacobi radius per (i,j) (Eq. 7) and the omega work array behind it (2 n0 n1)
     double* d_ghost[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     long face_len[6] = {0, 0, 0, 0, 0, 0};
     bool ghost_nonzero = false;
+    int inner_lmax = -1;            // order of the inner multipole moments held in d_scal + 300 (-1: none)
     // scratch vectors (lazily allocated)
     std::vector<double*> vec;
     pb::RedBuf red{nullptr, nullptr};
@@ -245,6 +249,16 @@ int launch_rbsor_pp(poisson_ctx* ctx, const Op& op, double** cur, double* a, dou
 int launch_rbsor_pp32(poisson_ctx* ctx, const Op& op, float** cur, float* a, float* b, const float* rhs, float omega,
                       int nsweeps);
 void* sor_scratch(poisson_ctx* ctx, size_t bytes);  // nullptr on OOM
+int sor_fused_seq(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, const double* omegas,
+                  int nsweeps, bool ug, double** result);
+int sor_fused_precond(poisson_ctx* ctx, const Op& op, const double* zin, double* zout, const double* f, bool symmetric);
+int launch_rbsor_half(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, double omega, int colour,
+                      bool ug, int kid);
+int launch_rbsor_seq(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, const double* omegas,
+                     int nsweeps, bool ug);
+int launch_rbsor_local(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, const double* d_rj,
+                       double* d_om, int nsweeps, int start_n, bool ug);
+int launch_pcg_dot(poisson_ctx* ctx, const double* r, const double* z);
 
 // Lean 7-point apply / residual for non-periodic Cartesian grids (k_apply7.cu), fp64 and fp32
 bool apply7_ok(const poisson_ctx* ctx, const Op& op);
@@ -294,7 +308,7 @@ int mgv_vcycles(poisson_ctx* ctx, double* phi, const double* rhs, int nu1, int n
 void mgv_destroy(poisson_ctx* ctx);
 
 // Multipole
-int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q);
-int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, double G, int lmax);
+int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, bool inner);
+int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, const double* d_qbar, double G, int lmax);
 
 }  // namespace pb

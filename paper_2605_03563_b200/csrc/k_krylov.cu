@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(BX* BY)
     double vals[1] = {acc};
     grid_reduce<1>(vals, rb, [=](const double* t) {
         ctl->pq = t[0];
-        ctl->alpha = ctl->rr / t[0];
+        ctl->alpha = (ctl->pcg ? ctl->rz : ctl->rr) / t[0];
     });
 }
 
@@ -117,11 +117,31 @@ __global__ void __launch_bounds__(256)
             ctl->status = POISSON_OK;
         } else if (ctl->it >= ctl->max_it) {
             ctl->done = 1;
-        } else {
-            ctl->beta = rr_new / ctl->rr;
+        } else if (!ctl->pcg) {
+            ctl->beta = rr_new / ctl->rr;  // preconditioned CG takes beta from r.z after the preconditioner (k_pcg_dot)
         }
         ctl->rr = rr_new;
         ctl->mu = mu;
+    });
+}
+
+// Preconditioned CG (Saad Alg. 9.1): rz = r . z after z = M^-1 r; beta = rz_new / rz_old (0 before the first iteration).
+__global__ void __launch_bounds__(256)
+    k_pcg_dot(size_t n, const double* __restrict__ r, const double* __restrict__ z, KrylovCtl* ctl, RedBuf rb) {
+    if (ctl->done) return;
+    double s = 0.0;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (size_t)gridDim.x * blockDim.x)
+        s = fma(r[p], z[p], s);
+    double vals[1] = {s};
+    grid_reduce<1>(vals, rb, [=](const double* t) {
+        const double rz_new = t[0];
+        if (!isfinite(rz_new) || rz_new == 0.0) {
+            ctl->done = 1;
+            ctl->status = POISSON_BREAKDOWN;
+            return;
+        }
+        ctl->beta = ctl->it == 0 ? 0.0 : rz_new / ctl->rz;
+        ctl->rz = rz_new;
     });
 }
 
@@ -401,6 +421,12 @@ int launch_cg_passA(poisson_ctx* ctx, const double* r, const double* p_old, doub
 int launch_cg_passB(poisson_ctx* ctx, double* r, const double* q) {
     PB_LAUNCH(ctx, KID_CG_PASS_B, (k_cg_passB<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(
                                       ctx->npts, r, q, ctx->d_ctl, ctx->d_hist, ctx->red)));
+    return POISSON_OK;
+}
+
+int launch_pcg_dot(poisson_ctx* ctx, const double* r, const double* z) {
+    PB_LAUNCH(ctx, KID_PCG_PRECOND,
+              (k_pcg_dot<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, r, z, ctx->d_ctl, ctx->red)));
     return POISSON_OK;
 }
 

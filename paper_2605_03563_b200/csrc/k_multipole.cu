@@ -8,6 +8,8 @@
 //   r^l S_l0 = Q_l^0 ;  r^l S_{l,m} = N_lm Q_l^m A_m ;  r^l S_{l,-m} = N_lm Q_l^m B_m ;  N_lm = sqrt(2 (l-m)!/(l+m)!).
 // One fused pass over rho accumulates all (lmax+1)^2 moments per thread in registers, then warp shuffles, a block
 // reduction and a last-block final sum (fixed order -> deterministic).  The pass is fp64-ALU bound at lmax = 8.
+#include <cmath>
+
 #include "stencil.cuh"
 
 namespace pb {
@@ -35,15 +37,24 @@ struct MpGeom {
     double origin[3], h[3];
     // spherical 1-D tables (device): centre radius, sin/cos theta, cos/sin phi, volume factors
     const double *rc, *st, *ct, *cph, *sph_, *vr, *vt, *vp;
-    double r_ghost;
+    double r_ghost, r_ghost_in;
 };
 
 // One point's contribution to all moments, WITHOUT the normalisation N_lm (applied once per thread at the end).
 // Per (l, m): one multiply, one fma and one scaling for the recurrence, one fma (two for m > 0) for the sums; the
 // products (2l-1) z and k r^2 are formed once per point.
-template <int L>
+// INNER: the inner multipoles of Eq. 22, qbar_lm = sum rho r^-(l+1) S_lm dV = sum rho (r^l S_lm) r^-(2l+1) dV — the same
+// solid harmonics with the weight scaled by r^-(2l+1) per degree.
+template <int L, bool INNER>
 __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], double x, double y, double z, double w) {
     const double r2 = fma(z, z, fma(y, y, x * x));
+    double pw[L + 1];  // r^-(2l+1)
+    if (INNER) {
+        const double rinv = 1.0 / sqrt(r2), rinv2 = rinv * rinv;
+        pw[0] = rinv;
+#pragma unroll
+        for (int l = 1; l <= L; ++l) pw[l] = pw[l - 1] * rinv2;
+    }
     double cz[L + 2], kr2[2 * L + 2];
 #pragma unroll
     for (int l = 0; l <= L; ++l) cz[l] = (2 * l - 1) * z;
@@ -63,11 +74,12 @@ __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], dou
                 ql = cz[l] * qm1;
             else
                 ql = fma(cz[l], qm1, -(kr2[l + m - 1] * qm2)) * (1.0 / (l - m));
+            const double qw = INNER ? ql * pw[l] : ql;
             if (m == 0) {
-                acc[l * l + l] = fma(wa, ql, acc[l * l + l]);
+                acc[l * l + l] = fma(wa, qw, acc[l * l + l]);
             } else {
-                acc[l * l + l + m] = fma(wa, ql, acc[l * l + l + m]);
-                acc[l * l + l - m] = fma(wb, ql, acc[l * l + l - m]);
+                acc[l * l + l + m] = fma(wa, qw, acc[l * l + l + m]);
+                acc[l * l + l - m] = fma(wb, qw, acc[l * l + l - m]);
             }
             qm2 = qm1;
             qm1 = ql;
@@ -79,7 +91,7 @@ __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], dou
     }
 }
 
-template <int L>
+template <int L, bool INNER>
 __global__ void __launch_bounds__(256, 1)
     k_moments(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
               double* __restrict__ q_out) {
@@ -112,7 +124,7 @@ __global__ void __launch_bounds__(256, 1)
             z = fma((double)k, g.h[2], g.origin[2]);
             w = d * dV;
         }
-        accumulate<L>(acc, x, y, z, w);
+        accumulate<L, INNER>(acc, x, y, z, w);
     }
 #pragma unroll
     for (int s = 0; s < NQ; ++s) acc[s] *= g.norm[s];  // N_lm, once per thread instead of once per point
@@ -147,12 +159,13 @@ __global__ void __launch_bounds__(256, 1)
 }
 
 // Phi at one exterior point from the moments.
+// inner: Eq. 21, Phi = -G sum qbar_lm r^l S_lm (no inverse powers of r).
 __device__ __forceinline__ double expansion(const double* __restrict__ norm, const double* __restrict__ q, int lmax,
-                                            double G, double x, double y, double z) {
+                                            double G, double x, double y, double z, bool inner) {
     const double r2 = fma(z, z, fma(y, y, x * x));
-    const double rinv = 1.0 / sqrt(r2), rinv2 = rinv * rinv;
+    const double rinv = inner ? 1.0 : 1.0 / sqrt(r2), rinv2 = rinv * rinv;
     double A = 1.0, B = 0.0, dfact = 1.0, acc = 0.0;
-    double pw_m = rinv;  // r^-(2m+1)
+    double pw_m = rinv;  // r^-(2m+1)  (1 for the inner expansion)
     for (int m = 0; m <= lmax; ++m) {
         double qm2 = 0.0, qm1 = dfact, pw = pw_m;  // pw = r^-(2l+1)
         for (int l = m; l <= lmax; ++l) {
@@ -183,7 +196,8 @@ __device__ __forceinline__ double expansion(const double* __restrict__ norm, con
 }
 
 __global__ void __launch_bounds__(256)
-    k_ghost_eval(MpGeom g, int face, int R, const double* __restrict__ q, double G, int lmax, double* __restrict__ out) {
+    k_ghost_eval(MpGeom g, int face, int R, const double* __restrict__ q, double G, int lmax, double* __restrict__ out,
+                 bool inner) {
     const int a = face / 2, a1 = (a == 0) ? 1 : 0, a2 = (a == 2) ? 1 : 2;
     const long len = (long)R * g.n[a1] * g.n[a2];
     const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -191,10 +205,11 @@ __global__ void __launch_bounds__(256)
     const int q1 = (int)(t % g.n[a1]), q2 = (int)((t / g.n[a1]) % g.n[a2]), layer = (int)(t / ((long)g.n[a1] * g.n[a2]));
     double x, y, z;
     if (g.sph) {
-        const double rs = g.r_ghost * g.st[q1];
+        const double rg = inner ? g.r_ghost_in : g.r_ghost;
+        const double rs = rg * g.st[q1];
         x = rs * g.cph[q2];
         y = rs * g.sph_[q2];
-        z = g.r_ghost * g.ct[q1];
+        z = rg * g.ct[q1];
     } else {
         int id[3];
         id[a] = (face & 1) ? g.n[a] + layer : -1 - layer;
@@ -204,7 +219,7 @@ __global__ void __launch_bounds__(256)
         y = fma((double)id[1], g.h[1], g.origin[1]);
         z = fma((double)id[2], g.h[2], g.origin[2]);
     }
-    out[t] = expansion(g.norm, q, lmax, G, x, y, z);
+    out[t] = expansion(g.norm, q, lmax, G, x, y, z, inner);
 }
 
 static MpGeom make_geom(poisson_ctx* ctx) {
@@ -228,16 +243,20 @@ static MpGeom make_geom(poisson_ctx* ctx) {
         g.vt = b + 2 * nr + 2 * nt + 2 * np;
         g.vp = b + 2 * nr + 3 * nt + 2 * np;
         g.r_ghost = ctx->r_ghost_out;
+        g.r_ghost_in = ctx->edges[0][0] * std::sqrt(ctx->edges[0][0] / ctx->edges[0][1]);
     }
     return g;
 }
 
 template <int L>
-static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, double* d_q, int blocks) {
-    k_moments<L><<<blocks, 256, 0, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, double* d_q, int blocks, bool inner) {
+    if (inner)
+        k_moments<L, true><<<blocks, 256, 0, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+    else
+        k_moments<L, false><<<blocks, 256, 0, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
 }
 
-int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
+int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, bool inner) {
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     const MpGeom g = make_geom(ctx);
     int blocks = ctx->num_sms * 2;
@@ -245,15 +264,15 @@ int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
     if ((size_t)blocks > maxb) blocks = (int)maxb;
     pre_launch(ctx, KID_MP_MOMENTS);
     switch (lmax) {
-        case 0: moments_launch<0>(ctx, g, rho, d_q, blocks); break;
-        case 1: moments_launch<1>(ctx, g, rho, d_q, blocks); break;
-        case 2: moments_launch<2>(ctx, g, rho, d_q, blocks); break;
-        case 3: moments_launch<3>(ctx, g, rho, d_q, blocks); break;
-        case 4: moments_launch<4>(ctx, g, rho, d_q, blocks); break;
-        case 5: moments_launch<5>(ctx, g, rho, d_q, blocks); break;
-        case 6: moments_launch<6>(ctx, g, rho, d_q, blocks); break;
-        case 7: moments_launch<7>(ctx, g, rho, d_q, blocks); break;
-        case 8: moments_launch<8>(ctx, g, rho, d_q, blocks); break;
+        case 0: moments_launch<0>(ctx, g, rho, d_q, blocks, inner); break;
+        case 1: moments_launch<1>(ctx, g, rho, d_q, blocks, inner); break;
+        case 2: moments_launch<2>(ctx, g, rho, d_q, blocks, inner); break;
+        case 3: moments_launch<3>(ctx, g, rho, d_q, blocks, inner); break;
+        case 4: moments_launch<4>(ctx, g, rho, d_q, blocks, inner); break;
+        case 5: moments_launch<5>(ctx, g, rho, d_q, blocks, inner); break;
+        case 6: moments_launch<6>(ctx, g, rho, d_q, blocks, inner); break;
+        case 7: moments_launch<7>(ctx, g, rho, d_q, blocks, inner); break;
+        case 8: moments_launch<8>(ctx, g, rho, d_q, blocks, inner); break;
         default: break;  // range checked by the caller
     }
     post_launch(ctx, KID_MP_MOMENTS);
@@ -261,14 +280,17 @@ int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q) {
     return POISSON_OK;
 }
 
-int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, double G, int lmax) {
+// d_qbar: inner moments (Eq. 22), used for the inner radial shell of a spherical grid (face 0) when it is a Dirichlet face.
+int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, const double* d_qbar, double G, int lmax) {
     const MpGeom g = make_geom(ctx);
     for (int f = 0; f < 6; ++f) {
         if (ctx->op.bc[f] != POISSON_BC_DIRICHLET_GHOST || !ctx->d_ghost[f]) continue;
-        if (g.sph && f != 1) continue;  // only the outer radial shell carries Eq. 19
+        if (g.sph && f > 1) continue;  // only the radial shells carry Eq. 19 / Eq. 21
+        const bool inner = g.sph && f == 0;
+        if (inner && !d_qbar) continue;
         const long len = ctx->face_len[f];
         PB_LAUNCH(ctx, KID_MP_GHOSTS, (k_ghost_eval<<<(int)((len + 255) / 256), 256, 0, ctx->stream>>>(
-                                          g, f, ctx->op.R, d_q, G, lmax, ctx->d_ghost[f])));
+                                          g, f, ctx->op.R, inner ? d_qbar : d_q, G, lmax, ctx->d_ghost[f], inner)));
     }
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;

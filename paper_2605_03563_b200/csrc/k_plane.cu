@@ -209,7 +209,7 @@ struct EpCgA {  // stores p_new and q = L p_new, sum p.q -> alpha (the x-update 
     }
     __device__ __forceinline__ void finish(const double* t) const {
         ctl->pq = t[0];
-        ctl->alpha = ctl->rr / t[0];
+        ctl->alpha = (ctl->pcg ? ctl->rz : ctl->rr) / t[0];
     }
 };
 

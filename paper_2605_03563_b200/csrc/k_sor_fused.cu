@@ -129,10 +129,18 @@ struct SorTile {
     static constexpr int MINB = (NT <= 320) ? 2 : 1;  // fp64 needs ~105 registers per thread
 };
 
+// One overrelaxation factor per colour half-step of the pass (constant omega: all equal; the Chebyshev sequence of
+// PAPER.md:81-88 Eq. 6: consecutive members; a factor of 0 turns a half-step into a no-op, which makes the
+// red-black-red symmetric Gauss-Seidel sweep of the CG preconditioner out of a four-half-step pass).
+template <typename T>
+struct OmegaSet {
+    T w[4];
+};
+
 template <typename T, class Cfg, bool PLAIN>
 __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
-    k_sor_fused(const Op op, const T* __restrict__ in, T* __restrict__ out, const T* __restrict__ rhs, const T omega,
-                const bool ug_in, const SorGeom g) {
+    k_sor_fused(const Op op, const T* __restrict__ in, T* __restrict__ out, const T* __restrict__ rhs,
+                const OmegaSet<T> om, const bool ug_in, const SorGeom g) {
     using P2 = typename PairT<T>::type;
     constexpr int NHS = Cfg::NHS, D = Cfg::D, SW = Cfg::SW, SLOT = Cfg::SLOT, PXN = Cfg::PXN, EY = Cfg::EY;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -319,7 +327,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                     }
                     const T s = fma_(zm + zp, c2, sxy[h - 1]);
                     const T gs = div_by<T>(s - f, d, rd);
-                    const T nw = fma_(omega, gs - old, old);
+                    const T nw = fma_(om.w[h - 1], gs - old, old);
                     if (upd) {
                         if (actA) qA[ph] = nw; else qB[ph] = nw;
                         (actA ? mineA : mineB)[((u - h + D) % D) * SLOT] = nw;
@@ -366,8 +374,8 @@ static double sor_cfg_cost(const poisson_ctx* ctx, const Op& op, size_t esize, S
 }
 
 template <typename T, class Cfg>
-static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, T omega, bool ug,
-                          const SorGeom& g, int grid) {
+static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, const OmegaSet<T>& omega,
+                          bool ug, const SorGeom& g, int grid) {
     bool plain = op.gamma == 0.0;
     for (int f = 0; f < 6; ++f) plain = plain && op.bc[f] != POISSON_BC_NEUMANN0;
     const size_t smem = (size_t)Cfg::D * Cfg::SLOT * sizeof(T);
@@ -383,7 +391,8 @@ static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, c
 
 // Tile choice: the compiled configuration with the smallest estimated pass time (POISSON_OPT_TILE_CFG overrides).
 template <typename T, int NHS>
-static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, T omega, bool ug) {
+static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, const OmegaSet<T>& omega,
+                          bool ug) {
     using C0 = SorTile<NHS, 32 + NHS, 14 + 2 * NHS>;   // 64 x 14 valid, 612 threads at NHS = 2 (best at 256^3 on B200)
     using C1 = SorTile<NHS, 16 + NHS, 28 + 2 * NHS>;   // 32 x 28 valid, 576 threads
     using C2 = SorTile<NHS, 16 + NHS, 10 + 2 * NHS>;   // 32 x 10 valid, 252 threads, two CTAs per SM
@@ -415,9 +424,10 @@ bool sor_fused_ok(const poisson_ctx* ctx, const Op& op) {
 }
 
 // nsweeps full sweeps phi -> phi through the ping-pong buffer tmp (same size as phi).
+// omegas == nullptr: the constant `omega`; else 2 nsweeps factors, one per colour half-sweep (red, black, red, ...).
 template <typename T>
 static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* rhs, T omega, int nsweeps, bool ug,
-                       T** result) {
+                       T** result, const double* omegas = nullptr) {
     T *src = phi, *dst = tmp;
     int left = nsweeps;
     // two sweeps per pass (NHS = 4) pay on large grids: fp64 from 2^23 points (122 vs 117 Gpoint/s at 256^3), fp32 from 2^21; 0 = this automatic choice
@@ -428,15 +438,20 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
     // (measured: 2 x NHS=2 beats NHS=4 + copy at 256^3; in fp32 the single pass + copy is the faster one).
     int n4 = two ? nsweeps / 2 : 0;
     if (!result && sizeof(T) == 8 && n4 > 0 && ((n4 + (nsweeps - 2 * n4)) & 1)) --n4;
+    int half = 0;  // colour half-sweeps done so far
     while (left > 0) {
         int rc;
+        OmegaSet<T> os;
+        for (int h = 0; h < 4; ++h) os.w[h] = omegas ? (half + h < 2 * nsweeps ? (T)omegas[half + h] : (T)0) : omega;
         if (n4 > 0) {
             --n4;
-            rc = sor_fused_pass<T, 4>(ctx, op, src, dst, rhs, omega, ug);
+            rc = sor_fused_pass<T, 4>(ctx, op, src, dst, rhs, os, ug);
             left -= 2;
+            half += 4;
         } else {
-            rc = sor_fused_pass<T, 2>(ctx, op, src, dst, rhs, omega, ug);
+            rc = sor_fused_pass<T, 2>(ctx, op, src, dst, rhs, os, ug);
             left -= 1;
+            half += 2;
         }
         if (rc != POISSON_OK) return rc;
         std::swap(src, dst);
@@ -454,6 +469,23 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
 int sor_fused(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, double omega, int nsweeps,
               bool ug, double** result) {
     return sor_fused_t<double>(ctx, op, phi, tmp, rhs, omega, nsweeps, ug, result);
+}
+int sor_fused_seq(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, const double* omegas,
+                  int nsweeps, bool ug, double** result) {
+    return sor_fused_t<double>(ctx, op, phi, tmp, rhs, 1.0, nsweeps, ug, result, omegas);
+}
+// z = (symmetric ? red-black-red : red-black) Gauss-Seidel sweep on L z = f from z = 0 (zin must hold zeros): the
+// multi-colour preconditioner of PAPER.md:107-123 Eq. 10 in ONE pass over HBM.  The result lands in zout.
+int sor_fused_precond(poisson_ctx* ctx, const Op& op, const double* zin, double* zout, const double* f, bool symmetric) {
+    OmegaSet<double> os;
+    os.w[0] = os.w[1] = 1.0;
+    os.w[2] = symmetric ? 1.0 : 0.0;
+    os.w[3] = 0.0;
+    const int rc = symmetric ? sor_fused_pass<double, 4>(ctx, op, zin, zout, f, os, false)
+                             : sor_fused_pass<double, 2>(ctx, op, zin, zout, f, os, false);
+    if (rc != POISSON_OK) return rc;
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
 }
 int sor_fused32(poisson_ctx* ctx, const Op& op, float* phi, float* tmp, const float* rhs, float omega, int nsweeps,
                 float** result) {

@@ -65,6 +65,34 @@ __global__ void __launch_bounds__(BX* BY)
     }
 }
 
+// The same half-sweep with a position-dependent factor omega(i,j) (Eq. 7: "the values of omega_n are not
+// uniform, but depend on position on the grid"); om holds the current member of the sequence of Eq. 6 per (i,j).
+template <typename T, int KIND>
+__global__ void __launch_bounds__(BX* BY)
+    k_rbsor_half_local(Op op, T* phi, const T* __restrict__ rhs, const double* __restrict__ om, int colour, bool ug, int kc) {
+    const int ti = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    if (j >= op.n[1]) return;
+    for (int k = k0; k < k1; ++k) {
+        const int i = 2 * ti + ((j + k + colour) & 1);
+        if (i >= op.n[0]) continue;
+        const size_t p = gidx(op, i, j, k);
+        const T s = row_offsum<T, KIND>(op, ArrLd<T>{phi}, i, j, k, ug);
+        const T d = row_diag<T, KIND>(op, i, j, k);
+        const T gs = (s - rhs[p]) / d;
+        const T old = phi[p];
+        phi[p] = fma_((T)om[(size_t)j * op.n[0] + i], gs - old, old);
+    }
+}
+
+// Eq. 6 advanced by one member per (i,j): omega_0 = 1, omega_1 = 1/(1 - rJ^2/2), omega_{n+1} = 1/(1 - rJ^2 omega_n/4).
+__global__ void __launch_bounds__(256) k_omega_advance(size_t n, const double* __restrict__ rj, double* __restrict__ om, int n_next) {
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n) return;
+    const double r = rj[q];
+    om[q] = n_next == 0 ? 1.0 : (n_next == 1 ? 1.0 / (1.0 - 0.5 * r * r) : 1.0 / (1.0 - 0.25 * r * r * om[q]));
+}
+
 static dim3 grid_for(const Op& op, int kc, bool half_x) {
     const int nxe = half_x ? (op.n[0] + 1) / 2 : op.n[0];
     return dim3((nxe + BX - 1) / BX, (op.n[1] + BY - 1) / BY, (op.n[2] + kc - 1) / kc);
@@ -127,6 +155,58 @@ static int rbsor_dispatch(poisson_ctx* ctx, const Op& op, T* phi, const T* rhs, 
         for (int colour = 0; colour < 2; ++colour) {
             PB_LAUNCH(ctx, KID_RBSOR, (k_rbsor_half<T, KIND><<<g, b, 0, ctx->stream>>>(op, phi, rhs, omega, colour, ug, kc)));
         }
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+// One colour half-sweep with the generic kernel (building block of the preconditioner and of the omega sequences).
+int launch_rbsor_half(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, double omega, int colour,
+                      bool ug, int kid) {
+    if (kind == KIND_CART6)
+        return fail(ctx, POISSON_UNSUPPORTED, "red-black sweeps need a radius-1 stencil (two colours, PAPER.md:61)");
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc, true), b(BX, BY);
+    if (kind == KIND_CART2)
+        PB_LAUNCH(ctx, kid, (k_rbsor_half<double, KIND_CART2><<<g, b, 0, ctx->stream>>>(op, phi, rhs, omega, colour, ug, kc)));
+    else
+        PB_LAUNCH(ctx, kid, (k_rbsor_half<double, KIND_SPH><<<g, b, 0, ctx->stream>>>(op, phi, rhs, omega, colour, ug, kc)));
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+// nsweeps sweeps with one factor per colour half-sweep: omegas[0 .. 2 nsweeps) (Eq. 6).
+int launch_rbsor_seq(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, const double* omegas,
+                     int nsweeps, bool ug) {
+    if (kind == KIND_CART2 && nsweeps > 0 && sor_fused_ok(ctx, op)) {
+        double* tmp = (double*)sor_scratch(ctx, (size_t)op.n[0] * op.n[1] * op.n[2] * sizeof(double));
+        if (!tmp) return POISSON_OUT_OF_MEMORY;
+        return sor_fused_seq(ctx, op, phi, tmp, rhs, omegas, nsweeps, ug, nullptr);
+    }
+    for (int m = 0; m < 2 * nsweeps; ++m) {
+        const int rc = launch_rbsor_half(ctx, op, kind, phi, rhs, omegas[m], m & 1, ug, KID_RBSOR);
+        if (rc != POISSON_OK) return rc;
+    }
+    return POISSON_OK;
+}
+
+// nsweeps sweeps with the position-dependent sequence: d_rj = local Jacobi radius per (i,j), d_om = work array.
+int launch_rbsor_local(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, const double* d_rj,
+                       double* d_om, int nsweeps, int start_n, bool ug) {
+    if (kind == KIND_CART6)
+        return fail(ctx, POISSON_UNSUPPORTED, "red-black sweeps need a radius-1 stencil (two colours, PAPER.md:61)");
+    const size_t n2d = (size_t)op.n[0] * op.n[1];
+    const int ob = (int)((n2d + 255) / 256);
+    for (int n = 0; n <= start_n; ++n)
+        PB_LAUNCH(ctx, KID_RBSOR, (k_omega_advance<<<ob, 256, 0, ctx->stream>>>(n2d, d_rj, d_om, n)));
+    const int kc = pick_kc(op, ctx->num_sms);
+    const dim3 g = grid_for(op, kc, true), b(BX, BY);
+    for (int m = 0; m < 2 * nsweeps; ++m) {
+        if (kind == KIND_CART2)
+            PB_LAUNCH(ctx, KID_RBSOR, (k_rbsor_half_local<double, KIND_CART2><<<g, b, 0, ctx->stream>>>(op, phi, rhs, d_om, m & 1, ug, kc)));
+        else
+            PB_LAUNCH(ctx, KID_RBSOR, (k_rbsor_half_local<double, KIND_SPH><<<g, b, 0, ctx->stream>>>(op, phi, rhs, d_om, m & 1, ug, kc)));
+        PB_LAUNCH(ctx, KID_RBSOR, (k_omega_advance<<<ob, 256, 0, ctx->stream>>>(n2d, d_rj, d_om, m + start_n + 1)));
+    }
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
