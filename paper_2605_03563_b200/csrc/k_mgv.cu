@@ -10,12 +10,14 @@
 // (centre | face | edge | corner), formed on the device from the definition R A P.
 //
 // Hot kernel k_spai: one pass over HBM per smoothing step (read x, b; write x: 24 B/point in fp64, 12 in fp32 storage).
-// A CTA of NTX x NTY threads owns the xy tile of residual points (output tile + 1 halo) and marches z.  Both
-// 27-point applications are evaluated from per-plane partial sums kept in registers along z,
+// A CTA of 32 x NTY threads owns an xy tile of 32 x (NTY RY) residual points (output tile + 1 halo) and marches z; a
+// thread owns RY consecutive rows of one column.  Both 27-point applications are evaluated from in-plane sums,
 //   Q0 = v(c), Q1 = sum of the 4 in-plane face neighbours, Q2 = sum of the 4 in-plane diagonal neighbours,
-//   (S v)(k) = s0 Q0(k) + s1 [Q1(k) + Q0(k-1) + Q0(k+1)] + s2 [Q2(k) + Q1(k-1) + Q1(k+1)] + s3 [Q2(k-1) + Q2(k+1)],
-// so only ONE plane of x and ONE plane of r is shared at a time (double-buffered, two barriers per plane) and a
-// point costs 9 + 9 shared-memory loads instead of 27 + 27.
+//   (S v)(k) = C(k) + U(k-1) + U(k+1),  C = s0 Q0 + s1 Q1 + s2 Q2,  U = s1 Q0 + s2 Q1 + s3 Q2,
+// so a plane contributes to three output planes through two numbers per point, the running sums live in registers
+// along z (two doubles per point and operator), only ONE plane of x and ONE plane of r is shared at a time
+// (double-buffered, two barriers per plane), and the in-plane sums of the RY rows share their row loads:
+// 3 (RY + 2) / RY shared-memory loads per point and operator instead of 27.
 #include <algorithm>
 #include <functional>
 
@@ -25,116 +27,224 @@ namespace pb {
 
 namespace mgv {
 
-constexpr int NTX = 32, NTY = 16;          // threads = residual tile; output tile (NTX-2) x (NTY-2)
-constexpr int VX = NTX - 2, VY = NTY - 2;
-constexpr int XW = NTX + 2, XH = NTY + 2;  // x plane with its halo
-constexpr int NHALO = 2 * XW + 2 * NTY;    // ring of x points around the residual tile
+constexpr int NTX = 32, NTY = 8, RY = 2;   // threads; rows per thread (measured at 255^3 / 511^3: 8x2 0.62 / 4.16 ms per 4 steps; 4x4 0.77 / 5.11; 16x1 0.77 / 5.25; 16x2 0.70 / 4.73)
+constexpr int TY = NTY * RY;               // residual tile NTX x TY; output tile (NTX-2) x (TY-2)
+constexpr int VX = NTX - 2, VY = TY - 2;
+constexpr int XW = NTX + 2, XH = TY + 2;   // x plane with its halo (and the r plane with an unused zero border)
+constexpr int NHALO = 2 * XW + 2 * TY;     // ring of x points around the residual tile
+constexpr int NT = NTX * NTY;
 
 template <typename S>
 __device__ __forceinline__ double ldv(const S* p) { return (double)*p; }
-
-struct Sten {  // symmetric 27-point stencil: centre, face, edge, corner
-    double s0, s1, s2, s3;
-};
 
 struct Plan {
     int n0, n1, n2;
     int ntx, nty, nz, kc;  // tiles and z chunks
 };
 
+constexpr int NS = 5, PD = 3;  // planes in the staging rings; loads run PD planes ahead (a slot is reused NS - PD = 2 barriers later)
+
+// 4- or 8-byte asynchronous copy global -> shared (LDGSTS); `ok` false zero-fills the destination instead.
+template <typename S>
+__device__ __forceinline__ void cp_async_fast(unsigned d, const void* gsrc) {  // d: shared-window address
+    if constexpr (sizeof(S) == 8)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+template <typename S>
+__device__ __forceinline__ void cp_async(S* smem_dst, const S* gsrc, bool ok) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    const int nbytes = ok ? (int)sizeof(S) : 0;
+    if constexpr (sizeof(S) == 8)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(nbytes) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(d), "l"(gsrc), "r"(nbytes) : "memory");
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// In-plane sums of the RY owned rows from a shared plane (row pitch XW): rows row0 .. row0+RY+1, columns tx .. tx+2.
+template <typename S>
+__device__ __forceinline__ void plane_sums(const S* pl, int tx, int row0, double (&q0)[RY], double (&q1)[RY],
+                                           double (&q2)[RY], bool want_q2) {
+    double h[RY + 2], c[RY + 2];
+#pragma unroll
+    for (int w = 0; w < RY + 2; ++w) {
+        const S* rowp = pl + (row0 + w) * XW;
+        c[w] = (double)rowp[tx + 1];
+        h[w] = (double)rowp[tx] + (double)rowp[tx + 2];
+    }
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        q0[r] = c[r + 1];
+        q1[r] = h[r + 1] + (c[r] + c[r + 2]);
+        q2[r] = want_q2 ? h[r] + h[r + 2] : 0.0;
+    }
+}
+
+template <typename SX, typename SB>
+constexpr size_t spai_smem() {
+    return (size_t)NS * XH * XW * sizeof(SX) + (size_t)NS * TY * NTX * sizeof(SB) + (size_t)2 * XH * XW * sizeof(double);
+}
+
 // MODE 0: out = x + omega M (bsign b - A x)      (one SPAI step, Eq. 15)
 // MODE 1: out = bsign b - A x                    (residual, for the restriction)
 // SEVEN: A has no edge / corner coefficients (level 0: the 7-point operator).
+// Planes of x (with halo) and b are staged by asynchronous copies PD planes ahead of their use: no staging registers,
+// PD planes of loads in flight per CTA.
 template <typename SX, typename SB, typename SO, int MODE, bool SEVEN>
-__global__ void __launch_bounds__(NTX* NTY)
+__global__ void __launch_bounds__(NT)
     k_spai(const Plan pl, const SX* __restrict__ x, const SB* __restrict__ b, SO* __restrict__ out,
            const double* __restrict__ a4 /* A: centre, face, edge, corner */, const double bsign, const double omega,
            const double m0, const double m1, const double m2, const double m3) {
-    __shared__ double xs[2][XH][XW];
-    __shared__ double rs[2][NTY][NTX];
+    extern __shared__ __align__(16) unsigned char smraw[];
+    double* const rs = reinterpret_cast<double*>(smraw);                       // [2][XH][XW]
+    SX* const xs = reinterpret_cast<SX*>(rs + 2 * XH * XW);                    // [NS][XH][XW]
+    SB* const bs = reinterpret_cast<SB*>(xs + NS * XH * XW);                   // [NS][TY][NTX]
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * NTX + tx;
     const int tile = blockIdx.x % (pl.ntx * pl.nty), zc = blockIdx.x / (pl.ntx * pl.nty);
     const int i0 = (tile % pl.ntx) * VX, j0 = (tile / pl.ntx) * VY;
     const int k0 = zc * pl.kc, k1 = min(pl.n2, k0 + pl.kc);
     const int n0 = pl.n0, n1 = pl.n1, n2 = pl.n2;
-    const int i = i0 - 1 + tx, j = j0 - 1 + ty;  // this thread's residual point
-    const bool in = i >= 0 && i < n0 && j >= 0 && j < n1;
-    const bool owner = in && tx >= 1 && tx <= VX && ty >= 1 && ty <= VY;
+    const int i = i0 - 1 + tx, jb = j0 - 1 + ty * RY;  // this thread's residual points: (i, jb + r)
     const size_t plane = (size_t)n0 * n1;
-    const size_t col = in ? (size_t)j * n0 + i : 0;
+    bool in[RY], owner[RY];
+    size_t col[RY];
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        const int j = jb + r, row = ty * RY + r;
+        in[r] = i >= 0 && i < n0 && j >= 0 && j < n1;
+        owner[r] = in[r] && tx >= 1 && tx <= VX && row >= 1 && row <= VY;
+        col[r] = in[r] ? (size_t)j * n0 + i : 0;
+    }
     // this thread's halo point of the x plane (ring around the residual tile), if any
     int hx = -1, hy = -1;
     if (tid < NHALO) {
         if (tid < XW) { hx = tid; hy = 0; }
         else if (tid < 2 * XW) { hx = tid - XW; hy = XH - 1; }
-        else if (tid < 2 * XW + NTY) { hx = 0; hy = 1 + tid - 2 * XW; }
-        else { hx = XW - 1; hy = 1 + tid - 2 * XW - NTY; }
+        else if (tid < 2 * XW + TY) { hx = 0; hy = 1 + tid - 2 * XW; }
+        else { hx = XW - 1; hy = 1 + tid - 2 * XW - TY; }
     }
     const int hi = i0 - 2 + hx, hj = j0 - 2 + hy;
     const bool hin = hx >= 0 && hi >= 0 && hi < n0 && hj >= 0 && hj < n1;
     const size_t hcol = hin ? (size_t)hj * n0 + hi : 0;
     const double s0 = a4[0], s1 = a4[1], s2 = SEVEN ? 0.0 : a4[2], s3 = SEVEN ? 0.0 : a4[3];
+    for (int e = tid; e < 2 * XH * XW; e += NT) rs[e] = 0.0;  // the border of the r planes stays zero
 
-    double q0m = 0, q1m = 0, q2m = 0, q0c = 0, q1c = 0, q2c = 0;  // x partial sums of planes kx-2, kx-1
-    double p0m = 0, p1m = 0, p2m = 0, p0c = 0, p1c = 0, p2c = 0;  // r partial sums of planes kx-3, kx-2
-    // software pipeline: the values of plane kx are loaded one iteration before they are shared
-    auto ldx = [&](int kk, bool ok, size_t c) -> double {
-        return (ok && kk >= 0 && kk < n2) ? ldv(x + (size_t)kk * plane + c) : 0.0;
-    };
-    auto ldb = [&](int kk) -> double { return (in && kk >= 0 && kk < n2) ? bsign * ldv(b + (size_t)kk * plane + col) : 0.0; };
+    // stage x plane kk (own points + halo ring) and b plane kk-1 (consumed in the same iteration) into ring slot
+    // `slot` (= kk mod NS); planes outside the grid and points outside the domain are zero-filled.  One commit group
+    // per call, always (uniform group counting).  The slot written in iteration kx was last read in iteration kx-2:
+    // the barrier of iteration kx-1 lies in between.  Tiles whose points (halo ring included) all lie in the domain
+    // take a path without per-copy predicates when both planes exist.
+    bool tile_inside = hx < 0 || hin;
+#pragma unroll
+    for (int r = 0; r < RY; ++r) tile_inside = tile_inside && in[r];
+    tile_inside = __syncthreads_and(tile_inside);
+    SX* const xown = xs + (ty * RY + 1) * XW + tx + 1;
+    SB* const bown = bs + (ty * RY) * NTX + tx;
+    SX* const xhal = xs + (hx >= 0 ? hy * XW + hx : 0);
+    // fast path state: shared-window addresses of slot 0 and running global pointers of the next plane to stage
+    const unsigned sx0 = (unsigned)__cvta_generic_to_shared(xown), sb0 = (unsigned)__cvta_generic_to_shared(bown),
+                   sh0 = (unsigned)__cvta_generic_to_shared(xhal);
     const int kx0 = (MODE == 0 ? k0 - 2 : k0 - 1);
-    double xn = ldx(kx0, in, col), hn = ldx(kx0, hin, hcol), bn = ldb(kx0 - 1);
-    for (int kx = kx0; kx <= k1 + (MODE == 0 ? 1 : 0); ++kx) {
-        const int par = kx & 1;
-        xs[par][ty + 1][tx + 1] = xn;
-        if (hx >= 0) xs[par][hy][hx] = hn;
-        const double bcur = bn;  // b of plane kx-1
-        xn = ldx(kx + 1, in, col);
-        hn = ldx(kx + 1, hin, hcol);
-        bn = ldb(kx);
-        __syncthreads();
-        // partial sums of x plane kx at this thread's residual point
-        const double q0p = xs[par][ty + 1][tx + 1];
-        const double q1p = (xs[par][ty + 1][tx] + xs[par][ty + 1][tx + 2]) + (xs[par][ty][tx + 1] + xs[par][ty + 2][tx + 1]);
-        double q2p = 0.0;
-        if (!SEVEN) q2p = (xs[par][ty][tx] + xs[par][ty][tx + 2]) + (xs[par][ty + 2][tx] + xs[par][ty + 2][tx + 2]);
-        // residual of plane kx-1 (zero outside the domain: Dirichlet vertices carry no residual)
-        const int kr = kx - 1;
-        double r = 0.0;
-        if (in && kr >= 0 && kr < n2) {
-            double ax = s0 * q0c;
-            ax = fma(s1, q1c + (q0m + q0p), ax);
-            if (!SEVEN) {
-                ax = fma(s2, q2c + (q1m + q1p), ax);
-                ax = fma(s3, q2m + q2p, ax);
+    const char* gx = reinterpret_cast<const char*>(x) + ((ptrdiff_t)kx0 * (ptrdiff_t)plane + (ptrdiff_t)col[0]) * (ptrdiff_t)sizeof(SX);
+    const char* gh = reinterpret_cast<const char*>(x) + ((ptrdiff_t)kx0 * (ptrdiff_t)plane + (ptrdiff_t)hcol) * (ptrdiff_t)sizeof(SX);
+    const char* gb = reinterpret_cast<const char*>(b) + ((ptrdiff_t)(kx0 - 1) * (ptrdiff_t)plane + (ptrdiff_t)col[0]) * (ptrdiff_t)sizeof(SB);
+    const size_t pbx = plane * sizeof(SX), pbb = plane * sizeof(SB), rbx = (size_t)n0 * sizeof(SX), rbb = (size_t)n0 * sizeof(SB);
+    // stage(kk, slot) must be called for consecutive kk starting at kx0 (the running pointers advance by one plane)
+    auto stage = [&](int kk, int slot) {
+        const bool kin = kk >= 0 && kk < n2, kbin = kk - 1 >= 0 && kk - 1 < n2;
+        if (tile_inside && kin && kbin) {
+            const unsigned ox = slot * (unsigned)(XH * XW * sizeof(SX)), ob = slot * (unsigned)(TY * NTX * sizeof(SB));
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                cp_async_fast<SX>(sx0 + ox + r * (unsigned)(XW * sizeof(SX)), gx + r * rbx);
+                cp_async_fast<SB>(sb0 + ob + r * (unsigned)(NTX * sizeof(SB)), gb + r * rbb);
             }
-            r = bcur - ax;
+            if (hx >= 0) cp_async_fast<SX>(sh0 + ox, gh);
+        } else {
+            SX* const xp = xown + slot * (XH * XW);
+            SB* const bp = bown + slot * (TY * NTX);
+            const size_t off = kin ? (size_t)kk * plane : 0, offb = kbin ? (size_t)(kk - 1) * plane : 0;
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                cp_async(xp + r * XW, x + off + col[r], kin && in[r]);
+                cp_async(bp + r * NTX, b + offb + col[r], kbin && in[r]);
+            }
+            if (hx >= 0) cp_async(xhal + slot * (XH * XW), x + off + hcol, kin && hin);
+        }
+        gx += pbx;
+        gh += pbx;
+        gb += pbb;
+        cp_commit();
+    };
+
+    double accA[RY], uA[RY], accM[RY], uM[RY], x1[RY], x2[RY];  // running sums along z; x of planes kx-1, kx-2
+#pragma unroll
+    for (int r = 0; r < RY; ++r) accA[r] = uA[r] = accM[r] = uM[r] = x1[r] = x2[r] = 0.0;
+    const int kx_end = k1 + (MODE == 0 ? 1 : 0);
+#pragma unroll
+    for (int d = 0; d < PD; ++d) stage(kx0 + d, d);
+    int slot = 0, slot_pd = PD;  // ring slots of planes kx and kx + PD
+    size_t oo = (size_t)(kx0 - (MODE == 0 ? 2 : 1)) * plane;  // offset of the plane written in this iteration
+    for (int kx = kx0; kx <= kx_end; ++kx, oo += plane) {
+        stage(kx + PD, slot_pd);
+        cp_wait<PD>();   // everything up to plane kx has landed (this thread's copies)
+        __syncthreads();  // ... and everybody else's
+        const SX* const xp = xs + slot * (XH * XW);
+        const SB* const bp = bs + slot * (TY * NTX);
+        slot = slot + 1 == NS ? 0 : slot + 1;
+        slot_pd = slot_pd + 1 == NS ? 0 : slot_pd + 1;
+        const int par = kx & 1;
+        double q0[RY], q1[RY], q2[RY], rv[RY];
+        plane_sums<SX>(xp, tx, ty * RY, q0, q1, q2, !SEVEN);
+        const int kr = kx - 1;
+        const bool krin = kr >= 0 && kr < n2;
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            // residual of plane kx-1 (zero outside the domain: Dirichlet vertices carry no residual)
+            double u = s1 * q0[r], c = fma(s1, q1[r], s0 * q0[r]);
+            if (!SEVEN) {
+                u = fma(s3, q2[r], fma(s2, q1[r], u));
+                c = fma(s2, q2[r], c);
+            }
+            const double ax = accA[r] + u;  // C(kx-1) + U(kx-2) + U(kx)
+            accA[r] = c + uA[r];
+            uA[r] = u;
+            rv[r] = (in[r] && krin) ? bsign * (double)bp[(ty * RY + r) * NTX + tx] - ax : 0.0;
         }
         if (MODE == 1) {
-            if (owner && kr >= k0 && kr < k1) out[(size_t)kr * plane + col] = (SO)r;
+#pragma unroll
+            for (int r = 0; r < RY; ++r)
+                if (owner[r] && kr >= k0 && kr < k1) out[oo + col[r]] = (SO)rv[r];
         } else {
-            rs[par][ty][tx] = r;
+            double* const rp = rs + par * (XH * XW);
+#pragma unroll
+            for (int r = 0; r < RY; ++r) rp[(ty * RY + r + 1) * XW + tx + 1] = rv[r];
             __syncthreads();
-            if (owner) {  // only owners have all their in-plane neighbours inside the tile
-                const double p0p = r;
-                const double p1p = (rs[par][ty][tx - 1] + rs[par][ty][tx + 1]) + (rs[par][ty - 1][tx] + rs[par][ty + 1][tx]);
-                const double p2p = (rs[par][ty - 1][tx - 1] + rs[par][ty - 1][tx + 1]) +
-                                   (rs[par][ty + 1][tx - 1] + rs[par][ty + 1][tx + 1]);
-                const int ko = kx - 2;
-                if (ko >= k0 && ko < k1) {
-                    double mr = m0 * p0c;
-                    mr = fma(m1, p1c + (p0m + p0p), mr);
-                    mr = fma(m2, p2c + (p1m + p1p), mr);
-                    mr = fma(m3, p2m + p2p, mr);
-                    out[(size_t)ko * plane + col] = (SO)fma(omega, mr, q0m);  // q0m = x of plane kx-2
-                }
-                p0m = p0c; p1m = p1c; p2m = p2c;
-                p0c = p0p; p1c = p1p; p2c = p2p;
+            double p0[RY], p1[RY], p2[RY];
+            plane_sums<double>(rp, tx, ty * RY, p0, p1, p2, true);
+            const int ko = kx - 2;
+            const bool koin = ko >= k0 && ko < k1;
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                const double u = fma(m3, p2[r], fma(m2, p1[r], m1 * p0[r]));
+                const double c = fma(m2, p2[r], fma(m1, p1[r], m0 * p0[r]));
+                const double mr = accM[r] + u;  // (M r)(kx-2)
+                accM[r] = c + uM[r];
+                uM[r] = u;
+                if (owner[r] && koin) out[oo + col[r]] = (SO)fma(omega, mr, x2[r]);
             }
         }
-        q0m = q0c; q1m = q1c; q2m = q2c;
-        q0c = q0p; q1c = q1p; q2c = q2p;
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            x2[r] = x1[r];
+            x1[r] = q0[r];
+        }
     }
+    cp_wait<0>();
 }
 
 // b_c = R r (Eq. 13): coarse vertex I sits on fine vertex 2I+1; all 27 fine points are interior.
@@ -283,35 +393,54 @@ __global__ void __launch_bounds__(512)
 // ---- host side ---------------------------------------------------------------------------------------------------------
 using mgv::Plan;
 
-static Plan make_plan(const poisson_ctx* ctx, const int n[3]) {
+// z chunks: the number of chunks that minimises (waves of resident CTAs) x (planes marched per CTA, 4 lead-in planes
+// included) — a partly filled last wave costs as much as a full one.
+static Plan make_plan(const poisson_ctx* ctx, const int n[3], int resident) {
     Plan pl;
     pl.n0 = n[0];
     pl.n1 = n[1];
     pl.n2 = n[2];
     pl.ntx = (n[0] + mgv::VX - 1) / mgv::VX;
     pl.nty = (n[1] + mgv::VY - 1) / mgv::VY;
-    // z chunks: enough CTAs for ~3 waves of 4 resident CTAs per SM, chunks of at least 16 planes (4 lead-in planes each)
-    const long tiles = (long)pl.ntx * pl.nty, want = 12L * ctx->num_sms;
-    int nz = (int)std::max(1L, std::min((long)std::max(1, n[2] / 16), (want + tiles - 1) / tiles));
-    pl.kc = (n[2] + nz - 1) / nz;
-    pl.nz = (n[2] + pl.kc - 1) / pl.kc;
+    const long tiles = (long)pl.ntx * pl.nty, slots = (long)ctx->num_sms * std::max(1, resident);
+    double best = 1e300;
+    pl.kc = n[2];
+    pl.nz = 1;
+    for (int nz = 1; nz <= std::max(1, n[2] / 8); ++nz) {
+        const int kc = (n[2] + nz - 1) / nz, nzz = (n[2] + kc - 1) / kc;
+        const double cost = (double)((tiles * nzz + slots - 1) / slots) * (kc + 4 + 2);
+        if (cost < best - 1e-9) {
+            best = cost;
+            pl.kc = kc;
+            pl.nz = nzz;
+        }
+    }
     return pl;
+}
+
+template <typename SX, typename SB, typename SO, int MODE, bool SEVEN>
+static int spai_launch_k(poisson_ctx* ctx, int kid, const int n[3], const SX* x, const SB* b, SO* out, const double* a4,
+                         double bsign, const double spai[5], double h) {
+    auto kern = mgv::k_spai<SX, SB, SO, MODE, SEVEN>;
+    constexpr size_t smem = mgv::spai_smem<SX, SB>();
+    int resident = 0;
+    const int rc = kernel_ready(ctx, kern, mgv::NT, smem, &resident);
+    if (rc != POISSON_OK) return rc;
+    const Plan pl = make_plan(ctx, n, resident);
+    const dim3 blk(mgv::NTX, mgv::NTY), grid((unsigned)(pl.ntx * pl.nty * pl.nz));
+    const double h2 = h * h, om = spai ? spai[0] : 0.0;
+    const double m0 = spai ? spai[1] * h2 : 0, m1 = spai ? spai[2] * h2 : 0, m2 = spai ? spai[3] * h2 : 0,
+                 m3 = spai ? spai[4] * h2 : 0;
+    PB_LAUNCH(ctx, kid, (kern<<<grid, blk, smem, ctx->stream>>>(pl, x, b, out, a4, bsign, om, m0, m1, m2, m3)));
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
 }
 
 template <typename SX, typename SB, typename SO, int MODE>
 static int spai_launch(poisson_ctx* ctx, int kid, const int n[3], bool seven, const SX* x, const SB* b, SO* out,
                        const double* a4, double bsign, const double spai[5], double h) {
-    const Plan pl = make_plan(ctx, n);
-    const dim3 blk(mgv::NTX, mgv::NTY), grid((unsigned)(pl.ntx * pl.nty * pl.nz));
-    const double h2 = h * h, om = spai ? spai[0] : 0.0;
-    const double m0 = spai ? spai[1] * h2 : 0, m1 = spai ? spai[2] * h2 : 0, m2 = spai ? spai[3] * h2 : 0,
-                 m3 = spai ? spai[4] * h2 : 0;
-    if (seven)
-        PB_LAUNCH(ctx, kid, (mgv::k_spai<SX, SB, SO, MODE, true><<<grid, blk, 0, ctx->stream>>>(pl, x, b, out, a4, bsign, om, m0, m1, m2, m3)));
-    else
-        PB_LAUNCH(ctx, kid, (mgv::k_spai<SX, SB, SO, MODE, false><<<grid, blk, 0, ctx->stream>>>(pl, x, b, out, a4, bsign, om, m0, m1, m2, m3)));
-    PB_CUDA_OK(cudaGetLastError());
-    return POISSON_OK;
+    if (seven) return spai_launch_k<SX, SB, SO, MODE, true>(ctx, kid, n, x, b, out, a4, bsign, spai, h);
+    return spai_launch_k<SX, SB, SO, MODE, false>(ctx, kid, n, x, b, out, a4, bsign, spai, h);
 }
 
 // Level bookkeeping lives in the handle (common.cuh MgvLevel); built lazily, rebuilt when the parameters change.
