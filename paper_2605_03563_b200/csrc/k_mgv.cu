@@ -39,7 +39,8 @@ __device__ __forceinline__ double ldv(const S* p) { return (double)*p; }
 
 struct Plan {
     int n0, n1, n2;
-    int ntx, nty, nz, kc;  // tiles and z chunks
+    int ntx, nty, nz, kc;  // tiles and z chunks (MODE 2: chunks of kc COARSE planes)
+    int nc0, nc1, nc2;     // MODE 2: the coarse grid
 };
 
 constexpr int NS = 5, PD = 3;  // planes in the staging rings; loads run PD planes ahead (a slot is reused NS - PD = 2 barriers later)
@@ -90,7 +91,10 @@ constexpr size_t spai_smem() {
 }
 
 // MODE 0: out = x + omega M (bsign b - A x)      (one SPAI step, Eq. 15)
-// MODE 1: out = bsign b - A x                    (residual, for the restriction)
+// MODE 1: out = bsign b - A x                    (residual)
+// MODE 2: out = R (bsign b - A x) on the coarse grid (residual + full weighting Eq. 13 in one pass: the fine residual
+//         never goes to memory; the in-plane part of R is the same partial sums, W = P0/4 + P1/8 + P2/16 at the fine
+//         vertices that carry a coarse vertex, and b_c(K) = W(2K)/4 + W(2K+1)/2 + W(2K+2)/4 is a running sum along z)
 // SEVEN: A has no edge / corner coefficients (level 0: the 7-point operator).
 // Planes of x (with halo) and b are staged by asynchronous copies PD planes ahead of their use: no staging registers,
 // PD planes of loads in flight per CTA.
@@ -106,7 +110,10 @@ __global__ void __launch_bounds__(NT)
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * NTX + tx;
     const int tile = blockIdx.x % (pl.ntx * pl.nty), zc = blockIdx.x / (pl.ntx * pl.nty);
     const int i0 = (tile % pl.ntx) * VX, j0 = (tile / pl.ntx) * VY;
-    const int k0 = zc * pl.kc, k1 = min(pl.n2, k0 + pl.kc);
+    // output planes [k0, k1): fine planes (MODE 0, 1) or coarse planes (MODE 2); r planes needed: [kr_first, kr_last]
+    const int k0 = zc * pl.kc, k1 = min(MODE == 2 ? pl.nc2 : pl.n2, k0 + pl.kc);
+    const int kr_first = MODE == 0 ? k0 - 1 : (MODE == 1 ? k0 : 2 * k0);
+    const int kr_last = MODE == 0 ? k1 : (MODE == 1 ? k1 - 1 : 2 * k1);
     const int n0 = pl.n0, n1 = pl.n1, n2 = pl.n2;
     const int i = i0 - 1 + tx, jb = j0 - 1 + ty * RY;  // this thread's residual points: (i, jb + r)
     const size_t plane = (size_t)n0 * n1;
@@ -148,7 +155,7 @@ __global__ void __launch_bounds__(NT)
     // fast path state: shared-window addresses of slot 0 and running global pointers of the next plane to stage
     const unsigned sx0 = (unsigned)__cvta_generic_to_shared(xown), sb0 = (unsigned)__cvta_generic_to_shared(bown),
                    sh0 = (unsigned)__cvta_generic_to_shared(xhal);
-    const int kx0 = (MODE == 0 ? k0 - 2 : k0 - 1);
+    const int kx0 = kr_first - 1;
     const char* gx = reinterpret_cast<const char*>(x) + ((ptrdiff_t)kx0 * (ptrdiff_t)plane + (ptrdiff_t)col[0]) * (ptrdiff_t)sizeof(SX);
     const char* gh = reinterpret_cast<const char*>(x) + ((ptrdiff_t)kx0 * (ptrdiff_t)plane + (ptrdiff_t)hcol) * (ptrdiff_t)sizeof(SX);
     const char* gb = reinterpret_cast<const char*>(b) + ((ptrdiff_t)(kx0 - 1) * (ptrdiff_t)plane + (ptrdiff_t)col[0]) * (ptrdiff_t)sizeof(SB);
@@ -184,11 +191,14 @@ __global__ void __launch_bounds__(NT)
     double accA[RY], uA[RY], accM[RY], uM[RY], x1[RY], x2[RY];  // running sums along z; x of planes kx-1, kx-2
 #pragma unroll
     for (int r = 0; r < RY; ++r) accA[r] = uA[r] = accM[r] = uM[r] = x1[r] = x2[r] = 0.0;
-    const int kx_end = k1 + (MODE == 0 ? 1 : 0);
+    const int kx_end = kr_last + 1;
+    double accR[RY];  // MODE 2: running z sum of the restriction
+#pragma unroll
+    for (int r = 0; r < RY; ++r) accR[r] = 0.0;
 #pragma unroll
     for (int d = 0; d < PD; ++d) stage(kx0 + d, d);
     int slot = 0, slot_pd = PD;  // ring slots of planes kx and kx + PD
-    size_t oo = (size_t)(kx0 - (MODE == 0 ? 2 : 1)) * plane;  // offset of the plane written in this iteration
+    size_t oo = (size_t)(kx0 - (MODE == 0 ? 2 : 1)) * plane;  // offset of the fine plane written in this iteration (MODE 0, 1)
     for (int kx = kx0; kx <= kx_end; ++kx, oo += plane) {
         stage(kx + PD, slot_pd);
         cp_wait<PD>();   // everything up to plane kx has landed (this thread's copies)
@@ -219,6 +229,26 @@ __global__ void __launch_bounds__(NT)
 #pragma unroll
             for (int r = 0; r < RY; ++r)
                 if (owner[r] && kr >= k0 && kr < k1) out[oo + col[r]] = (SO)rv[r];
+        } else if (MODE == 2) {
+            double* const rp = rs + par * (XH * XW);
+#pragma unroll
+            for (int r = 0; r < RY; ++r) rp[(ty * RY + r + 1) * XW + tx + 1] = rv[r];
+            __syncthreads();
+            double p0[RY], p1[RY], p2[RY];
+            plane_sums<double>(rp, tx, ty * RY, p0, p1, p2, true);
+            const int K = kr >> 1;  // kr even: the plane between coarse planes K-1 and K; odd: the plane of coarse K
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                const double w = fma(0.0625, p2[r], fma(0.125, p1[r], 0.25 * p0[r]));
+                if (kr & 1) {
+                    accR[r] = fma(0.5, w, accR[r]);
+                } else {
+                    const int j = jb + r;
+                    if (owner[r] && (i & 1) && (j & 1) && K - 1 >= k0 && K - 1 < k1)
+                        out[((size_t)(K - 1) * pl.nc1 + (j >> 1)) * pl.nc0 + (i >> 1)] = (SO)fma(0.25, w, accR[r]);
+                    accR[r] = 0.25 * w;
+                }
+            }
         } else {
             double* const rp = rs + par * (XH * XW);
 #pragma unroll
@@ -247,41 +277,46 @@ __global__ void __launch_bounds__(NT)
     cp_wait<0>();
 }
 
-// b_c = R r (Eq. 13): coarse vertex I sits on fine vertex 2I+1; all 27 fine points are interior.
-template <typename SO>
-__global__ void __launch_bounds__(256)
-    k_restrict27(int nc0, int nc1, int nc2, int n0, int n1, const double* __restrict__ r, SO* __restrict__ bc) {
-    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
-    if (I >= nc0 || J >= nc1 || K >= nc2) return;
-    const double w[3] = {0.25, 0.5, 0.25};
-    double s = 0.0;
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-        for (int bb = 0; bb < 3; ++bb) {
-            const double* row = r + ((size_t)(2 * K + c) * n1 + (2 * J + bb)) * n0 + 2 * I;
-            s = fma(w[bb] * w[c], fma(0.25, row[0] + row[2], 0.5 * row[1]), s);
-        }
-    bc[((size_t)K * nc1 + J) * nc0 + I] = (SO)s;
-}
-
 // x += P e_c, P = 8 R^T: odd fine indices sit on a coarse vertex, even ones half-way between two (zero beyond the boundary).
+// One thread per coarse slot (I,J,K), 0 <= I <= nc: it reads the 2 x 2 x 2 coarse values e(I-1..I, J-1..J, K-1..K) once and
+// updates its (up to) 8 fine points (2I+a, 2J+b, 2K+c): per axis an even fine index averages the two coarse
+// neighbours, an odd one copies the coarse vertex it sits on.
 template <typename SX, typename SE>
 __global__ void __launch_bounds__(256)
     k_prolong27(int n0, int n1, int n2, int nc0, int nc1, int nc2, const SE* __restrict__ ec, SX* __restrict__ x) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
-    if (i >= n0 || j >= n1 || k >= n2) return;
-    const int I0 = (i - 1) >> 1, J0 = (j - 1) >> 1, K0 = (k - 1) >> 1;
-    const int ni = (i & 1) ? 1 : 2, nj = (j & 1) ? 1 : 2, nk = (k & 1) ? 1 : 2;
-    double s = 0.0;
-    for (int c = 0; c < nk; ++c)
-        for (int bb = 0; bb < nj; ++bb)
-            for (int a = 0; a < ni; ++a) {
-                const int I = I0 + a, J = J0 + bb, K = K0 + c;
-                if (I >= 0 && I < nc0 && J >= 0 && J < nc1 && K >= 0 && K < nc2) s += ldv(ec + ((size_t)K * nc1 + J) * nc0 + I);
+    const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y * blockDim.y + threadIdx.y, K = blockIdx.z;
+    if (I > nc0 || J > nc1) return;
+    double e[2][2][2];  // [gamma][beta][alpha]
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+                const int Ic = I - 1 + a, Jc = J - 1 + bb, Kc = K - 1 + c;
+                const bool ok = Ic >= 0 && Ic < nc0 && Jc >= 0 && Jc < nc1 && Kc >= 0 && Kc < nc2;
+                e[c][bb][a] = ok ? ldv(ec + ((size_t)Kc * nc1 + Jc) * nc0 + Ic) : 0.0;
             }
-    const size_t p = ((size_t)k * n1 + j) * n0 + i;
-    x[p] = (SX)(ldv(x + p) + s / (double)(ni * nj * nk));
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+                const int i = 2 * I + a, j = 2 * J + bb, k = 2 * K + c;
+                if (i >= n0 || j >= n1 || k >= n2) continue;
+                // even index: both coarse neighbours (in the oracle's order: gamma, beta, alpha ascending); odd: the upper one
+                double sum = 0.0;
+#pragma unroll
+                for (int g = (c ? 1 : 0); g < 2; ++g)
+#pragma unroll
+                    for (int bt = (bb ? 1 : 0); bt < 2; ++bt)
+#pragma unroll
+                        for (int al = (a ? 1 : 0); al < 2; ++al) sum += e[g][bt][al];
+                const double w = (a ? 1.0 : 0.5) * (bb ? 1.0 : 0.5) * (c ? 1.0 : 0.5);
+                const size_t p = ((size_t)k * n1 + j) * n0 + i;
+                x[p] = (SX)(ldv(x + p) + sum * w);
+            }
 }
 
 // Galerkin product of a constant symmetric 27-point stencil (Eq. 14 with P = 8 R^T), from its definition: entry O of
@@ -395,20 +430,28 @@ using mgv::Plan;
 
 // z chunks: the number of chunks that minimises (waves of resident CTAs) x (planes marched per CTA, 4 lead-in planes
 // included) — a partly filled last wave costs as much as a full one.
-static Plan make_plan(const poisson_ctx* ctx, const int n[3], int resident) {
+static Plan make_plan(const poisson_ctx* ctx, const int n[3], int resident, const int* nc = nullptr) {
     Plan pl;
     pl.n0 = n[0];
     pl.n1 = n[1];
     pl.n2 = n[2];
+    pl.nc0 = pl.nc1 = pl.nc2 = 0;
+    if (nc) {  // residual + restriction: chunks of coarse planes, each costing two fine planes
+        pl.nc0 = nc[0];
+        pl.nc1 = nc[1];
+        pl.nc2 = nc[2];
+    }
+    const int nplanes = nc ? nc[2] : n[2], per = nc ? 2 : 1;
     pl.ntx = (n[0] + mgv::VX - 1) / mgv::VX;
     pl.nty = (n[1] + mgv::VY - 1) / mgv::VY;
     const long tiles = (long)pl.ntx * pl.nty, slots = (long)ctx->num_sms * std::max(1, resident);
     double best = 1e300;
     pl.kc = n[2];
     pl.nz = 1;
-    for (int nz = 1; nz <= std::max(1, n[2] / 8); ++nz) {
-        const int kc = (n[2] + nz - 1) / nz, nzz = (n[2] + kc - 1) / kc;
-        const double cost = (double)((tiles * nzz + slots - 1) / slots) * (kc + 4 + 2);
+    pl.kc = nplanes;
+    for (int nz = 1; nz <= std::max(1, per * nplanes / 8); ++nz) {
+        const int kc = (nplanes + nz - 1) / nz, nzz = (nplanes + kc - 1) / kc;
+        const double cost = (double)((tiles * nzz + slots - 1) / slots) * (per * kc + 4 + 2);
         if (cost < best - 1e-9) {
             best = cost;
             pl.kc = kc;
@@ -420,13 +463,13 @@ static Plan make_plan(const poisson_ctx* ctx, const int n[3], int resident) {
 
 template <typename SX, typename SB, typename SO, int MODE, bool SEVEN>
 static int spai_launch_k(poisson_ctx* ctx, int kid, const int n[3], const SX* x, const SB* b, SO* out, const double* a4,
-                         double bsign, const double spai[5], double h) {
+                         double bsign, const double spai[5], double h, const int* nc) {
     auto kern = mgv::k_spai<SX, SB, SO, MODE, SEVEN>;
     constexpr size_t smem = mgv::spai_smem<SX, SB>();
     int resident = 0;
     const int rc = kernel_ready(ctx, kern, mgv::NT, smem, &resident);
     if (rc != POISSON_OK) return rc;
-    const Plan pl = make_plan(ctx, n, resident);
+    const Plan pl = make_plan(ctx, n, resident, nc);
     const dim3 blk(mgv::NTX, mgv::NTY), grid((unsigned)(pl.ntx * pl.nty * pl.nz));
     const double h2 = h * h, om = spai ? spai[0] : 0.0;
     const double m0 = spai ? spai[1] * h2 : 0, m1 = spai ? spai[2] * h2 : 0, m2 = spai ? spai[3] * h2 : 0,
@@ -438,9 +481,9 @@ static int spai_launch_k(poisson_ctx* ctx, int kid, const int n[3], const SX* x,
 
 template <typename SX, typename SB, typename SO, int MODE>
 static int spai_launch(poisson_ctx* ctx, int kid, const int n[3], bool seven, const SX* x, const SB* b, SO* out,
-                       const double* a4, double bsign, const double spai[5], double h) {
-    if (seven) return spai_launch_k<SX, SB, SO, MODE, true>(ctx, kid, n, x, b, out, a4, bsign, spai, h);
-    return spai_launch_k<SX, SB, SO, MODE, false>(ctx, kid, n, x, b, out, a4, bsign, spai, h);
+                       const double* a4, double bsign, const double spai[5], double h, const int* nc = nullptr) {
+    if (seven) return spai_launch_k<SX, SB, SO, MODE, true>(ctx, kid, n, x, b, out, a4, bsign, spai, h, nc);
+    return spai_launch_k<SX, SB, SO, MODE, false>(ctx, kid, n, x, b, out, a4, bsign, spai, h, nc);
 }
 
 // Level bookkeeping lives in the handle (common.cuh MgvLevel); built lazily, rebuilt when the parameters change.
@@ -539,17 +582,13 @@ static int mgv_cycle(poisson_ctx* ctx, size_t l, int nu1, int nu2, const double*
         if ((rc = spai_launch<S, S, S, 0>(ctx, KID_MGV_SMOOTH, L.n, false, cur, b, oth, a4, 1.0, spai, L.h)) != POISSON_OK) return rc;
         std::swap(cur, oth);
     }
-    double* r = (double*)L.t;
-    if ((rc = spai_launch<S, S, double, 1>(ctx, KID_MGV_RESTRICT, L.n, false, cur, b, r, a4, 1.0, nullptr, L.h)) != POISSON_OK) return rc;
     MgvLevel& C = ctx->vlevels[l + 1];
-    {
-        const dim3 blk(32, 8), grid((C.n[0] + 31) / 32, (C.n[1] + 7) / 8, C.n[2]);
-        PB_LAUNCH(ctx, KID_MGV_RESTRICT, (mgv::k_restrict27<S><<<grid, blk, 0, ctx->stream>>>(C.n[0], C.n[1], C.n[2], L.n[0], L.n[1], r, (S*)C.b)));
-    }
+    // residual + full weighting in one pass: b_c = R (b - A x)
+    if ((rc = spai_launch<S, S, S, 2>(ctx, KID_MGV_RESTRICT, L.n, false, cur, b, (S*)C.b, a4, 1.0, nullptr, L.h, C.n)) != POISSON_OK) return rc;
     S* ec = nullptr;
     if ((rc = mgv_cycle<S>(ctx, l + 1, nu1, nu2, spai, cg_rtol, &ec)) != POISSON_OK) return rc;
     {
-        const dim3 blk(64, 4), grid((L.n[0] + 63) / 64, (L.n[1] + 3) / 4, L.n[2]);
+        const dim3 blk(32, 8), grid((C.n[0] + 1 + 31) / 32, (C.n[1] + 1 + 7) / 8, C.n[2] + 1);
         PB_LAUNCH(ctx, KID_MGV_PROLONG, (mgv::k_prolong27<S, S><<<grid, blk, 0, ctx->stream>>>(L.n[0], L.n[1], L.n[2], C.n[0], C.n[1], C.n[2], ec, cur)));
     }
     for (int s = 0; s < nu2; ++s) {
@@ -606,16 +645,12 @@ static int mgv_vcycles_t(poisson_ctx* ctx, double* phi, const double* rhs, int n
             if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, true, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
             std::swap(cur, oth);
         }
-        if ((rc = spai_launch<double, double, double, 1>(ctx, KID_MGV_RESTRICT, L0.n, true, cur, bt, oth, ctx->v_sten, -1.0, nullptr, L0.h)) != POISSON_OK) return rc;
         MgvLevel& C = ctx->vlevels[1];
-        {
-            const dim3 blk(32, 8), grid((C.n[0] + 31) / 32, (C.n[1] + 7) / 8, C.n[2]);
-            PB_LAUNCH(ctx, KID_MGV_RESTRICT, (mgv::k_restrict27<S><<<grid, blk, 0, ctx->stream>>>(C.n[0], C.n[1], C.n[2], L0.n[0], L0.n[1], oth, (S*)C.b)));
-        }
+        if ((rc = spai_launch<double, double, S, 2>(ctx, KID_MGV_RESTRICT, L0.n, true, cur, bt, (S*)C.b, ctx->v_sten, -1.0, nullptr, L0.h, C.n)) != POISSON_OK) return rc;
         S* ec = nullptr;
         if ((rc = mgv_cycle<S>(ctx, 1, nu1, nu2, spai, cg_rtol, &ec)) != POISSON_OK) return rc;
         {
-            const dim3 blk(64, 4), grid((L0.n[0] + 63) / 64, (L0.n[1] + 3) / 4, L0.n[2]);
+            const dim3 blk(32, 8), grid((C.n[0] + 1 + 31) / 32, (C.n[1] + 1 + 7) / 8, C.n[2] + 1);
             PB_LAUNCH(ctx, KID_MGV_PROLONG, (mgv::k_prolong27<double, S><<<grid, blk, 0, ctx->stream>>>(L0.n[0], L0.n[1], L0.n[2], C.n[0], C.n[1], C.n[2], ec, cur)));
         }
         for (int s = 0; s < nu2; ++s) {
