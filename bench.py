@@ -48,6 +48,13 @@ ROW_BYTES = {
     "multipole_bc": 8, "apply_laplacian": 16, "rbsor_sweep": 12,   # 24/T, T = 2 sweeps per HBM pass (NHS = 4) on grids >= 2^21 points
     "mg_vcycle_f64": 75, "mg_vcycle_mixed": 66,
     "residual_norm": 16, "cg_iteration_19pt": 72, "multipole_bc_spherical": 8, "bicgstab_iteration": 136,
+    # SURVEY.md §8(f) rows (measured after the timed step; not part of `value`):
+    "spai_smooth": 24,              # f1: read x, b; write x
+    "mgv_vcycle_f64": 94,           # f2: V(1,1): (2 x 24 smoothing + 17 residual/restriction + 17 prolongation) x 8/7
+    "mgv_vcycle_mixed": 88,         # f2: the same with the coarse levels (1/7 of the points) stored in fp32
+    "pcg_iteration": 112,           # f3: pass A 48 + pass B 24 + fused symmetric GS sweep 24 + r.z 16
+    "rbsor_cheby_sweep": 12,        # f4: the fused kernel with one omega per half-step: 24/T, T = 2
+    "rbsor_local_sweep": 48,        # f4: spherical, position-dependent omega: two unfused half-sweeps
 }
 NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 250
 ROW_CITE = {
@@ -55,6 +62,8 @@ ROW_CITE = {
     "mg_vcycle_f64": "a5 PAPER.md:125-152", "mg_vcycle_mixed": "a5 PAPER.md:205", "residual_norm": "a7 PAPER.md:55",
     "cg_iteration_19pt": "a3 PAPER.md:95-105,172", "multipole_bc_spherical": "a6 PAPER.md:222",
     "bicgstab_iteration": "a4 PAPER.md:105",
+    "spai_smooth": "f1 PAPER.md:154-184", "mgv_vcycle_f64": "f2 PAPER.md:125-152", "mgv_vcycle_mixed": "f2 PAPER.md:205",
+    "pcg_iteration": "f3 PAPER.md:107-123", "rbsor_cheby_sweep": "f4 PAPER.md:81-88", "rbsor_local_sweep": "f4 PAPER.md:88-93",
 }
 
 
@@ -86,8 +95,10 @@ def measured_peak():
 
 
 def stored_traffic():
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.csv:
-    lines `kernel,dram_bytes_per_launch`), or None."""
+    """DRAM bytes from the committed ncu captures (profiles/traffic.csv, lines `key,bytes`): `cg_pass_a` etc. = bytes per
+    launch of that kernel class, `row:<name>` = bytes per point-update of that bench row (dram__bytes_read.sum +
+    dram__bytes_write.sum of all its kernels / its point-updates).  ncu cannot run inside the timed bench, so these are
+    the stored figures of the capture profiles/README.md names, not a measurement of this run."""
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     out = {}
     try:
@@ -172,6 +183,53 @@ def build_inputs(p):
     w4 = wl.config4(p["n4"])
     w5 = wl.config5(*p["n5"])
     return w3, w4, w5
+
+
+def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
+    """SURVEY.md §8(f) rows, each timed on its own after the step (CUDA events, warm-up + repeats); not in `value`."""
+    reps = 3 if not args.small else 1
+
+    def timed(fn, units):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    out = []
+    # f1 / f2: the paper's own multigrid on the vertex-centred 2^N k - 1 grid next to config 3's (255^3), two-sphere density
+    nv = p["n3"] - 1
+    wv = wl.two_spheres(nv, cell_centred=False)
+    gv = pb.Poisson(wv["shape"], wv["spacing"], wv["origin"], bc=wv["bc"], stream=stream.cuda_stream)
+    gv.set_ghost_faces([torch.from_numpy(f).cuda() for f in wl.analytic_ghost_faces(wv, wv["potential"])])
+    rhs = torch.from_numpy(np.ascontiguousarray(wv["rhs"])).cuda()
+    phi = torch.zeros_like(rhs)
+    nsm, ncyc = (8, 10) if not args.small else (2, 2)
+    out.append(("spai_smooth", nv ** 3, nsm, timed(lambda: gv.spai_smooth(phi, rhs, nsteps=nsm), nsm)))
+    for name, prec in (("mgv_vcycle_f64", pb.F64), ("mgv_vcycle_mixed", pb.MIXED)):
+        def cyc():
+            phi.zero_()
+            gv.mgv_vcycle(phi, rhs, nu1=1, nu2=1, precision=prec, ncycles=ncyc, want_resnorms=False)
+        out.append((name, nv ** 3, ncyc, timed(cyc, ncyc)))
+    del gv, rhs, phi
+    # f3: Gauss-Seidel-preconditioned CG, f4: Chebyshev omega sequence, both on the config-3 grid (7-point, Dirichlet)
+    npcg, nsw = (50, 20) if not args.small else (5, 4)
+
+    def pcg():
+        d["phi3"].zero_()
+        res = g3.pcg_solve(d["phi3"], d["rhs3"], fixed_iters=npcg)
+        if res["status"] != pb.OK or res["iters"] != npcg:
+            raise SystemExit("bench: PCG ended early (status %d, %d iterations)" % (res["status"], res["iters"]))
+    out.append(("pcg_iteration", p["n3"] ** 3, npcg, timed(pcg, npcg)))
+    out.append(("rbsor_cheby_sweep", p["n3"] ** 3, nsw, timed(lambda: g3.rbsor_cheby(d["sor3"], d["rhs3"], nsw), nsw)))
+    n5 = p["n5"][0] * p["n5"][1] * p["n5"][2]
+    nloc = 4
+    out.append(("rbsor_local_sweep", n5, nloc, timed(lambda: g5.rbsor_local(d["phi5"], d["rhs5"], nloc), nloc)))
+    return out
 
 
 def run_ours(args):
@@ -358,32 +416,54 @@ def run_ours(args):
                 ktab["%s:%s" % (gname, kname)] = {"launches": cnt, "avg_ms": ms / cnt, "total_ms": ms}
         g.set_option(pb.OPT_TIME_KERNELS, -1)
 
+    next_rows = measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3) if not args.rows else []
+
     ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, "cuda")
     total_updates = sum(pts * u for _, pts, u in units)
     peak, peak_src = measured_peak()
-    rows = []
-    for (name, pts, u), ms in zip(units, row_ms):
+    tr = stored_traffic() or {}
+    rows = {}
+
+    def add_row(name, pts, u, ms, in_value):
+        # per row: Gpoint-updates/s, algorithmic B/point, achieved algorithmic GB/s, fraction of the measured HBM peak,
+        # and the DRAM bytes per point-update ncu counted for the row's kernels (profiles/traffic.csv), with the GB/s
+        # that figure implies
         gpts = pts * u / (ms * 1e-3) / 1e9
         gbs = gpts * ROW_BYTES[name]
-        row = {"row": name, "cite": ROW_CITE[name], "points": pts, "units_per_step": u, "ms": round(ms, 4),
-               "gpoint_updates_per_s": round(gpts, 3), "algorithmic_bytes_per_point": ROW_BYTES[name],
-               "algorithmic_gbs": round(gbs, 1), "frac_of_hbm_peak": round(gbs / peak, 4), "bound": "hbm"}
+        dram = tr.get("row:" + name)
+        row = {"cite": ROW_CITE[name], "pts": pts, "units": u, "ms": round(ms, 4), "gpts": round(gpts, 2),
+               "B_pt": ROW_BYTES[name], "alg_gbs": round(gbs), "frac": round(gbs / peak, 3),
+               "dram_B_pt": dram, "dram_gbs": round(gpts * dram) if dram else None, "in_value": in_value}
         if name.startswith("multipole_bc"):
-            # lmax = 8 moments are bound by the plain fp64 ALUs, not HBM: ~250 fp64-pipe instructions per point
-            # (DMUL + DFMA + DADD of one point in the SASS of k_moments<8>); peak = SMs x 64 fp64 lanes x max SM clock
-            alu_peak = NUM_SMS * 64 * FP64_CLOCK_HZ
-            row.update(bound="alu", alu_dp_instr_per_point=MOMENTS_DP_INSTR,
-                       alu_peak_dp_instr_per_s=alu_peak,
-                       frac_of_fp64_alu_peak=round(gpts * 1e9 * MOMENTS_DP_INSTR / alu_peak, 4))
-        rows.append(row)
+            # lmax = 8 moments are bound by the plain fp64 ALUs, not HBM: fp64-pipe instructions per
+            # point counted by ncu (sm__inst_executed_pipe_fp64 x 32 / points; profiles/traffic.csv), else the SASS
+            # count; peak = SMs x 64 fp64 lanes x max SM clock
+            instr = tr.get("fp64_instr_per_point:" + name, MOMENTS_DP_INSTR)
+            row.update(bound="alu", fp64_instr_pt=instr,
+                       frac_alu=round(gpts * 1e9 * instr / (NUM_SMS * 64 * FP64_CLOCK_HZ), 3))
+        rows[name] = row
+
+    for (name, pts, u), ms in zip(units, row_ms):
+        add_row(name, pts, u, ms, True)
+    for name, pts, u, ms in next_rows:
+        add_row(name, pts, u, ms, False)
     n4 = p["n4"] ** 3
     achieved = 48.0 * n4 / (dom_ms / max(dom_cnt, 1) * 1e-3) / 1e9 if dom_cnt else None
-    tr = stored_traffic()
     out = {
         "metric": METRIC, "value": round(aggregate_value(total_updates, world, ms_total, args.steps), 3),
         "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": round(ms_total / args.steps, 3), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "rows": rows,
+        "roofline": {"kernel": "cg_pass_a (19-point, 512^3): x += a p_old; p = r + b p_old; q = L p; sum p.q",
+                     "bound": "hbm", "achieved": round(achieved, 1) if achieved else None, "peak": peak,
+                     "unit": "GB/s", "frac": round(achieved / peak, 4) if achieved else None,
+                     "traffic": tr.get("cg_pass_a"), "traffic_source": "profiles/traffic.csv (ncu --set full, stored)",
+                     "algorithmic_bytes_per_launch": 48 * n4, "avg_launch_ms": round(dom_ms / max(dom_cnt, 1), 4),
+                     "launches_timed": dom_cnt, "peak_source": peak_src},
+        "e2e": {"value": round(aggregate_value(total_updates, world, ms_e2e, e2e_steps), 3), "unit": UNIT,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
+                "ms_per_step": round(ms_e2e / e2e_steps, 3)},
         "config": {"workload": "one pass over all hot-path rows: config 3 grid 256^3 (multipole lmax 8, apply x%d, "
                                "RB-SOR x%d sweeps, V(2,2) x%d fp64 + x%d mixed, residual norm), config 4 grid 512^3 "
                                "periodic 19-point CG x%d iterations, config 5 grid 256x128x256 spherical multipole "
@@ -394,18 +474,7 @@ def run_ours(args):
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "gpu_launches": launches,
         "clocks": clocks,
-        "e2e": {"value": round(aggregate_value(total_updates, world, ms_e2e, e2e_steps), 3), "unit": UNIT,
-                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
-                "ms_per_step": round(ms_e2e / e2e_steps, 3)},
-        "roofline": {"kernel": "cg_pass_a (19-point, 512^3): x += a p_old; p = r + b p_old; q = L p; sum p.q",
-                     "bound": "hbm", "achieved": round(achieved, 1) if achieved else None, "peak": peak,
-                     "unit": "GB/s", "frac": round(achieved / peak, 4) if achieved else None,
-                     "traffic": (tr or {}).get("cg_pass_a"),
-                     "algorithmic_bytes_per_launch": 48 * n4, "avg_launch_ms": round(dom_ms / max(dom_cnt, 1), 4),
-                     "launches_timed": dom_cnt, "peak_source": peak_src},
-        "rows": rows,
-        "kernels": {k: {"launches": v["launches"], "avg_ms": round(v["avg_ms"], 4), "total_ms": round(v["total_ms"], 3)}
-                    for k, v in ktab.items()},
+        "kernels": {k: [v["launches"], round(v["avg_ms"], 4)] for k, v in ktab.items()},   # class: [launches, avg ms]
     }
     if rank == 0:
         if not args.no_cpu and world == 1:
