@@ -54,7 +54,10 @@ enum {
     POISSON_OPT_RESTRICTION = 1,   /* V-cycle restriction: 0 = (1/8)[1 3 3 1]^3 (transpose of trilinear),
                                       1 = mean of the 8 children (reading C7) */
     POISSON_OPT_POLL_INTERVAL = 2, /* Krylov solvers poll the device convergence flag every this many iterations */
-    POISSON_OPT_JACOBI = 3,        /* BiCGSTAB right Jacobi scaling: 1 (default) on, 0 off (reading C10) */
+    POISSON_OPT_JACOBI = 3,        /* BiCGSTAB right preconditioner: 1 (default) Jacobi scaling (reading C10),
+                                      0 none, 2 the multi-colour Gauss-Seidel preconditioner of PAPER.md:107-123
+                                      Eq. 10 (p^ = B^-1 p by one red-black Gauss-Seidel sweep from zero; radius-1
+                                      stencils, Cartesian or spherical) */
     POISSON_OPT_RECORD_HISTORY = 4,/* 1: record ||r_k||/||r_0|| per Krylov iteration for poisson_get_history */
     POISSON_OPT_SOR_HALFSTEPS = 6, /* red-black colour half-steps fused per HBM pass (temporal blocking): 2 = one
                                       full sweep per pass, 4 = two sweeps per pass, 0 = automatic (default: 4 on

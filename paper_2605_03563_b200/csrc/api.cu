@@ -344,7 +344,8 @@ int poisson_set_option(poisson_t ctx, int option, int value) {
             ctx->opt_poll = value;
             return POISSON_OK;
         case POISSON_OPT_JACOBI:
-            ctx->opt_jacobi = value ? 1 : 0;
+            if (value < 0 || value > 2) return fail(ctx, POISSON_INVALID_ARG, "BiCGSTAB preconditioner must be 0, 1 or 2");
+            ctx->opt_jacobi = value;
             return POISSON_OK;
         case POISSON_OPT_RECORD_HISTORY:
             ctx->opt_history = value ? 1 : 0;
@@ -581,6 +582,19 @@ int poisson_cg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double r
     return c.status;
 }
 
+// z = B^-1 f, B = the colour-block lower-triangular part of L_h (Eq. 10): one red-black Gauss-Seidel sweep
+// on L_h z = f from z = 0; symmetric: a second red half-sweep (the CG preconditioner).  One fused pass where the fused
+// kernel applies (zeros = an all-zero vector it reads as the initial guess), else half-sweep kernels.
+static int gs_precond_apply(poisson_ctx* ctx, const double* f, double* z, const double* zeros, bool symmetric) {
+    if (ctx->kind == KIND_CART2 && sor_fused_ok(ctx, ctx->op)) return sor_fused_precond(ctx, ctx->op, zeros, z, f, symmetric);
+    PB_CUDA_OK(cudaMemsetAsync(z, 0, ctx->npts * sizeof(double), ctx->stream));
+    for (int h = 0; h < (symmetric ? 3 : 2); ++h) {
+        const int rc = launch_rbsor_half(ctx, ctx->op, ctx->kind, z, f, 1.0, h & 1, false, KID_PCG_PRECOND);
+        if (rc != POISSON_OK) return rc;
+    }
+    return POISSON_OK;
+}
+
 int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter,
                            int fixed_iters, int* iters, double* relres) {
     const DeviceGuard on_device(ctx);
@@ -589,6 +603,17 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
     double *r = scratch(ctx, 0), *r0 = scratch(ctx, 1), *P[2] = {scratch(ctx, 2), scratch(ctx, 3)},
            *V[2] = {scratch(ctx, 4), scratch(ctx, 5)}, *s = scratch(ctx, 6), *t = scratch(ctx, 7);
     if (!r || !r0 || !P[0] || !P[1] || !V[0] || !V[1] || !s || !t) return POISSON_OUT_OF_MEMORY;
+    const bool gs = ctx->opt_jacobi == 2;  // right-preconditioned by the Gauss-Seidel sweep of Eq. 10
+    double *ph = nullptr, *sh = nullptr, *zeros = nullptr;
+    if (gs) {
+        if (ctx->kind == KIND_CART6)
+            return fail(ctx, POISSON_UNSUPPORTED, "the two-colour Gauss-Seidel preconditioner needs a radius-1 stencil (PAPER.md:113)");
+        ph = scratch(ctx, 8);
+        sh = scratch(ctx, 9);
+        zeros = scratch(ctx, 10);
+        if (!ph || !sh || !zeros) return POISSON_OUT_OF_MEMORY;
+        PB_CUDA_OK(cudaMemsetAsync(zeros, 0, ctx->npts * sizeof(double), ctx->stream));
+    }
     int rc = krylov_setup(ctx, rtol, max_iter, fixed_iters, false);
     if (rc != POISSON_OK) return rc;
     for (double* z : {P[0], P[1], V[0], V[1]}) PB_CUDA_OK(cudaMemsetAsync(z, 0, ctx->npts * sizeof(double), ctx->stream));
@@ -600,6 +625,16 @@ int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, do
         const int chunk = std::min(ctx->opt_poll, nit - j);
         for (int c = 0; c < chunk; ++c, ++j) {
             const int o = j & 1, n = (j + 1) & 1;
+            if (gs) {  // p and v are updated in place (P[0], V[0]): nothing reads a neighbour of the vector being written
+                if ((rc = launch_gsb_p(ctx, r, P[0], V[0], r0)) != POISSON_OK) return rc;
+                if ((rc = gs_precond_apply(ctx, P[0], ph, zeros, false)) != POISSON_OK) return rc;
+                if ((rc = launch_gsb_matvec(ctx, 1, ph, V[0], r0)) != POISSON_OK) return rc;
+                if ((rc = launch_gsb_s(ctx, r, V[0], s)) != POISSON_OK) return rc;
+                if ((rc = gs_precond_apply(ctx, s, sh, zeros, false)) != POISSON_OK) return rc;
+                if ((rc = launch_gsb_matvec(ctx, 2, sh, t, s)) != POISSON_OK) return rc;
+                if ((rc = launch_gsb_update(ctx, d_phi, ph, sh, s, t, r0, r)) != POISSON_OK) return rc;
+                continue;
+            }
             if ((rc = launch_bicg_pass1(ctx, r, P[o], V[o], r0, P[n], V[n])) != POISSON_OK) return rc;
             if ((rc = launch_bicg_pass2(ctx, r, V[n], s, t)) != POISSON_OK) return rc;
             if ((rc = launch_bicg_pass3(ctx, d_phi, P[n], s, t, r0, r)) != POISSON_OK) return rc;
@@ -967,15 +1002,8 @@ int poisson_rbsor_local(poisson_t ctx, double* d_phi, const double* d_rhs, int n
     return POISSON_OK;
 }
 
-// z = M^-1 r: the symmetrised red-black Gauss-Seidel sweep (red, black, red) on L z = r from z = 0.
 static int gs_precond(poisson_ctx* ctx, const double* r, double* z, const double* zeros) {
-    if (sor_fused_ok(ctx, ctx->op)) return sor_fused_precond(ctx, ctx->op, zeros, z, r, true);
-    PB_CUDA_OK(cudaMemsetAsync(z, 0, ctx->npts * sizeof(double), ctx->stream));
-    for (int colour : {0, 1, 0}) {
-        const int rc = launch_rbsor_half(ctx, ctx->op, ctx->kind, z, r, 1.0, colour, false, KID_PCG_PRECOND);
-        if (rc != POISSON_OK) return rc;
-    }
-    return POISSON_OK;
+    return gs_precond_apply(ctx, r, z, zeros, true);  // red, black, red
 }
 
 int poisson_pcg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,

@@ -259,6 +259,12 @@ int launch_rbsor_seq(poisson_ctx* ctx, const Op& op, int kind, double* phi, cons
 int launch_rbsor_local(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, const double* d_rj,
                        double* d_om, int nsweeps, int start_n, bool ug);
 int launch_pcg_dot(poisson_ctx* ctx, const double* r, const double* z);
+// BiCGSTAB right-preconditioned by the Gauss-Seidel sweep of Eq. 10: the pieces between the preconditioner solves
+int launch_gsb_p(poisson_ctx* ctx, const double* r, double* p, const double* v, double* r0);
+int launch_gsb_s(poisson_ctx* ctx, const double* r, const double* v, double* s);
+int launch_gsb_matvec(poisson_ctx* ctx, int which, const double* in, double* out, const double* other);
+int launch_gsb_update(poisson_ctx* ctx, double* x, const double* ph, const double* sh, const double* s, const double* t,
+                      const double* r0, double* r);
 
 // Lean 7-point apply / residual for non-periodic Cartesian grids (k_apply7.cu), fp64 and fp32
 bool apply7_ok(const poisson_ctx* ctx, const Op& op);

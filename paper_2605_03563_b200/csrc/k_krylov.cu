@@ -371,6 +371,91 @@ __global__ void __launch_bounds__(BX* BY)
     grid_reduce<2>(vals, rb, [=](const double* tot) { bicg_finish_iteration(ctl, hist, tot); });
 }
 
+// ---- BiCGSTAB right-preconditioned by the multi-colour Gauss-Seidel sweep of PAPER.md:107-123 Eq. 10 (row f3) ---------
+// The preconditioner solve p^ = B^-1 p is a red-black sweep over the grid (k_sor_fused / k_rbsor_half), so the
+// iteration is cut at it:  p = r + beta (p - omega v) | p^ = B^-1 p | v = L p^, r0^.v -> alpha | s = r - alpha v |
+// s^ = B^-1 s | t = L s^, t.s, t.t -> omega | x += alpha p^ + omega s^, r = s - omega t, r.r, r0^.r -> beta.
+__global__ void __launch_bounds__(256)
+    k_gsb_p(size_t n, const double* __restrict__ r, double* __restrict__ p, const double* __restrict__ v,
+            double* __restrict__ r0, KrylovCtl* ctl) {
+    if (ctl->done) return;
+    const double beta = ctl->beta, omega = ctl->omega;
+    const int restart = ctl->restart;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        const double rv = r[q];
+        p[q] = fma(beta, fma(-omega, v[q], p[q]), rv);
+        if (restart) r0[q] = rv;  // near-breakdown restart: r^_0 := r (reading C4)
+    }
+}
+
+__global__ void __launch_bounds__(256)
+    k_gsb_s(size_t n, const double* __restrict__ r, const double* __restrict__ v, double* __restrict__ s, const KrylovCtl* ctl) {
+    if (ctl->done) return;
+    const double alpha = ctl->alpha;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x)
+        s[q] = fma(-alpha, v[q], r[q]);
+}
+
+// out = L in (homogeneous ghosts).  WHICH 1: sum other.out (other = r^_0) -> alpha; WHICH 2: sum out.other, out.out
+// (other = s) -> omega.
+template <int KIND, int WHICH>
+__global__ void __launch_bounds__(BX* BY)
+    k_gsb_matvec(Op op, const double* __restrict__ in, double* __restrict__ out, const double* __restrict__ other,
+                 KrylovCtl* ctl, int kc, RedBuf rb) {
+    if (ctl->done) return;
+    const int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
+    const int k0 = blockIdx.z * kc, k1 = min(op.n[2], k0 + kc);
+    double a0 = 0.0, a1 = 0.0;
+    if (i < op.n[0] && j < op.n[1])
+        for (int k = k0; k < k1; ++k) {
+            const size_t q = gidx(op, i, j, k);
+            const double o = row_apply<double, KIND>(op, ArrLd<double>{in}, i, j, k, false);
+            out[q] = o;
+            a0 = fma(other[q], o, a0);
+            if (WHICH == 2) a1 = fma(o, o, a1);
+        }
+    double vals[2] = {a0, a1};
+    grid_reduce<2>(vals, rb, [=](const double* t) {
+        if (WHICH == 1) {
+            const double r0v = t[0];
+            ctl->r0v = r0v;
+            if (!(fabs(r0v) > 0.0) || !isfinite(r0v) || !(fabs(ctl->rho) > 0.0)) {
+                ctl->status = POISSON_BREAKDOWN;
+                ctl->done = 1;
+            } else {
+                ctl->alpha = ctl->rho / r0v;
+            }
+        } else {
+            ctl->ts = t[0];
+            ctl->tt = t[1];
+            if (!(t[1] > 0.0) || !isfinite(t[1])) {
+                ctl->status = POISSON_BREAKDOWN;
+                ctl->done = 1;
+            } else {
+                ctl->omega = t[0] / t[1];
+            }
+        }
+    });
+}
+
+__global__ void __launch_bounds__(256)
+    k_gsb_update(size_t n, double* __restrict__ x, const double* __restrict__ ph, const double* __restrict__ sh,
+                 const double* __restrict__ s, const double* __restrict__ t, const double* __restrict__ r0,
+                 double* __restrict__ r, KrylovCtl* ctl, double* hist, RedBuf rb) {
+    if (ctl->done) return;
+    const double alpha = ctl->alpha, omega = ctl->omega;
+    double a_rr = 0.0, a_r0r = 0.0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x) {
+        x[q] = fma(omega, sh[q], fma(alpha, ph[q], x[q]));
+        const double rn = fma(-omega, t[q], s[q]);
+        r[q] = rn;
+        a_rr = fma(rn, rn, a_rr);
+        a_r0r = fma(r0[q], rn, a_r0r);
+    }
+    double vals[2] = {a_rr, a_r0r};
+    grid_reduce<2>(vals, rb, [=](const double* tot) { bicg_finish_iteration(ctl, hist, tot); });
+}
+
 // ---- launch wrappers --------------------------------------------------------------------------------------------------
 #define KIND_SWITCH(kind, CALL)                       \
     switch (kind) {                                   \
@@ -474,6 +559,38 @@ int launch_bicg_pass2(poisson_ctx* ctx, const double* r, const double* v, double
     KIND_SWITCH(ctx->kind, (k_bicg_pass2<K><<<g, b, 0, ctx->stream>>>(op, r, v, s, t, ctx->d_ctl, ctx->opt_jacobi, kc,
                                                                         ctx->red)));
     post_launch(ctx, KID_BICG_PASS2);
+    return POISSON_OK;
+}
+
+int launch_gsb_p(poisson_ctx* ctx, const double* r, double* p, const double* v, double* r0) {
+    PB_LAUNCH(ctx, KID_BICG_PASS1, (k_gsb_p<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, r, p, v, r0, ctx->d_ctl)));
+    return POISSON_OK;
+}
+int launch_gsb_s(poisson_ctx* ctx, const double* r, const double* v, double* s) {
+    PB_LAUNCH(ctx, KID_BICG_PASS2, (k_gsb_s<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(ctx->npts, r, v, s, ctx->d_ctl)));
+    return POISSON_OK;
+}
+int launch_gsb_matvec(poisson_ctx* ctx, int which, const double* in, double* out, const double* other) {
+    const Op& op = ctx->op;
+    int kc = pick_kc(op, ctx->num_sms);
+    dim3 g;
+    const dim3 b(BX, BY);
+    const int rcg = fit_grid(ctx, op, op.n[0], &kc, &g);
+    if (rcg != POISSON_OK) return rcg;
+    const int kid = which == 1 ? KID_BICG_PASS1 : KID_BICG_PASS2;
+    pre_launch(ctx, kid);
+    if (which == 1) {
+        KIND_SWITCH(ctx->kind, (k_gsb_matvec<K, 1><<<g, b, 0, ctx->stream>>>(op, in, out, other, ctx->d_ctl, kc, ctx->red)));
+    } else {
+        KIND_SWITCH(ctx->kind, (k_gsb_matvec<K, 2><<<g, b, 0, ctx->stream>>>(op, in, out, other, ctx->d_ctl, kc, ctx->red)));
+    }
+    post_launch(ctx, kid);
+    return POISSON_OK;
+}
+int launch_gsb_update(poisson_ctx* ctx, double* x, const double* ph, const double* sh, const double* s, const double* t,
+                      const double* r0, double* r) {
+    PB_LAUNCH(ctx, KID_BICG_PASS3, (k_gsb_update<<<stream_blocks(ctx, ctx->npts), 256, 0, ctx->stream>>>(
+                                       ctx->npts, x, ph, sh, s, t, r0, r, ctx->d_ctl, ctx->d_hist, ctx->red)));
     return POISSON_OK;
 }
 
