@@ -16,6 +16,11 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-fm
          "--extended-lambda", "-Xcompiler", "-fPIC"]
 
 
+# Files whose results are compared with the oracle at a tolerance (1e-12 for the multipole sums), not bit for bit: the
+# compiler may contract a * b + c into fma there.  Everything else keeps -fmad=false (explicit fma only, C1b).
+CONTRACT_OK = {"k_multipole.cu"}
+
+
 def sources():
     return sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
 
@@ -45,7 +50,8 @@ def build(force=False, verbose=False):
         if not force and not verbose and os.path.exists(obj) and \
                 os.path.getmtime(obj) > max(hdr_mtime, os.path.getmtime(os.path.join(CSRC, src))):
             return obj  # up to date
-        cmd = [NVCC] + FLAGS + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
+        flags = [f for f in FLAGS if not (src in CONTRACT_OK and f == "-fmad=false")]
+        cmd = [NVCC] + flags + extra + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, r.stdout, r.stderr))
