@@ -185,11 +185,28 @@ def build_inputs(p):
     return w3, w4, w5
 
 
+ALL_ROWS = list(ROW_BYTES)
+_marker = {}
+
+
+def row_marker(args, torch, index):
+    """--mark (profiling aid): index + 1 consecutive launches of a tiny torch kernel (int32 add) announce the row that
+    follows, so that a kernel list captured by ncu can be cut into rows (profiles/README.md)."""
+    if not args.mark:
+        return
+    if "t" not in _marker:
+        _marker["t"] = torch.zeros(8, device="cuda", dtype=torch.int32)
+    for _ in range(index + 1):
+        _marker["t"].add_(1)
+
+
 def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
     """SURVEY.md §8(f) rows, each timed on its own after the step (CUDA events, warm-up + repeats); not in `value`."""
-    reps = 3 if not args.small else 1
+    light = args.small or args.divide > 1   # functional / profiling runs: few units, one repeat
+    reps = 1 if light else 3
 
-    def timed(fn, units):
+    def timed(fn, units, name):
+        row_marker(args, torch, ALL_ROWS.index(name))
         fn()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -198,6 +215,7 @@ def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
             fn()
         e1.record()
         torch.cuda.synchronize()
+        row_marker(args, torch, len(ALL_ROWS))
         return e0.elapsed_time(e1) / reps
 
     out = []
@@ -208,27 +226,29 @@ def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
     gv.set_ghost_faces([torch.from_numpy(f).cuda() for f in wl.analytic_ghost_faces(wv, wv["potential"])])
     rhs = torch.from_numpy(np.ascontiguousarray(wv["rhs"])).cuda()
     phi = torch.zeros_like(rhs)
-    nsm, ncyc = (8, 10) if not args.small else (2, 2)
-    out.append(("spai_smooth", nv ** 3, nsm, timed(lambda: gv.spai_smooth(phi, rhs, nsteps=nsm), nsm)))
+    nsm, ncyc = (2, 2) if light else (8, 10)
+    out.append(("spai_smooth", nv ** 3, nsm, timed(lambda: gv.spai_smooth(phi, rhs, nsteps=nsm), nsm, "spai_smooth")))
     for name, prec in (("mgv_vcycle_f64", pb.F64), ("mgv_vcycle_mixed", pb.MIXED)):
         def cyc():
             phi.zero_()
             gv.mgv_vcycle(phi, rhs, nu1=1, nu2=1, precision=prec, ncycles=ncyc, want_resnorms=False)
-        out.append((name, nv ** 3, ncyc, timed(cyc, ncyc)))
+        out.append((name, nv ** 3, ncyc, timed(cyc, ncyc, name)))
     del gv, rhs, phi
     # f3: Gauss-Seidel-preconditioned CG, f4: Chebyshev omega sequence, both on the config-3 grid (7-point, Dirichlet)
-    npcg, nsw = (50, 20) if not args.small else (5, 4)
+    npcg, nsw = (5, 4) if light else (50, 20)
 
     def pcg():
         d["phi3"].zero_()
         res = g3.pcg_solve(d["phi3"], d["rhs3"], fixed_iters=npcg)
         if res["status"] != pb.OK or res["iters"] != npcg:
             raise SystemExit("bench: PCG ended early (status %d, %d iterations)" % (res["status"], res["iters"]))
-    out.append(("pcg_iteration", p["n3"] ** 3, npcg, timed(pcg, npcg)))
-    out.append(("rbsor_cheby_sweep", p["n3"] ** 3, nsw, timed(lambda: g3.rbsor_cheby(d["sor3"], d["rhs3"], nsw), nsw)))
+    out.append(("pcg_iteration", p["n3"] ** 3, npcg, timed(pcg, npcg, "pcg_iteration")))
+    out.append(("rbsor_cheby_sweep", p["n3"] ** 3, nsw,
+                timed(lambda: g3.rbsor_cheby(d["sor3"], d["rhs3"], nsw), nsw, "rbsor_cheby_sweep")))
     n5 = p["n5"][0] * p["n5"][1] * p["n5"][2]
     nloc = 4
-    out.append(("rbsor_local_sweep", n5, nloc, timed(lambda: g5.rbsor_local(d["phi5"], d["rhs5"], nloc), nloc)))
+    out.append(("rbsor_local_sweep", n5, nloc,
+                timed(lambda: g5.rbsor_local(d["phi5"], d["rhs5"], nloc), nloc, "rbsor_local_sweep")))
     return out
 
 
@@ -319,8 +339,10 @@ def run_ours(args):
             else (lambda: None)
         mark()
         for name in row_names:
+            row_marker(args, torch, ALL_ROWS.index(name))
             row_fn[name]()
             mark()
+        row_marker(args, torch, len(ALL_ROWS))   # "no row": what follows belongs to the harness
 
     def _apply_host():
         for _ in range(p["apply"]):
@@ -618,6 +640,7 @@ def main():
     ap.add_argument("--path", type=int, default=None, help="force POISSON_OPT_KERNEL_PATH (1 generic, 2 plane)")
     ap.add_argument("--rows", default=None, help="comma list of row names: time only these (profiling aid)")
     ap.add_argument("--divide", type=int, default=1, help="divide the per-row unit counts (profiling aid)")
+    ap.add_argument("--mark", action="store_true", help="launch a marker kernel before every row (profiling aid)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
