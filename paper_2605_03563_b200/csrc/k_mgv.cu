@@ -449,7 +449,7 @@ static Plan make_plan(const poisson_ctx* ctx, const int n[3], int resident, cons
     pl.kc = n[2];
     pl.nz = 1;
     pl.kc = nplanes;
-    for (int nz = 1; nz <= std::max(1, per * nplanes / 8); ++nz) {
+    for (int nz = 1; nz <= std::max(1, per * nplanes / 2); ++nz) {  // chunks down to two fine planes: small levels are latency-bound
         const int kc = (nplanes + nz - 1) / nz, nzz = (nplanes + kc - 1) / kc;
         const double cost = (double)((tiles * nzz + slots - 1) / slots) * (per * kc + 4 + 2);
         if (cost < best - 1e-9) {
