@@ -8,6 +8,7 @@
 //   r^l S_l0 = Q_l^0 ;  r^l S_{l,m} = N_lm Q_l^m A_m ;  r^l S_{l,-m} = N_lm Q_l^m B_m ;  N_lm = sqrt(2 (l-m)!/(l+m)!).
 // One fused pass over rho accumulates all (lmax+1)^2 moments per thread in registers, then warp shuffles, a block
 // reduction and a last-block final sum (fixed order -> deterministic).  The pass is fp64-ALU bound at lmax = 8.
+#include <algorithm>
 #include <cmath>
 
 #include "stencil.cuh"
@@ -45,7 +46,9 @@ struct MpGeom {
 // products (2l-1) z and k r^2 are formed once per point.
 // INNER: the inner multipoles of Eq. 22, qbar_lm = sum rho r^-(l+1) S_lm dV = sum rho (r^l S_lm) r^-(2l+1) dV — the same
 // solid harmonics with the weight scaled by r^-(2l+1) per degree.
-template <int L, bool INNER>
+// Only the orders M0 <= m <= M1 are accumulated (the unrolled loops touch no other accumulator, so the rest of `acc`
+// never exists in registers).
+template <int L, bool INNER, int M0, int M1>
 __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], double x, double y, double z, double w) {
     const double r2 = fma(z, z, fma(y, y, x * x));
     double pw[L + 1];  // r^-(2l+1)
@@ -62,27 +65,29 @@ __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], dou
     for (int k = 0; k <= 2 * L; ++k) kr2[k] = k * r2;
     double A = 1.0, B = 0.0, dfact = 1.0;  // (x+iy)^m, (2m-1)!!
 #pragma unroll
-    for (int m = 0; m <= L; ++m) {
-        double qm2 = 0.0, qm1 = dfact;  // Q_{l-2}^m, Q_{l-1}^m while walking l = m..L
-        const double wa = w * A, wb = w * B;
+    for (int m = 0; m <= M1; ++m) {
+        if (m >= M0) {
+            double qm2 = 0.0, qm1 = dfact;  // Q_{l-2}^m, Q_{l-1}^m while walking l = m..L
+            const double wa = w * A, wb = w * B;
 #pragma unroll
-        for (int l = m; l <= L; ++l) {
-            double ql;
-            if (l == m)
-                ql = dfact;
-            else if (l == m + 1)
-                ql = cz[l] * qm1;
-            else
-                ql = fma(cz[l], qm1, -(kr2[l + m - 1] * qm2)) * (1.0 / (l - m));
-            const double qw = INNER ? ql * pw[l] : ql;
-            if (m == 0) {
-                acc[l * l + l] = fma(wa, qw, acc[l * l + l]);
-            } else {
-                acc[l * l + l + m] = fma(wa, qw, acc[l * l + l + m]);
-                acc[l * l + l - m] = fma(wb, qw, acc[l * l + l - m]);
+            for (int l = m; l <= L; ++l) {
+                double ql;
+                if (l == m)
+                    ql = dfact;
+                else if (l == m + 1)
+                    ql = cz[l] * qm1;
+                else
+                    ql = fma(cz[l], qm1, -(kr2[l + m - 1] * qm2)) * (1.0 / (l - m));
+                const double qw = INNER ? ql * pw[l] : ql;
+                if (m == 0) {
+                    acc[l * l + l] = fma(wa, qw, acc[l * l + l]);
+                } else {
+                    acc[l * l + l + m] = fma(wa, qw, acc[l * l + l + m]);
+                    acc[l * l + l - m] = fma(wb, qw, acc[l * l + l - m]);
+                }
+                qm2 = qm1;
+                qm1 = ql;
             }
-            qm2 = qm1;
-            qm1 = ql;
         }
         const double An = x * A - y * B, Bn = fma(y, A, x * B);
         A = An;
@@ -91,10 +96,30 @@ __device__ __forceinline__ void accumulate(double (&acc)[(L + 1) * (L + 1)], dou
     }
 }
 
-template <int L, bool INNER>
-__global__ void __launch_bounds__(256, 1)
-    k_moments(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
-              double* __restrict__ q_out) {
+// |m| of moment index s = l*l + l + m.
+__host__ __device__ constexpr int abs_m_of(int s) {
+    int l = 0;
+    while ((l + 1) * (l + 1) <= s) ++l;
+    const int m = s - l * l - l;
+    return m < 0 ? -m : m;
+}
+// The orders are cut in two halves of about equal work: half 0 takes m < split, half 1 the rest.  At l_max = 8 that is
+// 24 + 21 (l, |m|) pairs and ~40 accumulators per thread instead of 81: 128 registers and two CTAs per SM instead of
+// 255 and one (ncu: the one-CTA kernel sat at 8 warps per SM with its loads exposed).  Each half walks rho once.
+__host__ __device__ constexpr int m_split(int L) {
+    int total = 0;
+    for (int m = 0; m <= L; ++m) total += L - m + 1;
+    int acc = 0;
+    for (int m = 0; m <= L; ++m) {
+        acc += L - m + 1;
+        if (2 * acc >= total) return m + 1;
+    }
+    return L + 1;
+}
+
+template <int L, bool INNER, int M0, int M1>
+__device__ __forceinline__ void moments_half(const MpGeom& g, const double* __restrict__ rho, double* __restrict__ partials,
+                                             unsigned bid, unsigned nblk, double (*sm)[(L + 1) * (L + 1)]) {
     constexpr int NQ = (L + 1) * (L + 1);
     double acc[NQ];
 #pragma unroll
@@ -103,8 +128,7 @@ __global__ void __launch_bounds__(256, 1)
     const size_t plane = (size_t)g.n[0] * g.n[1];
     const double dV = g.h[0] * g.h[1] * g.h[2];
     // whole warps walk consecutive points; a warp whose 32 densities are all zero skips the arithmetic
-    for (size_t base = ((size_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31)); base < n;
-         base += (size_t)gridDim.x * blockDim.x) {
+    for (size_t base = ((size_t)bid * blockDim.x + (threadIdx.x & ~31)); base < n; base += (size_t)nblk * blockDim.x) {
         const size_t p = base + (threadIdx.x & 31);
         const double d = p < n ? rho[p] : 0.0;
         if (__all_sync(0xffffffffu, d == 0.0)) continue;
@@ -124,25 +148,42 @@ __global__ void __launch_bounds__(256, 1)
             z = fma((double)k, g.h[2], g.origin[2]);
             w = d * dV;
         }
-        accumulate<L, INNER>(acc, x, y, z, w);
+        accumulate<L, INNER, M0, M1>(acc, x, y, z, w);
     }
-#pragma unroll
-    for (int s = 0; s < NQ; ++s) acc[s] *= g.norm[s];  // N_lm, once per thread instead of once per point
-    // block reduction: warp shuffles, then shared memory across the 8 warps
-    __shared__ double sm[8][NQ];
-    __shared__ int is_last;
+    // N_lm once per thread instead of once per point, then warp shuffles and shared memory across the 8 warps
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
     for (int s = 0; s < NQ; ++s) {
-        const double v = warp_sum(acc[s]);
+        if (abs_m_of(s) < M0 || abs_m_of(s) > M1) continue;  // compile-time after unrolling
+        const double v = warp_sum(acc[s] * g.norm[s]);
         if (lane == 0) sm[wid][s] = v;
     }
     __syncthreads();
     for (int s = threadIdx.x; s < NQ; s += blockDim.x) {
+        if (abs_m_of(s) < M0 || abs_m_of(s) > M1) continue;
         double v = 0.0;
         for (int ww = 0; ww < 8; ++ww) v += sm[ww][s];
         partials[(size_t)blockIdx.x * NQ + s] = v;
     }
+}
+
+// Grid: 2 G blocks; block b works on half b & 1 as block b >> 1 of G.  The last block adds, per moment, the partials of
+// the blocks of its half in a fixed order.
+template <int L, bool INNER>
+__global__ void __launch_bounds__(256, 2)
+    k_moments(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
+              double* __restrict__ q_out) {
+    constexpr int NQ = (L + 1) * (L + 1);
+    constexpr int MS = m_split(L);
+    __shared__ double sm[8][NQ];
+    __shared__ int is_last;
+    const unsigned half = MS <= L ? (blockIdx.x & 1u) : 0u;
+    const unsigned nhalf = MS <= L ? 2u : 1u;
+    const unsigned bid = blockIdx.x / nhalf, nblk = gridDim.x / nhalf;
+    if (half == 0)
+        moments_half<L, INNER, 0, (MS <= L ? MS - 1 : L)>(g, rho, partials, bid, nblk, sm);
+    else
+        moments_half<L, INNER, (MS <= L ? MS : L), L>(g, rho, partials, bid, nblk, sm);
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
@@ -152,8 +193,9 @@ __global__ void __launch_bounds__(256, 1)
     if (!is_last) return;
     __threadfence();
     for (int s = threadIdx.x; s < NQ; s += blockDim.x) {
+        const unsigned h = (MS <= L && abs_m_of(s) >= MS) ? 1u : 0u;
         double v = 0.0;
-        for (unsigned b = 0; b < gridDim.x; ++b) v += __ldcg(&partials[(size_t)b * NQ + s]);
+        for (unsigned b = h; b < gridDim.x; b += nhalf) v += __ldcg(&partials[(size_t)b * NQ + s]);
         q_out[s] = v;
     }
 }
@@ -259,9 +301,11 @@ static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho,
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, bool inner) {
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     const MpGeom g = make_geom(ctx);
+    // two resident CTAs per SM; for l_max >= 1 the grid is made of pairs of blocks (one per half of the orders)
     int blocks = ctx->num_sms * 2;
     const size_t maxb = (ctx->npts + 255) / 256;
     if ((size_t)blocks > maxb) blocks = (int)maxb;
+    if (lmax >= 1) blocks = 2 * std::max(1, blocks);  // G blocks per half (m_split(L) <= L for every L >= 1)
     pre_launch(ctx, KID_MP_MOMENTS);
     switch (lmax) {
         case 0: moments_launch<0>(ctx, g, rho, d_q, blocks, inner); break;
