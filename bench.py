@@ -104,9 +104,12 @@ def stored_traffic():
     try:
         for line in open(path):
             f = [x.strip() for x in line.split(",")]
-            if len(f) >= 2 and f[0] and not f[0].startswith(("#", '"')) and f[0] != "kernel":
-                out[f[0]] = float(f[1])
-    except Exception:
+            if len(f) >= 2 and f[0] and not f[0].startswith(("#", '"')):
+                try:
+                    out[f[0]] = float(f[1])
+                except ValueError:
+                    pass   # header line
+    except OSError:
         return None
     return out or None
 
