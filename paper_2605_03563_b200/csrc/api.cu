@@ -145,7 +145,7 @@ static int setup_spherical(poisson_ctx* ctx) {
         dt[j] = (at_m[j] + at_p[j]) + 2.0 * cp[j];
     }
     PB_CUDA_OK(cudaMalloc((void**)&ctx->d_coef, coef.size() * sizeof(double)));
-    PB_CUDA_OK(cudaMemcpy(ctx->d_coef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice));
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_coef, coef.data(), coef.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     Op& op = ctx->op;
     op.ar_m = ctx->d_coef;
     op.ar_p = op.ar_m + nr;
@@ -174,7 +174,8 @@ static int setup_spherical(poisson_ctx* ctx) {
     for (int j = 0; j < nt; ++j) vt[j] = std::cos(te[j]) - std::cos(te[j + 1]);
     for (int k = 0; k < np; ++k) vp[k] = pe[k + 1] - pe[k];
     PB_CUDA_OK(cudaMalloc((void**)&ctx->d_ctr, tab.size() * sizeof(double)));
-    PB_CUDA_OK(cudaMemcpy(ctx->d_ctr, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice));
+    PB_CUDA_OK(cudaMemcpyAsync(ctx->d_ctr, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));  // coef and tab are local vectors; the uploads are ordered on the handle's stream
     return POISSON_OK;
 }
 
@@ -994,7 +995,8 @@ int poisson_rbsor_local(poisson_t ctx, double* d_phi, const double* d_rhs, int n
                 }
             }
         PB_CUDA_OK(cudaMalloc((void**)&ctx->d_rj, 2 * n2d * sizeof(double)));
-        PB_CUDA_OK(cudaMemcpy(ctx->d_rj, rj.data(), n2d * sizeof(double), cudaMemcpyHostToDevice));
+        PB_CUDA_OK(cudaMemcpyAsync(ctx->d_rj, rj.data(), n2d * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));  // rj is a local vector
     }
     int rc = launch_rbsor_local(ctx, ctx->op, ctx->kind, d_phi, d_rhs, ctx->d_rj, ctx->d_rj + n2d, nsweeps, start_n, true);
     if (rc != POISSON_OK) return rc;
