@@ -325,6 +325,7 @@ int poisson_create(poisson_t* out, const int shape[3], const double spacing[3], 
             return rc;
         }
     }
+    CREATE_OK(cudaDeviceSynchronize());  // the set-up copies and fills are complete whatever stream the caller uses next
     *out = ctx;
     return POISSON_OK;
 }

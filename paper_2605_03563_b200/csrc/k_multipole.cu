@@ -127,25 +127,34 @@ __device__ __forceinline__ void moments_half(const MpGeom& g, const double* __re
     const size_t n = (size_t)g.n[0] * g.n[1] * g.n[2];
     const size_t plane = (size_t)g.n[0] * g.n[1];
     const double dV = g.h[0] * g.h[1] * g.h[2];
-    // whole warps walk consecutive points; a warp whose 32 densities are all zero skips the arithmetic
-    for (size_t base = ((size_t)bid * blockDim.x + (threadIdx.x & ~31)); base < n; base += (size_t)nblk * blockDim.x) {
-        const size_t p = base + (threadIdx.x & 31);
+    // whole warps walk consecutive points; a warp whose 32 densities are all zero skips the arithmetic.  The point
+    // index is decoded once; every further step adds the (decoded) grid stride with carries — no division per point
+    const size_t stride = (size_t)nblk * blockDim.x;
+    const int n0 = g.n[0], n1 = g.n[1];
+    const int di = (int)(stride % n0), dj = (int)((stride / n0) % n1), dk = (int)(stride / plane);
+    size_t p = (size_t)bid * blockDim.x + threadIdx.x;
+    int k = (int)(p / plane), j = (int)((p - (size_t)k * plane) / n0), i = (int)(p - (size_t)k * plane - (size_t)j * n0);
+    for (size_t base = ((size_t)bid * blockDim.x + (threadIdx.x & ~31)); base < n; base += stride, p += stride) {
+        const int ci = i, cj = j, ck = k;  // this iteration's point
+        i += di;
+        if (i >= n0) { i -= n0; ++j; }
+        j += dj;
+        if (j >= n1) { j -= n1; ++k; }
+        k += dk;
         const double d = p < n ? rho[p] : 0.0;
         if (__all_sync(0xffffffffu, d == 0.0)) continue;
         if (d == 0.0) continue;
-        const int k = (int)(p / plane), rem = (int)(p - (size_t)k * plane);
-        const int j = rem / g.n[0], i = rem - j * g.n[0];
         double x, y, z, w;
         if (g.sph) {
-            const double r = g.rc[i], rs = r * g.st[j];
-            x = rs * g.cph[k];
-            y = rs * g.sph_[k];
-            z = r * g.ct[j];
-            w = d * (g.vr[i] * g.vt[j] * g.vp[k]);
+            const double r = g.rc[ci], rs = r * g.st[cj];
+            x = rs * g.cph[ck];
+            y = rs * g.sph_[ck];
+            z = r * g.ct[cj];
+            w = d * (g.vr[ci] * g.vt[cj] * g.vp[ck]);
         } else {
-            x = fma((double)i, g.h[0], g.origin[0]);
-            y = fma((double)j, g.h[1], g.origin[1]);
-            z = fma((double)k, g.h[2], g.origin[2]);
+            x = fma((double)ci, g.h[0], g.origin[0]);
+            y = fma((double)cj, g.h[1], g.origin[1]);
+            z = fma((double)ck, g.h[2], g.origin[2]);
             w = d * dV;
         }
         accumulate<L, INNER, M0, M1>(acc, x, y, z, w);
@@ -237,12 +246,26 @@ __device__ __forceinline__ double expansion(const double* __restrict__ norm, con
     return -G * acc;
 }
 
-__global__ void __launch_bounds__(256)
-    k_ghost_eval(MpGeom g, int face, int R, const double* __restrict__ q, double G, int lmax, double* __restrict__ out,
-                 bool inner) {
+// All ghost faces in ONE launch (six launches of a few thousand threads each cost six launch latencies): block b
+// belongs to the face whose block range contains it.
+struct GhostFaces {
+    int nf;
+    int face[6], first_block[7];  // first_block[nf] = total
+    double* out[6];
+    const double* q[6];
+    int inner[6];
+};
+
+__global__ void __launch_bounds__(256) k_ghost_eval(MpGeom g, GhostFaces gf, int R, double G, int lmax) {
+    int s = 0;
+#pragma unroll
+    for (int m = 1; m < 6; ++m)
+        if (m < gf.nf && (int)blockIdx.x >= gf.first_block[m]) s = m;
+    const int face = gf.face[s];
+    const bool inner = gf.inner[s] != 0;
     const int a = face / 2, a1 = (a == 0) ? 1 : 0, a2 = (a == 2) ? 1 : 2;
     const long len = (long)R * g.n[a1] * g.n[a2];
-    const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long t = (long)(blockIdx.x - gf.first_block[s]) * blockDim.x + threadIdx.x;
     if (t >= len) return;
     const int q1 = (int)(t % g.n[a1]), q2 = (int)((t / g.n[a1]) % g.n[a2]), layer = (int)(t / ((long)g.n[a1] * g.n[a2]));
     double x, y, z;
@@ -261,7 +284,7 @@ __global__ void __launch_bounds__(256)
         y = fma((double)id[1], g.h[1], g.origin[1]);
         z = fma((double)id[2], g.h[2], g.origin[2]);
     }
-    out[t] = expansion(g.norm, q, lmax, G, x, y, z, inner);
+    gf.out[s][t] = expansion(g.norm, gf.q[s], lmax, G, x, y, z, inner);
 }
 
 static MpGeom make_geom(poisson_ctx* ctx) {
@@ -327,15 +350,23 @@ int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, b
 // d_qbar: inner moments (Eq. 22), used for the inner radial shell of a spherical grid (face 0) when it is a Dirichlet face.
 int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, const double* d_qbar, double G, int lmax) {
     const MpGeom g = make_geom(ctx);
+    GhostFaces gf{};
+    int blocks = 0;
     for (int f = 0; f < 6; ++f) {
         if (ctx->op.bc[f] != POISSON_BC_DIRICHLET_GHOST || !ctx->d_ghost[f]) continue;
         if (g.sph && f > 1) continue;  // only the radial shells carry Eq. 19 / Eq. 21
         const bool inner = g.sph && f == 0;
         if (inner && !d_qbar) continue;
-        const long len = ctx->face_len[f];
-        PB_LAUNCH(ctx, KID_MP_GHOSTS, (k_ghost_eval<<<(int)((len + 255) / 256), 256, 0, ctx->stream>>>(
-                                          g, f, ctx->op.R, inner ? d_qbar : d_q, G, lmax, ctx->d_ghost[f], inner)));
+        gf.face[gf.nf] = f;
+        gf.first_block[gf.nf] = blocks;
+        gf.out[gf.nf] = ctx->d_ghost[f];
+        gf.q[gf.nf] = inner ? d_qbar : d_q;
+        gf.inner[gf.nf] = inner ? 1 : 0;
+        blocks += (int)((ctx->face_len[f] + 255) / 256);
+        ++gf.nf;
     }
+    gf.first_block[gf.nf] = blocks;
+    if (blocks > 0) PB_LAUNCH(ctx, KID_MP_GHOSTS, (k_ghost_eval<<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G, lmax)));
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
