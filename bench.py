@@ -55,6 +55,7 @@ ROW_BYTES = {
     "pcg_iteration": 112,           # f3: pass A 48 + pass B 24 + fused symmetric GS sweep 24 + r.z 16
     "rbsor_cheby_sweep": 12,        # f4: the fused kernel with one omega per half-step: 24/T, T = 2
     "rbsor_local_sweep": 48,        # f4: spherical, position-dependent omega: two unfused half-sweeps
+    "mgv_vcycle_f64_511": 94,       # f2 at the paper's own size (Table 2: 511^3, seven coarse levels, nu = 1)
 }
 NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 250
 ROW_CITE = {
@@ -64,6 +65,7 @@ ROW_CITE = {
     "bicgstab_iteration": "a4 PAPER.md:105",
     "spai_smooth": "f1 PAPER.md:154-184", "mgv_vcycle_f64": "f2 PAPER.md:125-152", "mgv_vcycle_mixed": "f2 PAPER.md:205",
     "pcg_iteration": "f3 PAPER.md:107-123", "rbsor_cheby_sweep": "f4 PAPER.md:81-88", "rbsor_local_sweep": "f4 PAPER.md:88-93",
+    "mgv_vcycle_f64_511": "f2 PAPER.md:186-195 Table 2 (paper: 34.8 ms per V(1,1) cycle = 3.83 Gzups, hardware not stated)",
 }
 
 
@@ -237,6 +239,21 @@ def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
             gv.mgv_vcycle(phi, rhs, nu1=1, nu2=1, precision=prec, ncycles=ncyc, want_resnorms=False)
         out.append((name, nv ** 3, ncyc, timed(cyc, ncyc, name)))
     del gv, rhs, phi
+    if not light:
+        # the paper's own Table 2 configuration: 511^3, seven coarse levels, V(1,1), order 2, fp64
+        n5v = 2 * p["n3"] - 1
+        wv = wl.two_spheres(n5v, cell_centred=False)
+        gv = pb.Poisson(wv["shape"], wv["spacing"], wv["origin"], bc=wv["bc"], stream=stream.cuda_stream)
+        gv.set_ghost_faces([torch.from_numpy(f).cuda() for f in wl.analytic_ghost_faces(wv, wv["potential"])])
+        rhs = torch.from_numpy(np.ascontiguousarray(wv["rhs"])).cuda()
+        del wv
+        phi = torch.zeros_like(rhs)
+
+        def cyc511():
+            phi.zero_()
+            gv.mgv_vcycle(phi, rhs, nu1=1, nu2=1, precision=pb.F64, ncycles=ncyc, want_resnorms=False)
+        out.append(("mgv_vcycle_f64_511", n5v ** 3, ncyc, timed(cyc511, ncyc, "mgv_vcycle_f64_511")))
+        del gv, rhs, phi
     # f3: Gauss-Seidel-preconditioned CG, f4: Chebyshev omega sequence, both on the config-3 grid (7-point, Dirichlet)
     npcg, nsw = (5, 4) if light else (50, 20)
 
