@@ -12,12 +12,12 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libpoisson_b200.so")
 OBJ = os.path.join(HERE, "build")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-fmad=false", "-lineinfo",
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++20", "-fmad=false", "-lineinfo",
          "--extended-lambda", "-Xcompiler", "-fPIC"]
 
 
 # Files whose results are compared with the oracle at a tolerance (1e-12 for the multipole sums), not bit for bit: the
-# compiler may contract a * b + c into fma there.  Everything else keeps -fmad=false (explicit fma only, C1b).
+# compiler may contract a * b + c into fma there.  Everything else keeps -fmad=false (explicit fma only, C1b).  C++20: `requires` in plane.cuh.
 CONTRACT_OK = {"k_multipole.cu"}
 
 

@@ -21,6 +21,7 @@ struct LdArr {  // v itself
     __device__ __forceinline__ void prepare() {}
     __device__ __forceinline__ Raw load(size_t p) const { return Raw{ld2(v + p)}; }
     __device__ __forceinline__ Raw load_own(size_t p) const { return load(p); }
+    __device__ __forceinline__ void prefetch_own(size_t p) const { asm volatile("prefetch.global.L2 [%0];" ::"l"(v + p)); }
     __device__ __forceinline__ void side(const Raw&, size_t) const {}
     __device__ __forceinline__ double2 form(const Op&, const Raw& r, int, int, int) const { return r.a; }
     __device__ __forceinline__ double at(const Op&, size_t p, int, int, int) const { return v[p]; }
@@ -43,6 +44,11 @@ struct LdPnew {  // p_new = (r - mu) + beta p_old; side effect on owned points: 
     }
     __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q), mk2(0.0, 0.0)}; }
     __device__ __forceinline__ Raw load_own(size_t q) const { return Raw{ld2(r + q), ld2(p + q), ld2(x + q)}; }
+    __device__ __forceinline__ void prefetch_own(size_t q) const {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(r + q));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p + q));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(x + q));
+    }
     __device__ __forceinline__ void side(const Raw& w, size_t q) const {
         st2(x + q, mk2(fma(alpha_prev, w.p.x, w.x.x), fma(alpha_prev, w.p.y, w.x.y)));
     }
@@ -81,6 +87,11 @@ struct LdPhat {  // p^ = (r + beta (p_old - omega v_old)) / D; side effect on ow
     }
     __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(p + q), ld2(v + q)}; }
     __device__ __forceinline__ Raw load_own(size_t q) const { return load(q); }
+    __device__ __forceinline__ void prefetch_own(size_t q) const {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(r + q));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(p + q));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(v + q));
+    }
     __device__ __forceinline__ void side(const Raw& w, size_t q) const {
         st2(p_new + q, mk2(fma(beta, fma(-omega, w.v.x, w.p.x), w.r.x), fma(beta, fma(-omega, w.v.y, w.p.y), w.r.y)));
         if (restart) st2(r0w + q, w.r);  // r^_0 := r; the epilogue of this same thread reads it back for r^_0 . v
@@ -113,6 +124,10 @@ struct LdShat {  // s^ = (r - alpha v) / D; side effect on owned points: store s
     __device__ __forceinline__ void prepare() { alpha = ctl->alpha; }
     __device__ __forceinline__ Raw load(size_t q) const { return Raw{ld2(r + q), ld2(v + q)}; }
     __device__ __forceinline__ Raw load_own(size_t q) const { return load(q); }
+    __device__ __forceinline__ void prefetch_own(size_t q) const {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(r + q));
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(v + q));
+    }
     __device__ __forceinline__ void side(const Raw& w, size_t q) const {
         st2(s + q, mk2(fma(-alpha, w.v.x, w.r.x), fma(-alpha, w.v.y, w.r.y)));
     }

@@ -251,6 +251,17 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                 if (act[r]) s.o[r] = ld.load_own(off + base0 + (size_t)r * n0);
                 else if constexpr (Ld::PLAIN) s.o[r].a = bpair(i, jrow + r, s.kw);
             }
+            if constexpr (requires { ld.prefetch_own((size_t)0); }) {
+                // The demand loads run one plane ahead in registers (two planes spill); with one CTA per SM that is
+                // ~50 KB in flight per SM, marginal against the HBM latency.  One lane per 128 bytes also pulls the
+                // plane after that into L2 (no register): cg_pass_a 1.447 -> 1.321 ms at 512^3 (distance 2: 1.333,
+                // 3: 1.380, 4: no gain).  The same two lines made the register-capped fused SOR kernel 20 % slower.
+                if ((lx & 7) == 0 && s.kw + 1 < n2) {
+#pragma unroll
+                    for (int r = 0; r < RPT; ++r)
+                        if (act[r]) ld.prefetch_own(off + plane + base0 + (size_t)r * n0);
+                }
+            }
 #pragma unroll
             for (int m = 0; m < NH; ++m) {
                 if (hcls[m] == 1) s.h[m] = ld.load(off + (size_t)hwj[m] * n0 + hwi[m]);
