@@ -134,14 +134,16 @@ __device__ __forceinline__ void moments_half(const MpGeom& g, const double* __re
     const int di = (int)(stride % n0), dj = (int)((stride / n0) % n1), dk = (int)(stride / plane);
     size_t p = (size_t)bid * blockDim.x + threadIdx.x;
     int k = (int)(p / plane), j = (int)((p - (size_t)k * plane) / n0), i = (int)(p - (size_t)k * plane - (size_t)j * n0);
+    double dnext = p < n ? rho[p] : 0.0;  // the density is loaded one step ahead of its use
     for (size_t base = ((size_t)bid * blockDim.x + (threadIdx.x & ~31)); base < n; base += stride, p += stride) {
         const int ci = i, cj = j, ck = k;  // this iteration's point
+        const double d = dnext;
+        dnext = p + stride < n ? rho[p + stride] : 0.0;
         i += di;
         if (i >= n0) { i -= n0; ++j; }
         j += dj;
         if (j >= n1) { j -= n1; ++k; }
         k += dk;
-        const double d = p < n ? rho[p] : 0.0;
         if (__all_sync(0xffffffffu, d == 0.0)) continue;
         if (d == 0.0) continue;
         double x, y, z, w;
