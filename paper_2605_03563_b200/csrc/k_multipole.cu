@@ -213,10 +213,12 @@ __global__ void __launch_bounds__(256, 2)
 
 // Phi at one exterior point from the moments.
 // inner: Eq. 21, Phi = -G sum qbar_lm r^l S_lm (no inverse powers of r).
-__device__ __forceinline__ double expansion(const double* __restrict__ norm, const double* __restrict__ q, int lmax,
-                                            double G, double x, double y, double z, bool inner) {
+// qn = q_lm N_lm (shared memory).
+__device__ __forceinline__ double expansion(const double* __restrict__ qn, int lmax, double G, double x, double y, double z,
+                                            bool inner) {
     const double r2 = fma(z, z, fma(y, y, x * x));
     const double rinv = inner ? 1.0 : 1.0 / sqrt(r2), rinv2 = rinv * rinv;
+    const double rk[9] = {0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8};  // 1 / (l - m)
     double A = 1.0, B = 0.0, dfact = 1.0, acc = 0.0;
     double pw_m = rinv;  // r^-(2m+1)  (1 for the inner expansion)
     for (int m = 0; m <= lmax; ++m) {
@@ -228,13 +230,11 @@ __device__ __forceinline__ double expansion(const double* __restrict__ norm, con
             else if (l == m + 1)
                 ql = (2 * m + 1) * z * qm1;
             else
-                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) / (double)(l - m);
+                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) * rk[l - m];
             if (m == 0)
-                acc = fma(q[l * l + l] * ql, pw, acc);
-            else {
-                const double nq = norm[l * l + l + m] * ql;
-                acc = fma((q[l * l + l + m] * A + q[l * l + l - m] * B) * nq, pw, acc);
-            }
+                acc = fma(qn[l * l + l] * ql, pw, acc);
+            else
+                acc = fma((qn[l * l + l + m] * A + qn[l * l + l - m] * B) * ql, pw, acc);
             qm2 = qm1;
             qm1 = ql;
             pw *= rinv2;
@@ -265,6 +265,9 @@ __global__ void __launch_bounds__(256) k_ghost_eval(MpGeom g, GhostFaces gf, int
         if (m < gf.nf && (int)blockIdx.x >= gf.first_block[m]) s = m;
     const int face = gf.face[s];
     const bool inner = gf.inner[s] != 0;
+    __shared__ double qn[kNQ];  // this face's moments times N_lm, read 81 times by every thread
+    for (int e = threadIdx.x; e < (lmax + 1) * (lmax + 1); e += blockDim.x) qn[e] = gf.q[s][e] * g.norm[e];
+    __syncthreads();
     const int a = face / 2, a1 = (a == 0) ? 1 : 0, a2 = (a == 2) ? 1 : 2;
     const long len = (long)R * g.n[a1] * g.n[a2];
     const long t = (long)(blockIdx.x - gf.first_block[s]) * blockDim.x + threadIdx.x;
@@ -286,7 +289,7 @@ __global__ void __launch_bounds__(256) k_ghost_eval(MpGeom g, GhostFaces gf, int
         y = fma((double)id[1], g.h[1], g.origin[1]);
         z = fma((double)id[2], g.h[2], g.origin[2]);
     }
-    gf.out[s][t] = expansion(g.norm, gf.q[s], lmax, G, x, y, z, inner);
+    gf.out[s][t] = expansion(qn, lmax, G, x, y, z, inner);
 }
 
 static MpGeom make_geom(poisson_ctx* ctx) {
