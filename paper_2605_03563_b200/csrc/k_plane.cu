@@ -138,6 +138,12 @@ struct LdShat {  // s^ = (r - alpha v) / D; side effect on owned points: store s
     __device__ __forceinline__ double2 form_own(const Raw& w, double d0, double d1) const {
         return mk2(fma(-alpha, w.v.x, w.r.x) / (jacobi ? -d0 : 1.0), fma(-alpha, w.v.y, w.r.y) / (jacobi ? -d1 : 1.0));
     }
+    // the same quotients from a divisor that does not change along z and its reciprocal (div_by: correctly rounded)
+    static constexpr bool RECIP = true;
+    __device__ __forceinline__ double divisor(double d) const { return jacobi ? -d : 1.0; }
+    __device__ __forceinline__ double2 form_own_rd(const Raw& w, double v0, double v1, double r0, double r1) const {
+        return mk2(div_by<double>(fma(-alpha, w.v.x, w.r.x), v0, r0), div_by<double>(fma(-alpha, w.v.y, w.r.y), v1, r1));
+    }
     __device__ __forceinline__ double at(const Op& op, size_t q, int i, int j, int k) const {
         return fma(-alpha, v[q], r[q]) / jac_<KIND>(op, i, j, k, jacobi);
     }

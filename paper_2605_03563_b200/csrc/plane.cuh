@@ -230,6 +230,25 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
         }
     }
 
+    // spherical operator + a loader that divides by the diagonal and asks for it (Ld::RECIP; it pays where registers
+    // allow: BiCGSTAB pass 2 86 -> 80 us, pass 1 97 -> 104 us): divisor and reciprocal once per column, not per plane
+    constexpr bool sph_rd = KIND == KIND_SPH && [] { if constexpr (requires { Ld::RECIP; }) return Ld::USES_DIAG && Ld::RECIP; else return false; }();
+    double odv[RPT][2], ord_[RPT][2];
+    if constexpr (sph_rd) {
+#pragma unroll
+        for (int r = 0; r < RPT; ++r)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                odv[r][e] = ld.divisor(fma(rc.ir2[e], rc.dt[r], rc.dr[e]));
+                ord_[r][e] = 1.0 / odv[r][e];
+            }
+#pragma unroll
+        for (int m = 0; m < NH; ++m) {  // hd0 / hd1 become divisor, and two more registers hold the reciprocals
+            hd0[m] = ld.divisor(hd0[m]);
+            hd1[m] = ld.divisor(hd1[m]);
+        }
+    }
+
     // ---- plane staging --------------------------------------------------------------------------------------------
     struct Staged {
         typename Ld::Raw o[RPT], h[NH];
@@ -301,7 +320,10 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                         // the row diagonals of the two owned points from the coefficients already in registers
                         // (same expressions as stencil.cuh row_diag, so the quotients are the same bits)
                         double d0, d1;
-                        if constexpr (KIND == KIND_SPH) {
+                        if constexpr (sph_rd) {
+                            fv = ld.form_own_rd(s.o[r], odv[r][0], odv[r][1], ord_[r][0], ord_[r][1]);
+                            d0 = d1 = 0.0;
+                        } else if constexpr (KIND == KIND_SPH) {
                             d0 = fma(rc.ir2[0], rc.dt[r], rc.dr[0]);
                             d1 = fma(rc.ir2[1], rc.dt[r], rc.dr[1]);
                         } else if constexpr (KIND == KIND_CART6) {
@@ -310,7 +332,7 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                             d0 = rc.plain ? rc.d : row_diag<double, KIND_CART2>(op, i, jrow + r, s.kw);
                             d1 = rc.plain ? rc.d : row_diag<double, KIND_CART2>(op, i + 1, jrow + r, s.kw);
                         }
-                        fv = ld.form_own(s.o[r], d0, d1);
+                        if constexpr (!sph_rd) fv = ld.form_own(s.o[r], d0, d1);
                     } else {
                         fv = ld.form(op, s.o[r], i, jrow + r, s.kw);
                     }
@@ -328,7 +350,12 @@ __global__ void __launch_bounds__(PlaneGeom<KIND, Cfg>::NT, Cfg::MINB)
                 if (hcls[m] == 1)
                 {
                     if constexpr (Ld::USES_DIAG && KIND == KIND_SPH)
-                        st2(slot + hso[m], ld.form_own(s.h[m], hd0[m], hd1[m]));  // spherical diagonal: no k dependence
+                    {
+                        if constexpr (sph_rd)
+                            st2(slot + hso[m], ld.form_own_rd(s.h[m], hd0[m], hd1[m], 1.0 / hd0[m], 1.0 / hd1[m]));
+                        else
+                            st2(slot + hso[m], ld.form_own(s.h[m], hd0[m], hd1[m]));  // spherical diagonal: no k dependence
+                    }
                     else
                         st2(slot + hso[m], ld.form(op, s.h[m], hwi[m], hwj[m], s.kw));
                 }
