@@ -52,7 +52,7 @@ ROW_BYTES = {
     "spai_smooth": 24,              # f1: read x, b; write x
     "mgv_vcycle_f64": 94,           # f2: V(1,1): (2 x 24 smoothing + 17 residual/restriction + 17 prolongation) x 8/7
     "mgv_vcycle_mixed": 88,         # f2: the same with the coarse levels (1/7 of the points) stored in fp32
-    "pcg_iteration": 112,           # f3: pass A 48 + pass B 24 + fused symmetric GS sweep 24 + r.z 16
+    "pcg_iteration": 88,            # f3: pass A 48 + pass B 24 + fused symmetric GS sweep from zero with r.z 16
     "rbsor_cheby_sweep": 12,        # f4: the fused kernel with one omega per half-step: 24/T, T = 2
     "rbsor_local_sweep": 48,        # f4: spherical, position-dependent omega: two unfused half-sweeps
     "mgv_vcycle_f64_511": 94,       # f2 at the paper's own size (Table 2: 511^3, seven coarse levels, nu = 1)

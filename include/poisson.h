@@ -63,7 +63,8 @@ enum {
                                       full sweep per pass, 4 = two sweeps per pass, 0 = automatic (default: 4 on
                                       grids of >= 2^21 points, else 2); the results do not depend on it */
     POISSON_OPT_FUSED_RESTRICT = 7,/* V-cycle: residual + restriction fused into one pass over the level (no fine residual
-                                      in memory): 0 = automatic (fp32 levels of the mixed cycle), 1 = always, 2 = never;
+                                      in memory): 0 = automatic (fp32 levels of the mixed cycle, fp64 levels below 2^21 points),
+                                      1 = always, 2 = never;
                                       the results do not depend on it */
     POISSON_OPT_TIME_KERNELS = 5,  /* bracket every launch of one kernel class (0..poisson_kernel_classes()-1) with
                                       CUDA events on the handle's stream; -2 = every class, -1 = off (default) */

@@ -587,14 +587,17 @@ int poisson_cg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double r
 // z = B^-1 f, B = the colour-block lower-triangular part of L_h (Eq. 10): one red-black Gauss-Seidel sweep
 // on L_h z = f from z = 0; symmetric: a second red half-sweep (the CG preconditioner).  One fused pass where the fused
 // kernel applies (zeros = an all-zero vector it reads as the initial guess), else half-sweep kernels.
-static int gs_precond_apply(poisson_ctx* ctx, const double* f, double* z, const double* zeros, bool symmetric) {
-    if (ctx->kind == KIND_CART2 && sor_fused_ok(ctx, ctx->op)) return sor_fused_precond(ctx, ctx->op, zeros, z, f, symmetric);
+// with_rz (preconditioned CG): r . z and beta follow in the control block, inside the fused pass or by k_pcg_dot.
+static int gs_precond_apply(poisson_ctx* ctx, const double* f, double* z, const double* zeros, bool symmetric,
+                            bool with_rz = false) {
+    if (ctx->kind == KIND_CART2 && sor_fused_ok(ctx, ctx->op))
+        return sor_fused_precond(ctx, ctx->op, zeros, z, f, symmetric, with_rz);
     PB_CUDA_OK(cudaMemsetAsync(z, 0, ctx->npts * sizeof(double), ctx->stream));
     for (int h = 0; h < (symmetric ? 3 : 2); ++h) {
         const int rc = launch_rbsor_half(ctx, ctx->op, ctx->kind, z, f, 1.0, h & 1, false, KID_PCG_PRECOND);
         if (rc != POISSON_OK) return rc;
     }
-    return POISSON_OK;
+    return with_rz ? launch_pcg_dot(ctx, f, z) : POISSON_OK;
 }
 
 int poisson_bicgstab_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter,
@@ -756,9 +759,11 @@ static int cycle64(poisson_ctx* ctx, size_t l, double* phi, const double* rhs, b
     MgLevel& C = ctx->levels[l + 1];
     double* cur = phi;
     if ((rc = launch_rbsor_pp(ctx, L.op, &cur, phi, L.alt, rhs, 1.0, nu1, ug)) != POISSON_OK) return rc;
-    // residual and restriction in one pass (no fine residual in memory): in fp64 the two separate kernels are still
-    // ~10 % faster at 256^3 (the 64-term ordered sum stalls the CTA), so the fused kernel is opt-in there
-    if (ctx->opt_fused_restrict == 1 && resid_restrict_ok(ctx, L.op, C.op)) {
+    // residual and restriction in one pass (no fine residual in memory).  fp64, measured: 13 / 12 us against 20 / 18 us
+    // for the two kernels at 64^3 / 32^3, the same at 128^3, 181 against 153 us at 256^3 (one 704-thread CTA per SM
+    // with a barrier per plane, against the TMA-staged residual kernel with three small CTAs): fused below 2^21 points
+    const bool fuse = ctx->opt_fused_restrict == 1 || (ctx->opt_fused_restrict == 0 && L.npts < ((size_t)1 << 21));
+    if (fuse && resid_restrict_ok(ctx, L.op, C.op)) {
         if ((rc = resid_restrict(ctx, L.op, C.op, cur, rhs, C.rhs, ug)) != POISSON_OK) return rc;
     } else {
         if ((rc = launch_apply(ctx, L.op, KIND_CART2, cur, rhs, L.res, 1, ug, false)) != POISSON_OK) return rc;
@@ -1006,7 +1011,7 @@ int poisson_rbsor_local(poisson_t ctx, double* d_phi, const double* d_rhs, int n
 }
 
 static int gs_precond(poisson_ctx* ctx, const double* r, double* z, const double* zeros) {
-    return gs_precond_apply(ctx, r, z, zeros, true);  // red, black, red
+    return gs_precond_apply(ctx, r, z, zeros, true, true);  // red, black, red; then r . z
 }
 
 int poisson_pcg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double rtol, int max_iter, int fixed_iters,
@@ -1027,7 +1032,6 @@ int poisson_pcg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double 
     for (double* v : {P[0], P[1], zeros}) PB_CUDA_OK(cudaMemsetAsync(v, 0, ctx->npts * sizeof(double), ctx->stream));
     if ((rc = launch_krylov_init(ctx, d_phi, d_rhs, r, false, nullptr)) != POISSON_OK) return rc;
     if ((rc = gs_precond(ctx, r, z, zeros)) != POISSON_OK) return rc;
-    if ((rc = launch_pcg_dot(ctx, r, z)) != POISSON_OK) return rc;
     const int nit = fixed_iters > 0 ? fixed_iters : max_iter;
     for (int j = 0; j < nit;) {
         const int chunk = std::min(ctx->opt_poll, nit - j);
@@ -1036,7 +1040,6 @@ int poisson_pcg_solve(poisson_t ctx, double* d_phi, const double* d_rhs, double 
             if ((rc = launch_cg_passA(ctx, z, P[j & 1], P[(j + 1) & 1], q, d_phi)) != POISSON_OK) return rc;
             if ((rc = launch_cg_passB(ctx, r, q)) != POISSON_OK) return rc;
             if ((rc = gs_precond(ctx, r, z, zeros)) != POISSON_OK) return rc;
-            if ((rc = launch_pcg_dot(ctx, r, z)) != POISSON_OK) return rc;
         }
         PB_CUDA_OK(cudaGetLastError());
         if (fixed_iters <= 0) {

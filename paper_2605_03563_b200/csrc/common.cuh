@@ -144,7 +144,7 @@ struct poisson_ctx {
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
     int opt_sor_nhs = 0;             // colour half-steps fused per HBM pass of the red-black kernel (2, 4; 0 = auto)
     double opt_bicg_restart_eps = 1e-12;  // BiCGSTAB restart threshold (0 = never), reading C4
-    int opt_fused_restrict = 0;      // V-cycle residual + restriction in one kernel: 0 auto (fp32 levels only), 1 always, 2 never
+    int opt_fused_restrict = 0;      // V-cycle residual + restriction in one kernel: 0 auto (fp32 levels; fp64 levels below 2^21 points), 1 always, 2 never
     void* sor_tmp = nullptr;         // ping-pong buffer of the fused red-black kernel
     size_t sor_tmp_bytes = 0;
     long launches = 0;
@@ -251,7 +251,8 @@ int launch_rbsor_pp32(poisson_ctx* ctx, const Op& op, float** cur, float* a, flo
 void* sor_scratch(poisson_ctx* ctx, size_t bytes);  // nullptr on OOM
 int sor_fused_seq(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, const double* rhs, const double* omegas,
                   int nsweeps, bool ug, double** result);
-int sor_fused_precond(poisson_ctx* ctx, const Op& op, const double* zin, double* zout, const double* f, bool symmetric);
+int sor_fused_precond(poisson_ctx* ctx, const Op& op, const double* zin, double* zout, const double* f, bool symmetric,
+                      bool with_rz);
 int launch_rbsor_half(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, double omega, int colour,
                       bool ug, int kid);
 int launch_rbsor_seq(poisson_ctx* ctx, const Op& op, int kind, double* phi, const double* rhs, const double* omegas,

@@ -4,12 +4,14 @@
 //
 // Structure = k_apply7.cu (a thread owns a 16-byte pair of x-adjacent fine columns (2I, 2I+1) = the two x children of
 // coarse column I, keeps planes k-1, k, k+1 of phi in registers, publishes the arriving plane to a ring of three
-// shared-memory planes) plus a ring of four shared-memory RESIDUAL planes.  The tile carries two halo rows / one halo
-// pair of phi on each side so that the residual is available one fine cell beyond the valid tile, which is what the
-// (1/8)[1 3 3 1]^3 weights of coarse cell (I,J,K) — fine cells 2I-1..2I+2 per axis — reach.  When fine plane 2K+2 has
-// been computed, the first (VX/2)(VY/2) threads sum the 64 weighted residuals of their coarse cell out of shared
-// memory, in the order and with the weights of k_restrict / the oracle (z outer, y, x inner; fine cells outside the
-// domain skipped), so the result is bit-identical to residual kernel + k_restrict.  Work items are (tile, COARSE plane).
+// shared-memory planes).  The tile carries two halo rows / one halo pair of phi on each side so that the residual is
+// available one fine cell beyond the valid tile, which is what the (1/8)[1 3 3 1]^3 weights of coarse cell (I,J,K) —
+// fine cells 2I-1..2I+2 per axis — reach.  The restriction runs axis by axis (fw_acc, stencil.cuh) as a three-stage
+// pipeline behind the residual, one barrier per fine plane: in the iteration that forms the residual of plane k, the
+// x sums of plane k-1 are taken (own pair + one value of each neighbour pair, from a two-plane residual ring) and the
+// y sums of plane k-2 (own row + three rows of a two-plane ring of x sums) are added into the z sums of the two coarse
+// planes that fine plane touches, which live in the registers of the thread that owns fine row 2J.  Same bits as the
+// residual kernel followed by k_restrict.  Work items are (tile, COARSE plane).
 #include <algorithm>
 #include <cstdlib>
 
@@ -39,7 +41,9 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     constexpr int SW = Cfg::SW, SLOT = Cfg::SLOT, PXN = Cfg::PXN, EY = Cfg::EY;
     extern __shared__ __align__(16) unsigned char smraw[];
     T* const ring = reinterpret_cast<T*>(smraw);   // 3 planes of phi
-    T* const rres = ring + 3 * SLOT;               // 4 planes of residual
+    T* const rres = ring + 3 * SLOT;               // 2 planes of residual (pairs, the layout of the phi ring)
+    constexpr int XSLOT = PXN * EY;
+    T* const xbuf = rres + 2 * SLOT;               // 2 planes of x sums (one value per pair)
     const int n0 = op.n[0], n1 = op.n[1], n2 = op.n[2], nc2 = cop.n[2];
     const int tid = threadIdx.x;
     const bool live = tid < PXN * EY;
@@ -53,10 +57,8 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
     const bool rrow = live && ly >= 1 && ly < EY - 1;  // rows on which the residual is formed
     // shared-memory offsets of the x neighbours, clamped inside the row (the clamped ones feed only unused residuals)
     const int o_xl = lx > 0 ? -1 : 0, o_xr = lx < PXN - 1 ? 2 : 1;
-    // the coarse cell this thread restricts (threads 0 .. NC-1)
-    const bool cth = tid < Cfg::NC;
-    const int cI = cth ? tid % (Cfg::VX / 2) : 0, cJ = cth ? tid / (Cfg::VX / 2) : 0;
-    const double W[4] = {0.125, 0.375, 0.375, 0.125};
+    // the pair of thread lx = cI + 1 is the pair of x children (2I, 2I+1) of the tile's coarse column cI
+    const bool xth = live && lx >= 1 && lx <= PXN - 2;
 
     const long total = (long)g.ntx * g.nty * nc2;
     long pos = (long)blockIdx.x * g.items;
@@ -128,16 +130,27 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
             vp += vs;
         }
         frq[0] = frq[1] = frq[2] = P2T<T>::make((T)0, (T)0);
-        __syncthreads();  // the previous segment's readers are done with both rings
-        for (int kin0 = kbeg; kin0 <= kend; kin0 += 3) {
+        // restriction state of this thread: its residual pair of the previous plane, its x sum of the plane before,
+        // and the z sums of the two coarse planes the current fine plane contributes to
+        P2 res_prev = P2T<T>::make((T)0, (T)0);
+        T x_prev = (T)0, zA = (T)0, zB = (T)0;
+        const bool xrow = xth && rrow && col_in;                    // forms x sums (fine columns 2I, 2I+1 = its own pair)
+        const bool own = xrow && (ly & 1) == 0 && ly >= 2 && ly <= EY - 4;  // fine row 2J: forms y and z sums, stores
+        const bool has_l = i - 1 >= 0, has_r = i + 2 < n0, has_d = j - 1 >= 0, has_u = j + 2 < n1;
+        T* const fcp = own ? fc + (size_t)(j >> 1) * cop.n[0] + (i >> 1) : fc;
+        const size_t cplane = (size_t)cop.n[0] * cop.n[1];
+        __syncthreads();  // the previous segment's readers are done with the rings
+        for (int kin0 = kbeg; kin0 <= kend + 2; kin0 += 3) {
 #pragma unroll
             for (int u = 0; u < 3; ++u) {
                 const int kin = kin0 + u;
-                if (kin > kend) break;
-                const P2 nv = nvq[u % PF];
-                q[u] = nv;
-                if (live) *reinterpret_cast<P2*>(mine + u * SLOT) = nv;
-                if (kin + PF <= kend) nvq[u % PF] = loadv(kin + PF);
+                if (kin > kend + 2) break;
+                if (kin <= kend) {
+                    const P2 nv = nvq[u % PF];
+                    q[u] = nv;
+                    if (live) *reinterpret_cast<P2*>(mine + u * SLOT) = nv;
+                    if (kin + PF <= kend) nvq[u % PF] = loadv(kin + PF);
+                }
                 vp += vs;
                 // rhs of plane kin + 1 (used two iterations later)
                 frq[(u + 1) % 3] = P2T<T>::make((T)0, (T)0);
@@ -146,7 +159,60 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
                 const P2 f = frq[(u + 2) % 3];  // rhs of plane kin - 1
                 __syncthreads();
                 const int k = kin - 1;          // residual plane of this iteration
-                if (kin > kbeg + 0 && live) {
+                // (c) y and z sums of plane k - 2, whose x sums were published one iteration ago
+                {
+                    const int kz = k - 2;
+                    if (own && kz > kbeg && kz < kend && kz >= 0 && kz < n2) {
+                        const T* const xs = xbuf + ((kz + 8) & 1) * XSLOT + ly * PXN + lx;
+                        if (restriction == 1) {
+                            const T y = x_prev + xs[PXN];
+                            if (kz & 1) {
+                                const int K = kz >> 1;
+                                if (K >= K0 && K < K1) fcp[(size_t)K * cplane] = (zA + y) * (T)0.125;
+                            } else {
+                                zA = y;
+                            }
+                        } else {
+                            T y = (T)0;
+                            if (has_d) y = fw_acc<T>(y, 0, xs[-PXN]);
+                            y = fw_acc<T>(y, 1, x_prev);
+                            y = fw_acc<T>(y, 2, xs[PXN]);
+                            if (has_u) y = fw_acc<T>(y, 3, xs[2 * PXN]);
+                            if (kz & 1) {  // fine plane 2m+1: weight 2 of coarse plane m, weight 0 of m + 1
+                                zA = fw_acc<T>(zA, 2, y);
+                                zB = fw_acc<T>((T)0, 0, y);
+                                const int K = kz >> 1;
+                                if (kz == n2 - 1 && K >= K0 && K < K1) fcp[(size_t)K * cplane] = zA;
+                            } else {       // fine plane 2m: weight 3 of coarse plane m - 1 (now complete), weight 1 of m
+                                zA = fw_acc<T>(zA, 3, y);
+                                const int K = (kz >> 1) - 1;
+                                if (K >= K0 && K < K1) fcp[(size_t)K * cplane] = zA;
+                                zA = fw_acc<T>(zB, 1, y);
+                                zB = (T)0;
+                            }
+                        }
+                    }
+                }
+                // (b) x sums of plane k - 1, whose residuals were published one iteration ago
+                {
+                    const int kx = k - 1;
+                    if (xrow && kx > kbeg && kx < kend && kx >= 0 && kx < n2) {
+                        const T* const rp = rres + ((kx + 8) & 1) * SLOT + so;
+                        T x = (T)0;
+                        if (restriction == 1) {
+                            x = res_prev.x + res_prev.y;
+                        } else {
+                            if (has_l) x = fw_acc<T>(x, 0, rp[-1]);
+                            x = fw_acc<T>(x, 1, res_prev.x);
+                            x = fw_acc<T>(x, 2, res_prev.y);
+                            if (has_r) x = fw_acc<T>(x, 3, rp[2]);
+                        }
+                        xbuf[((kx + 8) & 1) * XSLOT + ly * PXN + lx] = x;
+                        x_prev = x;
+                    }
+                }
+                // (a) residual of plane k
+                if (kin > kbeg && kin <= kend && live) {
                     P2 res = P2T<T>::make((T)0, (T)0);
                     if (rown && k >= 0 && k < n2 && kin >= kbeg + 2) {
                         const T* const sp = mine + ((u + 2) % 3) * SLOT;
@@ -167,44 +233,8 @@ __global__ void __launch_bounds__(Cfg::NT, 1)
                         s = fma_(zm.y + zp.y, c2, s);
                         res.y = f.y - fma_(-d1, C.y, s);
                     }
-                    *reinterpret_cast<P2*>(rres + ((k + 8) & 3) * SLOT + so) = res;
-                }
-                // coarse plane K is complete once fine residual plane 2K+2 is in shared memory
-                if ((k & 1) == 0 && k >= 2 * K0 + 2 && k <= 2 * K1) {
-                    __syncthreads();
-                    const int K = k / 2 - 1;
-                    const int I = tx * (Cfg::VX / 2) + cI, J = ty * (Cfg::VY / 2) + cJ;
-                    if (cth && I < cop.n[0] && J < cop.n[1]) {
-                        // fine cell (2I-1+a, 2J-1+b, 2K-1+c) sits at tile-local (2cI+1+a, 2cJ+1+b), residual slot (2K-1+c) & 3
-                        const T* const base = rres + (2 * cJ + 1) * SW + (2 * cI + 1);
-                        T acc = 0;
-                        if (restriction == 1) {
-                            for (int c = 0; c < 2; ++c)
-                                for (int b = 0; b < 2; ++b)
-                                    for (int a = 0; a < 2; ++a)
-                                        acc += base[((2 * K + c + 8) & 3) * SLOT + (b + 1) * SW + (a + 1)];
-                            acc *= (T)0.125;
-                        } else {
-#pragma unroll
-                            for (int c = 0; c < 4; ++c) {
-                                const int kk = 2 * K - 1 + c;
-                                if (kk < 0 || kk >= n2) continue;
-                                const T* const pl = base + ((kk + 8) & 3) * SLOT;
-#pragma unroll
-                                for (int b = 0; b < 4; ++b) {
-                                    const int jj = 2 * J - 1 + b;
-                                    if (jj < 0 || jj >= n1) continue;
-#pragma unroll
-                                    for (int a = 0; a < 4; ++a) {
-                                        const int ii = 2 * I - 1 + a;
-                                        if (ii < 0 || ii >= n0) continue;
-                                        acc += (T)(W[a] * W[b] * W[c]) * pl[b * SW + a];
-                                    }
-                                }
-                            }
-                        }
-                        fc[((size_t)K * cop.n[1] + J) * cop.n[0] + I] = acc;
-                    }
+                    *reinterpret_cast<P2*>(rres + ((k + 8) & 1) * SLOT + so) = res;
+                    res_prev = res;
                 }
             }
         }
@@ -233,7 +263,7 @@ static int rr_launch(poisson_ctx* ctx, const Op& fine, const Op& coarse, const T
     const long total = (long)g.ntx * g.nty * coarse.n[2];
     g.items = std::max(2L, (total + ctx->num_sms - 1) / ctx->num_sms);
     const int grid = (int)((total + g.items - 1) / g.items);
-    const size_t smem = (size_t)7 * Cfg::SLOT * sizeof(T);
+    const size_t smem = (size_t)6 * Cfg::SLOT * sizeof(T);
     int rc = kernel_ready(ctx, k_resid_restrict<T, Cfg, true>, Cfg::NT, smem);
     if (rc == POISSON_OK) rc = kernel_ready(ctx, k_resid_restrict<T, Cfg, false>, Cfg::NT, smem);
     if (rc != POISSON_OK) return rc;

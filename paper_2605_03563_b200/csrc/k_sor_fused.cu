@@ -119,13 +119,20 @@ __device__ __forceinline__ typename PairT<T>::type sor_bpair(const Op& op, int i
 }
 
 // Tile configuration: extended tile of PXN pairs x EY rows (threads in use = PXN * EY), NHS colour half-steps per pass.
-template <int NHS_, int PXN_, int EY_, int PF_ = 1>
+// NACT <= NHS of the half-steps do work (the rest are no-ops that only delay the plane: the three-half-step symmetric
+// Gauss-Seidel sweep of the CG preconditioner runs in the four-half-step geometry, whose even depth the colour
+// bookkeeping needs); the y halo is NACT rows, the x halo stays NHS columns (16-byte pairs start at even columns).
+// ZIN: the input field is known to be zero and is not read.  DOT: the kernel also forms sum rhs . out over the grid
+// (r . z of preconditioned CG) from the values it holds when it stores a plane.
+template <int NHS_, int PXN_, int EY_, int PF_ = 1, int NACT_ = NHS_, bool ZIN_ = false, bool DOT_ = false>
 struct SorTile {
     static constexpr int NHS = NHS_, PXN = PXN_, EY = EY_, PF = PF_;  // PF = planes of load prefetch (1 or 2)
+    static constexpr int NACT = NACT_, HY = NACT_;
+    static constexpr bool ZIN = ZIN_, DOT = DOT_;
     static constexpr int D = NHS + 2;                       // queue depth = ring slots
     static constexpr int NT = ((PXN * EY + 31) / 32) * 32;  // threads per CTA
     static constexpr int SW = 2 * PXN, SLOT = SW * EY;
-    static constexpr int VX = 2 * PXN - 2 * NHS, VY = EY - 2 * NHS;
+    static constexpr int VX = 2 * PXN - 2 * NHS, VY = EY - 2 * HY;
     static constexpr int MINB = (NT <= 320) ? 2 : 1;  // fp64 needs ~105 registers per thread
 };
 
@@ -140,7 +147,7 @@ struct OmegaSet {
 template <typename T, class Cfg, bool PLAIN>
 __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
     k_sor_fused(const Op op, const T* __restrict__ in, T* __restrict__ out, const T* __restrict__ rhs,
-                const OmegaSet<T> om, const bool ug_in, const SorGeom g) {
+                const OmegaSet<T> om, const bool ug_in, const SorGeom g, KrylovCtl* const ctl, const RedBuf rb) {
     using P2 = typename PairT<T>::type;
     constexpr int NHS = Cfg::NHS, D = Cfg::D, SW = Cfg::SW, SLOT = Cfg::SLOT, PXN = Cfg::PXN, EY = Cfg::EY;
     extern __shared__ __align__(16) unsigned char smraw[];
@@ -158,6 +165,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
     // one column parity by consecutive lanes are consecutive words (no bank conflicts; the interleaved layout had 2-way)
     T* const mine = ring + ly * SW + lx;  // column 0 of this thread's pair in slot 0; column 1 is PXN words further
 
+    [[maybe_unused]] double dot = 0.0;
     const long total = (long)g.ntx * g.nty * n2;
     long pos = (long)blockIdx.x * g.items;
     const long end = min(total, pos + g.items);
@@ -166,7 +174,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
         const int k1 = (int)min((long)n2, (long)k0 + (end - pos));
         pos += k1 - k0;
         const int tx = t % g.ntx, ty = t / g.ntx;
-        const int i = tx * Cfg::VX - NHS + 2 * lx, j = ty * Cfg::VY - NHS + ly;
+        const int i = tx * Cfg::VX - NHS + 2 * lx, j = ty * Cfg::VY - Cfg::HY + ly;
         const bool col_in = live && i >= 0 && i < n0 && j >= 0 && j < n1;
         const bool st_ok = col_in && i >= tx * Cfg::VX && i < (tx + 1) * Cfg::VX && j >= ty * Cfg::VY &&
                            j < (ty + 1) * Cfg::VY;
@@ -226,6 +234,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
         // vp / prh point at plane kk (the next plane to load); they are only dereferenced when that plane exists
         auto loadv = [&](int kk) -> P2 {
             P2 v = PairT<T>::make((T)0, (T)0);
+            if (Cfg::ZIN) return v;
             if (kk >= 0 && kk < n2) {
                 if (kind == 1 || kind == 4) v = *reinterpret_cast<const P2*>(vp);
                 else if (kind == 2) v.y = *vp;
@@ -244,6 +253,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
         // the same loads for a plane known to exist (FAST blocks)
         auto loadv_in = [&]() -> P2 {
             P2 v = PairT<T>::make((T)0, (T)0);
+            if (Cfg::ZIN) return v;
             if (kind == 1 || kind == 4) v = *reinterpret_cast<const P2*>(vp);
             else if (kind == 2) v.y = *vp;
             else if (kind == 3) v.x = *vp;
@@ -303,7 +313,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                 const bool actA = (u % 2) == 0;
                 T sxy[NHS];
 #pragma unroll
-                for (int h = 1; h <= NHS; ++h) {
+                for (int h = 1; h <= Cfg::NACT; ++h) {
                     const T* const sp = mine + ((u - h + D) % D) * SLOT;
                     const int ph = (h - u + 2 * D) % D;
                     const T partner = actA ? qB[ph] : qA[ph];
@@ -313,7 +323,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                 }
                 // (2) the dependent chain plane kin-1 -> kin-2 -> ... through the z neighbours, in registers
 #pragma unroll
-                for (int h = 1; h <= NHS; ++h) {
+                for (int h = 1; h <= Cfg::NACT; ++h) {
                     const int kz = kin - h;
                     const bool upd = FAST ? col_in : (col_in && kz >= 0 && kz < n2);
                     const int ph = (h - u + 2 * D) % D, pm = (h + 1 - u + 2 * D) % D, pp = (h - 1 - u + 2 * D) % D;
@@ -337,6 +347,7 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
                 if (FAST ? st_ok : (st_ok && ko >= k0 && ko < k1)) {
                     const int po = (NHS - u + 2 * D) % D;
                     *reinterpret_cast<P2*>(pout) = cA ? PairT<T>::make(qB[po], qA[po]) : PairT<T>::make(qA[po], qB[po]);
+                    if constexpr (Cfg::DOT) dot = fma((double)fB[po], (double)qB[po], fma((double)fA[po], (double)qA[po], dot));
                 }
             }
         };
@@ -346,6 +357,20 @@ __global__ void __launch_bounds__(Cfg::NT, Cfg::MINB)
             if (fast) block(FastTag<true>{}, kin0);
             else block(FastTag<false>{}, kin0);
         }
+    }
+    if constexpr (Cfg::DOT) {  // beta = rz_new / rz_old (0 before the first iteration), Saad Alg. 9.1
+        double vals[1] = {dot};
+        grid_reduce<1>(vals, rb, [=](const double* t) {
+            if (ctl->done) return;
+            const double rz_new = t[0];
+            if (!isfinite(rz_new) || rz_new == 0.0) {
+                ctl->done = 1;
+                ctl->status = POISSON_BREAKDOWN;
+                return;
+            }
+            ctl->beta = ctl->it == 0 ? 0.0 : rz_new / ctl->rz;
+            ctl->rz = rz_new;
+        });
     }
 }
 
@@ -379,24 +404,26 @@ static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, c
     bool plain = op.gamma == 0.0;
     for (int f = 0; f < 6; ++f) plain = plain && op.bc[f] != POISSON_BC_NEUMANN0;
     const size_t smem = (size_t)Cfg::D * Cfg::SLOT * sizeof(T);
+    if (Cfg::DOT && grid > kMaxRedBlocks) return POISSON_UNSUPPORTED;
     int rc = kernel_ready(ctx, k_sor_fused<T, Cfg, true>, Cfg::NT, smem);
     if (rc == POISSON_OK) rc = kernel_ready(ctx, k_sor_fused<T, Cfg, false>, Cfg::NT, smem);
     if (rc != POISSON_OK) return rc;
     if (plain)
-        PB_LAUNCH(ctx, KID_RBSOR, (k_sor_fused<T, Cfg, true><<<grid, Cfg::NT, smem, ctx->stream>>>(op, in, out, rhs, omega, ug, g)));
+        PB_LAUNCH(ctx, KID_RBSOR, (k_sor_fused<T, Cfg, true><<<grid, Cfg::NT, smem, ctx->stream>>>(op, in, out, rhs, omega, ug, g, ctx->d_ctl, ctx->red)));
     else
-        PB_LAUNCH(ctx, KID_RBSOR, (k_sor_fused<T, Cfg, false><<<grid, Cfg::NT, smem, ctx->stream>>>(op, in, out, rhs, omega, ug, g)));
+        PB_LAUNCH(ctx, KID_RBSOR, (k_sor_fused<T, Cfg, false><<<grid, Cfg::NT, smem, ctx->stream>>>(op, in, out, rhs, omega, ug, g, ctx->d_ctl, ctx->red)));
     return POISSON_OK;
 }
 
 // Tile choice: the compiled configuration with the smallest estimated pass time (POISSON_OPT_TILE_CFG overrides).
-template <typename T, int NHS>
+template <typename T, int NHS, int NACT = NHS, bool ZIN = false, bool DOT = false>
 static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, const OmegaSet<T>& omega,
                           bool ug) {
-    using C0 = SorTile<NHS, 32 + NHS, 14 + 2 * NHS>;   // 64 x 14 valid, 612 threads at NHS = 2 (best at 256^3 on B200)
-    using C1 = SorTile<NHS, 16 + NHS, 28 + 2 * NHS>;   // 32 x 28 valid, 576 threads
-    using C2 = SorTile<NHS, 16 + NHS, 10 + 2 * NHS>;   // 32 x 10 valid, 252 threads, two CTAs per SM
-    using C3 = SorTile<NHS, 32 + NHS, 8 + 2 * NHS>;    // 64 x 8 valid, 408 threads
+    constexpr int V0 = NACT < NHS ? 16 : 14;             // a narrower y halo leaves room for two more valid rows
+    using C0 = SorTile<NHS, 32 + NHS, V0 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 64 x 14 valid, 612 threads at NHS = 2 (best at 256^3 on B200)
+    using C1 = SorTile<NHS, 16 + NHS, 28 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 32 x 28 valid, 576 threads
+    using C2 = SorTile<NHS, 16 + NHS, 10 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 32 x 10 valid, 252 threads, two CTAs per SM
+    using C3 = SorTile<NHS, 32 + NHS, 8 + 2 * NACT, 1, NACT, ZIN, DOT>;   // 64 x 8 valid, 408 threads
     SorGeom g[4];
     int grid[4];
     double cost[4] = {sor_cfg_cost<C0>(ctx, op, sizeof(T), &g[0], &grid[0]), sor_cfg_cost<C1>(ctx, op, sizeof(T), &g[1], &grid[1]),
@@ -476,13 +503,17 @@ int sor_fused_seq(poisson_ctx* ctx, const Op& op, double* phi, double* tmp, cons
 }
 // z = (symmetric ? red-black-red : red-black) Gauss-Seidel sweep on L z = f from z = 0 (zin must hold zeros): the
 // multi-colour preconditioner of PAPER.md:107-123 Eq. 10 in ONE pass over HBM.  The result lands in zout.
-int sor_fused_precond(poisson_ctx* ctx, const Op& op, const double* zin, double* zout, const double* f, bool symmetric) {
+// with_rz: the pass also leaves r . z and beta in the Krylov control block (what k_pcg_dot does as a pass of its own).
+int sor_fused_precond(poisson_ctx* ctx, const Op& op, const double* zin, double* zout, const double* f, bool symmetric,
+                      bool with_rz) {
     OmegaSet<double> os;
     os.w[0] = os.w[1] = 1.0;
     os.w[2] = symmetric ? 1.0 : 0.0;
     os.w[3] = 0.0;
-    const int rc = symmetric ? sor_fused_pass<double, 4>(ctx, op, zin, zout, f, os, false)
-                             : sor_fused_pass<double, 2>(ctx, op, zin, zout, f, os, false);
+    if (with_rz && !symmetric) return POISSON_INVALID_ARG;
+    const int rc = !symmetric ? sor_fused_pass<double, 2, 2, true>(ctx, op, zin, zout, f, os, false)
+                   : with_rz  ? sor_fused_pass<double, 4, 3, true, true>(ctx, op, zin, zout, f, os, false)
+                              : sor_fused_pass<double, 4, 3, true>(ctx, op, zin, zout, f, os, false);
     if (rc != POISSON_OK) return rc;
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;

@@ -143,6 +143,18 @@ __device__ __forceinline__ T div_by(T a, T d, T rd) {
     return fma_(r, rd, q);
 }
 
+// ---- full-weighting restriction, one axis at a time -------------------------------------------------------------------
+// R = (1/8)[1 3 3 1] per axis (cell-centred 2:1 coarsening, the transpose of trilinear interpolation).
+// Every restriction kernel evaluates it axis by axis — x, then y, then z — each axis as acc = fma(w_a, v_a, acc) over
+// a = 0..3 from acc = 0, cells outside the domain skipped: 12 multiply-adds per coarse cell instead of the 64 of the
+// tensor-product sum, and the same bits from every kernel (the one-kernel-per-operator path, the bottom-of-the-cycle
+// kernel, the fused residual + restriction pass, whose z sum runs along with the planes).  The values differ from the
+// 64-term sum only by the rounding of the partial sums.  The 8-cell average sums pairs the same way: x, y, z, then / 8.
+template <typename T>
+__device__ __forceinline__ T fw_acc(T acc, int a, T v) {
+    return fma_((a == 0 || a == 3) ? (T)0.125 : (T)0.375, v, acc);
+}
+
 // ---- single-pass grid reduction -------------------------------------------------------------------------------------
 __device__ __forceinline__ double warp_sum(double x) {
 #pragma unroll
