@@ -201,6 +201,21 @@ int poisson_get_ghost_face(poisson_t h, int face, double* d_out);
 long poisson_face_len(poisson_t h, int face);
 /* ||rhs - L phi||_2 with the handle's ghosts. */
 int poisson_residual_norm(poisson_t h, const double* d_phi, const double* d_rhs, double* h_norm);
+/* The same norm for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): no handle, and NO cudaMalloc / cudaFree / allocating library call inside.  L is the Cartesian 7-point
+ * Laplacian (Eq. 1) of the grid `shape` (x fastest) with spacing `spacing`, phi = 0 outside the grid
+ * (what a fresh handle with six DIRICHLET_GHOST faces computes).  d_phi, d_rhs: DEVICE arrays of shape[0] shape[1]
+ * shape[2] doubles on the current device (the caller's; not modified); d_norm: DEVICE double, receives the norm when
+ * the work queued on `cuda_stream` (a cudaStream_t, NULL = default stream) has run — the call does not synchronise.
+ * The block partial sums live in a static 256 KiB device array of the library (every GPU that loads the library holds
+ * it until exit): ceil(shape[0]/32) ceil(shape[1]/8) ceil(shape[2]/16) must not exceed 32768 (512^3 points fit) —
+ * larger grids return UNSUPPORTED.  All calls on a device share that array: calls that overlap on the GPU (different
+ * streams, two threads) race; calls queued on one stream do not.  The first call on a device resolves the array's
+ * address (make it before starting a capture).  Errors: INVALID_ARG (NULL / host / other-device pointers, bad shape),
+ * UNSUPPORTED, CUDA_ERROR; poisson_residual_norm_static_error() describes the calling thread's last one. */
+int poisson_residual_norm_static(const int shape[3], const double spacing[3], const double* d_phi,
+                                 const double* d_rhs, double* d_norm, void* cuda_stream);
+const char* poisson_residual_norm_static_error(void);
 /* Relative residual history of the last Krylov solve (needs POISSON_OPT_RECORD_HISTORY): h_out[0..n-1]. */
 int poisson_get_history(poisson_t h, double* h_out, int n);
 /* Near-breakdown restarts taken and true-residual confirmations that failed in the last BiCGSTAB solve (nullable). */

@@ -31,6 +31,7 @@ SYMBOLS = [
     "poisson_bicgstab_solve_host", "poisson_mg_vcycle_host", "poisson_multipole_bc_host",
     "poisson_spai_smooth", "poisson_mgv_vcycle", "poisson_mgv_vcycle_host",
     "poisson_rbsor_cheby", "poisson_rbsor_local", "poisson_pcg_solve", "poisson_multipole_inner_moments",
+    "poisson_residual_norm_static", "poisson_residual_norm_static_error",
 ]
 
 _lib = None
@@ -52,6 +53,8 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.poisson_last_error.restype = C.c_char_p
         L.poisson_last_error.argtypes = [C.c_void_p]
+        L.poisson_residual_norm_static_error.restype = C.c_char_p
+        L.poisson_residual_norm_static_error.argtypes = []
         L.poisson_face_len.restype = C.c_long
         L.poisson_face_len.argtypes = [C.c_void_p, C.c_int]
         L.poisson_kernel_launches.restype = C.c_long
@@ -81,6 +84,17 @@ def _ptr(t):
         return C.c_void_p(t.ctypes.data)
     assert t.is_contiguous(), "arrays must be contiguous"
     return C.c_void_p(t.data_ptr())
+
+
+def residual_norm_static(shape, spacing, d_phi, d_rhs, d_norm, stream=0):
+    """||rhs - L phi||_2 into the device double d_norm, through the entry point that allocates nothing (static
+    scratch; include/poisson.h).  Queued on `stream` (a raw cudaStream_t, 0 = default stream); does not synchronise."""
+    rc = lib().poisson_residual_norm_static((C.c_int * 3)(*[int(s) for s in shape]),
+                                            (C.c_double * 3)(*[float(h) for h in spacing]), _ptr(d_phi), _ptr(d_rhs),
+                                            _ptr(d_norm), C.c_void_p(int(stream)))
+    if rc != OK:
+        raise PoissonError(rc, lib().poisson_residual_norm_static_error().decode())
+    return rc
 
 
 class Poisson:
