@@ -139,15 +139,17 @@ void orc_prolong_add(void* h, const double* ec, double* phi, double coarse_gamma
     prolong_add(*g, c, ec, phi);
 }
 
-void orc_spai_smooth(void* h, double* phi, const double* rhs, const double* spai, int nsteps) {
-    spai_smooth(*(Grid*)h, phi, rhs, spai, nsteps);
+void orc_spai_smooth(void* h, double* phi, const double* rhs, const double* spai, int nsteps, int order) {
+    spai_smooth(*(Grid*)h, phi, rhs, spai, nsteps, order);
 }
 int orc_mgv_vcycle(void* h, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, const double* spai,
-                   double cg_rtol, int storage_f32, int ncycles, double* resnorms) {
-    return mgv_vcycle(*(Grid*)h, phi, rhs, nu1, nu2, coarsest_n, spai, cg_rtol, storage_f32, ncycles, resnorms);
+                   double cg_rtol, int storage_f32, int ncycles, double* resnorms, int order) {
+    return mgv_vcycle(*(Grid*)h, phi, rhs, nu1, nu2, coarsest_n, spai, cg_rtol, storage_f32, ncycles, resnorms, order);
 }
-int orc_mgv_galerkin_stencil(void* h, int level, int I, int J, int K, double* out27) {
-    return mgv_galerkin_stencil(*(Grid*)h, level, I, J, K, out27);
+int orc_compact_apply(void* h, int order, const double* v, double* out) { return compact_apply(*(Grid*)h, order, v, out); }
+int orc_compact_rhs(const int* n, int order, const double* f_ext, double* out) { return compact_rhs(n, order, f_ext, out); }
+int orc_mgv_galerkin_stencil(void* h, int level, int I, int J, int K, double* out27, int order) {
+    return mgv_galerkin_stencil(*(Grid*)h, level, I, J, K, out27, order);
 }
 void orc_mgv_restrict(void* h, const double* r, double* bc) { mgv_restrict(*(Grid*)h, r, bc); }
 void orc_mgv_prolong_add(void* h, const double* ec, double* x) { mgv_prolong_add(*(Grid*)h, ec, x); }

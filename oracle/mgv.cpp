@@ -48,17 +48,41 @@ inline double row27(const VLevel& L, const double* v, int i, int j, int k) {
     return s;
 }
 
-// Level 0: the 7-point operator A = -L_h as 27 coefficients per point (PAPER.md:43-45 with the sign of PAPER.md:105).
-VLevel level0(const Grid& g) {
+// The compact radius-1 discretisations of the Laplacian ("compact stencils of radius unity even for
+// fourth order, or, assuming isotropic spacing, even for sixth order (Spotz & Carey 1996)").  PAPER.md prints no
+// coefficients; they follow from the Taylor expansion (reading C19).  With the 1-D second difference d_a^2
+// (= h^2 D_a^2 + h^4 D_a^4 / 12 + h^6 D_a^6 / 360 + ...) and S1 = sum_a d_a^2, S2 = sum_{a<b} d_a^2 d_b^2,
+// S3 = d_x^2 d_y^2 d_z^2:
+//   order 2:  L_h = S1 / h^2                        = lap + O(h^2)                                      7 points
+//   order 4:  L_h = (S1 + S2/6) / h^2               = lap + h^2/12 lap^2 + O(h^4)                       19 points
+//   order 6:  L_h = (S1 + S2/6 + S3/30) / h^2       = lap + h^2/12 lap^2 + h^4/360 [lap^3 + 2 (D_x^2 D_y^2 + D_y^2 D_z^2
+//                                                     + D_z^2 D_x^2) lap] + O(h^6)                      27 points
+// so that L_h u = (the same operators applied to f) for lap u = f: see compact_rhs below.  In weights per number of
+// non-zero offsets (centre, 6 faces, 12 edges, 8 corners) x 1/h^2:
+//   order 2: -6, 1, 0, 0      order 4: -4, 1/3, 1/6, 0  (= (-24, 2, 1, 0)/6)
+//   order 6: -64/15, 7/15, 1/10, 1/30  (= (-128, 14, 3, 1)/30)
+bool compact_weights(int order, double w[4]) {
+    if (order == 2) { w[0] = -6.0; w[1] = 1.0; w[2] = 0.0; w[3] = 0.0; return true; }
+    if (order == 4) { w[0] = -4.0; w[1] = 1.0 / 3.0; w[2] = 1.0 / 6.0; w[3] = 0.0; return true; }
+    if (order == 6) { w[0] = -64.0 / 15.0; w[1] = 7.0 / 15.0; w[2] = 1.0 / 10.0; w[3] = 1.0 / 30.0; return true; }
+    return false;
+}
+
+// Level 0: A = -L_h as 27 coefficients per point (PAPER.md:43-45 with the sign of PAPER.md:105); order 2: 7-point.
+VLevel level0(const Grid& g, int order = 2) {
     VLevel L;
     for (int a = 0; a < 3; ++a) L.n[a] = g.n[a];
     L.h = g.h[0];
     L.coef.assign(L.size() * 27, 0.0);
     const double c = 1.0 / (L.h * L.h);
+    double w[4];
+    compact_weights(order, w);
     for (size_t p = 0; p < L.size(); ++p) {
         double* q = &L.coef[p * 27];
-        q[13] = 6.0 * c;
-        q[12] = q[14] = q[10] = q[16] = q[4] = q[22] = -c;
+        for (int dk = -1; dk <= 1; ++dk)
+            for (int dj = -1; dj <= 1; ++dj)
+                for (int di = -1; di <= 1; ++di)
+                    q[((dk + 1) * 3 + (dj + 1)) * 3 + (di + 1)] = -w[(di != 0) + (dj != 0) + (dk != 0)] * c;
     }
     return L;
 }
@@ -268,14 +292,14 @@ void cycle_coarse(const Hier& H, size_t l, std::vector<double>& e, std::vector<d
     }
 }
 
-Hier build(const Grid& g, int nu1, int nu2, int coarsest_n, const double spai[5], double cg_rtol, int f32) {
+Hier build(const Grid& g, int nu1, int nu2, int coarsest_n, const double spai[5], double cg_rtol, int f32, int order) {
     Hier H;
     H.nu1 = nu1;
     H.nu2 = nu2;
     H.cg_rtol = cg_rtol;
     H.f32 = f32 != 0;
     for (int c = 0; c < 5; ++c) H.sp[c] = spai[c];
-    H.lv.push_back(level0(g));
+    H.lv.push_back(level0(g, order));
     while (true) {
         const VLevel& F = H.lv.back();
         bool ok = true;
@@ -293,18 +317,84 @@ Hier build(const Grid& g, int nu1, int nu2, int coarsest_n, const double spai[5]
 }  // namespace
 
 // x <- x + omega M (rhs-form residual) on the user's grid: nsteps SPAI steps of Eq. 15 for L_h phi = rhs.
-void spai_smooth(const Grid& g, double* phi, const double* rhs, const double spai[5], int nsteps) {
-    VLevel L0 = level0(g);
+// order 2: the grid's 7-point operator with its ghost faces; order 4 / 6: the compact operator with ZERO Dirichlet values
+// (boundary data belong in the right-hand side there) and rhs = the transformed right-hand side of compact_rhs.
+void residual_level0(const Grid& g, const VLevel& L0, int order, const double* x, const double* rhs, double* r) {
+    if (order == 2) {
+        residual0(g, x, rhs, r);
+        return;
+    }
+    std::vector<double> b(L0.size());
+    for (size_t m = 0; m < b.size(); ++m) b[m] = -rhs[m];
+    residual27(L0, x, b.data(), r);
+}
+
+void spai_smooth(const Grid& g, double* phi, const double* rhs, const double spai[5], int nsteps, int order) {
+    VLevel L0 = level0(g, order);
     std::vector<double> r(L0.size());
     for (int s = 0; s < nsteps; ++s) {
-        residual0(g, phi, rhs, r.data());
+        residual_level0(g, L0, order, phi, rhs, r.data());
         spai_update(L0, phi, r.data(), spai);
     }
 }
 
+// out = L_h v, the compact Laplacian of the given order with zero Dirichlet values outside the grid.
+int compact_apply(const Grid& g, int order, const double* v, double* out) {
+    double w[4];
+    if (!compact_weights(order, w) || g.h[0] != g.h[1] || g.h[0] != g.h[2]) return -1;
+    VLevel L0 = level0(g, order);
+    for (int k = 0; k < g.n[2]; ++k)
+        for (int j = 0; j < g.n[1]; ++j)
+            for (int i = 0; i < g.n[0]; ++i) out[L0.idx(i, j, k)] = -row27(L0, v, i, j, k);
+    return 0;
+}
+
+// Right-hand side of the compact schemes: for lap u = f the discrete equation is L_h u = B f with
+//   order 4:  B f = f + h^2/12 lap f                                   -> f + S1 f / 12
+//   order 6:  B f = f + h^2/12 lap f + h^4/360 [lap^2 f + 2 (f_xxyy + f_yyzz + f_zzxx)]
+//                 -> f + S1 f / 12 - (sum_a d_a^4 f) / 240 + S2 f / 90
+// (lap f = S1 f / h^2 - h^2/12 sum_a D_a^4 f + O(h^4) moves -1/144 + 1/360 = -1/240 onto the fourth differences, which
+// reach two points out; lap^2 f + 2 (...) = sum_a D_a^4 f + 4 sum_{a<b} D_a^2 D_b^2 f.)
+// f_ext: f on the grid extended by TWO layers per side, (n0+4)(n1+4)(n2+4) values, x fastest; order 2: a copy.
+int compact_rhs(const int n[3], int order, const double* f_ext, double* out) {
+    if (order != 2 && order != 4 && order != 6) return -1;
+    const int e0 = n[0] + 4, e1 = n[1] + 4;
+    auto F = [&](int i, int j, int k) -> double { return f_ext[((size_t)(k + 2) * e1 + (j + 2)) * e0 + (i + 2)]; };
+    for (int k = 0; k < n[2]; ++k)
+        for (int j = 0; j < n[1]; ++j)
+            for (int i = 0; i < n[0]; ++i) {
+                const double f0 = F(i, j, k);
+                double v = f0;
+                if (order >= 4) {
+                    const double s1 = (F(i - 1, j, k) + F(i + 1, j, k)) + (F(i, j - 1, k) + F(i, j + 1, k)) +
+                                      (F(i, j, k - 1) + F(i, j, k + 1)) - 6.0 * f0;
+                    v += s1 / 12.0;
+                }
+                if (order == 6) {
+                    auto d4 = [&](int di, int dj, int dk) -> double {
+                        return F(i - 2 * di, j - 2 * dj, k - 2 * dk) - 4.0 * F(i - di, j - dj, k - dk) + 6.0 * f0 -
+                               4.0 * F(i + di, j + dj, k + dk) + F(i + 2 * di, j + 2 * dj, k + 2 * dk);
+                    };
+                    // d_a^2 d_b^2 f: the 9-point cross difference in the plane of axes a, b
+                    auto d22 = [&](int ai, int aj, int ak, int bi, int bj, int bk) -> double {
+                        double s = 0.0;
+                        const double c1[3] = {1.0, -2.0, 1.0};
+                        for (int p = -1; p <= 1; ++p)
+                            for (int q = -1; q <= 1; ++q)
+                                s += c1[p + 1] * c1[q + 1] * F(i + p * ai + q * bi, j + p * aj + q * bj, k + p * ak + q * bk);
+                        return s;
+                    };
+                    v -= (d4(1, 0, 0) + d4(0, 1, 0) + d4(0, 0, 1)) / 240.0;
+                    v += (d22(1, 0, 0, 0, 1, 0) + d22(0, 1, 0, 0, 0, 1) + d22(0, 0, 1, 1, 0, 0)) / 90.0;
+                }
+                out[((size_t)k * n[1] + j) * n[0] + i] = v;
+            }
+    return 0;
+}
+
 // Galerkin stencil of coarse level `level` (>= 1) at coarse point (I,J,K): 27 coefficients.
-int mgv_galerkin_stencil(const Grid& g, int level, int I, int J, int K, double* out27) {
-    VLevel L = level0(g);
+int mgv_galerkin_stencil(const Grid& g, int level, int I, int J, int K, double* out27, int order) {
+    VLevel L = level0(g, order);
     for (int l = 0; l < level; ++l) {
         for (int a = 0; a < 3; ++a)
             if (L.n[a] % 2 == 0 || L.n[a] < 3) return -1;
@@ -328,15 +418,27 @@ void mgv_prolong_add(const Grid& g, const double* ec, double* x) {
 
 // ncycles V-cycles (Eq. 11) on L_h phi = rhs; storage_f32: coarse levels stored in fp32.
 // resnorms (nullable, ncycles+1): ||rhs - L_h phi||_2 before the first and after every cycle (for Eq. 18).
+// order: the level-0 discretisation (2: the grid's 7-point operator and ghost faces; 4, 6: compact, zero boundary values,
+// rhs = compact_rhs output; the norms are then those of the compact residual).
 int mgv_vcycle(const Grid& g, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, const double spai[5],
-               double cg_rtol, int storage_f32, int ncycles, double* resnorms) {
+               double cg_rtol, int storage_f32, int ncycles, double* resnorms, int order) {
     if (g.coord != CARTESIAN || g.order != 2 || g.h[0] != g.h[1] || g.h[0] != g.h[2]) return -1;
+    if (order != 2 && order != 4 && order != 6) return -1;
     for (int f = 0; f < 6; ++f)
         if (g.bc[f] != BC_DIRICHLET_GHOST) return -1;
-    Hier H = build(g, nu1, nu2, coarsest_n, spai, cg_rtol, storage_f32);
+    Hier H = build(g, nu1, nu2, coarsest_n, spai, cg_rtol, storage_f32, order);
     const VLevel& L0 = H.lv[0];
     std::vector<double> r(L0.size());
-    if (resnorms) resnorms[0] = residual_norm(g, phi, rhs, true);
+    auto residual0 = [&](const Grid& gg, const double* x, const double* f, double* out) {
+        residual_level0(gg, L0, order, x, f, out);
+    };
+    auto norm0 = [&]() -> double {
+        if (order == 2) return residual_norm(g, phi, rhs, true);
+        std::vector<double> t(L0.size());
+        residual0(g, phi, rhs, t.data());
+        return (double)sqrtl(dotv(t, t));
+    };
+    if (resnorms) resnorms[0] = norm0();
     for (int c = 0; c < ncycles; ++c) {
         if (H.lv.size() == 1) {
             // no coarse level: the "coarsest solve" is CG on the error equation A e = r
@@ -360,7 +462,7 @@ int mgv_vcycle(const Grid& g, double* phi, const double* rhs, int nu1, int nu2, 
                 spai_update(L0, phi, r.data(), H.sp);
             }
         }
-        if (resnorms) resnorms[c + 1] = residual_norm(g, phi, rhs, true);
+        if (resnorms) resnorms[c + 1] = norm0();
     }
     return ST_OK;
 }

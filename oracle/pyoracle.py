@@ -16,6 +16,12 @@ BC_DIRICHLET_GHOST, BC_PERIODIC, BC_NEUMANN0, BC_AXIS = 0, 1, 2, 3
 
 # PAPER.md:176-182 Table 1, row "Order 2": omega, alpha, beta, gamma, delta of the SPAI smoother (Eq. 15-16)
 SPAI_ORDER2 = (1.3699, 0.1432, 0.0284, 0.0081, 0.0025)
+# rows "Order 4" and "Order 6" (for the compact radius-1 discretisations of PAPER.md:172).  The delta of order 6 is
+# printed as 0.0909, a copy of the mu column (reading C20): taken as 0.0150, the middle of the interval
+# [0.0140, 0.0160] on which the local-Fourier smoothing factor of Eq. 17 is smallest with the other printed values.
+SPAI_ORDER4 = (0.9363, 0.2807, 0.0329, 0.0166, 0.0044)
+SPAI_ORDER6 = (0.3543, 0.7064, 0.1005, 0.0363, 0.0150)
+SPAI = {2: SPAI_ORDER2, 4: SPAI_ORDER4, 6: SPAI_ORDER6}
 
 _lib = None
 
@@ -245,26 +251,35 @@ class Oracle:
         lib().orc_prolong_add(self.h, _p(ec), _p(phi), C.c_double(coarse_gamma))
 
     # ---- the paper's own multigrid (oracle/mgv.cpp) ----
-    def spai_smooth(self, phi, rhs, spai=SPAI_ORDER2, nsteps=1):
+    def spai_smooth(self, phi, rhs, spai=None, nsteps=1, order=2):
+        """order 4 / 6: the compact operator, zero boundary values, rhs = compact_rhs(...) (oracle/mgv.cpp)."""
         assert phi.dtype == np.float64 and phi.flags.c_contiguous
-        rhs, sp = _f64(rhs), _f64(np.array(spai))
-        lib().orc_spai_smooth(self.h, _p(phi), _p(rhs), _p(sp), int(nsteps))
+        rhs, sp = _f64(rhs), _f64(np.array(SPAI[order] if spai is None else spai))
+        lib().orc_spai_smooth(self.h, _p(phi), _p(rhs), _p(sp), int(nsteps), int(order))
 
-    def mgv_vcycle(self, phi, rhs, nu1=1, nu2=1, coarsest_n=3, spai=SPAI_ORDER2, cg_rtol=1e-3, storage_f32=False,
-                   ncycles=1):
+    def mgv_vcycle(self, phi, rhs, nu1=1, nu2=1, coarsest_n=3, spai=None, cg_rtol=1e-3, storage_f32=False,
+                   ncycles=1, order=2):
         assert phi.dtype == np.float64 and phi.flags.c_contiguous
-        rhs, sp = _f64(rhs), _f64(np.array(spai))
+        rhs, sp = _f64(rhs), _f64(np.array(SPAI[order] if spai is None else spai))
         rn = np.zeros(ncycles + 1)
         fn = lib().orc_mgv_vcycle
         fn.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_double, C.c_int,
-                       C.c_int, C.c_void_p]
+                       C.c_int, C.c_void_p, C.c_int]
         st = fn(self.h, phi.ctypes.data, rhs.ctypes.data, int(nu1), int(nu2), int(coarsest_n), sp.ctypes.data,
-                float(cg_rtol), int(bool(storage_f32)), int(ncycles), rn.ctypes.data)
+                float(cg_rtol), int(bool(storage_f32)), int(ncycles), rn.ctypes.data, int(order))
         return dict(status=int(st), resnorms=rn)
 
-    def mgv_galerkin_stencil(self, level, I, J, K):
+    def compact_apply(self, v, order):
+        """L_h v with the compact radius-1 Laplacian of the given order, zero values outside the grid."""
+        v = _f64(v)
+        out = np.zeros_like(v)
+        rc = lib().orc_compact_apply(self.h, int(order), _p(v), _p(out))
+        assert rc == 0
+        return out
+
+    def mgv_galerkin_stencil(self, level, I, J, K, order=2):
         out = np.zeros(27)
-        rc = lib().orc_mgv_galerkin_stencil(self.h, int(level), int(I), int(J), int(K), _p(out))
+        rc = lib().orc_mgv_galerkin_stencil(self.h, int(level), int(I), int(J), int(K), _p(out), int(order))
         assert rc == 0
         return out.reshape(3, 3, 3)
 
@@ -298,6 +313,19 @@ class Oracle:
 
     def r_ghost_out(self):
         return float(lib().orc_r_ghost_out(self.h))
+
+
+def compact_rhs(f_ext, order):
+    """B f of the compact scheme of the given order (oracle/mgv.cpp compact_rhs): f_ext carries two extra layers per side
+    (numpy shape (n2+4, n1+4, n0+4)); returns shape (n2, n1, n0)."""
+    f_ext = _f64(f_ext)
+    n = (C.c_int * 3)(f_ext.shape[2] - 4, f_ext.shape[1] - 4, f_ext.shape[0] - 4)
+    out = np.zeros((f_ext.shape[0] - 4, f_ext.shape[1] - 4, f_ext.shape[2] - 4))
+    fn = lib().orc_compact_rhs
+    fn.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+    rc = fn(n, int(order), f_ext.ctypes.data, out.ctypes.data)
+    assert rc == 0
+    return out
 
 
 def multipole_inner_potential(qbar, lmax, G, x, y, z):

@@ -56,10 +56,13 @@ Grid coarsen(const Grid& fine, int level_of_coarse);
 
 // ---- the paper's own multigrid (mgv.cpp): vertex-centred, Galerkin, SPAI smoother, CG coarsest; PAPER.md:125-205 -------
 // spai[5] = {omega, alpha, beta, gamma, delta} of Eq. 15-16 (Table 1).
-void spai_smooth(const Grid& g, double* phi, const double* rhs, const double spai[5], int nsteps);
+void spai_smooth(const Grid& g, double* phi, const double* rhs, const double spai[5], int nsteps, int order = 2);
+// compact radius-1 discretisations of order 2 / 4 / 6: the operator and its right-hand-side transform
+int compact_apply(const Grid& g, int order, const double* v, double* out);
+int compact_rhs(const int n[3], int order, const double* f_ext, double* out);
 int mgv_vcycle(const Grid& g, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, const double spai[5],
-               double cg_rtol, int storage_f32, int ncycles, double* resnorms /* nullable, ncycles+1 */);
-int mgv_galerkin_stencil(const Grid& g, int level, int I, int J, int K, double* out27);
+               double cg_rtol, int storage_f32, int ncycles, double* resnorms /* nullable, ncycles+1 */, int order = 2);
+int mgv_galerkin_stencil(const Grid& g, int level, int I, int J, int K, double* out27, int order = 2);
 void mgv_restrict(const Grid& g, const double* r, double* bc);
 void mgv_prolong_add(const Grid& g, const double* ec, double* x);
 
