@@ -56,6 +56,8 @@ ROW_BYTES = {
     "rbsor_cheby_sweep": 12,        # f4: the fused kernel with one omega per half-step: 24/T, T = 2
     "rbsor_local_sweep": 48,        # f4: spherical, position-dependent omega: two unfused half-sweeps
     "mgv_vcycle_f64_511": 94,       # f2 at the paper's own size (Table 2: 511^3, seven coarse levels, nu = 1)
+    "spai_smooth_o6": 24,           # f1: the SPAI step on the compact 27-point sixth-order operator (same bytes, 27-point A)
+    "mgv_vcycle_o6_511": 94,        # f1 + f2: Table 2, order 6: 511^3, V(1,1)
 }
 NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 250
 ROW_CITE = {
@@ -66,6 +68,8 @@ ROW_CITE = {
     "spai_smooth": "f1 PAPER.md:154-184", "mgv_vcycle_f64": "f2 PAPER.md:125-152", "mgv_vcycle_mixed": "f2 PAPER.md:205",
     "pcg_iteration": "f3 PAPER.md:107-123", "rbsor_cheby_sweep": "f4 PAPER.md:81-88", "rbsor_local_sweep": "f4 PAPER.md:88-93",
     "mgv_vcycle_f64_511": "f2 PAPER.md:186-195 Table 2 (paper: 34.8 ms per V(1,1) cycle = 3.83 Gzups, hardware not stated)",
+    "spai_smooth_o6": "f1 PAPER.md:172-182 (compact order 6, Table 1 row 6)",
+    "mgv_vcycle_o6_511": "f1 PAPER.md:186-195 Table 2 order 6 (paper: 35.3 ms per V(1,1) cycle)",
 }
 
 
@@ -238,6 +242,10 @@ def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
             phi.zero_()
             gv.mgv_vcycle(phi, rhs, nu1=1, nu2=1, precision=prec, ncycles=ncyc, want_resnorms=False)
         out.append((name, nv ** 3, ncyc, timed(cyc, ncyc, name)))
+    del gv
+    gv = pb.Poisson((nv,) * 3, (2.0 / (nv + 1),) * 3, (-1 + 2.0 / (nv + 1),) * 3, bc=(0,) * 6, stream=stream.cuda_stream)
+    gv.set_option(pb.OPT_COMPACT_ORDER, 6)
+    out.append(("spai_smooth_o6", nv ** 3, nsm, timed(lambda: gv.spai_smooth(phi, rhs, nsteps=nsm), nsm, "spai_smooth_o6")))
     del gv, rhs, phi
     if not light:
         # the paper's own Table 2 configuration: 511^3, seven coarse levels, V(1,1), order 2, fp64
@@ -253,6 +261,11 @@ def measure_next_rows(p, args, pb, torch, stream, g3, g5, d, omega3):
             phi.zero_()
             gv.mgv_vcycle(phi, rhs, nu1=1, nu2=1, precision=pb.F64, ncycles=ncyc, want_resnorms=False)
         out.append(("mgv_vcycle_f64_511", n5v ** 3, ncyc, timed(cyc511, ncyc, "mgv_vcycle_f64_511")))
+        # f1: the compact sixth-order discretisation (zero boundary values, right-hand side taken as it is)
+        del gv
+        gv = pb.Poisson((n5v,) * 3, (2.0 / (n5v + 1),) * 3, (-1 + 2.0 / (n5v + 1),) * 3, bc=(0,) * 6, stream=stream.cuda_stream)
+        gv.set_option(pb.OPT_COMPACT_ORDER, 6)
+        out.append(("mgv_vcycle_o6_511", n5v ** 3, ncyc, timed(cyc511, ncyc, "mgv_vcycle_o6_511")))
         del gv, rhs, phi
     # f3: Gauss-Seidel-preconditioned CG, f4: Chebyshev omega sequence, both on the config-3 grid (7-point, Dirichlet)
     npcg, nsw = (5, 4) if light else (50, 20)

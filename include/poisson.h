@@ -72,6 +72,9 @@ enum {
     POISSON_OPT_TILE_CFG = 9,      /* index of the compiled tile configuration of the fused SOR / lean apply kernels */
     POISSON_OPT_PLANE_SPLIT = 10,  /* plane engine: 1 = always split the (tile, plane) items linearly, 0 = never */
     POISSON_OPT_APPLY_BULK = 11,   /* TMA-staged 7-point apply: 1 = whenever eligible, 0 = never */
+    POISSON_OPT_COMPACT_ORDER = 12,/* level-0 discretisation of poisson_spai_smooth / poisson_mgv_vcycle: 2 (default; the
+                                      handle's 7-point operator with its ghost faces), 4 or 6 = the compact radius-1
+                                      19- / 27-point discretisations of PAPER.md:172 (see poisson_compact_rhs) */
     /* floating-point options (poisson_set_option_f64) */
     POISSON_OPT_BICG_RESTART_EPS = 8 /* BiCGSTAB near-breakdown restart threshold on |r0^.r| / (|r0^| |r|); default
                                       1e-12 (reading C4), 0 = never restart */
@@ -179,6 +182,19 @@ int poisson_mg_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1, 
  *   in fp32, all arithmetic in fp64.  UNSUPPORTED when the grid admits no coarse level.
  *   h_resnorms (nullable, ncycles+1): ||rhs - L phi||_2 before the first and after every cycle (for Eq. 18). */
 int poisson_spai_smooth(poisson_t h, double* d_phi, const double* d_rhs, const double* spai, int nsteps);
+/* Compact discretisations (radius-1 stencils of 4th and, on isotropic grids, 6th order; the paper
+ * prints no coefficients — DESIGN.md reading C19).  With POISSON_OPT_COMPACT_ORDER = 4 or 6, poisson_spai_smooth and
+ * poisson_mgv_vcycle work on L_h phi = d_rhs with
+ *   L_h = (S1 + S2/6 [+ S3/30]) / h^2,  S1 = sum_a d_a^2, S2 = sum_{a<b} d_a^2 d_b^2, S3 = d_x^2 d_y^2 d_z^2
+ * (stencil weights (-24, 2, 1, 0)/6h^2 and (-128, 14, 3, 1)/30h^2 on centre, faces, edges, corners), ZERO values on the
+ * boundary vertices (the handle's ghost faces must be unset: fold boundary data into the right-hand side), the SPAI
+ * rows 4 / 6 of Table 1 by default (delta of row 6: 0.0150, reading C20), and d_rhs = the TRANSFORMED right-hand side
+ * that poisson_compact_rhs computes for lap u = f:
+ *   order 4: f + S1 f / 12;   order 6: f + S1 f / 12 - (sum_a d_a^4 f) / 240 + S2 f / 90;   order 2: f.
+ * d_f_ext: DEVICE array of (n0+4)(n1+4)(n2+4) doubles, f on the grid extended by two layers per side (x fastest);
+ * d_out: DEVICE array of n0 n1 n2 doubles.  The residual norms poisson_mgv_vcycle reports are then those of this
+ * operator.  Errors: INVALID_ARG, UNSUPPORTED (non-Cartesian, anisotropic, ghosts set). */
+int poisson_compact_rhs(poisson_t h, const double* d_f_ext, double* d_out);
 int poisson_mgv_vcycle(poisson_t h, double* d_phi, const double* d_rhs, int nu1, int nu2, int coarsest_n,
                        const double* spai, double cg_rtol, int precision, int ncycles, double* h_resnorms);
 

@@ -17,7 +17,7 @@ OK, NOT_CONVERGED, BREAKDOWN = 0, 1, 2
 INVALID_ARG, UNSUPPORTED, CUDA_ERROR, OUT_OF_MEMORY = -1, -2, -3, -4
 OPT_KERNEL_PATH, OPT_RESTRICTION, OPT_POLL_INTERVAL, OPT_JACOBI, OPT_RECORD_HISTORY, OPT_TIME_KERNELS = 0, 1, 2, 3, 4, 5
 OPT_SOR_HALFSTEPS, OPT_FUSED_RESTRICT, OPT_BICG_RESTART_EPS = 6, 7, 8
-OPT_TILE_CFG, OPT_PLANE_SPLIT, OPT_APPLY_BULK = 9, 10, 11
+OPT_TILE_CFG, OPT_PLANE_SPLIT, OPT_APPLY_BULK, OPT_COMPACT_ORDER = 9, 10, 11, 12
 PATH_AUTO, PATH_GENERIC, PATH_PLANE = 0, 1, 2
 
 SYMBOLS = [
@@ -31,7 +31,7 @@ SYMBOLS = [
     "poisson_bicgstab_solve_host", "poisson_mg_vcycle_host", "poisson_multipole_bc_host",
     "poisson_spai_smooth", "poisson_mgv_vcycle", "poisson_mgv_vcycle_host",
     "poisson_rbsor_cheby", "poisson_rbsor_local", "poisson_pcg_solve", "poisson_multipole_inner_moments",
-    "poisson_residual_norm_static", "poisson_residual_norm_static_error",
+    "poisson_residual_norm_static", "poisson_residual_norm_static_error", "poisson_compact_rhs",
 ]
 
 _lib = None
@@ -258,6 +258,9 @@ class Poisson:
     def spai_smooth(self, d_phi, d_rhs, spai=None, nsteps=1):
         sp = (C.c_double * 5)(*spai) if spai is not None else None
         self._check(lib().poisson_spai_smooth(self.h, _ptr(d_phi), _ptr(d_rhs), sp, int(nsteps)))
+
+    def compact_rhs(self, d_f_ext, d_out):
+        self._check(lib().poisson_compact_rhs(self.h, _ptr(d_f_ext), _ptr(d_out)))
 
     def mgv_vcycle(self, d_phi, d_rhs, nu1=1, nu2=1, coarsest_n=3, spai=None, cg_rtol=1e-3, precision=F64, ncycles=1,
                    want_resnorms=True, _fn=None):

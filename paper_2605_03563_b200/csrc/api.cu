@@ -370,6 +370,12 @@ int poisson_set_option(poisson_t ctx, int option, int value) {
         case POISSON_OPT_APPLY_BULK:
             ctx->opt_apply_bulk = value < 0 ? -1 : (value ? 1 : 0);
             return POISSON_OK;
+        case POISSON_OPT_COMPACT_ORDER:
+            if (value != 2 && value != 4 && value != 6) return fail(ctx, POISSON_INVALID_ARG, "compact order must be 2, 4 or 6");
+            if (value != 2 && (ctx->kind != KIND_CART2 || ctx->h[0] != ctx->h[1] || ctx->h[0] != ctx->h[2]))
+                return fail(ctx, POISSON_UNSUPPORTED, "compact orders 4 / 6: Cartesian grid with isotropic spacing, created with stencil order 2 (PAPER.md:172)");
+            ctx->opt_compact_order = value;
+            return POISSON_OK;
         case POISSON_OPT_TIME_KERNELS:
             if (value < -2 || value >= KID_COUNT) return fail(ctx, POISSON_INVALID_ARG, "bad kernel class");
             ctx->time_kid = value;
@@ -884,7 +890,10 @@ int poisson_mgv_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu
         return fail(ctx, POISSON_INVALID_ARG, "bad V-cycle parameters");
     auto record_norm = [&](int slot) -> int {
         if (!h_resnorms) return POISSON_OK;
-        int r2 = launch_apply(ctx, ctx->op, ctx->kind, d_phi, d_rhs, nullptr, 1, true, true);
+        // order 2: the handle's 7-point residual with its ghosts; compact orders: the residual of the compact operator
+        int r2 = ctx->opt_compact_order == 2
+                     ? launch_apply(ctx, ctx->op, ctx->kind, d_phi, d_rhs, nullptr, 1, true, true)
+                     : mgv_residual_norm2(ctx, d_phi, d_rhs, coarsest_n, precision == POISSON_MIXED);
         if (r2 != POISSON_OK) return r2;
         PB_CUDA_OK(cudaMemcpyAsync(ctx->d_scal + 16 + slot, ctx->d_scal, sizeof(double), cudaMemcpyDeviceToDevice,
                                    ctx->stream));
@@ -902,6 +911,14 @@ int poisson_mgv_vcycle(poisson_t ctx, double* d_phi, const double* d_rhs, int nu
         for (int c = 0; c <= ncycles; ++c) h_resnorms[c] = std::sqrt(ctx->h_scal[c]);
     }
     return POISSON_OK;
+}
+
+int poisson_compact_rhs(poisson_t ctx, const double* d_f_ext, double* d_out) {
+    const DeviceGuard on_device(ctx);
+    if (!ctx || !d_f_ext || !d_out) return fail(ctx, POISSON_INVALID_ARG, "bad pointers");
+    if (ctx->kind != KIND_CART2 || ctx->h[0] != ctx->h[1] || ctx->h[0] != ctx->h[2])
+        return fail(ctx, POISSON_UNSUPPORTED, "compact right-hand side: Cartesian grid with isotropic spacing (PAPER.md:172)");
+    return mgv_compact_rhs(ctx, d_f_ext, d_out);
 }
 
 // ---- multipole boundary -------------------------------------------------------------------------------------------------

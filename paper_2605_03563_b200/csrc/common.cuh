@@ -139,7 +139,8 @@ struct poisson_ctx {
     int mg_coarsest_n = -1;
     std::vector<pb::MgvLevel> vlevels;  // the paper's vertex-centred hierarchy
     double* v_sten = nullptr;           // 4 stencil coefficients per level (device)
-    int v_key[2] = {-1, -1};            // (coarsest_n, fp32 storage) the hierarchy was built for
+    int v_key[3] = {-1, -1, -1};        // (coarsest_n, fp32 storage, compact order) the hierarchy was built for
+    int opt_compact_order = 2;          // level-0 discretisation of the SPAI / Galerkin multigrid: 2, 4 or 6
     // options
     int opt_path = 0, opt_restriction = 0, opt_poll = 16, opt_jacobi = 1, opt_history = 0;
     int opt_sor_nhs = 0;             // colour half-steps fused per HBM pass of the red-black kernel (2, 4; 0 = auto)
@@ -313,6 +314,8 @@ int mgv_spai_smooth(poisson_ctx* ctx, double* phi, const double* rhs, const doub
 int mgv_vcycles(poisson_ctx* ctx, double* phi, const double* rhs, int nu1, int nu2, int coarsest_n, const double* spai,
                 double cg_rtol, int storage_f32, int ncycles, const std::function<int(int)>& record);
 void mgv_destroy(poisson_ctx* ctx);
+int mgv_residual_norm2(poisson_ctx* ctx, const double* phi, const double* rhs, int coarsest_n, int storage_f32);
+int mgv_compact_rhs(poisson_ctx* ctx, const double* f_ext, double* out);
 
 // Multipole
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, bool inner);

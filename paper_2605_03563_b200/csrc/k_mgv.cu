@@ -355,6 +355,44 @@ __global__ void __launch_bounds__(256) k_fold_ghosts(Op op, const double* __rest
     bt[p] = rhs[p] - g;
 }
 
+// Right-hand side of the compact schemes (reading C19): out = B f with
+//   order 4: B f = f + S1 f / 12;   order 6: B f = f + S1 f / 12 - (sum_a d_a^4 f) / 240 + S2 f / 90,
+// S1 = sum_a d_a^2, S2 = sum_{a<b} d_a^2 d_b^2 (second differences), d_a^4 = (d_a^2)^2 reaching two points out.
+// f_ext carries two extra layers per side: (n0+4)(n1+4)(n2+4) values.  One pass, done once per right-hand side.
+template <int ORDER>
+__global__ void __launch_bounds__(256)
+    k_compact_rhs(int n0, int n1, int n2, const double* __restrict__ fe, double* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+    if (i >= n0 || j >= n1) return;
+    const ptrdiff_t sx = 1, sy = n0 + 4, sz = (ptrdiff_t)(n0 + 4) * (n1 + 4);
+    const double* const c = fe + (k + 2) * sz + (j + 2) * sy + (i + 2);
+    const double f0 = c[0];
+    double v = f0;
+    if (ORDER >= 4) {
+        const double s1 = fma(-6.0, f0, ((c[-sx] + c[sx]) + (c[-sy] + c[sy])) + (c[-sz] + c[sz]));
+        v = fma(s1, 1.0 / 12.0, v);
+    }
+    if (ORDER == 6) {
+        auto d4 = [&](ptrdiff_t s) { return fma(6.0, f0, fma(-4.0, c[-s] + c[s], c[-2 * s] + c[2 * s])); };
+        auto d22 = [&](ptrdiff_t a, ptrdiff_t b) {
+            const double corners = (c[-a - b] + c[a + b]) + (c[-a + b] + c[a - b]);
+            const double faces = (c[-a] + c[a]) + (c[-b] + c[b]);
+            return fma(4.0, f0, fma(-2.0, faces, corners));
+        };
+        v = fma(-(d4(sx) + d4(sy) + d4(sz)), 1.0 / 240.0, v);
+        v = fma(d22(sx, sy) + d22(sy, sz) + d22(sz, sx), 1.0 / 90.0, v);
+    }
+    out[((size_t)k * n1 + j) * n0 + i] = v;
+}
+
+__global__ void __launch_bounds__(256) k_norm2(size_t n, const double* __restrict__ r, double* scal, RedBuf rb) {
+    double s = 0.0;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (size_t)gridDim.x * blockDim.x)
+        s = fma(r[q], r[q], s);
+    double vals[1] = {s};
+    grid_reduce<1>(vals, rb, [=](const double* t) { scal[0] = t[0]; });
+}
+
 // Coarsest level: CG (Saad Alg. 6.18) from e = 0 in ONE CTA, vectors in shared memory, to ||r|| <= rtol ||b|| or max_it.
 template <typename S>
 __global__ void __launch_bounds__(512)
@@ -496,13 +534,15 @@ static void mgv_free(poisson_ctx* ctx) {
     ctx->vlevels.clear();
     cudaFree(ctx->v_sten);
     ctx->v_sten = nullptr;
-    ctx->v_key[0] = ctx->v_key[1] = -1;
+    ctx->v_key[0] = ctx->v_key[1] = ctx->v_key[2] = -1;
 }
 
 void mgv_destroy(poisson_ctx* ctx) { mgv_free(ctx); }
 
 static int mgv_build(poisson_ctx* ctx, int coarsest_n, int f32) {
-    if (ctx->v_key[0] == coarsest_n && ctx->v_key[1] == f32 && !ctx->vlevels.empty()) return POISSON_OK;
+    const int order = ctx->opt_compact_order;
+    if (ctx->v_key[0] == coarsest_n && ctx->v_key[1] == f32 && ctx->v_key[2] == order && !ctx->vlevels.empty())
+        return POISSON_OK;
     mgv_free(ctx);
     MgvLevel L0;
     for (int a = 0; a < 3; ++a) L0.n[a] = ctx->op.n[a];
@@ -526,7 +566,12 @@ static int mgv_build(poisson_ctx* ctx, int coarsest_n, int f32) {
     const size_t nl = ctx->vlevels.size();
     PB_CUDA_OK(cudaMalloc((void**)&ctx->v_sten, nl * 4 * sizeof(double)));
     const double c = 1.0 / (ctx->h[0] * ctx->h[0]);
-    const double s0[4] = {6.0 * c, -c, 0.0, 0.0};  // A = -L_h: the 7-point operator as a symmetric 27-point stencil
+    // A = -L_h as a symmetric 27-point stencil (centre, faces, edges, corners): the 7-point operator, or the compact
+    // radius-1 discretisation of order 4 / 6: L_h = (S1 + S2/6 [+ S3/30]) / h^2 in second differences,
+    // i.e. (-24, 2, 1, 0)/6 and (-128, 14, 3, 1)/30 (reading C19)
+    const double s0[4] = {order == 2 ? 6.0 * c : order == 4 ? 4.0 * c : (64.0 / 15.0) * c,
+                          order == 2 ? -c : order == 4 ? -c / 3.0 : -(7.0 / 15.0) * c,
+                          order == 2 ? 0.0 : order == 4 ? -c / 6.0 : -c / 10.0, order == 6 ? -c / 30.0 : 0.0};
     PB_CUDA_OK(cudaMemcpyAsync(ctx->v_sten, s0, sizeof(s0), cudaMemcpyHostToDevice, ctx->stream));
     PB_CUDA_OK(cudaStreamSynchronize(ctx->stream));  // s0 is a stack array
     for (size_t l = 1; l < nl; ++l)
@@ -543,12 +588,30 @@ static int mgv_build(poisson_ctx* ctx, int coarsest_n, int f32) {
     }
     ctx->v_key[0] = coarsest_n;
     ctx->v_key[1] = f32;
+    ctx->v_key[2] = order;
     return POISSON_OK;
 }
 
-static const double kSpaiOrder2[5] = {1.3699, 0.1432, 0.0284, 0.0081, 0.0025};  // PAPER.md:176-182 Table 1, order 2
+// PAPER.md:176-182 Table 1.  The delta of row 6 is printed as 0.0909 (a copy of the mu column): 0.0150, the middle of
+// the interval on which the smoothing factor of Eq. 17 is smallest with the other printed values (reading C20).
+static const double kSpaiOrder2[5] = {1.3699, 0.1432, 0.0284, 0.0081, 0.0025};
+static const double kSpaiOrder4[5] = {0.9363, 0.2807, 0.0329, 0.0166, 0.0044};
+static const double kSpaiOrder6[5] = {0.3543, 0.7064, 0.1005, 0.0363, 0.0150};
+static const double* default_spai(const poisson_ctx* ctx) {
+    return ctx->opt_compact_order == 4 ? kSpaiOrder4 : ctx->opt_compact_order == 6 ? kSpaiOrder6 : kSpaiOrder2;
+}
 
-static int fold_ghosts(poisson_ctx* ctx, const double* rhs, double* bt) {
+// Level-0 right-hand side.  Order 2: the Dirichlet values of the ghost faces folded in (into bt).  Orders 4 / 6: the
+// caller's array as it is — a 27-point stencil would need ghost values on the edges and corners of the shell, which the
+// face arrays do not hold, so boundary data belong in the right-hand side there and the ghosts must be zero.
+static int fold_ghosts(poisson_ctx* ctx, const double* rhs, double* bt, const double** use) {
+    if (ctx->opt_compact_order != 2) {
+        if (ctx->ghost_nonzero)
+            return fail(ctx, POISSON_UNSUPPORTED, "compact order 4 / 6: ghost values are not used — fold the boundary data into the right-hand side");
+        *use = rhs;
+        return POISSON_OK;
+    }
+    *use = bt;
     const Op& op = ctx->op;
     const dim3 blk(64, 4), grid((op.n[0] + 63) / 64, (op.n[1] + 3) / 4, op.n[2]);
     PB_LAUNCH(ctx, KID_MGV_SETUP, (mgv::k_fold_ghosts<<<grid, blk, 0, ctx->stream>>>(op, rhs, bt)));
@@ -615,14 +678,15 @@ int mgv_spai_smooth(poisson_ctx* ctx, double* phi, const double* rhs, const doub
     int rc;
     if ((rc = mgv_check(ctx)) != POISSON_OK) return rc;
     if ((rc = mgv_build(ctx, ctx->v_key[0] < 0 ? 3 : ctx->v_key[0], ctx->v_key[1] < 0 ? 0 : ctx->v_key[1])) != POISSON_OK) return rc;
-    if (!spai) spai = kSpaiOrder2;
+    if (!spai) spai = default_spai(ctx);
+    const bool seven = ctx->opt_compact_order == 2;
     MgvLevel& L0 = ctx->vlevels[0];
-    double* bt = (double*)L0.b;
-    if ((rc = fold_ghosts(ctx, rhs, bt)) != POISSON_OK) return rc;
+    const double* bt = nullptr;
+    if ((rc = fold_ghosts(ctx, rhs, (double*)L0.b, &bt)) != POISSON_OK) return rc;
     double *cur = phi, *oth = (double*)L0.t;
     for (int s = 0; s < nsteps; ++s) {
         // level 0: b = -rhs~ (bsign = -1), A = -L_h
-        if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, true, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
+        if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, seven, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
         std::swap(cur, oth);
     }
     if (cur != phi) PB_CUDA_OK(cudaMemcpyAsync(phi, cur, ctx->npts * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
@@ -633,20 +697,21 @@ template <typename S>
 static int mgv_vcycles_t(poisson_ctx* ctx, double* phi, const double* rhs, int nu1, int nu2, const double* spai,
                          double cg_rtol, int ncycles, const std::function<int(int)>& record) {
     int rc;
+    const bool seven = ctx->opt_compact_order == 2;
     MgvLevel& L0 = ctx->vlevels[0];
-    double* bt = (double*)L0.b;
-    if ((rc = fold_ghosts(ctx, rhs, bt)) != POISSON_OK) return rc;
+    const double* bt = nullptr;
+    if ((rc = fold_ghosts(ctx, rhs, (double*)L0.b, &bt)) != POISSON_OK) return rc;
     for (int c = 0; c < ncycles; ++c) {
         double *cur = phi, *oth = (double*)L0.t;
         if (ctx->vlevels.size() == 1) {
             return fail(ctx, POISSON_UNSUPPORTED, "the grid admits no coarse level (sizes must be 2^N k - 1 >= 2 coarsest_n + 1, PAPER.md:152)");
         }
         for (int s = 0; s < nu1; ++s) {
-            if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, true, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
+            if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, seven, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
             std::swap(cur, oth);
         }
         MgvLevel& C = ctx->vlevels[1];
-        if ((rc = spai_launch<double, double, S, 2>(ctx, KID_MGV_RESTRICT, L0.n, true, cur, bt, (S*)C.b, ctx->v_sten, -1.0, nullptr, L0.h, C.n)) != POISSON_OK) return rc;
+        if ((rc = spai_launch<double, double, S, 2>(ctx, KID_MGV_RESTRICT, L0.n, seven, cur, bt, (S*)C.b, ctx->v_sten, -1.0, nullptr, L0.h, C.n)) != POISSON_OK) return rc;
         S* ec = nullptr;
         if ((rc = mgv_cycle<S>(ctx, 1, nu1, nu2, spai, cg_rtol, &ec)) != POISSON_OK) return rc;
         {
@@ -654,7 +719,7 @@ static int mgv_vcycles_t(poisson_ctx* ctx, double* phi, const double* rhs, int n
             PB_LAUNCH(ctx, KID_MGV_PROLONG, (mgv::k_prolong27<double, S><<<grid, blk, 0, ctx->stream>>>(L0.n[0], L0.n[1], L0.n[2], C.n[0], C.n[1], C.n[2], ec, cur)));
         }
         for (int s = 0; s < nu2; ++s) {
-            if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, true, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
+            if ((rc = spai_launch<double, double, double, 0>(ctx, KID_MGV_SMOOTH, L0.n, seven, cur, bt, oth, ctx->v_sten, -1.0, spai, L0.h)) != POISSON_OK) return rc;
             std::swap(cur, oth);
         }
         if (cur != phi) PB_CUDA_OK(cudaMemcpyAsync(phi, cur, ctx->npts * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream));
@@ -669,9 +734,40 @@ int mgv_vcycles(poisson_ctx* ctx, double* phi, const double* rhs, int nu1, int n
     int rc;
     if ((rc = mgv_check(ctx)) != POISSON_OK) return rc;
     if ((rc = mgv_build(ctx, coarsest_n, storage_f32 ? 1 : 0)) != POISSON_OK) return rc;
-    if (!spai) spai = kSpaiOrder2;
+    if (!spai) spai = default_spai(ctx);
     if (storage_f32) return mgv_vcycles_t<float>(ctx, phi, rhs, nu1, nu2, spai, cg_rtol, ncycles, record);
     return mgv_vcycles_t<double>(ctx, phi, rhs, nu1, nu2, spai, cg_rtol, ncycles, record);
+}
+
+// ||B f - L_h phi||_2^2 of the compact operator (orders 4 / 6) into d_scal[0]: residual pass + one reduction.
+int mgv_residual_norm2(poisson_ctx* ctx, const double* phi, const double* rhs, int coarsest_n, int storage_f32) {
+    int rc;
+    if ((rc = mgv_check(ctx)) != POISSON_OK) return rc;
+    if ((rc = mgv_build(ctx, coarsest_n, storage_f32 ? 1 : 0)) != POISSON_OK) return rc;
+    MgvLevel& L0 = ctx->vlevels[0];
+    const double* bt = nullptr;
+    if ((rc = fold_ghosts(ctx, rhs, (double*)L0.b, &bt)) != POISSON_OK) return rc;
+    double* r = (double*)L0.t;
+    if ((rc = spai_launch<double, double, double, 1>(ctx, KID_MGV_SMOOTH, L0.n, ctx->opt_compact_order == 2, phi, bt, r,
+                                                     ctx->v_sten, -1.0, nullptr, L0.h)) != POISSON_OK)
+        return rc;
+    const int blocks = (int)std::min<size_t>((ctx->npts + 255) / 256, (size_t)ctx->num_sms * 8);
+    PB_LAUNCH(ctx, KID_MGV_SMOOTH, (mgv::k_norm2<<<blocks, 256, 0, ctx->stream>>>(ctx->npts, r, ctx->d_scal, ctx->red)));
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
+}
+
+// out = B f (compact right-hand side of the handle's compact order) from f on the grid extended by two layers per side.
+int mgv_compact_rhs(poisson_ctx* ctx, const double* f_ext, double* out) {
+    const Op& op = ctx->op;
+    const dim3 blk(64, 4), grid((op.n[0] + 63) / 64, (op.n[1] + 3) / 4, op.n[2]);
+    switch (ctx->opt_compact_order) {
+        case 4: PB_LAUNCH(ctx, KID_MGV_SETUP, (mgv::k_compact_rhs<4><<<grid, blk, 0, ctx->stream>>>(op.n[0], op.n[1], op.n[2], f_ext, out))); break;
+        case 6: PB_LAUNCH(ctx, KID_MGV_SETUP, (mgv::k_compact_rhs<6><<<grid, blk, 0, ctx->stream>>>(op.n[0], op.n[1], op.n[2], f_ext, out))); break;
+        default: PB_LAUNCH(ctx, KID_MGV_SETUP, (mgv::k_compact_rhs<2><<<grid, blk, 0, ctx->stream>>>(op.n[0], op.n[1], op.n[2], f_ext, out))); break;
+    }
+    PB_CUDA_OK(cudaGetLastError());
+    return POISSON_OK;
 }
 
 }  // namespace pb

@@ -53,6 +53,38 @@ def test_mgv_vcycle_255_reproduces_table2_and_storage_precisions_agree(v255):
     assert (r3[2] / r3[0]) ** 0.5 == pytest.approx(0.013, rel=0.2)
 
 
+@pytest.mark.parametrize("order,rho1", [(4, 0.065), (6, 0.068)])
+def test_compact_orders_255_smoother_pointwise_and_table2_factors(v255, order, rho1):
+    """Row f1 at bench size: one SPAI step of the compact operator against the oracle element by element over the whole
+    grid; the V-cycle (whose oracle would take minutes) by the factors of PAPER.md Table 2 and by the agreement of the
+    two storage precisions.  Zero boundary values (the compact operators take no ghost faces)."""
+    w, _, _ = v255
+    o, g = make_pair(dict(shape=w["shape"], spacing=w["spacing"], origin=w["origin"], bc=w["bc"]))
+    g.set_option(pb.OPT_COMPACT_ORDER, order)
+    phi_c = wl.random_field(w["shape"], 14) * 0.1
+    d_phi, d_rhs = dev(phi_c), dev(w["rhs"])
+    o.spai_smooth(phi_c, w["rhs"], nsteps=1, order=order)
+    g.spai_smooth(d_phi, d_rhs, nsteps=1)
+    d = 6 / w["spacing"][0] ** 2
+    assert pointwise_scaled(host(d_phi), phi_c, stencil_scale(phi_c, w["rhs"] / d)) <= 1e-13
+    hist = {}
+    for prec in (pb.F64, pb.MIXED):
+        d_phi = dev(np.zeros_like(w["rhs"]))
+        hist[prec] = np.array(g.mgv_vcycle(d_phi, d_rhs, nu1=1, nu2=1, precision=prec, ncycles=8)["resnorms"])
+    r = hist[pb.F64]
+    assert np.all(r[1:] < r[:-1])
+    assert (r[8] / r[0]) ** (1 / 8) == pytest.approx(rho1, rel=0.2)          # measured 0.073 / 0.074
+    assert r[8] / r[7] == pytest.approx(0.080, abs=0.006)                    # settles to 0.079-0.081 at 255^3 and 511^3
+    assert np.allclose(hist[pb.MIXED][:7] / r[0], r[:7] / r[0], rtol=0.02)
+    # more smoothing steps: the same ordering as Table 2 (0.017 / 0.011 for order 4, 0.018 / 0.012 for order 6)
+    f = []
+    for nu in (2, 3):
+        d_phi = dev(np.zeros_like(w["rhs"]))
+        rn = np.array(g.mgv_vcycle(d_phi, d_rhs, nu1=nu, nu2=nu, ncycles=4)["resnorms"])
+        f.append((rn[4] / rn[0]) ** 0.25)
+    assert f[1] < f[0] < (r[4] / r[0]) ** 0.25 and f[0] < 0.04 and f[1] < 0.026
+
+
 @pytest.fixture(scope="module")
 def c3():
     w = wl.config3(256)
