@@ -36,7 +36,7 @@ def test_static_scratch_residual_norm_matches_the_handle_path_twice_in_a_row():
         got = float(out.item())
         assert want > 0 and abs(got - want) <= RTOL * want, (shape, got, want)
         if n > 0:   # (the first call may load the module) no device memory was taken by the call
-            assert torch.cuda.mem_get_info()[0] == free_before
+            assert torch.cuda.mem_get_info()[0] >= free_before
     # and again on the first inputs: same bits as the first time (fixed summation order, shared scratch overwritten)
     shape, spacing, g, phi, rhs = prepared[0]
     pb.residual_norm_static(shape, spacing, phi, rhs, out, stream)
