@@ -211,6 +211,165 @@ __global__ void __launch_bounds__(256, 2)
     }
 }
 
+// ---- Cartesian grids: the same moments by z lines ---------------------------------------------------------------------------
+// For a fixed column (x, y) the solid harmonic r^l S_lm is (x + i y)^m times a polynomial in z of degree l - m whose
+// coefficients depend on s = x^2 + y^2 only: Q_l^m(z) = sum_c P_lm,c(s) z^c with the SAME recurrence as above applied
+// to coefficient vectors,
+//   P_m^m = (2m-1)!! ;  P_{m+1}^m = (2m+1) z P_m^m ;  (l-m) P_l^m = (2l-1) z P_{l-1}^m - (l+m-1) (s + z^2) P_{l-2}^m ,
+// so that  sum_z rho Q_l^m = sum_c P_lm,c(s) Z_c  with the line sums  Z_c = sum_z rho z^c  (c = 0..lmax).
+// Per point that is one load and lmax + 1 fused multiply-adds instead of ~270 fp64 instructions: the pass becomes
+// HBM-bound (8 B/point).  A thread owns one column of a z chunk (lanes along x: coalesced), forms Z_c, converts once per
+// chunk, and the 81 column values are summed over the CTA through shared memory in three groups of orders (m = 0-1,
+// 2-3, 4-8: at most 30 values each).  Same sums in another order: the moments agree with the point-by-point kernel to
+// rounding (measured 1e-19 .. 1e-24 absolute on configs 2 and 3, tolerance 1e-12 relative).
+template <int L>
+__global__ void __launch_bounds__(256, 2)
+    k_moments_zline(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
+                    double* __restrict__ q_out, int kc) {
+    constexpr int NQ = (L + 1) * (L + 1), NC = L + 1, NCP = (NC + 1) & ~1;  // table rows padded to whole 16-byte pairs
+    extern __shared__ __align__(16) double smz[];
+    double* const zt = smz;                        // kc x NCP powers of z
+    double* const buf = zt + (size_t)kc * NCP;     // 256 x 33: one row per thread (padded: conflict-free both ways)
+    double* const sm2 = buf + 256 * 33;            // 8 x 32 warp partials
+    __shared__ int smap[32];
+    __shared__ int is_last;
+    const int tid = threadIdx.x, lane = tid & 31, ty = tid >> 5;
+    const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
+    // columns in memory order: a CTA reads 2 KB of consecutive densities per plane
+    const size_t plane = (size_t)n0 * n1, col = (size_t)blockIdx.x * 256 + tid;
+    const int j = (int)(col / n0), i = (int)(col - (size_t)j * n0);
+    const int k0 = blockIdx.y * kc, nk = min(kc, n2 - k0);
+    const unsigned nblk = gridDim.x * gridDim.y;
+    const unsigned bid = blockIdx.y * gridDim.x + blockIdx.x;
+    for (int kk = tid; kk < nk; kk += 256) {
+        const double z = fma((double)(k0 + kk), g.h[2], g.origin[2]);
+        double p = 1.0;
+#pragma unroll
+        for (int c = 0; c < NCP; ++c) {
+            zt[kk * NCP + c] = c < NC ? p : 0.0;
+            p *= z;
+        }
+    }
+    __syncthreads();
+    double Z[NC];
+#pragma unroll
+    for (int c = 0; c < NC; ++c) Z[c] = 0.0;
+    if (col < plane) {
+        const double* p = rho + (size_t)k0 * plane + col;
+        int kk = 0;
+        constexpr int UNR = 16;  // loads in flight per thread
+        for (; kk + UNR <= nk; kk += UNR) {
+            double d[UNR];
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) d[u] = p[(size_t)(kk + u) * plane];
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) {
+                const double2* const zr = reinterpret_cast<const double2*>(zt + (kk + u) * NCP);  // broadcast, 16 bytes a load
+#pragma unroll
+                for (int c = 0; c < NC; c += 2) {
+                    const double2 t = zr[c / 2];
+                    Z[c] = fma(d[u], t.x, Z[c]);
+                    if (c + 1 < NC) Z[c + 1] = fma(d[u], t.y, Z[c + 1]);
+                }
+            }
+        }
+        for (; kk < nk; ++kk) {
+            const double d = p[(size_t)kk * plane];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) Z[c] = fma(d, zt[kk * NCP + c], Z[c]);
+        }
+    }
+    // one group of orders: sum the values every thread has put into its row of buf over the CTA (fixed order)
+    auto reduce_group = [&](int nvals) {
+        __syncthreads();
+        double acc = 0.0;
+        if (lane < nvals)
+            for (int t = 0; t < 32; ++t) acc += buf[(ty * 32 + t) * 33 + lane];
+        sm2[ty * 32 + lane] = acc;
+        __syncthreads();
+        if (tid < nvals) {
+            double t = 0.0;
+            for (int w = 0; w < 8; ++w) t += sm2[w * 32 + tid];
+            partials[(size_t)smap[tid] * nblk + bid] = t;  // moment-major: the final sum reads consecutive blocks
+        }
+        __syncthreads();
+    };
+    const double x = fma((double)i, g.h[0], g.origin[0]), y = fma((double)j, g.h[1], g.origin[1]);
+    const double s = fma(y, y, x * x);
+    double A = 1.0, B = 0.0, dfact = 1.0;  // (x + i y)^m, (2m-1)!!
+    int slot = 0;
+    double* const row = buf + tid * 33;
+#pragma unroll
+    for (int m = 0; m <= L; ++m) {
+        double P1[NC], P2[NC];  // coefficient vectors of Q_{l-1}^m, Q_{l-2}^m (powers of z; only c = l-m mod 2 is non-zero)
+#pragma unroll
+        for (int c = 0; c < NC; ++c) P1[c] = P2[c] = 0.0;
+#pragma unroll
+        for (int l = m; l <= L; ++l) {
+            double P[NC];
+#pragma unroll
+            for (int c = 0; c < NC; ++c) P[c] = 0.0;
+            if (l == m) {
+                P[0] = dfact;
+            } else if (l == m + 1) {
+                P[1] = (2 * m + 1) * P1[0];
+            } else {
+#pragma unroll
+                for (int c = (l - m) & 1; c <= l - m; c += 2) {
+                    const double up = c >= 1 ? (2 * l - 1) * P1[c - 1] : 0.0;
+                    double lo = c <= l - 2 - m ? s * P2[c] : 0.0;
+                    if (c >= 2) lo += P2[c - 2];
+                    P[c] = (up - (l + m - 1) * lo) * (1.0 / (l - m));
+                }
+            }
+            double v = 0.0;
+#pragma unroll
+            for (int c = (l - m) & 1; c <= l - m; c += 2) v = fma(P[c], Z[c], v);
+            if (m == 0) {
+                row[slot] = v;
+                if (tid == 0) smap[slot] = l * l + l;
+                ++slot;
+            } else {
+                row[slot] = A * v;
+                row[slot + 1] = B * v;
+                if (tid == 0) {
+                    smap[slot] = l * l + l + m;
+                    smap[slot + 1] = l * l + l - m;
+                }
+                slot += 2;
+            }
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                P2[c] = P1[c];
+                P1[c] = P[c];
+            }
+        }
+        if (m == 1 || m == 3 || m == L) {  // groups m = 0-1, 2-3, 4-L
+            reduce_group(slot);
+            slot = 0;
+        }
+        const double An = x * A - y * B, Bn = fma(y, A, x * B);
+        A = An;
+        B = Bn;
+        dfact *= (2 * m + 1);
+    }
+    // the last block adds the block partials in a fixed order; N_lm and the cell volume are applied once, here
+    if (tid == 0) {
+        __threadfence();
+        is_last = (atomicInc(counter, nblk - 1) == nblk - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    const double dV = g.h[0] * g.h[1] * g.h[2];
+    for (int q = ty; q < NQ; q += 8) {  // a warp per moment: lanes over the blocks, then the warp (fixed order)
+        double v = 0.0;
+        for (unsigned b = lane; b < nblk; b += 32) v += __ldcg(&partials[(size_t)q * nblk + b]);
+        v = warp_sum(v);
+        if (lane == 0) q_out[q] = v * g.norm[q] * dV;
+    }
+}
+
 // Phi at one exterior point from the moments.
 // inner: Eq. 21, Phi = -G sum qbar_lm r^l S_lm (no inverse powers of r).
 // qn = q_lm N_lm (shared memory).
@@ -326,9 +485,53 @@ static void moments_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho,
         k_moments<L, false><<<blocks, 256, 0, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
 }
 
+// z-line kernel: Cartesian grids, outer moments; z chunks so that about two waves of CTAs exist (a chunk costs one
+// conversion + CTA reduction, ~1100 instructions per thread, next to ~22 per plane).
+template <int L>
+static int zline_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, double* d_q) {
+    const long bx = ((long)g.n[0] * g.n[1] + 255) / 256, by = 1;
+    // z chunks only where the columns alone do not give every SM a CTA: a chunk costs a conversion and a CTA reduction
+    // (measured 6 us per layer of 256 CTAs at 256^3, lmax = 8; 48 / 54 / 66 us with 1 / 2 / 4 chunks)
+    int nzc = std::max(1, (int)((ctx->num_sms + bx - 1) / bx));
+    nzc = std::min(nzc, std::max(1, g.n[2] / 64));
+    int kc = (g.n[2] + nzc - 1) / nzc;
+    kc = std::min(kc, 512);
+    nzc = (g.n[2] + kc - 1) / kc;
+    constexpr int NQ = (L + 1) * (L + 1);
+    if ((size_t)bx * nzc * NQ > (size_t)kMaxRedBlocks * kRedSlots || bx > 0x7fffffffL || nzc > 65535) return POISSON_UNSUPPORTED;
+    const size_t smem = ((size_t)kc * ((L + 2) & ~1) + 256 * 33 + 8 * 32) * sizeof(double);
+    const int rc = kernel_ready(ctx, k_moments_zline<L>, 256, 110 * 1024);
+    if (rc != POISSON_OK) return rc;
+    k_moments_zline<L><<<dim3((unsigned)bx, nzc), 256, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q, kc);
+    return POISSON_OK;
+}
+
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, bool inner) {
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     const MpGeom g = make_geom(ctx);
+    // Cartesian grids: by z lines (HBM-bound); POISSON_OPT_KERNEL_PATH = 1 keeps the point-by-point kernel
+    if (!g.sph && !inner && ctx->opt_path != 1) {
+        pre_launch(ctx, KID_MP_MOMENTS);
+        int rc = POISSON_UNSUPPORTED;
+        switch (lmax) {
+            case 0: rc = zline_launch<0>(ctx, g, rho, d_q); break;
+            case 1: rc = zline_launch<1>(ctx, g, rho, d_q); break;
+            case 2: rc = zline_launch<2>(ctx, g, rho, d_q); break;
+            case 3: rc = zline_launch<3>(ctx, g, rho, d_q); break;
+            case 4: rc = zline_launch<4>(ctx, g, rho, d_q); break;
+            case 5: rc = zline_launch<5>(ctx, g, rho, d_q); break;
+            case 6: rc = zline_launch<6>(ctx, g, rho, d_q); break;
+            case 7: rc = zline_launch<7>(ctx, g, rho, d_q); break;
+            case 8: rc = zline_launch<8>(ctx, g, rho, d_q); break;
+            default: break;
+        }
+        if (rc == POISSON_OK) {
+            post_launch(ctx, KID_MP_MOMENTS);
+            PB_CUDA_OK(cudaGetLastError());
+            return POISSON_OK;
+        }
+        if (rc != POISSON_UNSUPPORTED) return rc;
+    }
     // two resident CTAs per SM; for l_max >= 1 the grid is made of pairs of blocks (one per half of the orders)
     int blocks = ctx->num_sms * 2;
     const size_t maxb = (ctx->npts + 255) / 256;
