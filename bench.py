@@ -59,7 +59,6 @@ ROW_BYTES = {
     "spai_smooth_o6": 24,           # f1: the SPAI step on the compact 27-point sixth-order operator (same bytes, 27-point A)
     "mgv_vcycle_o6_511": 94,        # f1 + f2: Table 2, order 6: 511^3, V(1,1)
 }
-NUM_SMS, FP64_CLOCK_HZ, MOMENTS_DP_INSTR = 148, 1.965e9, 250
 ROW_CITE = {
     "multipole_bc": "a6 PAPER.md:213-222", "apply_laplacian": "a1 PAPER.md:43-49", "rbsor_sweep": "a2 PAPER.md:59-63",
     "mg_vcycle_f64": "a5 PAPER.md:125-152", "mg_vcycle_mixed": "a5 PAPER.md:205", "residual_norm": "a7 PAPER.md:55",
@@ -490,12 +489,9 @@ def run_ours(args):
                "B_pt": ROW_BYTES[name], "alg_gbs": round(gbs), "frac": round(gbs / peak, 3),
                "dram_B_pt": dram, "dram_gbs": round(gpts * dram) if dram else None, "in_value": in_value}
         if name.startswith("multipole_bc"):
-            # lmax = 8 moments are bound by the plain fp64 ALUs, not HBM: fp64-pipe instructions per
-            # point counted by ncu (sm__inst_executed_pipe_fp64 x 32 / points; profiles/traffic.csv), else the SASS
-            # count; peak = SMs x 64 fp64 lanes x max SM clock
-            instr = tr.get("fp64_instr_per_point:" + name, MOMENTS_DP_INSTR)
-            row.update(bound="alu", fp64_instr_pt=instr,
-                       frac_alu=round(gpts * 1e9 * instr / (NUM_SMS * 64 * FP64_CLOCK_HZ), 3))
+            # the moments are line sums since round 2 (z lines / radial lines: lmax + 1 multiply-adds per point, DESIGN.md
+            # §6): an HBM-bound pass of 8 B/point, no longer the fp64-ALU-bound one of the point-by-point kernel
+            row.update(bound="hbm")
         rows[name] = row
 
     for (name, pts, u), ms in zip(units, row_ms):

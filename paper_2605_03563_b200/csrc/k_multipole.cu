@@ -370,6 +370,154 @@ __global__ void __launch_bounds__(256, 2)
     }
 }
 
+// ---- spherical grids: the same moments by radial lines -----------------------------------------------------------------------
+// r^l S_lm(theta, phi) dV factorises on a spherical grid: q_lm = sum_{j,k} [N_lm P_l^m(cos theta_j) {cos, sin}(m phi_k)
+// vt_j vp_k] * R_l(j,k) with the radial line sums R_l = sum_i rho_ijk rc_i^l vr_i (inner moments, Eq. 22: rc_i^-(l+1)).
+// The radius is the fastest index: a warp walks one line (coalesced), every lane forms the lmax + 1 partial sums of its
+// points (one load, lmax multiplications and lmax + 1 fused multiply-adds per point instead of ~270 fp64 instructions),
+// the warp adds them, and then lane q owns the moments q, q + 32, q + 64: it evaluates their angular factor for the line
+// and accumulates.  The angular factors come from two tables every CTA builds once in shared memory — P_l^m(cos
+// theta_j) vt_j by its recurrence from the tabulated sin / cos theta, {cos, sin}(m phi_k) vp_k by powers of the
+// tabulated cos phi + i sin phi (no trigonometric call) — so a line costs each lane two loads and three multiply-adds
+// per moment it owns.
+template <int L, bool INNER>
+__global__ void __launch_bounds__(256, 2)
+    k_moments_rline(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
+                    double* __restrict__ q_out) {
+    constexpr int NQ = (L + 1) * (L + 1), NC = L + 1, NP = (L + 1) * (L + 2) / 2, NM = 2 * L + 1;
+    extern __shared__ double smr[];
+    const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
+    double* const rtab = smr;            // rc_i (inner: 1 / rc_i)
+    double* const vtab = rtab + n0;      // vr_i (inner: vr_i / rc_i)
+    double* const Rw = vtab + n0;        // 8 warps x 2 x 16: the line sums of the warp's two current lines
+    double* const accw = Rw + 8 * 32;    // 8 warps x 96: the warps' moments at the end
+    double* const PT = accw + 8 * 96;    // n1 x NP: P_l^m(cos theta_j) vt_j at l (l+1)/2 + m
+    double* const CS = PT + (size_t)n1 * NP;  // n2 x NM: cos(m phi_k) vp_k at m, sin(m phi_k) vp_k at L + m
+    __shared__ int is_last;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int i = tid; i < n0; i += 256) {
+        const double r = g.rc[i];
+        rtab[i] = INNER ? 1.0 / r : r;
+        vtab[i] = INNER ? g.vr[i] / r : g.vr[i];
+    }
+    for (int j = tid; j < n1; j += 256) {
+        const double ct = g.ct[j], st = g.st[j], vt = g.vt[j];
+        const double rk[9] = {0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8};  // 1 / (l - m)
+        double pmm = 1.0;  // P_m^m = (2m-1)!! sin^m theta, no Condon-Shortley phase
+#pragma unroll
+        for (int m = 0; m <= L; ++m) {
+            if (m > 0) pmm *= (2 * m - 1) * st;
+            double pm2 = 0.0, pm1 = pmm;
+#pragma unroll
+            for (int l = m; l <= L; ++l) {
+                double pl;
+                if (l == m)
+                    pl = pmm;
+                else if (l == m + 1)
+                    pl = (2 * m + 1) * ct * pm1;
+                else
+                    pl = ((2 * l - 1) * ct * pm1 - (l + m - 1) * pm2) * rk[l - m];
+                PT[(size_t)j * NP + l * (l + 1) / 2 + m] = pl * vt;
+                pm2 = pm1;
+                pm1 = pl;
+            }
+        }
+    }
+    for (int k = tid; k < n2; k += 256) {
+        const double cp = g.cph[k], sp = g.sph_[k], vp = g.vp[k];
+        double ca = 1.0, sa = 0.0;
+        CS[(size_t)k * NM] = vp;
+#pragma unroll
+        for (int m = 1; m <= L; ++m) {
+            const double cn = ca * cp - sa * sp, sn = fma(sa, cp, ca * sp);
+            ca = cn;
+            sa = sn;
+            CS[(size_t)k * NM + m] = ca * vp;
+            CS[(size_t)k * NM + L + m] = sa * vp;
+        }
+    }
+    __syncthreads();
+    // this lane's moments: index s = lane + 32 q, degree ls, order ms (sine harmonic for ms < 0)
+    int ls[3], pi[3], ci[3];  // degree (-1: none), index into a PT row, index into a CS row
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const int s = lane + 32 * q;
+        int l = 0;
+        while ((l + 1) * (l + 1) <= s) ++l;
+        const int m = s - l * l - l, am = m < 0 ? -m : m;
+        ls[q] = s < NQ ? l : -1;
+        pi[q] = s < NQ ? l * (l + 1) / 2 + am : 0;
+        ci[q] = s < NQ ? (m < 0 ? L + am : am) : 0;
+    }
+    double acc[3] = {0.0, 0.0, 0.0};
+    const long nlines = (long)n1 * n2, nw = (long)gridDim.x * 8;
+    // two lines per pass of the warp: twice the loads in flight and twice the independent reductions
+    for (long line0 = (long)blockIdx.x * 8 + wid; line0 < nlines; line0 += 2 * nw) {
+        const long line1 = line0 + nw;
+        const bool two = line1 < nlines;
+        const double* const p0 = rho + (size_t)line0 * n0;
+        const double* const p1 = rho + (size_t)(two ? line1 : line0) * n0;
+        double R0[NC], R1[NC];
+#pragma unroll
+        for (int l = 0; l < NC; ++l) R0[l] = R1[l] = 0.0;
+#pragma unroll 4
+        for (int i = lane; i < n0; i += 32) {
+            const double d0 = p0[i], d1 = p1[i], rr = rtab[i];
+            double rl = vtab[i];
+#pragma unroll
+            for (int l = 0; l < NC; ++l) {
+                R0[l] = fma(d0, rl, R0[l]);
+                R1[l] = fma(d1, rl, R1[l]);
+                rl *= rr;
+            }
+        }
+#pragma unroll
+        for (int l = 0; l < NC; ++l) {
+            const double t0 = warp_sum(R0[l]), t1 = warp_sum(R1[l]);
+            if (lane == l) {
+                Rw[wid * 32 + l] = t0;
+                Rw[wid * 32 + 16 + l] = t1;
+            }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (h == 1 && !two) break;
+            const long line = h ? line1 : line0;
+            const int k = (int)(line / n1), j = (int)(line - (long)k * n1);
+            const double* const pt = PT + (size_t)j * NP;
+            const double* const cs = CS + (size_t)k * NM;
+#pragma unroll
+            for (int q = 0; q < 3; ++q)
+                if (ls[q] >= 0) acc[q] = fma(pt[pi[q]] * cs[ci[q]], Rw[wid * 32 + 16 * h + ls[q]], acc[q]);
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int q = 0; q < 3; ++q) accw[wid * 96 + lane + 32 * q] = acc[q];
+    __syncthreads();
+    const unsigned nblk = gridDim.x, bid = blockIdx.x;
+    if (tid < NQ) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += accw[w * 96 + tid];
+        partials[(size_t)tid * nblk + bid] = t;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        is_last = (atomicInc(counter, nblk - 1) == nblk - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    for (int q = wid; q < NQ; q += 8) {  // a warp per moment: lanes over the blocks, then the warp (fixed order)
+        double v = 0.0;
+        for (unsigned b = lane; b < nblk; b += 32) v += __ldcg(&partials[(size_t)q * nblk + b]);
+        v = warp_sum(v);
+        if (lane == 0) q_out[q] = v * g.norm[q];
+    }
+}
+
 // Phi at one exterior point from the moments.
 // inner: Eq. 21, Phi = -G sum qbar_lm r^l S_lm (no inverse powers of r).
 // qn = q_lm N_lm (shared memory).
@@ -506,9 +654,49 @@ static int zline_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, do
     return POISSON_OK;
 }
 
+template <int L>
+static int rline_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, double* d_q, bool inner) {
+    const long nlines = (long)g.n[1] * g.n[2];
+    const int blocks = (int)std::max(1L, std::min<long>(2L * ctx->num_sms, (nlines + 7) / 8));
+    const size_t smem = ((size_t)2 * g.n[0] + 8 * 32 + 8 * 96 + (size_t)g.n[1] * ((L + 1) * (L + 2) / 2) +
+                         (size_t)g.n[2] * (2 * L + 1)) * sizeof(double);
+    if (smem > 100 * 1024) return POISSON_UNSUPPORTED;
+    int rc = kernel_ready(ctx, k_moments_rline<L, false>, 256, 100 * 1024);
+    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_moments_rline<L, true>, 256, 100 * 1024);
+    if (rc != POISSON_OK) return rc;
+    if (inner)
+        k_moments_rline<L, true><<<blocks, 256, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+    else
+        k_moments_rline<L, false><<<blocks, 256, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+    return POISSON_OK;
+}
+
 int launch_moments(poisson_ctx* ctx, const double* rho, int lmax, double* d_q, bool inner) {
     if (lmax < 0 || lmax > kMaxLmax) return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
     const MpGeom g = make_geom(ctx);
+    // spherical grids: by radial lines; POISSON_OPT_KERNEL_PATH = 1 keeps the point-by-point kernel
+    if (g.sph && ctx->opt_path != 1) {
+        pre_launch(ctx, KID_MP_MOMENTS);
+        int rc = POISSON_UNSUPPORTED;
+        switch (lmax) {
+            case 0: rc = rline_launch<0>(ctx, g, rho, d_q, inner); break;
+            case 1: rc = rline_launch<1>(ctx, g, rho, d_q, inner); break;
+            case 2: rc = rline_launch<2>(ctx, g, rho, d_q, inner); break;
+            case 3: rc = rline_launch<3>(ctx, g, rho, d_q, inner); break;
+            case 4: rc = rline_launch<4>(ctx, g, rho, d_q, inner); break;
+            case 5: rc = rline_launch<5>(ctx, g, rho, d_q, inner); break;
+            case 6: rc = rline_launch<6>(ctx, g, rho, d_q, inner); break;
+            case 7: rc = rline_launch<7>(ctx, g, rho, d_q, inner); break;
+            case 8: rc = rline_launch<8>(ctx, g, rho, d_q, inner); break;
+            default: break;
+        }
+        if (rc == POISSON_OK) {
+            post_launch(ctx, KID_MP_MOMENTS);
+            PB_CUDA_OK(cudaGetLastError());
+            return POISSON_OK;
+        }
+        if (rc != POISSON_UNSUPPORTED) return rc;
+    }
     // Cartesian grids: by z lines (HBM-bound); POISSON_OPT_KERNEL_PATH = 1 keeps the point-by-point kernel
     if (!g.sph && !inner && ctx->opt_path != 1) {
         pre_launch(ctx, KID_MP_MOMENTS);

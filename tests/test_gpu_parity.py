@@ -143,6 +143,38 @@ def test_multipole_moment_kernels_agree(shape):
             assert np.abs(qs[0][sl] - qs[1][sl]).max() <= 1e-13 * np.abs(qs[1][sl]).max() + 1e-15 * abs(qs[1][0]), (lmax, l)
 
 
+@pytest.mark.parametrize("shape", [(32, 16, 32), (50, 9, 7), (256, 16, 12)])
+def test_multipole_moment_kernels_agree_spherical(shape):
+    """The radial-line kernel (spherical default) against the point-by-point kernel (generic path): outer moments of a
+    grid with a Neumann inner face, outer and inner moments of one with a Dirichlet inner face.  Both sum the same terms
+    in another order: they agree to the rounding of the sum, 1e-13 of sum |rho| r^l dV (inner: r^-(l+1))."""
+    w = wl.config5(*shape)
+    re, te, pe = w["edges"]
+    rc = np.sqrt(re[:-1] * re[1:])
+    dV = ((re[1:] ** 3 - re[:-1] ** 3) / 3)[None, None, :] * (np.cos(te[:-1]) - np.cos(te[1:]))[None, :, None] \
+        * (pe[1:] - pe[:-1])[:, None, None]
+    mass = np.abs(w["rho"]) * dV
+    rho = dev(w["rho"])
+    for inner_dirichlet in (False, True):
+        bc = list(w["bc"])
+        if inner_dirichlet:
+            bc[0] = po.BC_DIRICHLET_GHOST
+        for lmax in (0, 2, 8):
+            qs = []
+            for path in (pb.PATH_PLANE, pb.PATH_GENERIC):
+                g = pb.Poisson(w["shape"], edges=w["edges"], coord=w["coord"], bc=tuple(bc))
+                g.set_option(pb.OPT_KERNEL_PATH, path)
+                q = [np.array(g.multipole_bc(rho, 1.0, lmax))]
+                if inner_dirichlet:
+                    q.append(np.array(g.multipole_inner_moments(lmax)))
+                qs.append(q)
+            for which in range(len(qs[0])):
+                for l in range(lmax + 1):
+                    sl = slice(l * l, (l + 1) * (l + 1))
+                    floor = np.sum(mass * (rc[None, None, :] ** (l if which == 0 else -(l + 1))))
+                    assert np.abs(qs[0][which][sl] - qs[1][which][sl]).max() <= 1e-13 * floor, (inner_dirichlet, which, lmax, l)
+
+
 def test_multipole_spherical():
     w = wl.config5(32, 16, 32)
     o, g = make_pair(w)
