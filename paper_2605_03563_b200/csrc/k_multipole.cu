@@ -521,15 +521,20 @@ __global__ void __launch_bounds__(256, 2)
 // Phi at one exterior point from the moments.
 // inner: Eq. 21, Phi = -G sum qbar_lm r^l S_lm (no inverse powers of r).
 // qn = q_lm N_lm (shared memory).
-__device__ __forceinline__ double expansion(const double* __restrict__ qn, int lmax, double G, double x, double y, double z,
+// LMAX is a template parameter: both loops unroll (no table of reciprocals in local memory, no loop bookkeeping —
+// the run-time-lmax version spent ~24 instructions per harmonic).
+template <int LMAX>
+__device__ __forceinline__ double expansion(const double* __restrict__ qn, double G, double x, double y, double z,
                                             bool inner) {
+    constexpr int lmax = LMAX;
     const double r2 = fma(z, z, fma(y, y, x * x));
     const double rinv = inner ? 1.0 : 1.0 / sqrt(r2), rinv2 = rinv * rinv;
-    const double rk[9] = {0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8};  // 1 / (l - m)
     double A = 1.0, B = 0.0, dfact = 1.0, acc = 0.0;
     double pw_m = rinv;  // r^-(2m+1)  (1 for the inner expansion)
+#pragma unroll
     for (int m = 0; m <= lmax; ++m) {
         double qm2 = 0.0, qm1 = dfact, pw = pw_m;  // pw = r^-(2l+1)
+#pragma unroll
         for (int l = m; l <= lmax; ++l) {
             double ql;
             if (l == m)
@@ -537,7 +542,7 @@ __device__ __forceinline__ double expansion(const double* __restrict__ qn, int l
             else if (l == m + 1)
                 ql = (2 * m + 1) * z * qm1;
             else
-                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) * rk[l - m];
+                ql = ((2 * l - 1) * z * qm1 - (l + m - 1) * r2 * qm2) * (1.0 / (l - m));
             if (m == 0)
                 acc = fma(qn[l * l + l] * ql, pw, acc);
             else
@@ -565,7 +570,9 @@ struct GhostFaces {
     int inner[6];
 };
 
-__global__ void __launch_bounds__(256) k_ghost_eval(MpGeom g, GhostFaces gf, int R, double G, int lmax) {
+template <int LMAX>
+__global__ void __launch_bounds__(256) k_ghost_eval(MpGeom g, GhostFaces gf, int R, double G) {
+    constexpr int lmax = LMAX;
     int s = 0;
 #pragma unroll
     for (int m = 1; m < 6; ++m)
@@ -596,7 +603,7 @@ __global__ void __launch_bounds__(256) k_ghost_eval(MpGeom g, GhostFaces gf, int
         y = fma((double)id[1], g.h[1], g.origin[1]);
         z = fma((double)id[2], g.h[2], g.origin[2]);
     }
-    gf.out[s][t] = expansion(qn, lmax, G, x, y, z, inner);
+    gf.out[s][t] = expansion<LMAX>(qn, G, x, y, z, inner);
 }
 
 static MpGeom make_geom(poisson_ctx* ctx) {
@@ -762,7 +769,22 @@ int launch_ghost_eval(poisson_ctx* ctx, const double* d_q, const double* d_qbar,
         ++gf.nf;
     }
     gf.first_block[gf.nf] = blocks;
-    if (blocks > 0) PB_LAUNCH(ctx, KID_MP_GHOSTS, (k_ghost_eval<<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G, lmax)));
+    if (blocks > 0) {
+        pre_launch(ctx, KID_MP_GHOSTS);
+        switch (lmax) {
+            case 0: k_ghost_eval<0><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 1: k_ghost_eval<1><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 2: k_ghost_eval<2><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 3: k_ghost_eval<3><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 4: k_ghost_eval<4><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 5: k_ghost_eval<5><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 6: k_ghost_eval<6><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 7: k_ghost_eval<7><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            case 8: k_ghost_eval<8><<<blocks, 256, 0, ctx->stream>>>(g, gf, ctx->op.R, G); break;
+            default: return fail(ctx, POISSON_INVALID_ARG, "lmax must be in 0..8");
+        }
+        post_launch(ctx, KID_MP_GHOSTS);
+    }
     PB_CUDA_OK(cudaGetLastError());
     return POISSON_OK;
 }
