@@ -380,8 +380,10 @@ __global__ void __launch_bounds__(256, 2)
 // theta_j) vt_j by its recurrence from the tabulated sin / cos theta, {cos, sin}(m phi_k) vp_k by powers of the
 // tabulated cos phi + i sin phi (no trigonometric call) — so a line costs each lane two loads and three multiply-adds
 // per moment it owns.
+constexpr int kRlineWarps = 16;  // one 512-thread CTA per SM
+
 template <int L, bool INNER>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(32 * kRlineWarps, 1)
     k_moments_rline(MpGeom g, const double* __restrict__ rho, double* __restrict__ partials, unsigned int* counter,
                     double* __restrict__ q_out) {
     constexpr int NQ = (L + 1) * (L + 1), NC = L + 1, NP = (L + 1) * (L + 2) / 2, NM = 2 * L + 1;
@@ -389,18 +391,20 @@ __global__ void __launch_bounds__(256, 2)
     const int n0 = g.n[0], n1 = g.n[1], n2 = g.n[2];
     double* const rtab = smr;            // rc_i (inner: 1 / rc_i)
     double* const vtab = rtab + n0;      // vr_i (inner: vr_i / rc_i)
-    double* const Rw = vtab + n0;        // 8 warps x 2 x 16: the line sums of the warp's two current lines
-    double* const accw = Rw + 8 * 32;    // 8 warps x 96: the warps' moments at the end
-    double* const PT = accw + 8 * 96;    // n1 x NP: P_l^m(cos theta_j) vt_j at l (l+1)/2 + m
+    constexpr int NW = kRlineWarps, NT = 32 * NW;
+    double* const Rw = vtab + n0;        // NW warps x 2 x 16: the line sums of the warp's two current lines
+    double* const accw = Rw + NW * 32;   // NW warps x 96: the warps' moments at the end
+    double* const PT = accw + NW * 96;   // n1 x NP: P_l^m(cos theta_j) vt_j at l (l+1)/2 + m
     double* const CS = PT + (size_t)n1 * NP;  // n2 x NM: cos(m phi_k) vp_k at m, sin(m phi_k) vp_k at L + m
+    double* const Rs = CS + (size_t)n2 * NM;  // NW warps x 2 NC x 33: the lanes' partial line sums, transposed to add
     __shared__ int is_last;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    for (int i = tid; i < n0; i += 256) {
+    for (int i = tid; i < n0; i += NT) {
         const double r = g.rc[i];
         rtab[i] = INNER ? 1.0 / r : r;
         vtab[i] = INNER ? g.vr[i] / r : g.vr[i];
     }
-    for (int j = tid; j < n1; j += 256) {
+    for (int j = tid; j < n1; j += NT) {
         const double ct = g.ct[j], st = g.st[j], vt = g.vt[j];
         const double rk[9] = {0.0, 1.0, 1.0 / 2, 1.0 / 3, 1.0 / 4, 1.0 / 5, 1.0 / 6, 1.0 / 7, 1.0 / 8};  // 1 / (l - m)
         double pmm = 1.0;  // P_m^m = (2m-1)!! sin^m theta, no Condon-Shortley phase
@@ -423,7 +427,7 @@ __global__ void __launch_bounds__(256, 2)
             }
         }
     }
-    for (int k = tid; k < n2; k += 256) {
+    for (int k = tid; k < n2; k += NT) {
         const double cp = g.cph[k], sp = g.sph_[k], vp = g.vp[k];
         double ca = 1.0, sa = 0.0;
         CS[(size_t)k * NM] = vp;
@@ -450,9 +454,10 @@ __global__ void __launch_bounds__(256, 2)
         ci[q] = s < NQ ? (m < 0 ? L + am : am) : 0;
     }
     double acc[3] = {0.0, 0.0, 0.0};
-    const long nlines = (long)n1 * n2, nw = (long)gridDim.x * 8;
+    const long nlines = (long)n1 * n2, nw = (long)gridDim.x * NW;
     // two lines per pass of the warp: twice the loads in flight and twice the independent reductions
-    for (long line0 = (long)blockIdx.x * 8 + wid; line0 < nlines; line0 += 2 * nw) {
+    double* const rs = Rs + (size_t)wid * (2 * NC * 33);
+    for (long line0 = (long)blockIdx.x * NW + wid; line0 < nlines; line0 += 2 * nw) {
         const long line1 = line0 + nw;
         const bool two = line1 < nlines;
         const double* const p0 = rho + (size_t)line0 * n0;
@@ -471,13 +476,19 @@ __global__ void __launch_bounds__(256, 2)
                 rl *= rr;
             }
         }
+        // the warp's sums through shared memory: every lane deposits its 2 NC partial sums, lane v adds row v
+        // (18 stores + 32 loads and additions per lane instead of 90 shuffle-and-add steps)
 #pragma unroll
         for (int l = 0; l < NC; ++l) {
-            const double t0 = warp_sum(R0[l]), t1 = warp_sum(R1[l]);
-            if (lane == l) {
-                Rw[wid * 32 + l] = t0;
-                Rw[wid * 32 + 16 + l] = t1;
-            }
+            rs[l * 33 + lane] = R0[l];
+            rs[(NC + l) * 33 + lane] = R1[l];
+        }
+        __syncwarp();
+        if (lane < 2 * NC) {
+            double t = 0.0;
+#pragma unroll 8
+            for (int u = 0; u < 32; ++u) t += rs[lane * 33 + u];
+            Rw[wid * 32 + (lane < NC ? lane : 16 + lane - NC)] = t;
         }
         __syncwarp();
 #pragma unroll
@@ -499,7 +510,7 @@ __global__ void __launch_bounds__(256, 2)
     const unsigned nblk = gridDim.x, bid = blockIdx.x;
     if (tid < NQ) {
         double t = 0.0;
-        for (int w = 0; w < 8; ++w) t += accw[w * 96 + tid];
+        for (int w = 0; w < NW; ++w) t += accw[w * 96 + tid];
         partials[(size_t)tid * nblk + bid] = t;
     }
     __syncthreads();
@@ -510,7 +521,7 @@ __global__ void __launch_bounds__(256, 2)
     __syncthreads();
     if (!is_last) return;
     __threadfence();
-    for (int q = wid; q < NQ; q += 8) {  // a warp per moment: lanes over the blocks, then the warp (fixed order)
+    for (int q = wid; q < NQ; q += NW) {  // a warp per moment: lanes over the blocks, then the warp (fixed order)
         double v = 0.0;
         for (unsigned b = lane; b < nblk; b += 32) v += __ldcg(&partials[(size_t)q * nblk + b]);
         v = warp_sum(v);
@@ -664,17 +675,18 @@ static int zline_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, do
 template <int L>
 static int rline_launch(poisson_ctx* ctx, const MpGeom& g, const double* rho, double* d_q, bool inner) {
     const long nlines = (long)g.n[1] * g.n[2];
-    const int blocks = (int)std::max(1L, std::min<long>(2L * ctx->num_sms, (nlines + 7) / 8));
-    const size_t smem = ((size_t)2 * g.n[0] + 8 * 32 + 8 * 96 + (size_t)g.n[1] * ((L + 1) * (L + 2) / 2) +
-                         (size_t)g.n[2] * (2 * L + 1)) * sizeof(double);
-    if (smem > 100 * 1024) return POISSON_UNSUPPORTED;
-    int rc = kernel_ready(ctx, k_moments_rline<L, false>, 256, 100 * 1024);
-    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_moments_rline<L, true>, 256, 100 * 1024);
+    constexpr int NW = kRlineWarps;
+    const int blocks = (int)std::max(1L, std::min<long>((long)ctx->num_sms, (nlines + 2 * NW - 1) / (2 * NW)));
+    const size_t smem = ((size_t)2 * g.n[0] + NW * 32 + NW * 96 + (size_t)g.n[1] * ((L + 1) * (L + 2) / 2) +
+                         (size_t)g.n[2] * (2 * L + 1) + (size_t)NW * 2 * (L + 1) * 33) * sizeof(double);
+    if (smem > 200 * 1024) return POISSON_UNSUPPORTED;
+    int rc = kernel_ready(ctx, k_moments_rline<L, false>, 32 * NW, 200 * 1024);
+    if (rc == POISSON_OK) rc = kernel_ready(ctx, k_moments_rline<L, true>, 32 * NW, 200 * 1024);
     if (rc != POISSON_OK) return rc;
     if (inner)
-        k_moments_rline<L, true><<<blocks, 256, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+        k_moments_rline<L, true><<<blocks, 32 * NW, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
     else
-        k_moments_rline<L, false><<<blocks, 256, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
+        k_moments_rline<L, false><<<blocks, 32 * NW, smem, ctx->stream>>>(g, rho, ctx->red.partials, ctx->red.counter, d_q);
     return POISSON_OK;
 }
 
