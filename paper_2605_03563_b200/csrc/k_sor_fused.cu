@@ -457,9 +457,10 @@ static int sor_fused_t(poisson_ctx* ctx, const Op& op, T* phi, T* tmp, const T* 
                        T** result, const double* omegas = nullptr) {
     T *src = phi, *dst = tmp;
     int left = nsweeps;
-    // two sweeps per pass (NHS = 4) pay on large grids: fp64 from 2^23 points (122 vs 117 Gpoint/s at 256^3), fp32 from 2^21; 0 = this automatic choice
+    // two sweeps per pass (NHS = 4) pay from 2^21 points (128^3: 22.9 vs 24.8 us per sweep in fp64; 256^3: 109 vs 138;
+    // 64^3: the same either way); 0 = this automatic choice
     const bool two = ctx->opt_sor_nhs == 4 ||
-                     (ctx->opt_sor_nhs == 0 && (size_t)op.n[0] * op.n[1] * op.n[2] >= ((size_t)1 << (sizeof(T) == 4 ? 21 : 23)));
+                     (ctx->opt_sor_nhs == 0 && (size_t)op.n[0] * op.n[1] * op.n[2] >= ((size_t)1 << 21));
     // Plan: n4 passes of two sweeps + n2 passes of one.  An odd number of passes ends in the ping-pong buffer and costs
     // a copy back (16 B/point): in fp64 one two-sweep pass is then split into two one-sweep passes instead
     // (measured: 2 x NHS=2 beats NHS=4 + copy at 256^3; in fp32 the single pass + copy is the faster one).
