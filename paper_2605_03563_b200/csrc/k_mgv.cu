@@ -27,7 +27,7 @@ namespace pb {
 
 namespace mgv {
 
-constexpr int NTX = 32, NTY = 8, RY = 2;   // threads; rows per thread (measured at 255^3 / 511^3: 8x2 0.62 / 4.16 ms per 4 steps; 4x4 0.77 / 5.11; 16x1 0.77 / 5.25; 16x2 0.70 / 4.73)
+constexpr int NTX = 32, NTY = 8, RY = 3;   // threads; rows per thread (ms per SPAI step at 255^3 / 511^3, 7-point A: 8x3 0.143 / 0.900, 8x2 0.140 / 0.920, 8x4 0.177 / 1.259 (128 registers, two CTAs per SM); V(1,1) cycle 0.728 / 3.81, 0.744 / 4.01, 0.902 / 5.10; earlier: 4x4, 16x1, 16x2 all 13-25 % behind 8x2)
 constexpr int TY = NTY * RY;               // residual tile NTX x TY; output tile (NTX-2) x (TY-2)
 constexpr int VX = NTX - 2, VY = TY - 2;
 constexpr int XW = NTX + 2, XH = TY + 2;   // x plane with its halo (and the r plane with an unused zero border)
