@@ -395,7 +395,8 @@ static double sor_cfg_cost(const poisson_ctx* ctx, const Op& op, size_t esize, S
     *g = s;
     *grid = (int)ctas;
     // time per plane ~ threads per SM; narrow tiles move shorter row segments (measured ~15 % slower per point)
-    return (double)(s.items + 2 * Cfg::NHS + 3) * Cfg::NT * conc * (Cfg::PXN < 32 ? 1.2 : 1.0);
+    // (the constant stands for the planes a run spends filling and draining the wavefront)
+    return (double)(s.items + 2 * Cfg::NHS + 8) * Cfg::NT * conc * (Cfg::PXN < 32 ? 1.2 : 1.0);
 }
 
 template <typename T, class Cfg>
@@ -419,8 +420,13 @@ static int sor_launch_cfg(poisson_ctx* ctx, const Op& op, const T* in, T* out, c
 template <typename T, int NHS, int NACT = NHS, bool ZIN = false, bool DOT = false>
 static int sor_fused_pass(poisson_ctx* ctx, const Op& op, const T* in, T* out, const T* rhs, const OmegaSet<T>& omega,
                           bool ug) {
-    constexpr int V0 = NACT < NHS ? 16 : 14;             // a narrower y halo leaves room for two more valid rows
-    using C0 = SorTile<NHS, 32 + NHS, V0 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 64 x 14 valid, 612 threads at NHS = 2 (best at 256^3 on B200)
+    // Configuration 0 is sized for 7 warps per scheduler: the register file is split over the SM's four schedulers
+    // (16384 registers each), so 25..28 warps all get 72 registers per thread and the kernel, which is latency-bound,
+    // wants as many as fit.  Four half-steps: 36 x 24 threads = 27 warps, 64 x 16 valid (measured at 256^3, us per
+    // sweep: 22 rows 109.4, 24 rows 99.5, 28 rows at 64 registers 104.3); two half-steps: 34 x 26 threads = 28 warps,
+    // 64 x 22 valid (18 rows 136.0, 22 rows 124.9, 26 rows 108.5, 30 rows at 64 registers 115.2)
+    constexpr int V0 = NHS == 4 ? (NACT < NHS ? 18 : 16) : 22;
+    using C0 = SorTile<NHS, 32 + NHS, V0 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 64 x V0 valid (best at 256^3 on B200)
     using C1 = SorTile<NHS, 16 + NHS, 28 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 32 x 28 valid, 576 threads
     using C2 = SorTile<NHS, 16 + NHS, 10 + 2 * NACT, 1, NACT, ZIN, DOT>;  // 32 x 10 valid, 252 threads, two CTAs per SM
     using C3 = SorTile<NHS, 32 + NHS, 8 + 2 * NACT, 1, NACT, ZIN, DOT>;   // 64 x 8 valid, 408 threads
